@@ -1,0 +1,181 @@
+/*
+ * acf.h -- C ABI of libacf: angular pair-count histograms (DD, DR, RR) and the
+ * w(theta) estimator of arXiv 1208.3658 (Bard et al., "Cosmological calculations on
+ * the GPU", sect. 2), computed by hand-written sm_100a CUDA kernels on one B200.
+ *
+ * Citations are lines of the paper text with the section they fall in.
+ *
+ * WHAT IS COMPUTED (the definition every kernel must reproduce bit for bit):
+ *   canonical vector  u = (cos d cos a, cos d sin a, sin d) of (RA a, Dec d)      PAPER.md:207-219 (App. A)
+ *   pair cosine       c = fma(x_i, x_j, fma(y_i, y_j, z_i * z_j)) in IEEE double,
+ *                     clamped to [-1, 1]; c is the C term of App. A = cos(theta)
+ *   range             a pair with c > e[0] or c < e[nbins] is dropped
+ *   bin               k such that e[k+1] < c <= e[k]; the last bin also takes
+ *                     c == e[nbins]  (theta_k <= theta < theta_k+1 in angle)
+ *   counts[k] += 1 ; weighted: wsums[k] += (double)w_i * (double)w_j
+ *   pair set          is_auto: unordered pairs i < j, n(n-1)/2 of them;
+ *                     cross: all n_a * n_b ordered pairs
+ *   estimator         w = (DD - 2 DR + RR) / RR on pair-normalised counts          PAPER.md:65-68 (Eq. 2)
+ * Counts are exact u64 integers under this double-precision definition whatever
+ * the internal arithmetic (fp32 is used only where a pair is provably more than a
+ * rounding bound away from every bin edge; every other pair is re-evaluated in
+ * fp64).  Weighted sums are fp64 sums of exact products; their summation order is
+ * unspecified (agreement with a long-double reference is ~1e-14 relative).
+ *
+ * CONVENTIONS
+ *   - "HOST" / "DEVICE" says where a pointer must live.  The caller owns every
+ *     buffer it passes; the library owns only the context and the scratch memory
+ *     inside it (grown lazily, freed by acf_destroy).  No PyTorch types cross the ABI.
+ *   - xyz arrays are structure-of-arrays doubles of length 3n: x[0..n) | y[0..n) | z[0..n).
+ *   - cos_edges: HOST, nbins+1 doubles, strictly descending, all within [-1, 1]
+ *     (cosines of ascending angle edges).  1 <= nbins <= ACF_MAX_BINS.
+ *   - Device work is enqueued on the context's stream and is asynchronous unless
+ *     stated; results in device buffers are valid after that stream is synchronised.
+ *   - Every function returns ACF_OK (0) or a negative ACF_E* code, never throws,
+ *     aborts or prints; acf_last_error() gives the message of the last failure on
+ *     that context.  A context is not thread-safe: one caller at a time.
+ *   - There is no CPU fallback: with no usable CUDA device acf_create fails.
+ */
+#ifndef ACF_H
+#define ACF_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define ACF_OK 0
+#define ACF_EINVAL (-1) /* bad argument: null pointer, bad edges, non-unit vectors, ... */
+#define ACF_ENOMEM (-2) /* host or device allocation failed */
+#define ACF_ECUDA (-3)  /* a CUDA runtime call or a kernel failed */
+
+#define ACF_MAX_BINS 1024
+
+typedef struct acf_ctx acf_ctx; /* opaque; library-owned */
+
+/* Options for acf_set_option. */
+enum {
+    /* Which pair kernel runs.  ACF_KERNEL_AUTO (default) = the fast fp32-certify path;
+     * ACF_KERNEL_FP64 = the reference kernel that evaluates the definition in double for
+     * every pair (slow; the arbiter the fast path defers to, kept callable for debugging). */
+    ACF_OPT_KERNEL = 1,
+    /* 1 (default): tile pairs that provably hold no in-range pair are skipped
+     * ("ignoring calculations that would fall outside the bin range");
+     * 0: every tile pair is evaluated. */
+    ACF_OPT_PRUNE = 2,
+    /* 1: collect acf_stats device counters (pairs evaluated, fp64 re-checks); default 1. */
+    ACF_OPT_STATS = 3
+};
+enum { ACF_KERNEL_AUTO = 0, ACF_KERNEL_FP64 = 1 };
+
+/* Counters of the most recent acf_pair_count* call on a context. */
+typedef struct acf_stats {
+    uint64_t pairs_nominal;      /* n(n-1)/2 or n_a*n_b (of the requested row range) */
+    uint64_t pairs_evaluated;    /* pair cosines actually computed on the device */
+    uint64_t pairs_fp64;         /* pairs re-evaluated in double (inside a guard band of an edge) */
+    uint64_t tile_pairs_total;   /* tile pairs the call is made of */
+    uint64_t tile_pairs_pruned;  /* tile pairs skipped as provably out of range */
+    uint64_t kernel_launches;    /* CUDA kernels launched by the call */
+    double device_ms;            /* device time of the call, CUDA events on the ctx stream */
+} acf_stats;
+
+/* Create a context on CUDA device `device`.  cuda_stream: a cudaStream_t (as void*) all
+ * work is enqueued on, or NULL for the legacy default stream.  *out is set on success.
+ * ACF_ECUDA if the device is missing or is not compute capability 10.x. */
+int acf_create(acf_ctx **out, int device, void *cuda_stream);
+
+/* Synchronise the stream, free the context and all its scratch.  NULL is a no-op. */
+void acf_destroy(acf_ctx *ctx);
+
+/* Message of the last failure on ctx (ctx-owned, valid until the next call); "" if none.
+ * With ctx == NULL: the message of the last failed acf_create in this thread. */
+const char *acf_last_error(const acf_ctx *ctx);
+
+/* Set ACF_OPT_* (see above).  ACF_EINVAL for an unknown option or value. */
+int acf_set_option(acf_ctx *ctx, int option, int64_t value);
+
+/* Change the stream later calls enqueue on (the previous one is synchronised first). */
+int acf_set_stream(acf_ctx *ctx, void *cuda_stream);
+
+/*
+ * Canonical unit vectors (App. A).  Pure host function, glibc sin/cos in
+ * double:  r = deg * (pi/180 as a double);  x = cos(d)*cos(a), y = cos(d)*sin(a), z = sin(d).
+ * ra_deg, dec_deg: HOST, n doubles (degrees).  xyz_host: HOST, 3n doubles, SoA, overwritten.
+ * This defines the vectors every count is made from; parity runs use it, not a device sincos.
+ */
+int acf_radec_to_xyz(const double *ra_deg, const double *dec_deg, size_t n, double *xyz_host);
+
+/*
+ * Pair-count histogram: DD or RR with is_auto = 1, DR with 0.
+ *   d_a, d_b : DEVICE, canonical xyz SoA of n_a / n_b points.  Components must be finite and
+ *              |x^2+y^2+z^2 - 1| <= 1e-6, else ACF_EINVAL (checked on the device; this
+ *              error is reported by this same call, which then synchronises).
+ *   is_auto  : 1 counts unordered pairs i<j of one catalogue (d_b must equal d_a and n_b n_a);
+ *              0 counts all n_a*n_b pairs.
+ *   d_counts : DEVICE, nbins uint64, overwritten.
+ * n = 0 (or n = 1 in auto mode) gives all-zero counts and ACF_OK.
+ */
+int acf_pair_count(acf_ctx *ctx, const double *d_a, size_t n_a, const double *d_b, size_t n_b,
+                   const double *cos_edges, int nbins, int is_auto, uint64_t *d_counts);
+
+/*
+ * Same, with pair weight w_i * w_j (not in the paper; BASELINE.json config 4).
+ *   d_wa, d_wb : DEVICE, n_a / n_b floats, finite and >= 0.  In auto mode d_wb must equal d_wa.
+ *   d_wsums    : DEVICE, nbins doubles, overwritten with sum over counted pairs of
+ *                (double)w_i * (double)w_j.  d_counts as above (unweighted), both are produced.
+ */
+int acf_pair_count_weighted(acf_ctx *ctx, const double *d_a, const float *d_wa, size_t n_a,
+                            const double *d_b, const float *d_wb, size_t n_b, const double *cos_edges,
+                            int nbins, int is_auto, uint64_t *d_counts, double *d_wsums);
+
+/*
+ * Row range of the pair matrix: rows i in [i_begin, i_end) of catalogue A against B (the
+ * paper's sub-matrix decomposition; basis of chunking and of sharding rows
+ * over GPUs).  In auto mode row i pairs with j > i only, so the counts of
+ * disjoint row ranges covering [0, n_a) add up to the full acf_pair_count result.
+ * d_wa/d_wb/d_wsums may all be NULL (unweighted).
+ */
+int acf_pair_count_rows(acf_ctx *ctx, const double *d_a, const float *d_wa, size_t n_a, size_t i_begin,
+                        size_t i_end, const double *d_b, const float *d_wb, size_t n_b,
+                        const double *cos_edges, int nbins, int is_auto, uint64_t *d_counts,
+                        double *d_wsums);
+
+/*
+ * Landy-Szalay estimator, Eq. 2, pure host, O(nbins):
+ *   w[k] = (dd - 2 dr + rr) / rr  with  dd = DD[k] / (n_d(n_d-1)/2),  dr = DR[k] / (n_d n_r),
+ *   rr = RR[k] / (n_r(n_r-1)/2);  NaN where RR[k] == 0.
+ * dd, dr, rr: HOST, nbins uint64.  w_host: HOST, nbins doubles, overwritten.
+ */
+int acf_wtheta(const uint64_t *dd, const uint64_t *dr, const uint64_t *rr, uint64_t n_d, uint64_t n_r,
+               int nbins, double *w_host);
+
+/* Weighted form: the same expression on weighted sums with normalisers
+ * ((sum w)^2 - sum w^2)/2 (auto) and (sum w_d)(sum w_r) (cross).  All pointers HOST. */
+int acf_wtheta_weighted(const double *wdd, const double *wdr, const double *wrr, const float *w_d,
+                        size_t n_d, const float *w_r, size_t n_r, int nbins, double *w_host);
+
+/*
+ * The whole job from HOST buffers: canonicalise both catalogues (acf_radec_to_xyz), copy them
+ * to the device, count DD, DR, RR, copy the histograms back and apply Eq. 2.  Synchronous.
+ *   ra_*, dec_* : HOST doubles (degrees);  w_d, w_r : HOST floats or both NULL (unweighted)
+ *   dd, dr, rr  : HOST, nbins uint64 each, overwritten
+ *   wdd, wdr, wrr : HOST, nbins doubles each (weighted sums) or all NULL when unweighted
+ *   w_host      : HOST, nbins doubles: the estimator (of the weighted sums when weighted)
+ */
+int acf_correlate_host(acf_ctx *ctx, const double *ra_d, const double *dec_d, const float *w_d, size_t n_d,
+                       const double *ra_r, const double *dec_r, const float *w_r, size_t n_r,
+                       const double *cos_edges, int nbins, uint64_t *dd, uint64_t *dr, uint64_t *rr,
+                       double *wdd, double *wdr, double *wrr, double *w_host);
+
+/* Counters of the last acf_pair_count* call (synchronises the stream). */
+int acf_get_stats(acf_ctx *ctx, acf_stats *out);
+
+/* Library version string, e.g. "acf-b200 0.1 (sm_100a)". */
+const char *acf_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ACF_H */

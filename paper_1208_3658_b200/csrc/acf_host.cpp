@@ -1,0 +1,71 @@
+// acf_host.cpp -- the pure-host entry points of libacf (no CUDA): canonical unit vectors and
+// the w(theta) estimator.  Compiled by g++ with -ffp-contract=off and no fast-math, so that
+// acf_radec_to_xyz is exactly "one rounded multiply per product around glibc sin/cos"
+// (include/acf.h; Appendix A, Eq. 2).
+#include <cmath>
+#include <cstddef>
+#include <cstdint>
+#include <limits>
+
+#include "acf.h"
+
+namespace {
+// pi/180 rounded to double; degrees -> radians is a single multiply by this constant.
+constexpr double kDegToRad = 0.017453292519943295;
+}  // namespace
+
+extern "C" int acf_radec_to_xyz(const double *ra_deg, const double *dec_deg, size_t n, double *xyz_host)
+{
+    if (n == 0) return ACF_OK;
+    if (!ra_deg || !dec_deg || !xyz_host) return ACF_EINVAL;
+    double *x = xyz_host, *y = xyz_host + n, *z = xyz_host + 2 * n;
+    for (size_t i = 0; i < n; ++i) {
+        const double alpha = ra_deg[i] * kDegToRad;
+        const double delta = dec_deg[i] * kDegToRad;
+        const double cos_delta = std::cos(delta);
+        x[i] = cos_delta * std::cos(alpha);
+        y[i] = cos_delta * std::sin(alpha);
+        z[i] = std::sin(delta);
+    }
+    return ACF_OK;
+}
+
+// Eq. 2 with pair-normalised terms (reading R2).
+static inline double landy_szalay(double dd, double dr, double rr, double ndd, double ndr, double nrr)
+{
+    if (!(rr > 0.0) || !(ndd > 0.0) || !(ndr > 0.0) || !(nrr > 0.0))
+        return std::numeric_limits<double>::quiet_NaN();
+    const double fdd = dd / ndd, fdr = dr / ndr, frr = rr / nrr;
+    return (fdd - 2.0 * fdr + frr) / frr;
+}
+
+extern "C" int acf_wtheta(const uint64_t *dd, const uint64_t *dr, const uint64_t *rr, uint64_t n_d,
+                          uint64_t n_r, int nbins, double *w_host)
+{
+    if (!dd || !dr || !rr || !w_host || nbins < 1) return ACF_EINVAL;
+    const double nd = (double)n_d, nr = (double)n_r;
+    const double ndd = nd * (nd - 1.0) / 2.0, ndr = nd * nr, nrr = nr * (nr - 1.0) / 2.0;
+    for (int k = 0; k < nbins; ++k)
+        w_host[k] = landy_szalay((double)dd[k], (double)dr[k], (double)rr[k], ndd, ndr, nrr);
+    return ACF_OK;
+}
+
+extern "C" int acf_wtheta_weighted(const double *wdd, const double *wdr, const double *wrr, const float *w_d,
+                                   size_t n_d, const float *w_r, size_t n_r, int nbins, double *w_host)
+{
+    if (!wdd || !wdr || !wrr || !w_host || nbins < 1) return ACF_EINVAL;
+    if ((n_d && !w_d) || (n_r && !w_r)) return ACF_EINVAL;
+    long double sd = 0, sd2 = 0, sr = 0, sr2 = 0;
+    for (size_t i = 0; i < n_d; ++i) {
+        sd += w_d[i];
+        sd2 += (long double)w_d[i] * w_d[i];
+    }
+    for (size_t i = 0; i < n_r; ++i) {
+        sr += w_r[i];
+        sr2 += (long double)w_r[i] * w_r[i];
+    }
+    const double ndd = (double)((sd * sd - sd2) / 2), ndr = (double)(sd * sr),
+                 nrr = (double)((sr * sr - sr2) / 2);
+    for (int k = 0; k < nbins; ++k) w_host[k] = landy_szalay(wdd[k], wdr[k], wrr[k], ndd, ndr, nrr);
+    return ACF_OK;
+}

@@ -1,0 +1,137 @@
+// acf_internal.h -- context, scratch buffers and kernel entry points shared by the .cu files
+// of libacf.  Nothing here is visible through the C ABI (include/acf.h).
+#pragma once
+
+#include <cuda_runtime.h>
+
+#include <cstdarg>
+#include <cstddef>
+#include <cstdint>
+#include <cstdio>
+
+#include "acf.h"
+
+namespace acf {
+
+// Device buffer that only ever grows; owned by the context.
+struct Scratch {
+    void *ptr = nullptr;
+    size_t bytes = 0;
+    cudaError_t reserve(size_t want)
+    {
+        if (want <= bytes) return cudaSuccess;
+        if (ptr) cudaFree(ptr);
+        ptr = nullptr;
+        bytes = 0;
+        size_t rounded = (want + 255) & ~size_t(255);
+        cudaError_t e = cudaMalloc(&ptr, rounded);
+        if (e == cudaSuccess) bytes = rounded;
+        return e;
+    }
+    void release()
+    {
+        if (ptr) cudaFree(ptr);
+        ptr = nullptr;
+        bytes = 0;
+    }
+    template <class T>
+    T *as() const
+    {
+        return static_cast<T *>(ptr);
+    }
+};
+
+// Device-side counters of one call (ACF_OPT_STATS).  Indexes into ctx->d_counters.
+enum Counter : int {
+    kCtrPairsEvaluated = 0,
+    kCtrPairsFp64 = 1,
+    kCtrTilePairsTotal = 2,
+    kCtrTilePairsPruned = 3,
+    kCtrBadInput = 4,   // number of points that failed validation
+    kCtrWorkHead = 5,   // persistent-kernel work counter
+    kCtrWorkCount = 6,  // number of work items produced on the device
+    kNumCounters = 8
+};
+
+// One catalogue prepared for the fast path (all device pointers live in ctx scratch).
+struct Prepared {
+    const double *xyz = nullptr;  // caller's canonical fp64 SoA (not owned)
+    const float *w = nullptr;     // caller's weights or nullptr
+    size_t n = 0;
+    float4 *pts = nullptr;        // spatially sorted fp32 {x, y, z, w}; padded to a tile multiple
+    uint32_t *perm = nullptr;     // sorted position -> original index
+    double4 *caps = nullptr;      // per tile: unit centre (x, y, z) and cos of the bounding radius
+    int n_tiles = 0;
+};
+
+}  // namespace acf
+
+struct acf_ctx {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    int num_sms = 0;
+    int max_smem_optin = 0;
+    char err[512] = {0};
+
+    int opt_kernel = ACF_KERNEL_AUTO;
+    int opt_prune = 1;
+    int opt_stats = 1;
+
+    cudaEvent_t ev_start = nullptr, ev_stop = nullptr, ev_flag = nullptr;
+    unsigned long long *d_counters = nullptr;  // acf::kNumCounters
+    unsigned long long *h_counters = nullptr;  // pinned mirror
+    acf_stats last{};
+    bool stats_pending = false;
+
+    // scratch, grown lazily
+    acf::Scratch s_edges;            // device copy of cos_edges (+ fp32 tables of the fast path)
+    acf::Scratch s_pts[2];           // sorted float4 points of catalogue a / b
+    acf::Scratch s_perm[2];          // permutations
+    acf::Scratch s_keys[2];          // sort keys (double-buffered inside)
+    acf::Scratch s_caps[2];          // tile caps
+    acf::Scratch s_work;             // work list
+    acf::Scratch s_misc;             // radix-sort histograms etc.
+    acf::Scratch s_host_stage[6];    // acf_correlate_host: device copies of xyz / weights / outputs
+    void *h_stage = nullptr;         // acf_correlate_host: pinned host staging
+    size_t h_stage_bytes = 0;
+};
+
+namespace acf {
+
+inline int fail(acf_ctx *ctx, int code, const char *fmt, ...)
+{
+    if (ctx) {
+        va_list ap;
+        va_start(ap, fmt);
+        vsnprintf(ctx->err, sizeof(ctx->err), fmt, ap);
+        va_end(ap);
+    }
+    return code;
+}
+
+#define ACF_CUDA_TRY(ctx, expr)                                                                   \
+    do {                                                                                          \
+        cudaError_t _e = (expr);                                                                  \
+        if (_e != cudaSuccess)                                                                    \
+            return acf::fail((ctx), _e == cudaErrorMemoryAllocation ? ACF_ENOMEM : ACF_ECUDA,     \
+                             "%s failed: %s (%s:%d)", #expr, cudaGetErrorString(_e), __FILE__,    \
+                             __LINE__);                                                           \
+    } while (0)
+
+// ---- kernels_ref.cu: the definition, one pair at a time, in double -------------------------
+// Adds into d_counts / d_wsums (which the caller has zeroed).  Rows [i_begin, i_end) of a.
+cudaError_t launch_pair_count_fp64(acf_ctx *ctx, const double *d_a, const float *d_wa, size_t n_a,
+                                   size_t i_begin, size_t i_end, const double *d_b, const float *d_wb,
+                                   size_t n_b, const double *d_edges, int nbins, int is_auto,
+                                   unsigned long long *d_counts, double *d_wsums);
+
+// ---- acf_pair.cu: the fast path (prep + fp32-certify pair kernel).  Enqueues everything needed
+// to add the counts of rows [i_begin, i_end) into d_counts / d_wsums.  Returns an ACF_* code.
+int run_pair_count_fast(acf_ctx *ctx, const double *d_a, const float *d_wa, size_t n_a, size_t i_begin,
+                        size_t i_end, const double *d_b, const float *d_wb, size_t n_b, const double *h_edges,
+                        int nbins, int is_auto, unsigned long long *d_counts, double *d_wsums);
+
+// Validates unit vectors (and weights): bumps counters[kCtrBadInput] per bad point.
+cudaError_t launch_validate(acf_ctx *ctx, const double *d_xyz, const float *d_w, size_t n);
+
+}  // namespace acf

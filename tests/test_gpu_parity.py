@@ -1,0 +1,284 @@
+"""GPU parity: the CUDA path (through the C ABI via the thin binding) against the CPU oracle,
+element by element on the same seeded inputs.  Counts must be equal as u64 integers; weighted
+sums within 1e-12 relative; w(theta) within 1e-10 absolute (north_star tolerances).
+
+Run on the B200 box:  python -m pytest tests -m gpu -x -q
+"""
+import math
+
+import numpy as np
+import pytest
+
+from workloads import cos_edges_from_theta_deg, full_sky, linear_theta_edges_deg, log_theta_edges_deg, make_config
+from workloads.catalogs import lognormal_weights, uniform_patch
+
+pytestmark = pytest.mark.gpu
+
+WSUM_RTOL = 1e-12   # north_star: weighted sums agree to <= 1e-12 relative
+WTHETA_ATOL = 1e-10  # north_star: w(theta) agrees to <= 1e-10 absolute
+
+
+@pytest.fixture(scope="module")
+def acf():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    import paper_1208_3658_b200 as P
+    return P
+
+
+@pytest.fixture(scope="module")
+def ctx(acf):
+    c = acf.acf_create(0)
+    yield c
+    acf.acf_destroy(c)
+
+
+def dev(x, dtype=None):
+    import torch
+    t = torch.from_numpy(np.ascontiguousarray(x))
+    if dtype is not None:
+        t = t.to(dtype)
+    return t.cuda()
+
+
+def gpu_counts(acf, ctx, xa, xb, edges, auto, wa=None, wb=None, rows=None, kernel=None):
+    """Run one pair count on the device and bring the result back as numpy."""
+    import torch
+    if kernel is not None:
+        acf.acf_set_option(ctx, acf.ACF_OPT_KERNEL, kernel)
+    try:
+        da = dev(xa)
+        db = None if auto else dev(xb)
+        n_a = xa.size // 3
+        i0, i1 = (0, n_a) if rows is None else rows
+        if wa is None:
+            if rows is None:
+                out = acf.acf_pair_count(ctx, da, db, edges, auto)
+            else:
+                out = acf.acf_pair_count_rows(ctx, da, None, i0, i1, db, None, edges, auto)
+            torch.cuda.synchronize()
+            return acf.counts_to_numpy(out)
+        dwa = dev(wa)
+        dwb = None if auto else dev(wb)
+        c, w = acf.acf_pair_count_rows(ctx, da, dwa, i0, i1, db, dwb, edges, auto)
+        torch.cuda.synchronize()
+        return acf.counts_to_numpy(c), w.cpu().numpy()
+    finally:
+        if kernel is not None:
+            acf.acf_set_option(ctx, acf.ACF_OPT_KERNEL, acf.ACF_KERNEL_AUTO)
+
+
+def soa(v):
+    v = np.asarray(v, dtype=np.float64)
+    return np.concatenate([v[:, 0], v[:, 1], v[:, 2]])
+
+
+def test_canonical_vectors_bit_equal(acf, oracle):
+    # both sides call glibc sin/cos on the same doubles: the arrays must be identical bit for bit
+    ra, dec = full_sky(20000, 3)
+    a = acf.acf_radec_to_xyz(ra, dec)
+    b = oracle.radec_to_xyz(ra, dec)
+    assert a.tobytes() == b.tobytes()
+
+
+@pytest.mark.parametrize("kernel", ["auto", "fp64"])
+@pytest.mark.parametrize("name,scale", [("tiny", 0.5), ("clustered_patch", 0.03), ("survey_scale", 0.006),
+                                        ("full_sky", 0.008), ("pruning_stress", 0.0012)])
+def test_config_parity(acf, ctx, oracle, name, scale, kernel):
+    """All five BASELINE configurations at a size the oracle finishes in seconds: several tiles
+    and ragged tails on both catalogues; DD, DR, RR and the estimator."""
+    kern = acf.ACF_KERNEL_FP64 if kernel == "fp64" else acf.ACF_KERNEL_AUTO
+    w = make_config(name, scale)
+    xd, xr = acf.acf_radec_to_xyz(w.ra_d, w.dec_d), acf.acf_radec_to_xyz(w.ra_r, w.dec_r)
+    assert xd.tobytes() == oracle.radec_to_xyz(w.ra_d, w.dec_d).tobytes()
+    res = {}
+    for key, (a, b, auto, wa, wb) in {"dd": (xd, None, True, w.w_d, None), "dr": (xd, xr, False, w.w_d, w.w_r),
+                                      "rr": (xr, None, True, w.w_r, None)}.items():
+        want = oracle.pair_count(a, b, w.cos_edges, auto, w_a=wa, w_b=wb)
+        got = gpu_counts(acf, ctx, a, b, w.cos_edges, auto, wa=wa, wb=wb, kernel=kern)
+        if wa is None:
+            assert got.tolist() == want.tolist(), key
+            res[key] = got
+        else:
+            assert got[0].tolist() == want[0].tolist(), key
+            np.testing.assert_allclose(got[1], want[1], rtol=WSUM_RTOL, atol=0, err_msg=key)
+            res[key] = got[0]
+            res["w" + key] = got[1]
+        st = acf.acf_get_stats(ctx)
+        n_a = a.size // 3
+        assert st["pairs_nominal"] == (n_a * (n_a - 1) // 2 if auto else n_a * (b.size // 3))
+        assert st["kernel_launches"] >= 1
+    assert int(res["dd"].sum()) > 0 and int(res["rr"].sum()) > 0
+    wt = acf.acf_wtheta(res["dd"], res["dr"], res["rr"], w.n_d, w.n_r)
+    wo = oracle.wtheta(res["dd"], res["dr"], res["rr"], w.n_d, w.n_r)
+    assert np.array_equal(np.isnan(wt), np.isnan(wo))
+    np.testing.assert_allclose(wt[~np.isnan(wt)], wo[~np.isnan(wo)], rtol=0, atol=WTHETA_ATOL)
+    if w.w_d is not None:
+        ww = acf.acf_wtheta_weighted(res["wdd"], res["wdr"], res["wrr"], w.w_d, w.w_r)
+        wwo = oracle.wtheta_weighted(res["wdd"], res["wdr"], res["wrr"], w.w_d, w.w_r)
+        np.testing.assert_allclose(ww, wwo, rtol=0, atol=WTHETA_ATOL, equal_nan=True)
+
+
+def test_polyhedra_and_full_range(acf, ctx, oracle):
+    phi = (1 + 5 ** 0.5) / 2
+    ico = []
+    for s1 in (-1, 1):
+        for s2 in (-1, 1):
+            ico += [(0, s1, s2 * phi), (s1, s2 * phi, 0), (s2 * phi, 0, s1)]
+    ico = np.array(ico, dtype=np.float64)
+    ico /= np.linalg.norm(ico, axis=1, keepdims=True)
+    xyz = soa(ico)
+    edges = np.array([1.0, 0.0, -0.9, -1.0])
+    assert gpu_counts(acf, ctx, xyz, None, edges, True).tolist() == [30, 30, 6]
+    assert gpu_counts(acf, ctx, xyz, xyz, edges, False).tolist() == [72, 60, 12]   # + 12 self pairs at c = 1
+    # totals when the bins cover [0, 180] deg: n(n-1)/2 and n_a n_b
+    ra, dec = full_sky(3000, 41)
+    rb, db_ = full_sky(2500, 42)
+    a, b = acf.acf_radec_to_xyz(ra, dec), acf.acf_radec_to_xyz(rb, db_)
+    full = cos_edges_from_theta_deg(np.array([0.0, 0.01, 1.0, 30.0, 90.0, 179.0, 180.0]))
+    ca = gpu_counts(acf, ctx, a, None, full, True)
+    cb = gpu_counts(acf, ctx, a, b, full, False)
+    assert int(ca.sum()) == 3000 * 2999 // 2 and int(cb.sum()) == 3000 * 2500
+    assert ca.tolist() == oracle.pair_count(a, None, full, True).tolist()
+    assert cb.tolist() == oracle.pair_count(a, b, full, False).tolist()
+    assert cb.tolist() == gpu_counts(acf, ctx, b, a, full, False).tolist()       # swap symmetry
+
+
+@pytest.mark.parametrize("kernel", ["auto", "fp64"])
+def test_edge_inclusivity_adversarial(acf, ctx, oracle, kernel):
+    """Pairs whose cosine is exactly an edge, or one ulp either side, through the xyz entry point:
+    a = (1,0,0), b = (c, sqrt(1-c^2), 0) makes the defined pair cosine equal c exactly."""
+    kern = acf.ACF_KERNEL_FP64 if kernel == "fp64" else acf.ACF_KERNEL_AUTO
+    edges = cos_edges_from_theta_deg(log_theta_edges_deg(0.05, 170.0, 12))
+    cs = []
+    for e in edges:
+        cs += [e, np.nextafter(e, 2.0), np.nextafter(e, -2.0), e + 3e-7, e - 3e-7, e + 1e-8, e - 1e-8]
+    cs += [1.0, -1.0, 0.0, 0.5]
+    cs = np.clip(np.array(cs), -1.0, 1.0)
+    b = np.stack([cs, np.sqrt(np.maximum(0.0, 1.0 - cs * cs)), np.zeros_like(cs)], axis=1)
+    # renormalising would move c; instead keep norms within the validator's 1e-6 (they are ~1e-16 off)
+    xa = soa([(1.0, 0.0, 0.0)])
+    xb = soa(b)
+    want = oracle.pair_count(xa, xb, edges, False)
+    got = gpu_counts(acf, ctx, xa, xb, edges, False, kernel=kern)
+    assert got.tolist() == want.tolist()
+    got = gpu_counts(acf, ctx, xb, xa, edges, False, kernel=kern)
+    assert got.tolist() == want.tolist()
+    # and one pair at a time, so that a compensating double error cannot hide
+    for c, row in zip(cs[:21], b[:21]):
+        one = soa([row])
+        assert gpu_counts(acf, ctx, xa, one, edges, False, kernel=kern).tolist() == oracle.pair_count(xa, one, edges, False).tolist(), c
+
+
+def test_duplicates_and_clamp(acf, ctx, oracle):
+    # coincident points: c may round above 1 and is clamped; counted iff e_0 = 1
+    ra, dec = full_sky(500, 7)
+    ra = np.concatenate([ra, ra[:100]])
+    dec = np.concatenate([dec, dec[:100]])
+    a = acf.acf_radec_to_xyz(ra, dec)
+    for edges in (cos_edges_from_theta_deg(np.array([0.0, 1.0, 90.0, 180.0])),
+                  cos_edges_from_theta_deg(np.array([1e-6, 1.0, 90.0, 180.0]))):
+        assert gpu_counts(acf, ctx, a, None, edges, True).tolist() == oracle.pair_count(a, None, edges, True).tolist()
+
+
+def test_degenerate_sizes(acf, ctx):
+    import torch
+    edges = np.array([1.0, 0.0, -1.0])
+    one = soa([(0.0, 0.0, 1.0)])
+    two = soa([(0.0, 0.0, 1.0), (0.0, 1.0, 0.0)])
+    empty = np.zeros(0)
+    assert gpu_counts(acf, ctx, one, None, edges, True).tolist() == [0, 0]          # n = 1, auto
+    assert gpu_counts(acf, ctx, two, None, edges, True).tolist() == [1, 0]          # c = 0 -> bin 0 (closed above)
+    assert gpu_counts(acf, ctx, one, two, edges, False).tolist() == [2, 0]
+    out = acf.acf_pair_count(ctx, torch.zeros(0, dtype=torch.float64, device="cuda"), None, edges, True)
+    torch.cuda.synchronize()
+    assert out.cpu().tolist() == [0, 0]
+    assert gpu_counts(acf, ctx, two, None, edges, True, rows=(1, 1)).tolist() == [0, 0]
+
+
+def test_row_ranges_add_up(acf, ctx, oracle):
+    # the pair matrix cut into sub-matrices; counts are additive over row ranges
+    w = make_config("clustered_patch", 0.02)
+    xd, xr = acf.acf_radec_to_xyz(w.ra_d, w.dec_d), acf.acf_radec_to_xyz(w.ra_r, w.dec_r)
+    n = w.n_d
+    cuts = [0, 1, 777, 1024, 2049, n]
+    for b, auto in ((None, True), (xr, False)):
+        whole = gpu_counts(acf, ctx, xd, b, w.cos_edges, auto)
+        parts = np.zeros_like(whole)
+        for lo, hi in zip(cuts[:-1], cuts[1:]):
+            p = gpu_counts(acf, ctx, xd, b, w.cos_edges, auto, rows=(lo, hi))
+            assert p.tolist() == oracle.pair_count(xd, b, w.cos_edges, auto, rows=(lo, hi)).tolist()
+            parts += p
+        assert parts.tolist() == whole.tolist()
+
+
+def test_linear_bins_many(acf, ctx, oracle):
+    # the paper's benchmark used 254 bins; even spacing is one of its presets
+    ra, dec = uniform_patch(6000, (0.0, 90.0), (0.0, 90.0), 5)   # the paper's octant footprint
+    a = acf.acf_radec_to_xyz(ra, dec)
+    for theta in (linear_theta_edges_deg(0.0, 120.0, 254), log_theta_edges_deg(0.01, 100.0, 254)):
+        edges = cos_edges_from_theta_deg(theta)
+        assert gpu_counts(acf, ctx, a, None, edges, True).tolist() == oracle.pair_count(a, None, edges, True).tolist()
+
+
+def test_weighted_dyadic_exact(acf, ctx):
+    # power-of-two weights: every product and partial sum is exact, so the sums must be exact too
+    ra, dec = full_sky(3000, 51)
+    a = acf.acf_radec_to_xyz(ra, dec)
+    rng = np.random.default_rng(52)
+    wa = (2.0 ** rng.integers(-3, 4, size=3000)).astype(np.float32)
+    edges = cos_edges_from_theta_deg(np.array([0.0, 40.0, 90.0, 130.0, 180.0]))
+    c, ws = gpu_counts(acf, ctx, a, None, edges, True, wa=wa)
+    c1, w1 = gpu_counts(acf, ctx, a, None, edges, True, wa=np.ones(3000, np.float32))
+    assert c.tolist() == c1.tolist() and w1.tolist() == c1.astype(np.float64).tolist()
+    assert np.all(ws * 64 == np.round(ws * 64))
+
+
+def test_invalid_arguments(acf, ctx):
+    import torch
+    ra, dec = full_sky(100, 1)
+    a = acf.acf_radec_to_xyz(ra, dec)
+    da = dev(a)
+    ok = np.array([1.0, 0.0, -1.0])
+    for bad in (np.array([0.0, 0.5]), np.array([1.5, 0.0]), np.array([0.5]), np.array([0.5, 0.5])):
+        with pytest.raises(acf.AcfError) as ei:
+            acf.acf_pair_count(ctx, da, None, bad, True)
+        assert ei.value.code == -1
+    with pytest.raises(acf.AcfError):
+        acf.acf_pair_count_rows(ctx, da, None, 5, 101, None, None, ok, True)      # row range outside
+    # non-unit and non-finite vectors are rejected by the device-side check
+    for poison in (2.0, float("nan"), float("inf")):
+        b = a.copy()
+        b[17] = poison
+        with pytest.raises(acf.AcfError) as ei:
+            acf.acf_pair_count(ctx, dev(b), None, ok, True)
+        assert ei.value.code == -1 and "unit" in str(ei.value)
+    with pytest.raises(acf.AcfError):
+        acf.acf_pair_count_rows(ctx, da, dev(-np.ones(100, np.float32)), 0, 100, None, None, ok, True)
+    # the context still works afterwards
+    out = acf.acf_pair_count(ctx, da, None, ok, True)
+    torch.cuda.synchronize()
+    assert int(out.sum()) == 100 * 99 // 2
+
+
+def test_correlate_host_end_to_end(acf, ctx, oracle):
+    w = make_config("full_sky", 0.004)
+    res = acf.acf_correlate_host(ctx, w.ra_d, w.dec_d, w.w_d, w.ra_r, w.dec_r, w.w_r, w.cos_edges)
+    xd, xr = oracle.radec_to_xyz(w.ra_d, w.dec_d), oracle.radec_to_xyz(w.ra_r, w.dec_r)
+    dd, wdd = oracle.pair_count(xd, None, w.cos_edges, True, w_a=w.w_d)
+    dr, wdr = oracle.pair_count(xd, xr, w.cos_edges, False, w_a=w.w_d, w_b=w.w_r)
+    rr, wrr = oracle.pair_count(xr, None, w.cos_edges, True, w_a=w.w_r)
+    assert res["dd"].tolist() == dd.tolist() and res["dr"].tolist() == dr.tolist() and res["rr"].tolist() == rr.tolist()
+    np.testing.assert_allclose(res["wdd"], wdd, rtol=WSUM_RTOL)
+    np.testing.assert_allclose(res["wdr"], wdr, rtol=WSUM_RTOL)
+    np.testing.assert_allclose(res["wrr"], wrr, rtol=WSUM_RTOL)
+    np.testing.assert_allclose(res["w"], oracle.wtheta_weighted(wdd, wdr, wrr, w.w_d, w.w_r), rtol=0, atol=WTHETA_ATOL,
+                               equal_nan=True)
+    t = make_config("tiny", 0.3)
+    res = acf.acf_correlate_host(ctx, t.ra_d, t.dec_d, None, t.ra_r, t.dec_r, None, t.cos_edges)
+    xd, xr = oracle.radec_to_xyz(t.ra_d, t.dec_d), oracle.radec_to_xyz(t.ra_r, t.dec_r)
+    dd, dr, rr = (oracle.pair_count(xd, None, t.cos_edges, True), oracle.pair_count(xd, xr, t.cos_edges, False),
+                  oracle.pair_count(xr, None, t.cos_edges, True))
+    assert res["dd"].tolist() == dd.tolist() and res["dr"].tolist() == dr.tolist() and res["rr"].tolist() == rr.tolist()
+    np.testing.assert_allclose(res["w"], oracle.wtheta(dd, dr, rr, t.n_d, t.n_r), rtol=0, atol=WTHETA_ATOL, equal_nan=True)

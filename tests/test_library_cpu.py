@@ -1,0 +1,84 @@
+"""CPU-side checks of libacf.so (-m "not gpu"): it builds, loads, exports every symbol that
+include/acf.h declares, its pure-host entry points agree with the oracle, and with no GPU it
+fails loudly instead of falling back."""
+import ctypes
+import math
+import os
+import re
+
+import numpy as np
+import pytest
+
+from conftest import ROOT, read_golden
+from workloads import full_sky
+
+
+@pytest.fixture(scope="module")
+def acf():
+    import paper_1208_3658_b200 as P
+    P.load_library()
+    return P
+
+
+def test_exports_match_header(acf):
+    header = open(os.path.join(ROOT, "include", "acf.h")).read()
+    header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
+    declared = set(re.findall(r"\b(acf_[a-z0-9_]+)\s*\(", header))
+    assert {"acf_create", "acf_pair_count", "acf_wtheta"} <= declared   # the names north_star fixes
+    lib = ctypes.CDLL(os.path.join(ROOT, "paper_1208_3658_b200", "libacf.so"))
+    for name in sorted(declared):
+        assert hasattr(lib, name), "libacf.so does not export %s" % name
+    from paper_1208_3658_b200.binding import EXPORTS
+    assert set(EXPORTS) == declared
+
+
+def test_no_gpu_means_error_not_fallback(acf):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    with pytest.raises(acf.AcfError) as ei:
+        acf.acf_create(0)
+    assert ei.value.code == -3
+    # straight through the C ABI as well
+    lib = acf.load_library()
+    ctx = ctypes.c_void_p()
+    assert lib.acf_create(ctypes.byref(ctx), 0, None) == -3
+    assert not ctx.value
+    assert b"no CUDA device" in lib.acf_last_error(None)
+
+
+def test_radec_to_xyz_matches_oracle_bitwise(acf, oracle):
+    ra, dec = full_sky(50000, 77)
+    assert acf.acf_radec_to_xyz(ra, dec).tobytes() == oracle.radec_to_xyz(ra, dec).tobytes()
+    rows = read_golden("radec_unit_vectors.txt")
+    xyz = acf.acf_radec_to_xyz([float(r[0]) for r in rows], [float(r[1]) for r in rows]).reshape(3, -1).T
+    want = np.array([[float(v) for v in r[2:5]] for r in rows])
+    assert np.max(np.abs(xyz - want)) < 3e-16
+
+
+def test_wtheta_golden_and_oracle(acf, oracle):
+    for r in read_golden("wtheta_examples.txt"):
+        n_d, n_r, dd, dr, rr = (int(v) for v in r[:5])
+        w = acf.acf_wtheta([dd], [dr], [rr], n_d, n_r)[0]
+        assert math.isnan(w) if r[5] == "nan" else abs(w - float(r[5])) < 1e-15
+    rng = np.random.default_rng(3)
+    dd, dr, rr = (rng.integers(0, 10 ** 9, size=40).astype(np.uint64) for _ in range(3))
+    rr[5] = 0
+    a = acf.acf_wtheta(dd, dr, rr, 123456, 234567)
+    b = oracle.wtheta(dd, dr, rr, 123456, 234567)
+    np.testing.assert_allclose(a, b, rtol=0, atol=1e-10, equal_nan=True)
+    wd = rng.lognormal(0, 0.3, 1000).astype(np.float32)
+    wr = rng.lognormal(0, 0.3, 1500).astype(np.float32)
+    x, y, z = (rng.uniform(1, 1e5, size=40) for _ in range(3))
+    np.testing.assert_allclose(acf.acf_wtheta_weighted(x, y, z, wd, wr), oracle.wtheta_weighted(x, y, z, wd, wr),
+                               rtol=0, atol=1e-10)
+
+
+def test_host_argument_errors(acf):
+    lib = acf.load_library()
+    assert lib.acf_wtheta(None, None, None, 1, 1, 3, None) == -1
+    assert lib.acf_radec_to_xyz(None, None, 5, None) == -1
+    assert lib.acf_radec_to_xyz(None, None, 0, None) == 0
+    assert lib.acf_set_option(None, 1, 0) == -1
+    assert lib.acf_get_stats(None, None) == -1
+    lib.acf_destroy(None)   # no-op
