@@ -170,17 +170,13 @@ extern "C" int acf_pair_count_rows(acf_ctx *ctx, const double *d_a, const float 
                                           sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
         ACF_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_flag, st));
 
-        ACF_CUDA_TRY(ctx, ctx->s_edges.reserve(sizeof(double) * (size_t)(nbins + 1)));
-        ACF_CUDA_TRY(ctx, cudaMemcpyAsync(ctx->s_edges.ptr, cos_edges, sizeof(double) * (size_t)(nbins + 1), cudaMemcpyHostToDevice, st));
-
-        bool done = false;
         if (ctx->opt_kernel == ACF_KERNEL_AUTO) {
             int rc = acf::run_pair_count_fast(ctx, d_a, d_wa, n_a, i_begin, i_end, d_b, d_wb, n_b, cos_edges, nbins,
                                               is_auto, reinterpret_cast<unsigned long long *>(d_counts), d_wsums);
             if (rc != ACF_OK) return rc;
-            done = true;
-        }
-        if (!done) {
+        } else {
+            ACF_CUDA_TRY(ctx, ctx->s_edges.reserve(sizeof(double) * (size_t)(nbins + 1)));
+            ACF_CUDA_TRY(ctx, cudaMemcpyAsync(ctx->s_edges.ptr, cos_edges, sizeof(double) * (size_t)(nbins + 1), cudaMemcpyHostToDevice, st));
             ACF_CUDA_TRY(ctx, acf::launch_pair_count_fp64(ctx, d_a, d_wa, n_a, i_begin, i_end, d_b, d_wb, n_b,
                                                           ctx->s_edges.as<double>(), nbins, is_auto,
                                                           reinterpret_cast<unsigned long long *>(d_counts), d_wsums));

@@ -53,11 +53,15 @@ enum Counter : int {
     kNumCounters = 8
 };
 
+constexpr int kTile = 1024;      // points per tile (both the register-resident i side and the staged j side)
+constexpr int kItemTiles = 8;    // at most this many consecutive j-tiles per work item
+
 // One catalogue prepared for the fast path (all device pointers live in ctx scratch).
 struct Prepared {
     const double *xyz = nullptr;  // caller's canonical fp64 SoA (not owned)
     const float *w = nullptr;     // caller's weights or nullptr
-    size_t n = 0;
+    size_t stride = 0;            // points in the caller's catalogue (SoA stride)
+    size_t n = 0;                 // points prepared
     float4 *pts = nullptr;        // spatially sorted fp32 {x, y, z, w}; padded to a tile multiple
     uint32_t *perm = nullptr;     // sorted position -> original index
     double4 *caps = nullptr;      // per tile: unit centre (x, y, z) and cos of the bounding radius
@@ -130,6 +134,13 @@ cudaError_t launch_pair_count_fp64(acf_ctx *ctx, const double *d_a, const float 
 int run_pair_count_fast(acf_ctx *ctx, const double *d_a, const float *d_wa, size_t n_a, size_t i_begin,
                         size_t i_end, const double *d_b, const float *d_wb, size_t n_b, const double *h_edges,
                         int nbins, int is_auto, unsigned long long *d_counts, double *d_wsums);
+
+// ---- acf_prep.cu: sort + gather + caps of points [off, off+cnt) of a catalogue with `stride` points;
+// and the work list of (i-tile, j-tile run) items for i-tiles [ti_begin, ti_end).
+int prepare_catalogue(acf_ctx *ctx, int slot, const double *xyz, size_t stride, size_t off, size_t cnt,
+                      const float *w, Prepared *out);
+int build_worklist(acf_ctx *ctx, const Prepared &a, int ti_begin, int ti_end, const Prepared &b, int is_auto,
+                   double e_first, double e_last, int3 *items, uint32_t capacity);
 
 // Validates unit vectors (and weights): bumps counters[kCtrBadInput] per bad point.
 cudaError_t launch_validate(acf_ctx *ctx, const double *d_xyz, const float *d_w, size_t n);

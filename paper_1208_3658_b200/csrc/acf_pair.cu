@@ -1,14 +1,500 @@
-// acf_pair.cu -- fast path (placeholder while the fp32-certify kernel is being written):
-// routes to the fp64 reference kernel.
+// acf_pair.cu -- the fast path of acf_pair_count*: fp32 pair cosine with certified binning,
+// fp64 re-check of every pair the fp32 test cannot certify.
+//
+// Per pair ("most of their time actually calculating the angular separations"):
+//   t32 = K - (x_i x_j + y_i y_j + z_i z_j)   three fp32 FMAs; K = 1 + 2^-18 keeps t32 > 0
+//   cell = float bits of t32 >> (23 - m)       log-spaced cells, 2^m per octave of t
+//   {thr, row} = LUT[cell]                     the one bin edge (as K - e) that can matter in the cell
+//   row += (t32 > thr)                         histogram row: 0 = closer than theta_min, 1..nbins = bins,
+//                                              nbins+1 = beyond theta_max (dropped)
+//   certified iff |t32 - thr| > G              G bounds |t32 - (K - c64)| + rounding of thr
+// A pair that is not certified is re-evaluated exactly as include/acf.h defines it (fp64 fma
+// chain on the caller's doubles, clamp, exact edge search) and the histogram is corrected, so
+// the counts equal the fp64 definition whatever the fp32 arithmetic did.
+//
+// Histograms are privatised per lane in shared memory (row-major [row][lane]: a lane owns a bank,
+// so updates never conflict and need no ordering -- PAPER.md:86 reports 5-50 % loss to atomic
+// serialisation), summed per warp with shuffles and flushed with global u64 / f64 atomics.
+// j-tiles are staged with cp.async.bulk (TMA, mbarrier completion) into a double buffer while
+// each thread holds kR i-points in registers.  Auto-correlations visit the upper triangle only.
+#include <cmath>
+#include <cstring>
+#include <vector>
+
+#include "acf_device.cuh"
 #include "acf_internal.h"
 
 namespace acf {
-int run_pair_count_fast(acf_ctx *ctx, const double *d_a, const float *d_wa, size_t n_a, size_t i_begin,
-                        size_t i_end, const double *d_b, const float *d_wb, size_t n_b, const double *,
-                        int nbins, int is_auto, unsigned long long *d_counts, double *d_wsums)
+
+namespace {
+
+constexpr int kThreads = 256;
+constexpr int kWarps = kThreads / 32;
+constexpr int kR = kTile / kThreads;  // i-points per thread
+constexpr float kK = 1.0f + 0x1p-18f;
+// |t32 - (K - c64)| <= 2u(1+1e-6) [input rounding, u = 2^-24] + 3 * 2^-23 [three roundings of values < 4]
+// = 4.77e-7; thr is K - e rounded to fp32: another 2^-23 at most.
+constexpr float kDelta = 5.5e-7f;
+constexpr float kGuard = kDelta + 0x1p-23f;
+constexpr int kExpLo = -19;  // t32 >= K - (1 + 1e-6) - kDelta > 2^-19
+constexpr int kExpHi = 2;    // t32 < 4
+constexpr int kMaxPrivateRows = 64;
+
+struct PairParams {
+    const float4 *pts_a, *pts_b;
+    const uint32_t *perm_a, *perm_b;
+    uint32_t n_a, n_b;
+    const double *xyz_a, *xyz_b;
+    size_t stride_a, stride_b;
+    const int3 *items;
+    uint32_t capacity;
+    const uint2 *lut;
+    int lut_len, key0, shift;
+    const double *edges;
+    int nbins;
+    unsigned long long *counts;
+    double *wsums;
+    unsigned long long *counters;
+    int is_auto;
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
 {
-    ACF_CUDA_TRY(ctx, launch_pair_count_fp64(ctx, d_a, d_wa, n_a, i_begin, i_end, d_b, d_wb, n_b,
-                                             ctx->s_edges.as<double>(), nbins, is_auto, d_counts, d_wsums));
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_LOOP:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra WAIT_DONE;\n"
+        "bra WAIT_LOOP;\n"
+        "WAIT_DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// TMA 1-D bulk copy global -> shared, completion signalled on an mbarrier (SASS: UBLKCP)
+__device__ __forceinline__ void bulk_load(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+
+// Exact histogram row of a pair: the definition of include/acf.h on the caller's doubles.
+__device__ __noinline__ int exact_row(const double *__restrict__ xyz_a, size_t stride_a, size_t gi,
+                                      const double *__restrict__ xyz_b, size_t stride_b, size_t gj,
+                                      const double *__restrict__ edges, int nbins)
+{
+    const double c = pair_cos_fp64(xyz_a[gi], xyz_a[stride_a + gi], xyz_a[2 * stride_a + gi], xyz_b[gj],
+                                   xyz_b[stride_b + gj], xyz_b[2 * stride_b + gj]);
+    const int k = bin_of_fp64(c, edges, nbins);
+    if (k >= 0) return k + 1;
+    return c > edges[0] ? 0 : nbins + 1;
+}
+
+template <bool kWeighted, bool kPrivate>
+struct Hist {
+    uint32_t *cnt;  // private: this warp's [rows][32]; shared: the CTA's [rows]
+    double *ws;     // same shapes (weighted only)
+    int lane;
+    __device__ __forceinline__ void add(uint32_t row)
+    {
+        if constexpr (kPrivate) atomicAdd(&cnt[row * 32 + lane], 1u);  // own bank: conflict-free, result unused -> RED
+        else atomicAdd(&cnt[row], 1u);
+    }
+    __device__ __forceinline__ void add_w(uint32_t row, double w)
+    {
+        if constexpr (kPrivate) ws[row * 32 + lane] += w;  // the lane owns the word: plain read-modify-write
+        else atomicAdd(&ws[row], w);
+    }
+    __device__ __forceinline__ void move(uint32_t from, uint32_t to)
+    {
+        if constexpr (kPrivate) {
+            cnt[from * 32 + lane] -= 1u;
+            cnt[to * 32 + lane] += 1u;
+        } else {
+            atomicSub(&cnt[from], 1u);
+            atomicAdd(&cnt[to], 1u);
+        }
+    }
+};
+
+// One j-tile against the kR register-resident i-points of every thread.
+// kMasked: pairs are individually enabled (ragged last i-tile, or the diagonal tile of an auto count
+// where only j > i is counted).
+template <bool kWeighted, bool kPrivate, bool kMasked>
+__device__ __forceinline__ void process_tile(const PairParams &p, Hist<kWeighted, kPrivate> &h, const float4 *__restrict__ tile,
+                                             int jn, const float (&nx)[kR], const float (&ny)[kR], const float (&nz)[kR],
+                                             const float (&wi)[kR], const uint2 *__restrict__ lut, uint32_t i_base,
+                                             uint32_t j_base, bool diag, uint32_t valid_mask, unsigned long long &n_fp64)
+{
+    const int shift = p.shift, key0 = p.key0;
+    const uint32_t tid = threadIdx.x;
+#pragma unroll 2
+    for (int jj = 0; jj < jn; ++jj) {
+        const float4 q = tile[jj];
+        bool amb_any = false;
+        bool amb[kR];
+        uint32_t row[kR];
+#pragma unroll
+        for (int r = 0; r < kR; ++r) {
+            const float t = fmaf(nx[r], q.x, fmaf(ny[r], q.y, fmaf(nz[r], q.z, kK)));
+            const uint2 e = lut[(int)(__float_as_uint(t) >> shift) - key0];
+            const float thr = __uint_as_float(e.x);
+            row[r] = e.y + (t > thr ? 1u : 0u);
+            amb[r] = !(fabsf(t - thr) > kGuard);  // also true for the NaN threshold of a crowded cell
+            if constexpr (kMasked) {
+                const bool on = ((valid_mask >> r) & 1u) && (!diag || (uint32_t)jj > (uint32_t)(r * kThreads) + tid);
+                amb[r] = amb[r] && on;
+                if (on) h.add(row[r]);
+                if constexpr (kWeighted)
+                    if (on && !amb[r]) h.add_w(row[r], (double)wi[r] * (double)q.w);
+            } else {
+                h.add(row[r]);
+                if constexpr (kWeighted)
+                    if (!amb[r]) h.add_w(row[r], (double)wi[r] * (double)q.w);
+            }
+            amb_any |= amb[r];
+        }
+        if (__any_sync(0xffffffffu, amb_any)) {
+#pragma unroll
+            for (int r = 0; r < kR; ++r) {
+                if (amb[r]) {
+                    const int exact = exact_row(p.xyz_a, p.stride_a, p.perm_a[i_base + r * kThreads + tid], p.xyz_b,
+                                                p.stride_b, p.perm_b[j_base + jj], p.edges, p.nbins);
+                    if ((uint32_t)exact != row[r]) h.move(row[r], (uint32_t)exact);
+                    if constexpr (kWeighted) h.add_w((uint32_t)exact, (double)wi[r] * (double)q.w);
+                    ++n_fp64;
+                }
+            }
+        }
+    }
+}
+
+template <bool kWeighted, bool kPrivate>
+__global__ void __launch_bounds__(kThreads, kWeighted ? 1 : 2) pair_kernel(const PairParams p)
+{
+    if (p.counters[kCtrBadInput] != 0) return;  // inputs failed validation: never index the LUT with garbage
+    extern __shared__ __align__(128) unsigned char smem[];
+    const int rows = p.nbins + 2;
+    // layout: [2 mbarriers][tile 0][tile 1][LUT][count rows][weighted rows]
+    uint64_t *bars = reinterpret_cast<uint64_t *>(smem);
+    float4 *tiles = reinterpret_cast<float4 *>(smem + 128);
+    uint2 *lut = reinterpret_cast<uint2 *>(smem + 128 + 2 * kTile * sizeof(float4));
+    const size_t cnt_words = kPrivate ? (size_t)kWarps * rows * 32 : (size_t)rows;
+    size_t off = 128 + 2 * kTile * sizeof(float4) + (size_t)p.lut_len * sizeof(uint2);
+    off = (off + 15) & ~size_t(15);
+    uint32_t *cnt_all = reinterpret_cast<uint32_t *>(smem + off);
+    off += cnt_words * sizeof(uint32_t);
+    off = (off + 15) & ~size_t(15);
+    double *ws_all = reinterpret_cast<double *>(smem + off);
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    for (int i = tid; i < p.lut_len; i += kThreads) lut[i] = p.lut[i];
+    for (size_t i = tid; i < cnt_words; i += kThreads) cnt_all[i] = 0;
+    if constexpr (kWeighted)
+        for (size_t i = tid; i < cnt_words; i += kThreads) ws_all[i] = 0.0;
+    if (tid == 0) {
+        mbar_init(&bars[0], 1);
+        mbar_init(&bars[1], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    Hist<kWeighted, kPrivate> h;
+    h.cnt = kPrivate ? cnt_all + (size_t)warp * rows * 32 : cnt_all;
+    h.ws = kPrivate ? ws_all + (size_t)warp * rows * 32 : ws_all;
+    h.lane = lane;
+
+    unsigned long long n_items = p.counters[kCtrWorkCount];
+    if (n_items > p.capacity) n_items = p.capacity;
+    __shared__ unsigned int s_item;
+    uint32_t consumed = 0;  // j-tiles this CTA has staged so far: buffer = consumed & 1, parity = (consumed >> 1) & 1
+    unsigned long long n_fp64 = 0, n_eval = 0;
+
+    while (true) {
+        if (tid == 0) s_item = (unsigned int)atomicAdd(&p.counters[kCtrWorkHead], 1ull);
+        __syncthreads();
+        const unsigned int item = s_item;
+        if (item >= n_items) break;
+        const int3 it = p.items[item];
+        const uint32_t i_base = (uint32_t)it.x * kTile;
+        float nx[kR], ny[kR], nz[kR], wi[kR];
+        uint32_t valid_mask = 0;
+#pragma unroll
+        for (int r = 0; r < kR; ++r) {
+            const uint32_t s = i_base + r * kThreads + tid;
+            const float4 v = p.pts_a[s];  // the array is padded to a whole tile
+            nx[r] = -v.x;
+            ny[r] = -v.y;
+            nz[r] = -v.z;
+            wi[r] = v.w;
+            valid_mask |= (s < p.n_a ? 1u : 0u) << r;
+        }
+        const bool i_full = i_base + kTile <= p.n_a;
+        const uint32_t n_i = i_full ? kTile : p.n_a - i_base;
+
+        auto tile_count = [&](int tj) -> uint32_t {
+            const uint32_t j0 = (uint32_t)tj * kTile;
+            return p.n_b - j0 < (uint32_t)kTile ? p.n_b - j0 : (uint32_t)kTile;
+        };
+        if (tid == 0) {
+            const uint32_t bytes = tile_count(it.y) * sizeof(float4);
+            uint64_t *bar = &bars[consumed & 1];
+            mbar_expect_tx(bar, bytes);
+            bulk_load(tiles + (size_t)(consumed & 1) * kTile, p.pts_b + (size_t)it.y * kTile, bytes, bar);
+        }
+        for (int t = 0; t < it.z; ++t) {
+            const int tj = it.y + t;
+            if (tid == 0 && t + 1 < it.z) {  // prefetch the next tile into the other buffer (released by the sync below)
+                const uint32_t bytes = tile_count(tj + 1) * sizeof(float4);
+                uint64_t *bar = &bars[(consumed + 1) & 1];
+                mbar_expect_tx(bar, bytes);
+                bulk_load(tiles + (size_t)((consumed + 1) & 1) * kTile, p.pts_b + (size_t)(tj + 1) * kTile, bytes, bar);
+            }
+            mbar_wait(&bars[consumed & 1], (consumed >> 1) & 1);
+            const float4 *tile = tiles + (size_t)(consumed & 1) * kTile;
+            const int jn = (int)tile_count(tj);
+            const bool diag = p.is_auto && tj == it.x;
+            const uint32_t j_base = (uint32_t)tj * kTile;
+            if (diag || !i_full)
+                process_tile<kWeighted, kPrivate, true>(p, h, tile, jn, nx, ny, nz, wi, lut, i_base, j_base, diag, valid_mask, n_fp64);
+            else
+                process_tile<kWeighted, kPrivate, false>(p, h, tile, jn, nx, ny, nz, wi, lut, i_base, j_base, false, valid_mask, n_fp64);
+            if (tid == 0) n_eval += diag ? (unsigned long long)n_i * (n_i - 1) / 2 : (unsigned long long)n_i * (unsigned)jn;
+            ++consumed;
+            __syncthreads();  // all reads of this buffer are done before it is refilled
+        }
+        if constexpr (!kPrivate) {
+            // the CTA-wide u32 rows could overflow over a CTA's lifetime: flush per item (<= 2^23 pairs)
+            for (int row = 1 + tid; row <= p.nbins; row += kThreads) {
+                const uint32_t v = cnt_all[row];
+                if (v) atomicAdd(&p.counts[row - 1], (unsigned long long)v);
+                cnt_all[row] = 0;
+                if constexpr (kWeighted) {
+                    const double w = ws_all[row];
+                    if (w != 0.0) atomicAdd(&p.wsums[row - 1], w);
+                    ws_all[row] = 0.0;
+                }
+            }
+            __syncthreads();
+        }
+    }
+
+    if constexpr (kPrivate) {
+        // per-lane u32 counters: a thread sees < 2^32 pairs in any call this library accepts per CTA
+        // (n_a, n_b < 2^31 and >= 148 CTAs share the work), so one flush at the end suffices.
+        __syncwarp();
+        for (int row = 1; row <= p.nbins; ++row) {
+            const unsigned long long v = warp_sum_u64((unsigned long long)h.cnt[row * 32 + lane]);
+            if (lane == 0 && v) atomicAdd(&p.counts[row - 1], v);
+            if constexpr (kWeighted) {
+                double w = h.ws[row * 32 + lane];
+#pragma unroll
+                for (int o = 16; o > 0; o >>= 1) w += __shfl_xor_sync(0xffffffffu, w, o);
+                if (lane == 0 && w != 0.0) atomicAdd(&p.wsums[row - 1], w);
+            }
+        }
+    }
+    n_fp64 = warp_sum_u64(n_fp64);
+    if (lane == 0 && n_fp64) atomicAdd(&p.counters[kCtrPairsFp64], n_fp64);
+    if (tid == 0 && n_eval) atomicAdd(&p.counters[kCtrPairsEvaluated], n_eval);
+}
+
+// ---- host: the cell table -------------------------------------------------------------------
+// Cells are the float values sharing the top (9 + m) bits; each gets the single edge (as K - e)
+// that can separate two rows inside it, or a NaN threshold when two or more edges crowd it.
+struct Lut {
+    std::vector<uint2> cells;
+    int m, shift, key0;
+};
+
+float bits_to_float(uint32_t b)
+{
+    float f;
+    memcpy(&f, &b, 4);
+    return f;
+}
+uint32_t float_to_bits(float f)
+{
+    uint32_t b;
+    memcpy(&b, &f, 4);
+    return b;
+}
+
+Lut build_lut(const double *edges, int nbins, int m)
+{
+    Lut L;
+    L.m = m;
+    L.shift = 23 - m;
+    L.key0 = (int)(float_to_bits(std::ldexp(1.0f, kExpLo)) >> L.shift);
+    const int key1 = (int)(float_to_bits(std::ldexp(1.0f, kExpHi)) >> L.shift);
+    L.cells.resize((size_t)(key1 - L.key0));
+    std::vector<double> te(nbins + 1);  // edges in the t domain, ascending
+    for (int k = 0; k <= nbins; ++k) te[k] = (double)kK - edges[k];
+    // The pair cosine is clamped to [-1, 1]: when the range reaches a pole nothing lies beyond it, so
+    // that edge must not be tested in fp32 (an unclamped c32 marginally outside would be misfiled).
+    if (edges[0] >= 1.0) te[0] = -1.0e300;
+    if (edges[nbins] <= -1.0) te[nbins] = 1.0e300;
+    const double G = (double)kGuard;
+    int crowded = 0;
+    for (int key = L.key0; key < key1; ++key) {
+        const double lo = (double)bits_to_float((uint32_t)key << L.shift);
+        const double hi = (double)bits_to_float((uint32_t)(key + 1) << L.shift);
+        int below = 0, inside = 0, first = -1;
+        for (int k = 0; k <= nbins; ++k) {
+            if (te[k] < lo - G) ++below;
+            else if (te[k] <= hi + G) {
+                if (!inside) first = k;
+                ++inside;
+            }
+        }
+        uint2 c;
+        c.y = (uint32_t)below;
+        if (inside == 0) c.x = float_to_bits(3.0e38f);
+        else if (inside == 1) c.x = float_to_bits((float)te[first]);
+        else {
+            c.x = 0x7fc00000u;  // NaN: every pair of the cell is re-checked
+            ++crowded;
+        }
+        L.cells[(size_t)(key - L.key0)] = c;
+    }
+    (void)crowded;
+    return L;
+}
+
+// number of cells that are crowded although they are wider than a few guard bands (i.e. a finer
+// table would resolve them)
+int crowded_resolvable(const Lut &L)
+{
+    int n = 0;
+    for (size_t i = 0; i < L.cells.size(); ++i) {
+        if (L.cells[i].x != 0x7fc00000u) continue;
+        const double lo = (double)bits_to_float((uint32_t)(L.key0 + (int)i) << L.shift);
+        const double hi = (double)bits_to_float((uint32_t)(L.key0 + (int)i + 1) << L.shift);
+        if (hi - lo > 8.0 * (double)kGuard) ++n;
+    }
+    return n;
+}
+
+template <bool kWeighted, bool kPrivate>
+cudaError_t launch(acf_ctx *ctx, const PairParams &p, size_t smem, int grid)
+{
+    auto kern = pair_kernel<kWeighted, kPrivate>;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    kern<<<grid, kThreads, smem, ctx->stream>>>(p);
+    ctx->last.kernel_launches++;
+    return cudaGetLastError();
+}
+
+int count_prepared(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_auto, const double *h_edges, int nbins,
+                   const Lut &L, const uint2 *d_lut, unsigned long long *d_counts, double *d_wsums)
+{
+    if (a.n == 0 || b.n == 0) return ACF_OK;
+    const bool weighted = d_wsums != nullptr;
+    const int rows = nbins + 2;
+    const bool priv = rows <= kMaxPrivateRows;
+    size_t smem = 128 + 2 * kTile * sizeof(float4) + L.cells.size() * sizeof(uint2);
+    smem = (smem + 15) & ~size_t(15);
+    const size_t cnt_words = priv ? (size_t)kWarps * rows * 32 : (size_t)rows;
+    smem += cnt_words * sizeof(uint32_t);
+    smem = (smem + 15) & ~size_t(15);
+    if (weighted) smem += cnt_words * sizeof(double);
+    if (smem > (size_t)ctx->max_smem_optin) return fail(ctx, ACF_EINVAL, "shared memory need %zu exceeds %d", smem, ctx->max_smem_optin);
+
+    // i-tiles are handed out in batches so that the item buffer stays bounded
+    // (worst case one item per surviving j-tile: survivors may alternate with pruned tiles)
+    const uint64_t items_per_ti = (uint64_t)b.n_tiles;
+    const uint64_t max_items = 8u << 20;
+    int ti_per_batch = (int)(max_items / items_per_ti);
+    if (ti_per_batch < 1) ti_per_batch = 1;
+    if (ti_per_batch > a.n_tiles) ti_per_batch = a.n_tiles;
+    const uint32_t capacity = (uint32_t)(items_per_ti * (uint64_t)ti_per_batch);
+    ACF_CUDA_TRY(ctx, ctx->s_work.reserve(sizeof(int3) * (size_t)capacity));
+
+    PairParams p{};
+    p.pts_a = a.pts;
+    p.pts_b = b.pts;
+    p.perm_a = a.perm;
+    p.perm_b = b.perm;
+    p.n_a = (uint32_t)a.n;
+    p.n_b = (uint32_t)b.n;
+    p.xyz_a = a.xyz;
+    p.xyz_b = b.xyz;
+    p.stride_a = a.stride;
+    p.stride_b = b.stride;
+    p.items = ctx->s_work.as<int3>();
+    p.capacity = capacity;
+    p.lut = d_lut;
+    p.lut_len = (int)L.cells.size();
+    p.key0 = L.key0;
+    p.shift = L.shift;
+    p.edges = ctx->s_edges.as<double>();
+    p.nbins = nbins;
+    p.counts = d_counts;
+    p.wsums = d_wsums;
+    p.counters = ctx->d_counters;
+    p.is_auto = is_auto;
+
+    const int ctas_per_sm = weighted ? 1 : (2 * smem <= (size_t)220 * 1024 ? 2 : 1);
+    const int grid = ctx->num_sms * ctas_per_sm;
+    for (int ti0 = 0; ti0 < a.n_tiles; ti0 += ti_per_batch) {
+        const int ti1 = ti0 + ti_per_batch < a.n_tiles ? ti0 + ti_per_batch : a.n_tiles;
+        ACF_CUDA_TRY(ctx, cudaMemsetAsync(&ctx->d_counters[kCtrWorkHead], 0, 2 * sizeof(unsigned long long), ctx->stream));
+        int rc = build_worklist(ctx, a, ti0, ti1, b, is_auto, h_edges[0], h_edges[nbins], ctx->s_work.as<int3>(), capacity);
+        if (rc != ACF_OK) return rc;
+        cudaError_t e;
+        if (weighted) e = priv ? launch<true, true>(ctx, p, smem, grid) : launch<true, false>(ctx, p, smem, grid);
+        else e = priv ? launch<false, true>(ctx, p, smem, grid) : launch<false, false>(ctx, p, smem, grid);
+        ACF_CUDA_TRY(ctx, e);
+    }
     return ACF_OK;
 }
+
+}  // namespace
+
+int run_pair_count_fast(acf_ctx *ctx, const double *d_a, const float *d_wa, size_t n_a, size_t i_begin,
+                        size_t i_end, const double *d_b, const float *d_wb, size_t n_b, const double *h_edges,
+                        int nbins, int is_auto, unsigned long long *d_counts, double *d_wsums)
+{
+    // cell table: the coarsest resolution that leaves no resolvable cell crowded
+    Lut L = build_lut(h_edges, nbins, 6);
+    for (int m = 7; m <= 9 && crowded_resolvable(L) > 0; ++m) L = build_lut(h_edges, nbins, m);
+    const size_t edge_bytes = (sizeof(double) * (size_t)(nbins + 1) + 15) & ~size_t(15);
+    ACF_CUDA_TRY(ctx, ctx->s_edges.reserve(edge_bytes + L.cells.size() * sizeof(uint2)));
+    ACF_CUDA_TRY(ctx, cudaMemcpyAsync(ctx->s_edges.ptr, h_edges, sizeof(double) * (size_t)(nbins + 1), cudaMemcpyHostToDevice, ctx->stream));
+    uint2 *d_lut = reinterpret_cast<uint2 *>(static_cast<char *>(ctx->s_edges.ptr) + edge_bytes);
+    ACF_CUDA_TRY(ctx, cudaMemcpyAsync(d_lut, L.cells.data(), L.cells.size() * sizeof(uint2), cudaMemcpyHostToDevice, ctx->stream));
+
+    Prepared a, b;
+    int rc;
+    if (is_auto) {
+        // rows [i_begin, i_end): pairs inside the row block, plus the block against everything after it
+        rc = prepare_catalogue(ctx, 0, d_a, n_a, i_begin, i_end - i_begin, d_wa, &a);
+        if (rc != ACF_OK) return rc;
+        rc = count_prepared(ctx, a, a, 1, h_edges, nbins, L, d_lut, d_counts, d_wsums);
+        if (rc != ACF_OK) return rc;
+        if (i_end < n_a) {
+            rc = prepare_catalogue(ctx, 1, d_a, n_a, i_end, n_a - i_end, d_wa, &b);
+            if (rc != ACF_OK) return rc;
+            rc = count_prepared(ctx, a, b, 0, h_edges, nbins, L, d_lut, d_counts, d_wsums);
+        }
+        return rc;
+    }
+    rc = prepare_catalogue(ctx, 0, d_a, n_a, i_begin, i_end - i_begin, d_wa, &a);
+    if (rc != ACF_OK) return rc;
+    rc = prepare_catalogue(ctx, 1, d_b, n_b, 0, n_b, d_wb, &b);
+    if (rc != ACF_OK) return rc;
+    return count_prepared(ctx, a, b, 0, h_edges, nbins, L, d_lut, d_counts, d_wsums);
+}
+
 }  // namespace acf

@@ -1,0 +1,354 @@
+// acf_prep.cu -- O(N) preparation of a catalogue for the pair kernel:
+//   1. spatial key of every point (3-D Morton code of the quantised unit vector),
+//   2. LSD radix sort of (key, index) -- own kernels, 4 passes of 8 bits,
+//   3. gather into sorted fp32 float4 {x, y, z, w} + per-tile bounding caps in fp64,
+//   4. the work list: (i-tile, run of j-tiles) items that may hold an in-range pair
+//      (calculations that fall outside the bin range need not be made;
+//       the pair matrix is walked sub-matrix by sub-matrix).
+// Pair counts do not depend on the order of the points, so sorting changes nothing in the
+// result; it makes tiles compact on the sky, which is what lets whole tile pairs be skipped.
+#include "acf_device.cuh"
+#include "acf_internal.h"
+
+namespace acf {
+
+namespace {
+
+// ------------------------------------------------------------------ keys
+__device__ __forceinline__ uint32_t spread10(uint32_t v)
+{
+    // 10 bits -> every third bit
+    v = (v | (v << 16)) & 0x030000FFu;
+    v = (v | (v << 8)) & 0x0300F00Fu;
+    v = (v | (v << 4)) & 0x030C30C3u;
+    v = (v | (v << 2)) & 0x09249249u;
+    return v;
+}
+
+__global__ void key_kernel(const double *__restrict__ xyz, size_t stride, size_t off, uint32_t n,
+                           uint32_t *__restrict__ keys, uint32_t *__restrict__ idx)
+{
+    for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const size_t g = off + i;
+        const float x = (float)xyz[g], y = (float)xyz[stride + g], z = (float)xyz[2 * stride + g];
+        // quantise [-1, 1] to 10 bits per axis (inputs are validated unit vectors; clamp anyway)
+        const uint32_t qx = (uint32_t)fminf(fmaxf((x + 1.0f) * 511.5f, 0.0f), 1023.0f);
+        const uint32_t qy = (uint32_t)fminf(fmaxf((y + 1.0f) * 511.5f, 0.0f), 1023.0f);
+        const uint32_t qz = (uint32_t)fminf(fmaxf((z + 1.0f) * 511.5f, 0.0f), 1023.0f);
+        keys[i] = (spread10(qz) << 2) | (spread10(qy) << 1) | spread10(qx);
+        idx[i] = i;
+    }
+}
+
+// ------------------------------------------------------------------ radix sort (stable, LSD)
+constexpr int kSortThreads = 256;
+constexpr int kSortWarps = kSortThreads / 32;
+constexpr int kSortPerLane = 16;                                  // elements per lane
+constexpr int kSortWarpChunk = 32 * kSortPerLane;                 // contiguous elements per warp
+constexpr int kSortBlockChunk = kSortWarps * kSortWarpChunk;      // 4096 per CTA
+
+// counts[d * nblocks + b] = number of keys of CTA b whose digit is d
+__global__ void __launch_bounds__(kSortThreads)
+radix_count_kernel(const uint32_t *__restrict__ keys, uint32_t n, int shift, uint32_t *__restrict__ counts, uint32_t nblocks)
+{
+    __shared__ uint32_t hist[256];
+    hist[threadIdx.x] = 0;
+    __syncthreads();
+    const uint32_t base = blockIdx.x * kSortBlockChunk;
+    for (int t = threadIdx.x; t < kSortBlockChunk; t += kSortThreads) {
+        const uint32_t i = base + t;
+        if (i < n) atomicAdd(&hist[(keys[i] >> shift) & 255u], 1u);
+    }
+    __syncthreads();
+    counts[threadIdx.x * nblocks + blockIdx.x] = hist[threadIdx.x];
+}
+
+// in-place exclusive scan of `len` counters by one CTA of 1024 threads
+__global__ void __launch_bounds__(1024) scan_kernel(uint32_t *__restrict__ data, uint32_t len)
+{
+    __shared__ uint32_t partial[1024];
+    const uint32_t per = (len + 1023u) / 1024u;
+    const uint32_t lo = threadIdx.x * per, hi = lo + per < len ? lo + per : len;
+    uint32_t sum = 0;
+    for (uint32_t i = lo; i < hi; ++i) sum += data[i];
+    partial[threadIdx.x] = sum;
+    __syncthreads();
+    // Hillis-Steele over the 1024 partial sums
+    for (int o = 1; o < 1024; o <<= 1) {
+        uint32_t v = threadIdx.x >= o ? partial[threadIdx.x - o] : 0u;
+        __syncthreads();
+        partial[threadIdx.x] += v;
+        __syncthreads();
+    }
+    uint32_t run = threadIdx.x ? partial[threadIdx.x - 1] : 0u;
+    for (uint32_t i = lo; i < hi; ++i) {
+        const uint32_t v = data[i];
+        data[i] = run;
+        run += v;
+    }
+}
+
+// Stable scatter.  Each warp owns a contiguous run of the CTA's chunk and walks it 32 keys at a
+// time; __match_any_sync ranks equal digits inside a round by lane order.
+__global__ void __launch_bounds__(kSortThreads)
+radix_scatter_kernel(const uint32_t *__restrict__ keys_in, const uint32_t *__restrict__ idx_in,
+                     uint32_t *__restrict__ keys_out, uint32_t *__restrict__ idx_out, uint32_t n, int shift,
+                     const uint32_t *__restrict__ offsets, uint32_t nblocks)
+{
+    __shared__ uint32_t whist[kSortWarps][256];  // per-warp digit counts, then running output positions
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    for (int t = threadIdx.x; t < kSortWarps * 256; t += kSortThreads) (&whist[0][0])[t] = 0;
+    __syncthreads();
+    const uint32_t wbase = blockIdx.x * kSortBlockChunk + warp * kSortWarpChunk;
+    for (int r = 0; r < kSortPerLane; ++r) {
+        const uint32_t i = wbase + r * 32 + lane;
+        if (i < n) atomicAdd(&whist[warp][(keys_in[i] >> shift) & 255u], 1u);
+    }
+    __syncthreads();
+    {   // digit d = threadIdx.x: global offset of this CTA's digit-d run, then split over warps in order
+        uint32_t run = offsets[threadIdx.x * nblocks + blockIdx.x];
+        for (int w = 0; w < kSortWarps; ++w) {
+            const uint32_t c = whist[w][threadIdx.x];
+            whist[w][threadIdx.x] = run;
+            run += c;
+        }
+    }
+    __syncthreads();
+    const uint32_t lt_mask = (1u << lane) - 1u;
+    for (int r = 0; r < kSortPerLane; ++r) {
+        const uint32_t i = wbase + r * 32 + lane;
+        const bool ok = i < n;
+        const uint32_t key = ok ? keys_in[i] : 0u;
+        const uint32_t digit = ok ? ((key >> shift) & 255u) : (256u + lane);  // invalid lanes match nobody
+        const uint32_t peers = __match_any_sync(0xffffffffu, digit);
+        uint32_t pos = 0;
+        if (ok) pos = whist[warp][digit] + __popc(peers & lt_mask);
+        __syncwarp();
+        if (ok && (peers & lt_mask) == 0) whist[warp][digit] += __popc(peers);  // first peer advances the cursor
+        __syncwarp();
+        if (ok) {
+            keys_out[pos] = key;
+            idx_out[pos] = idx_in[i];
+        }
+    }
+}
+
+// ------------------------------------------------------------------ gather + tile caps
+// One CTA per tile of kTile sorted points: writes the fp32 float4 records and the tile's bounding
+// cap {unit centre, cos(radius)} computed in fp64 from the fp64 vectors.
+__global__ void __launch_bounds__(256)
+gather_caps_kernel(const double *__restrict__ xyz, size_t stride, size_t off, const float *__restrict__ w,
+                   const uint32_t *__restrict__ idx, uint32_t n, float4 *__restrict__ pts,
+                   uint32_t *__restrict__ perm, double4 *__restrict__ caps)
+{
+    __shared__ double red[3][8];
+    __shared__ double centre[3];
+    constexpr int kPer = kTile / 256;
+    const uint32_t base = blockIdx.x * kTile;
+    double px[kPer], py[kPer], pz[kPer];
+    double sx = 0, sy = 0, sz = 0;
+#pragma unroll
+    for (int r = 0; r < kPer; ++r) {
+        const uint32_t s = base + r * 256 + threadIdx.x;
+        if (s < n) {
+            const uint32_t local = idx[s];
+            const size_t g = off + local;
+            px[r] = xyz[g];
+            py[r] = xyz[stride + g];
+            pz[r] = xyz[2 * stride + g];
+            const float wi = w ? w[g] : 1.0f;
+            pts[s] = make_float4((float)px[r], (float)py[r], (float)pz[r], wi);
+            perm[s] = (uint32_t)g;  // index into the caller's catalogue
+            sx += px[r];
+            sy += py[r];
+            sz += pz[r];
+        } else {
+            px[r] = py[r] = pz[r] = 0.0;
+            pts[s] = make_float4(0.f, 0.f, 0.f, 0.f);  // padding up to the tile boundary, never paired
+        }
+    }
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        sx += __shfl_xor_sync(0xffffffffu, sx, o);
+        sy += __shfl_xor_sync(0xffffffffu, sy, o);
+        sz += __shfl_xor_sync(0xffffffffu, sz, o);
+    }
+    if (lane == 0) {
+        red[0][warp] = sx;
+        red[1][warp] = sy;
+        red[2][warp] = sz;
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double cx = 0, cy = 0, cz = 0;
+        for (int k = 0; k < 8; ++k) {
+            cx += red[0][k];
+            cy += red[1][k];
+            cz += red[2][k];
+        }
+        const double nrm = sqrt(cx * cx + cy * cy + cz * cz);
+        if (nrm > 1e-9) {
+            centre[0] = cx / nrm;
+            centre[1] = cy / nrm;
+            centre[2] = cz / nrm;
+        } else {  // points spread over the whole sphere: any centre, the radius will say pi
+            centre[0] = 0.0;
+            centre[1] = 0.0;
+            centre[2] = 1.0;
+        }
+    }
+    __syncthreads();
+    const double cx = centre[0], cy = centre[1], cz = centre[2];
+    double mind = 2.0;
+#pragma unroll
+    for (int r = 0; r < kPer; ++r) {
+        const uint32_t s = base + r * 256 + threadIdx.x;
+        if (s < n) mind = fmin(mind, cx * px[r] + cy * py[r] + cz * pz[r]);
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) mind = fmin(mind, __shfl_xor_sync(0xffffffffu, mind, o));
+    __syncthreads();
+    if (lane == 0) red[0][warp] = mind;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        for (int k = 1; k < 8; ++k) mind = fmin(mind, red[0][k]);
+        // cos of the bounding radius, pushed outwards by far more than the rounding of the dots
+        caps[blockIdx.x] = make_double4(cx, cy, cz, fmax(-1.0, fmin(1.0, mind) - 1e-9));
+    }
+}
+
+// ------------------------------------------------------------------ work list
+// Angular bounds of all pairs between two caps, as cosines: every pair has
+// cos_lo <= c <= cos_hi.  Radii are padded by 1e-7 rad.
+__device__ __forceinline__ void cap_pair_bounds(const double4 a, const double4 b, double &cos_lo, double &cos_hi)
+{
+    const double d = fmin(1.0, fmax(-1.0, a.x * b.x + a.y * b.y + a.z * b.z));
+    const double th = acos(d), ra = acos(a.w), rb = acos(b.w);
+    const double pad = 1e-7;
+    const double tmin = th - ra - rb - pad, tmax = th + ra + rb + pad;
+    cos_hi = tmin <= 0.0 ? 1.0 : cos(tmin);
+    cos_lo = tmax >= 3.141592653589793 ? -1.0 : cos(tmax);
+}
+
+// One CTA per i-tile.  Tests every candidate j-tile cap, then one thread walks the survivor bitmap
+// and appends items {ti, first j-tile, number of j-tiles <= kItemTiles}.
+__global__ void __launch_bounds__(256)
+worklist_kernel(const double4 *__restrict__ caps_a, int ti_begin, int ti_end, const double4 *__restrict__ caps_b,
+                int n_tiles_b, int is_auto, int prune, double e_first, double e_last,
+                int3 *__restrict__ items, uint32_t capacity, unsigned long long *__restrict__ counters)
+{
+    extern __shared__ uint32_t keep[];  // bitmap over j tiles
+    const int ti = ti_begin + blockIdx.x;
+    if (ti >= ti_end) return;
+    const int words = (n_tiles_b + 31) / 32;
+    const int tj_first = is_auto ? ti : 0;
+    const double4 ca = caps_a[ti];
+    uint32_t pruned = 0;
+    for (int wbase = 0; wbase < words; wbase += blockDim.x / 32) {
+        const int word = wbase + (threadIdx.x >> 5);
+        const int tj = word * 32 + (threadIdx.x & 31);
+        bool k = false;
+        if (word < words && tj < n_tiles_b && tj >= tj_first) {
+            k = true;
+            if (prune) {
+                double lo, hi;
+                cap_pair_bounds(ca, caps_b[tj], lo, hi);
+                // no pair can be in range: all beyond theta_max, or all closer than theta_min
+                if (hi < e_last - 1e-12 || lo > e_first + 1e-12) k = false;
+            }
+            pruned += k ? 0u : 1u;
+        }
+        const uint32_t bits = __ballot_sync(0xffffffffu, k);
+        if ((threadIdx.x & 31) == 0 && word < words) keep[word] = bits;
+    }
+    pruned = __reduce_add_sync(0xffffffffu, pruned);
+    if ((threadIdx.x & 31) == 0) {
+        if (pruned) atomicAdd(&counters[kCtrTilePairsPruned], (unsigned long long)pruned);
+    }
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        atomicAdd(&counters[kCtrTilePairsTotal], (unsigned long long)(n_tiles_b - tj_first));
+        int tj = tj_first;
+        while (tj < n_tiles_b) {
+            // skip to the next surviving tile
+            uint32_t wv = keep[tj >> 5] >> (tj & 31);
+            if (wv == 0) {
+                tj = ((tj >> 5) + 1) << 5;
+                continue;
+            }
+            tj += __ffs(wv) - 1;
+            if (tj >= n_tiles_b) break;
+            int len = 1;
+            // the diagonal tile of an auto count is always an item of its own (it runs the i<j variant)
+            const bool diag = is_auto && tj == ti;
+            while (!diag && len < kItemTiles && tj + len < n_tiles_b && ((keep[(tj + len) >> 5] >> ((tj + len) & 31)) & 1u)) ++len;
+            const unsigned long long slot = atomicAdd(&counters[kCtrWorkCount], 1ull);
+            if (slot < capacity) items[slot] = make_int3(ti, tj, len);
+            tj += len;
+        }
+    }
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------ host side
+int prepare_catalogue(acf_ctx *ctx, int slot, const double *xyz, size_t stride, size_t off, size_t cnt,
+                      const float *w, Prepared *out)
+{
+    cudaStream_t st = ctx->stream;
+    const uint32_t n = (uint32_t)cnt;
+    const int n_tiles = (int)((cnt + kTile - 1) / kTile);
+    out->xyz = xyz;
+    out->w = w;
+    out->stride = stride;
+    out->n = cnt;
+    out->n_tiles = n_tiles;
+    if (cnt == 0) return ACF_OK;
+    const size_t padded = (size_t)n_tiles * kTile;
+    ACF_CUDA_TRY(ctx, ctx->s_pts[slot].reserve(sizeof(float4) * padded));
+    ACF_CUDA_TRY(ctx, ctx->s_perm[slot].reserve(sizeof(uint32_t) * padded));
+    ACF_CUDA_TRY(ctx, ctx->s_caps[slot].reserve(sizeof(double4) * (size_t)n_tiles));
+    ACF_CUDA_TRY(ctx, ctx->s_keys[slot].reserve(sizeof(uint32_t) * 4 * (size_t)n));  // keys x2, idx x2
+    const uint32_t nblocks = (n + kSortBlockChunk - 1) / kSortBlockChunk;
+    ACF_CUDA_TRY(ctx, ctx->s_misc.reserve(sizeof(uint32_t) * 256 * (size_t)nblocks));
+    out->pts = ctx->s_pts[slot].as<float4>();
+    out->perm = ctx->s_perm[slot].as<uint32_t>();
+    out->caps = ctx->s_caps[slot].as<double4>();
+    uint32_t *k0 = ctx->s_keys[slot].as<uint32_t>(), *k1 = k0 + n, *i0 = k1 + n, *i1 = i0 + n;
+    uint32_t *counts = ctx->s_misc.as<uint32_t>();
+
+    int blocks = (int)((n + 255) / 256);
+    if (blocks > ctx->num_sms * 16) blocks = ctx->num_sms * 16;
+    key_kernel<<<blocks, 256, 0, st>>>(xyz, stride, off, n, k0, i0);
+    ctx->last.kernel_launches++;
+    for (int pass = 0; pass < 4; ++pass) {
+        const int shift = 8 * pass;
+        radix_count_kernel<<<nblocks, kSortThreads, 0, st>>>(k0, n, shift, counts, nblocks);
+        scan_kernel<<<1, 1024, 0, st>>>(counts, 256u * nblocks);
+        radix_scatter_kernel<<<nblocks, kSortThreads, 0, st>>>(k0, i0, k1, i1, n, shift, counts, nblocks);
+        ctx->last.kernel_launches += 3;
+        uint32_t *t = k0; k0 = k1; k1 = t;
+        t = i0; i0 = i1; i1 = t;
+    }
+    gather_caps_kernel<<<n_tiles, 256, 0, st>>>(xyz, stride, off, w, i0, n, out->pts, out->perm, out->caps);
+    ctx->last.kernel_launches++;
+    ACF_CUDA_TRY(ctx, cudaGetLastError());
+    return ACF_OK;
+}
+
+int build_worklist(acf_ctx *ctx, const Prepared &a, int ti_begin, int ti_end, const Prepared &b, int is_auto,
+                   double e_first, double e_last, int3 *items, uint32_t capacity)
+{
+    const int n_ti = ti_end - ti_begin;
+    if (n_ti <= 0 || b.n_tiles == 0) return ACF_OK;
+    const size_t smem = sizeof(uint32_t) * (size_t)((b.n_tiles + 31) / 32);
+    if (smem > 48 * 1024) return fail(ctx, ACF_EINVAL, "catalogue too large for the work-list kernel (%d tiles)", b.n_tiles);
+    worklist_kernel<<<n_ti, 256, smem, ctx->stream>>>(a.caps, ti_begin, ti_end, b.caps, b.n_tiles, is_auto, ctx->opt_prune,
+                                                     e_first, e_last, items, capacity, ctx->d_counters);
+    ctx->last.kernel_launches++;
+    ACF_CUDA_TRY(ctx, cudaGetLastError());
+    return ACF_OK;
+}
+
+}  // namespace acf

@@ -189,8 +189,8 @@ def test_degenerate_sizes(acf, ctx):
     two = soa([(0.0, 0.0, 1.0), (0.0, 1.0, 0.0)])
     empty = np.zeros(0)
     assert gpu_counts(acf, ctx, one, None, edges, True).tolist() == [0, 0]          # n = 1, auto
-    assert gpu_counts(acf, ctx, two, None, edges, True).tolist() == [1, 0]          # c = 0 -> bin 0 (closed above)
-    assert gpu_counts(acf, ctx, one, two, edges, False).tolist() == [2, 0]
+    assert gpu_counts(acf, ctx, two, None, edges, True).tolist() == [0, 1]          # c = 0 = e_1 -> bin 1 (c <= e_1)
+    assert gpu_counts(acf, ctx, one, two, edges, False).tolist() == [1, 1]          # c = 1 -> bin 0, c = 0 -> bin 1
     out = acf.acf_pair_count(ctx, torch.zeros(0, dtype=torch.float64, device="cuda"), None, edges, True)
     torch.cuda.synchronize()
     assert out.cpu().tolist() == [0, 0]
