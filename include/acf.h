@@ -79,6 +79,7 @@ typedef struct acf_stats {
     uint64_t tile_pairs_pruned;  /* tile pairs skipped as provably out of range */
     uint64_t kernel_launches;    /* CUDA kernels launched by the call */
     double device_ms;            /* device time of the call, CUDA events on the ctx stream */
+    double pair_kernel_ms;       /* of which: first to last pair-kernel launch (the dominant kernel) */
 } acf_stats;
 
 /* Create a context on CUDA device `device`.  cuda_stream: a cudaStream_t (as void*) all

@@ -37,7 +37,7 @@ class acf_stats(ctypes.Structure):
     _fields_ = [
         ("pairs_nominal", ctypes.c_uint64), ("pairs_evaluated", ctypes.c_uint64), ("pairs_fp64", ctypes.c_uint64),
         ("tile_pairs_total", ctypes.c_uint64), ("tile_pairs_pruned", ctypes.c_uint64),
-        ("kernel_launches", ctypes.c_uint64), ("device_ms", ctypes.c_double),
+        ("kernel_launches", ctypes.c_uint64), ("device_ms", ctypes.c_double), ("pair_kernel_ms", ctypes.c_double),
     ]
 
     def as_dict(self):

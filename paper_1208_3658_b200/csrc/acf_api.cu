@@ -59,6 +59,7 @@ extern "C" int acf_create(acf_ctx **out, int device, void *cuda_stream)
     ctx->max_smem_optin = (int)prop.sharedMemPerBlockOptin;
     bool ok = cudaEventCreate(&ctx->ev_start) == cudaSuccess && cudaEventCreate(&ctx->ev_stop) == cudaSuccess &&
               cudaEventCreateWithFlags(&ctx->ev_flag, cudaEventDisableTiming) == cudaSuccess &&
+              cudaEventCreate(&ctx->ev_k0) == cudaSuccess && cudaEventCreate(&ctx->ev_k1) == cudaSuccess &&
               cudaMalloc(&ctx->d_counters, sizeof(unsigned long long) * acf::kNumCounters) == cudaSuccess &&
               cudaHostAlloc(&ctx->h_counters, sizeof(unsigned long long) * acf::kNumCounters, cudaHostAllocDefault) == cudaSuccess;
     if (!ok) {
@@ -93,6 +94,8 @@ extern "C" void acf_destroy(acf_ctx *ctx)
     if (ctx->ev_start) cudaEventDestroy(ctx->ev_start);
     if (ctx->ev_stop) cudaEventDestroy(ctx->ev_stop);
     if (ctx->ev_flag) cudaEventDestroy(ctx->ev_flag);
+    if (ctx->ev_k0) cudaEventDestroy(ctx->ev_k0);
+    if (ctx->ev_k1) cudaEventDestroy(ctx->ev_k1);
     delete ctx;
 }
 
@@ -148,6 +151,7 @@ extern "C" int acf_pair_count_rows(acf_ctx *ctx, const double *d_a, const float 
     ACF_CUDA_TRY(ctx, cudaSetDevice(ctx->device));
     cudaStream_t st = ctx->stream;
     ctx->last = acf_stats{};
+    ctx->pair_timed = false;
     {
         // pairs the call is defined over
         // auto: T(n - i_begin) - T(n - i_end) with T(m) = m(m-1)/2 pairs among the last m points
@@ -224,6 +228,7 @@ extern "C" int acf_get_stats(acf_ctx *ctx, acf_stats *out)
         ACF_CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
         float ms = 0.f;
         if (cudaEventElapsedTime(&ms, ctx->ev_start, ctx->ev_stop) == cudaSuccess) ctx->last.device_ms = ms;
+        if (ctx->pair_timed && cudaEventElapsedTime(&ms, ctx->ev_k0, ctx->ev_k1) == cudaSuccess) ctx->last.pair_kernel_ms = ms;
         ctx->last.pairs_evaluated = ctx->h_counters[acf::kCtrPairsEvaluated];
         ctx->last.pairs_fp64 = ctx->h_counters[acf::kCtrPairsFp64];
         ctx->last.tile_pairs_total = ctx->h_counters[acf::kCtrTilePairsTotal];

@@ -82,6 +82,8 @@ struct acf_ctx {
     int opt_stats = 1;
 
     cudaEvent_t ev_start = nullptr, ev_stop = nullptr, ev_flag = nullptr;
+    cudaEvent_t ev_k0 = nullptr, ev_k1 = nullptr;  // around the pair kernel(s) of the last call
+    bool pair_timed = false;
     unsigned long long *d_counters = nullptr;  // acf::kNumCounters
     unsigned long long *h_counters = nullptr;  // pinned mirror
     acf_stats last{};

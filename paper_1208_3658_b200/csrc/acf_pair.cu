@@ -453,9 +453,14 @@ int count_prepared(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_au
         int rc = build_worklist(ctx, a, ti0, ti1, b, is_auto, h_edges[0], h_edges[nbins], ctx->s_work.as<int3>(), capacity);
         if (rc != ACF_OK) return rc;
         cudaError_t e;
+        if (!ctx->pair_timed) {
+            ACF_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_k0, ctx->stream));
+            ctx->pair_timed = true;
+        }
         if (weighted) e = priv ? launch<true, true>(ctx, p, smem, grid) : launch<true, false>(ctx, p, smem, grid);
         else e = priv ? launch<false, true>(ctx, p, smem, grid) : launch<false, false>(ctx, p, smem, grid);
         ACF_CUDA_TRY(ctx, e);
+        ACF_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_k1, ctx->stream));
     }
     return ACF_OK;
 }

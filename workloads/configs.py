@@ -79,11 +79,12 @@ class Workload:
         return self.n_d * (self.n_d - 1) // 2 + self.n_d * self.n_r + self.n_r * (self.n_r - 1) // 2
 
 
-def make_config(name: str, scale: float = 1.0) -> Workload:
+def make_config(name: str, scale: float = 1.0, seed_offset: int = 0) -> Workload:
+    """seed_offset shifts every seed: another realisation of the same configuration."""
     spec = CONFIGS[name]
     n_d = max(2, int(round(spec["n_d"] * scale)))
     n_r = max(2, int(round(spec["n_r"] * scale)))
-    sd, sr = spec["seeds"]
+    sd, sr = (s + seed_offset for s in spec["seeds"])
     cl = spec["cluster"]
     if cl is None:
         ra_d, dec_d = uniform_patch(n_d, spec["ra"], spec["dec"], sd)
@@ -97,8 +98,8 @@ def make_config(name: str, scale: float = 1.0) -> Workload:
     ra_r, dec_r = uniform_patch(n_r, spec["ra"], spec["dec"], sr)
     w_d = w_r = None
     if spec["weights"] is not None:
-        w_d = lognormal_weights(n_d, spec["weights"][0])
-        w_r = lognormal_weights(n_r, spec["weights"][1])
+        w_d = lognormal_weights(n_d, spec["weights"][0] + seed_offset)
+        w_r = lognormal_weights(n_r, spec["weights"][1] + seed_offset)
     tmin, tmax, nb = spec["bins"]
     theta = log_theta_edges_deg(tmin, tmax, nb)
     return Workload(name=name, scale=scale, ra_d=ra_d, dec_d=dec_d, ra_r=ra_r, dec_r=dec_r,
