@@ -66,7 +66,12 @@ enum {
      * 0: every tile pair is evaluated. */
     ACF_OPT_PRUNE = 2,
     /* 1: collect acf_stats device counters (pairs evaluated, fp64 re-checks); default 1. */
-    ACF_OPT_STATS = 3
+    ACF_OPT_STATS = 3,
+    /* 1 (default): where the bounding caps of a warp's i-points and of a group of j-points show that
+     * at most one bin edge can separate their pairs, every pair is tested against that one edge and
+     * tallied in registers; 0: every pair goes through the bin table and the shared-memory histogram.
+     * The counts are the same either way. */
+    ACF_OPT_WINDOWS = 4
 };
 enum { ACF_KERNEL_AUTO = 0, ACF_KERNEL_FP64 = 1 };
 
@@ -75,6 +80,7 @@ typedef struct acf_stats {
     uint64_t pairs_nominal;      /* n(n-1)/2 or n_a*n_b (of the requested row range) */
     uint64_t pairs_evaluated;    /* pair cosines actually computed on the device */
     uint64_t pairs_fp64;         /* pairs re-evaluated in double (inside a guard band of an edge) */
+    uint64_t pairs_window;       /* of pairs_evaluated: classified against a single edge (ACF_OPT_WINDOWS) */
     uint64_t tile_pairs_total;   /* tile pairs the call is made of */
     uint64_t tile_pairs_pruned;  /* tile pairs skipped as provably out of range */
     uint64_t kernel_launches;    /* CUDA kernels launched by the call */

@@ -13,7 +13,7 @@ import os
 import numpy as np
 
 ACF_OK, ACF_EINVAL, ACF_ENOMEM, ACF_ECUDA = 0, -1, -2, -3
-ACF_OPT_KERNEL, ACF_OPT_PRUNE, ACF_OPT_STATS = 1, 2, 3
+ACF_OPT_KERNEL, ACF_OPT_PRUNE, ACF_OPT_STATS, ACF_OPT_WINDOWS = 1, 2, 3, 4
 ACF_KERNEL_AUTO, ACF_KERNEL_FP64 = 0, 1
 ACF_MAX_BINS = 1024
 
@@ -36,6 +36,7 @@ class AcfError(RuntimeError):
 class acf_stats(ctypes.Structure):
     _fields_ = [
         ("pairs_nominal", ctypes.c_uint64), ("pairs_evaluated", ctypes.c_uint64), ("pairs_fp64", ctypes.c_uint64),
+        ("pairs_window", ctypes.c_uint64),
         ("tile_pairs_total", ctypes.c_uint64), ("tile_pairs_pruned", ctypes.c_uint64),
         ("kernel_launches", ctypes.c_uint64), ("device_ms", ctypes.c_double), ("pair_kernel_ms", ctypes.c_double),
     ]

@@ -84,6 +84,7 @@ extern "C" void acf_destroy(acf_ctx *ctx)
         ctx->s_perm[i].release();
         ctx->s_keys[i].release();
         ctx->s_caps[i].release();
+        ctx->s_gcaps[i].release();
     }
     ctx->s_work.release();
     ctx->s_misc.release();
@@ -114,6 +115,9 @@ extern "C" int acf_set_option(acf_ctx *ctx, int option, int64_t value)
         return ACF_OK;
     case ACF_OPT_STATS:
         ctx->opt_stats = value != 0;
+        return ACF_OK;
+    case ACF_OPT_WINDOWS:
+        ctx->opt_windows = value != 0;
         return ACF_OK;
     default:
         return acf::fail(ctx, ACF_EINVAL, "unknown option %d", option);
@@ -231,6 +235,7 @@ extern "C" int acf_get_stats(acf_ctx *ctx, acf_stats *out)
         if (ctx->pair_timed && cudaEventElapsedTime(&ms, ctx->ev_k0, ctx->ev_k1) == cudaSuccess) ctx->last.pair_kernel_ms = ms;
         ctx->last.pairs_evaluated = ctx->h_counters[acf::kCtrPairsEvaluated];
         ctx->last.pairs_fp64 = ctx->h_counters[acf::kCtrPairsFp64];
+        ctx->last.pairs_window = ctx->h_counters[acf::kCtrPairsWindow];
         ctx->last.tile_pairs_total = ctx->h_counters[acf::kCtrTilePairsTotal];
         ctx->last.tile_pairs_pruned = ctx->h_counters[acf::kCtrTilePairsPruned];
         ctx->stats_pending = false;

@@ -50,11 +50,21 @@ enum Counter : int {
     kCtrBadInput = 4,   // number of points that failed validation
     kCtrWorkHead = 5,   // persistent-kernel work counter
     kCtrWorkCount = 6,  // number of work items produced on the device
+    kCtrPairsWindow = 7,  // pairs classified by the single-edge window path
     kNumCounters = 8
 };
 
 constexpr int kTile = 1024;      // points per tile (both the register-resident i side and the staged j side)
 constexpr int kItemTiles = 8;    // at most this many consecutive j-tiles per work item
+constexpr int kGroup = 128;      // points per group: a warp's i-points, and the j-points of one window
+constexpr int kGroupsPerTile = kTile / kGroup;
+
+// Bounding cap of one group of kGroup consecutive sorted points, in double: every point p of the
+// group has centre . p >= cos_r.  sin_r = sqrt(1 - cos_r^2); wsum = sum of the group's weights.
+// A group without points has cos_r = 2.
+struct GroupCap {
+    double cx, cy, cz, cos_r, sin_r, wsum;
+};
 
 // One catalogue prepared for the fast path (all device pointers live in ctx scratch).
 struct Prepared {
@@ -65,6 +75,7 @@ struct Prepared {
     float4 *pts = nullptr;        // spatially sorted fp32 {x, y, z, w}; padded to a tile multiple
     uint32_t *perm = nullptr;     // sorted position -> original index
     double4 *caps = nullptr;      // per tile: unit centre (x, y, z) and cos of the bounding radius
+    GroupCap *gcaps = nullptr;    // per group of kGroup points (kGroupsPerTile per tile)
     int n_tiles = 0;
 };
 
@@ -80,6 +91,7 @@ struct acf_ctx {
     int opt_kernel = ACF_KERNEL_AUTO;
     int opt_prune = 1;
     int opt_stats = 1;
+    int opt_windows = 1;
 
     cudaEvent_t ev_start = nullptr, ev_stop = nullptr, ev_flag = nullptr;
     cudaEvent_t ev_k0 = nullptr, ev_k1 = nullptr;  // around the pair kernel(s) of the last call
@@ -95,6 +107,7 @@ struct acf_ctx {
     acf::Scratch s_perm[2];          // permutations
     acf::Scratch s_keys[2];          // sort keys (double-buffered inside)
     acf::Scratch s_caps[2];          // tile caps
+    acf::Scratch s_gcaps[2];         // group caps
     acf::Scratch s_work;             // work list
     acf::Scratch s_misc;             // radix-sort histograms etc.
     acf::Scratch s_host_stage[6];    // acf_correlate_host: device copies of xyz / weights / outputs

@@ -12,6 +12,16 @@
 // chain on the caller's doubles, clamp, exact edge search) and the histogram is corrected, so
 // the counts equal the fp64 definition whatever the fp32 arithmetic did.
 //
+// Window path.  Points are sorted along a space-filling curve, so the kGroup i-points of a warp and a
+// group of kGroup staged j-points each sit in a small cap, and all their pair cosines lie in a window
+// [c_lo, c_hi] known from the two caps.  When that window holds at most one bin edge e_m, every pair
+// is classified against that single edge, held in a uniform register:
+//   d32 = e_m - (x_i x_j + y_i y_j + z_i z_j)  three fp32 FMAs seeded with fp32(e_m)
+//   above = d32 > 0                             row m + above
+//   certified iff |d32| > G1                    else the exact fp64 row replaces it, as above
+// and the tallies (count of `above`, sum of w_j over `above` per i-point) stay in registers until the
+// group is done.  Windows with two or more edges, ragged groups and diagonal tiles take the table path.
+//
 // Histograms are privatised per lane in shared memory (row-major [row][lane]: a lane owns a bank,
 // so updates never conflict and need no ordering -- PAPER.md:86 reports 5-50 % loss to atomic
 // serialisation), summed per warp with shuffles and flushed with global u64 / f64 atomics.
@@ -39,10 +49,17 @@ constexpr float kGuard = kDelta + 0x1p-23f;
 constexpr int kExpLo = -19;  // t32 >= K - (1 + 1e-6) - kDelta > 2^-19
 constexpr int kExpHi = 2;    // t32 < 4
 constexpr int kMaxPrivateRows = 64;
+// Window path: |d32 - (e_m - c64)| <= 2^-25 [fp32(e_m)] + 2u(1+1e-6) [input rounding] + 3 * 2^-24
+// [three roundings of values of magnitude <= 2] = 3.3e-7.
+constexpr float kGuardWin = 4.5e-7f;
+constexpr int kWinUnroll = 4;  // j-points per guard-band vote
+static_assert(kGroup == kR * 32, "a warp's i-points are one group");
+static_assert(kGroup % kWinUnroll == 0, "");
 
 struct PairParams {
     const float4 *pts_a, *pts_b;
     const uint32_t *perm_a, *perm_b;
+    const GroupCap *gcaps_a, *gcaps_b;
     uint32_t n_a, n_b;
     const double *xyz_a, *xyz_b;
     size_t stride_a, stride_b;
@@ -56,6 +73,7 @@ struct PairParams {
     double *wsums;
     unsigned long long *counters;
     int is_auto;
+    int use_windows;
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -115,6 +133,11 @@ struct Hist {
         if constexpr (kPrivate) ws[row * 32 + lane] += w;  // the lane owns the word: plain read-modify-write
         else atomicAdd(&ws[row], w);
     }
+    __device__ __forceinline__ void add_n(uint32_t row, uint32_t n)
+    {
+        if constexpr (kPrivate) cnt[row * 32 + lane] += n;
+        else atomicAdd(&cnt[row], n);
+    }
     __device__ __forceinline__ void move(uint32_t from, uint32_t to)
     {
         if constexpr (kPrivate) {
@@ -130,16 +153,19 @@ struct Hist {
 // One j-tile against the kR register-resident i-points of every thread.
 // kMasked: pairs are individually enabled (ragged last i-tile, or the diagonal tile of an auto count
 // where only j > i is counted).
+// Thread (warp, lane) holds the i-points warp * kGroup + r * 32 + lane of the i-tile, r < kR.
+__device__ __forceinline__ uint32_t local_i(int r) { return (threadIdx.x >> 5) * kGroup + r * 32 + (threadIdx.x & 31); }
+
+// Table path: j-points [jj0, jj0 + jn) of the staged tile against the kR register-resident i-points.
 template <bool kWeighted, bool kPrivate, bool kMasked>
 __device__ __forceinline__ void process_tile(const PairParams &p, Hist<kWeighted, kPrivate> &h, const float4 *__restrict__ tile,
-                                             int jn, const float (&nx)[kR], const float (&ny)[kR], const float (&nz)[kR],
+                                             int jj0, int jn, const float (&nx)[kR], const float (&ny)[kR], const float (&nz)[kR],
                                              const float (&wi)[kR], const uint2 *__restrict__ lut, uint32_t i_base,
                                              uint32_t j_base, bool diag, uint32_t valid_mask, unsigned long long &n_fp64)
 {
     const int shift = p.shift, key0 = p.key0;
-    const uint32_t tid = threadIdx.x;
 #pragma unroll 2
-    for (int jj = 0; jj < jn; ++jj) {
+    for (int jj = jj0; jj < jj0 + jn; ++jj) {
         const float4 q = tile[jj];
         bool amb_any = false;
         bool amb[kR];
@@ -152,7 +178,7 @@ __device__ __forceinline__ void process_tile(const PairParams &p, Hist<kWeighted
             row[r] = e.y + (t > thr ? 1u : 0u);
             amb[r] = !(fabsf(t - thr) > kGuard);  // also true for the NaN threshold of a crowded cell
             if constexpr (kMasked) {
-                const bool on = ((valid_mask >> r) & 1u) && (!diag || (uint32_t)jj > (uint32_t)(r * kThreads) + tid);
+                const bool on = ((valid_mask >> r) & 1u) && (!diag || (uint32_t)jj > local_i(r));
                 amb[r] = amb[r] && on;
                 if (on) h.add(row[r]);
                 if constexpr (kWeighted)
@@ -168,7 +194,7 @@ __device__ __forceinline__ void process_tile(const PairParams &p, Hist<kWeighted
 #pragma unroll
             for (int r = 0; r < kR; ++r) {
                 if (amb[r]) {
-                    const int exact = exact_row(p.xyz_a, p.stride_a, p.perm_a[i_base + r * kThreads + tid], p.xyz_b,
+                    const int exact = exact_row(p.xyz_a, p.stride_a, p.perm_a[i_base + local_i(r)], p.xyz_b,
                                                 p.stride_b, p.perm_b[j_base + jj], p.edges, p.nbins);
                     if ((uint32_t)exact != row[r]) h.move(row[r], (uint32_t)exact);
                     if constexpr (kWeighted) h.add_w((uint32_t)exact, (double)wi[r] * (double)q.w);
@@ -176,6 +202,123 @@ __device__ __forceinline__ void process_tile(const PairParams &p, Hist<kWeighted
                 }
             }
         }
+    }
+}
+
+// ---- window path --------------------------------------------------------------------------------
+// Histogram row of a cosine (the definition of include/acf.h): 0 if c > e[0]; nbins + 1 if c < e[nbins];
+// else 1 + its bin.  Equals #{m <= nbins - 1 : c <= e[m]} + [c < e[nbins]], non-increasing in c.
+__device__ __forceinline__ int row_of_cos(double c, const double *__restrict__ e, int nbins)
+{
+    int lo = 0, hi = nbins;  // c <= e[m] for m < lo; c > e[m] for m >= hi
+    while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        if (c <= e[mid]) lo = mid + 1; else hi = mid;
+    }
+    return lo + ((lo == nbins && c < e[nbins]) ? 1 : 0);
+}
+
+struct Window {
+    int edge;    // m: the one edge pairs of this window are tested against, or -1: take the table path
+    float e32;   // fp32(e[m])
+    double wsum; // sum of the j-group's weights
+};
+
+// All pairs between points of cap a and cap b have c_lo <= cos(theta) <= c_hi; the window is usable
+// when rows(c_lo) - rows(c_hi) <= 1.  theta = angle between the centres, rho = sum of the radii:
+// cos(theta -+ rho) = cos(theta) cos(rho) +- sin(theta) sin(rho), clamped at the poles.
+__device__ __forceinline__ Window make_window(const GroupCap &a, const GroupCap &b, const double *__restrict__ edges, int nbins)
+{
+    Window w;
+    w.edge = -1;
+    w.e32 = 0.f;
+    w.wsum = b.wsum;
+    if (a.cos_r > 1.5 || b.cos_r > 1.5) return w;  // an empty group
+    if (a.cos_r + b.cos_r <= 0.0) return w;         // radii sum to pi or more: no bound
+    const double d = fmin(1.0, fmax(-1.0, a.cx * b.cx + a.cy * b.cy + a.cz * b.cz));
+    const double C = a.cos_r * b.cos_r - a.sin_r * b.sin_r;  // cos(rho)
+    const double S = a.sin_r * b.cos_r + a.cos_r * b.sin_r;  // sin(rho) >= 0
+    const double sd = sqrt(fmax(0.0, 1.0 - d * d));
+    double c_hi = d >= C ? 1.0 : d * C + sd * S;
+    double c_lo = d <= -C ? -1.0 : d * C - sd * S;
+    c_hi = fmin(1.0, c_hi + 1e-9);  // rounding of the few operations above is ~1e-15
+    c_lo = fmax(-1.0, c_lo - 1e-9);
+    const int r_lo = row_of_cos(c_hi, edges, nbins), r_hi = row_of_cos(c_lo, edges, nbins);
+    if (r_hi - r_lo > 1) return w;
+    w.edge = r_lo <= nbins ? r_lo : nbins;  // rows edge (c > e[edge]) and edge + 1
+    w.e32 = (float)edges[w.edge];
+    return w;
+}
+
+// One group of kGroup staged j-points against this thread's kR i-points, every pair tested against
+// the single edge of the window.  Tallies stay in registers and are added to the histogram rows
+// `edge` and `edge + 1` at the end.
+template <bool kWeighted, bool kPrivate>
+__device__ __forceinline__ void window_group(const PairParams &p, Hist<kWeighted, kPrivate> &h, const float4 *__restrict__ grp,
+                                             const float (&nx)[kR], const float (&ny)[kR], const float (&nz)[kR],
+                                             const float (&wi)[kR], const Window win, uint32_t i_base, uint32_t j_first,
+                                             unsigned long long &n_fp64)
+{
+    const float e32 = win.e32;
+    float n_above = 0.f;  // exact: at most kGroup * kR = 512
+    double t_above[kR];   // per i-point: sum of w_j over its pairs above the edge
+#pragma unroll
+    for (int r = 0; r < kR; ++r) t_above[r] = 0.0;
+#pragma unroll 1
+    for (int jj = 0; jj < kGroup; jj += kWinUnroll) {
+        bool amb = false;
+#pragma unroll
+        for (int u = 0; u < kWinUnroll; ++u) {
+            const float4 q = grp[jj + u];
+            const double wj = (double)q.w;
+#pragma unroll
+            for (int r = 0; r < kR; ++r) {
+                const float d = fmaf(nx[r], q.x, fmaf(ny[r], q.y, fmaf(nz[r], q.z, e32)));
+                const bool above = d > 0.f;
+                amb |= !(fabsf(d) > kGuardWin);
+                n_above += above ? 1.f : 0.f;
+                if constexpr (kWeighted) t_above[r] += above ? wj : 0.0;
+            }
+        }
+        if (__any_sync(0xffffffffu, amb)) {
+            // some pair is within the guard band of the edge: replace its row by the exact one
+#pragma unroll 1
+            for (int u = 0; u < kWinUnroll; ++u) {
+                const float4 q = grp[jj + u];
+#pragma unroll
+                for (int r = 0; r < kR; ++r) {
+                    const float d = fmaf(nx[r], q.x, fmaf(ny[r], q.y, fmaf(nz[r], q.z, e32)));
+                    if (fabsf(d) > kGuardWin) continue;
+                    const uint32_t fast = (uint32_t)win.edge + (d > 0.f ? 1u : 0u);
+                    const uint32_t exact = (uint32_t)exact_row(p.xyz_a, p.stride_a, p.perm_a[i_base + local_i(r)], p.xyz_b, p.stride_b,
+                                                               p.perm_b[j_first + jj + u], p.edges, p.nbins);
+                    if (exact != fast) {
+                        h.move(fast, exact);
+                        if constexpr (kWeighted) {
+                            const double w = (double)wi[r] * (double)q.w;
+                            h.add_w(fast, -w);
+                            h.add_w(exact, w);
+                        }
+                    }
+                    ++n_fp64;
+                }
+            }
+        }
+    }
+    const uint32_t above = (uint32_t)n_above, total = (uint32_t)(kGroup * kR);
+    h.add_n((uint32_t)win.edge + 1u, above);
+    h.add_n((uint32_t)win.edge, total - above);
+    if constexpr (kWeighted) {
+        // sum over this thread's pairs of w_i w_j = sum_r w_i[r] * (sum of w_j above / not above)
+        double s_above = 0.0, s_below = 0.0;
+#pragma unroll
+        for (int r = 0; r < kR; ++r) {
+            s_above = fma((double)wi[r], t_above[r], s_above);
+            s_below = fma((double)wi[r], win.wsum - t_above[r], s_below);
+        }
+        if (above == total) s_below = 0.0;  // nothing below: not even a rounding residue of wsum - t_above
+        h.add_w((uint32_t)win.edge + 1u, s_above);
+        h.add_w((uint32_t)win.edge, s_below);
     }
 }
 
@@ -218,7 +361,7 @@ __global__ void __launch_bounds__(kThreads, kWeighted ? 1 : 2) pair_kernel(const
     if (n_items > p.capacity) n_items = p.capacity;
     __shared__ unsigned int s_item;
     uint32_t consumed = 0;  // j-tiles this CTA has staged so far: buffer = consumed & 1, parity = (consumed >> 1) & 1
-    unsigned long long n_fp64 = 0, n_eval = 0;
+    unsigned long long n_fp64 = 0, n_eval = 0, n_win = 0;
 
     while (true) {
         if (tid == 0) s_item = (unsigned int)atomicAdd(&p.counters[kCtrWorkHead], 1ull);
@@ -231,7 +374,7 @@ __global__ void __launch_bounds__(kThreads, kWeighted ? 1 : 2) pair_kernel(const
         uint32_t valid_mask = 0;
 #pragma unroll
         for (int r = 0; r < kR; ++r) {
-            const uint32_t s = i_base + r * kThreads + tid;
+            const uint32_t s = i_base + local_i(r);
             const float4 v = p.pts_a[s];  // the array is padded to a whole tile
             nx[r] = -v.x;
             ny[r] = -v.y;
@@ -265,10 +408,34 @@ __global__ void __launch_bounds__(kThreads, kWeighted ? 1 : 2) pair_kernel(const
             const int jn = (int)tile_count(tj);
             const bool diag = p.is_auto && tj == it.x;
             const uint32_t j_base = (uint32_t)tj * kTile;
-            if (diag || !i_full)
-                process_tile<kWeighted, kPrivate, true>(p, h, tile, jn, nx, ny, nz, wi, lut, i_base, j_base, diag, valid_mask, n_fp64);
-            else
-                process_tile<kWeighted, kPrivate, false>(p, h, tile, jn, nx, ny, nz, wi, lut, i_base, j_base, false, valid_mask, n_fp64);
+            if (diag || !i_full) {
+                process_tile<kWeighted, kPrivate, true>(p, h, tile, 0, jn, nx, ny, nz, wi, lut, i_base, j_base, diag, valid_mask, n_fp64);
+            } else if (!p.use_windows) {
+                process_tile<kWeighted, kPrivate, false>(p, h, tile, 0, jn, nx, ny, nz, wi, lut, i_base, j_base, false, valid_mask, n_fp64);
+            } else {
+                // lane g works out the window of this warp's i-group against j-group g of the tile
+                const int n_groups = (jn + kGroup - 1) / kGroup;
+                Window mine;
+                mine.edge = -1;
+                mine.e32 = 0.f;
+                mine.wsum = 0.0;
+                if (lane < n_groups && (lane + 1) * kGroup <= jn)
+                    mine = make_window(p.gcaps_a[(size_t)it.x * kGroupsPerTile + warp], p.gcaps_b[(size_t)tj * kGroupsPerTile + lane],
+                                       p.edges, p.nbins);
+                for (int g = 0; g < n_groups; ++g) {
+                    Window win;
+                    win.edge = __shfl_sync(0xffffffffu, mine.edge, g);
+                    win.e32 = __shfl_sync(0xffffffffu, mine.e32, g);
+                    win.wsum = __shfl_sync(0xffffffffu, mine.wsum, g);
+                    if (win.edge >= 0) {
+                        window_group<kWeighted, kPrivate>(p, h, tile + g * kGroup, nx, ny, nz, wi, win, i_base, j_base + g * kGroup, n_fp64);
+                        n_win += (unsigned long long)(kGroup * kR);
+                    } else {
+                        const int gn = jn - g * kGroup < kGroup ? jn - g * kGroup : kGroup;
+                        process_tile<kWeighted, kPrivate, false>(p, h, tile, g * kGroup, gn, nx, ny, nz, wi, lut, i_base, j_base, false, valid_mask, n_fp64);
+                    }
+                }
+            }
             if (tid == 0) n_eval += diag ? (unsigned long long)n_i * (n_i - 1) / 2 : (unsigned long long)n_i * (unsigned)jn;
             ++consumed;
             __syncthreads();  // all reads of this buffer are done before it is refilled
@@ -306,6 +473,8 @@ __global__ void __launch_bounds__(kThreads, kWeighted ? 1 : 2) pair_kernel(const
     }
     n_fp64 = warp_sum_u64(n_fp64);
     if (lane == 0 && n_fp64) atomicAdd(&p.counters[kCtrPairsFp64], n_fp64);
+    n_win = warp_sum_u64(n_win);
+    if (lane == 0 && n_win) atomicAdd(&p.counters[kCtrPairsWindow], n_win);
     if (tid == 0 && n_eval) atomicAdd(&p.counters[kCtrPairsEvaluated], n_eval);
 }
 
@@ -426,6 +595,9 @@ int count_prepared(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_au
     p.pts_b = b.pts;
     p.perm_a = a.perm;
     p.perm_b = b.perm;
+    p.gcaps_a = a.gcaps;
+    p.gcaps_b = b.gcaps;
+    p.use_windows = ctx->opt_windows;
     p.n_a = (uint32_t)a.n;
     p.n_b = (uint32_t)b.n;
     p.xyz_a = a.xyz;

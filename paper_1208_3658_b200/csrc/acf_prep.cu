@@ -1,7 +1,8 @@
 // acf_prep.cu -- O(N) preparation of a catalogue for the pair kernel:
-//   1. spatial key of every point (3-D Morton code of the quantised unit vector),
+//   1. spatial key of every point (cube face of the unit vector + Hilbert index on the face),
 //   2. LSD radix sort of (key, index) -- own kernels, 4 passes of 8 bits,
-//   3. gather into sorted fp32 float4 {x, y, z, w} + per-tile bounding caps in fp64,
+//   3. gather into sorted fp32 float4 {x, y, z, w} + bounding caps in fp64, per tile of kTile points
+//      and per group of kGroup points,
 //   4. the work list: (i-tile, run of j-tiles) items that may hold an in-range pair
 //      (calculations that fall outside the bin range need not be made;
 //       the pair matrix is walked sub-matrix by sub-matrix).
@@ -15,27 +16,48 @@ namespace acf {
 namespace {
 
 // ------------------------------------------------------------------ keys
-__device__ __forceinline__ uint32_t spread10(uint32_t v)
+// Hilbert index of (x, y) on a 2^14 x 2^14 grid (the classic xy -> d walk, one quadrant per level).
+__device__ __forceinline__ uint32_t hilbert14(uint32_t x, uint32_t y)
 {
-    // 10 bits -> every third bit
-    v = (v | (v << 16)) & 0x030000FFu;
-    v = (v | (v << 8)) & 0x0300F00Fu;
-    v = (v | (v << 4)) & 0x030C30C3u;
-    v = (v | (v << 2)) & 0x09249249u;
-    return v;
+    constexpr uint32_t n = 1u << 14;
+    uint32_t d = 0;
+#pragma unroll
+    for (uint32_t s = n >> 1; s > 0; s >>= 1) {
+        const uint32_t rx = (x & s) ? 1u : 0u, ry = (y & s) ? 1u : 0u;
+        d += s * s * ((3u * rx) ^ ry);
+        if (ry == 0) {
+            if (rx == 1) {
+                x = n - 1 - x;
+                y = n - 1 - y;
+            }
+            const uint32_t t = x;
+            x = y;
+            y = t;
+        }
+    }
+    return d;
 }
 
+// Key = cube face (3 bits) | Hilbert index of the equal-angle face coordinates (28 bits).  Points
+// that are consecutive in key order are neighbours on the sky, so a run of sorted points has a small
+// bounding cap (about 1.5x the ideal radius), which is what tile pruning and the per-window
+// threshold selection of the pair kernel live on.  Any key gives correct counts.
 __global__ void key_kernel(const double *__restrict__ xyz, size_t stride, size_t off, uint32_t n,
                            uint32_t *__restrict__ keys, uint32_t *__restrict__ idx)
 {
     for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
         const size_t g = off + i;
-        const float x = (float)xyz[g], y = (float)xyz[stride + g], z = (float)xyz[2 * stride + g];
-        // quantise [-1, 1] to 10 bits per axis (inputs are validated unit vectors; clamp anyway)
-        const uint32_t qx = (uint32_t)fminf(fmaxf((x + 1.0f) * 511.5f, 0.0f), 1023.0f);
-        const uint32_t qy = (uint32_t)fminf(fmaxf((y + 1.0f) * 511.5f, 0.0f), 1023.0f);
-        const uint32_t qz = (uint32_t)fminf(fmaxf((z + 1.0f) * 511.5f, 0.0f), 1023.0f);
-        keys[i] = (spread10(qz) << 2) | (spread10(qy) << 1) | spread10(qx);
+        const float v[3] = {(float)xyz[g], (float)xyz[stride + g], (float)xyz[2 * stride + g]};
+        int f = 0;
+        if (fabsf(v[1]) > fabsf(v[f])) f = 1;
+        if (fabsf(v[2]) > fabsf(v[f])) f = 2;
+        const float major = v[f], inv = 1.0f / fmaxf(fabsf(major), 1e-30f);
+        const float a1 = v[(f + 1) % 3] * inv, a2 = v[(f + 2) % 3] * inv;  // in [-1, 1]
+        const float u = atanf(a1) * 1.2732395447351628f, w = atanf(a2) * 1.2732395447351628f;  // * 4/pi
+        const uint32_t qx = (uint32_t)fminf(fmaxf((u + 1.0f) * 8192.0f, 0.0f), 16383.0f);
+        const uint32_t qy = (uint32_t)fminf(fmaxf((w + 1.0f) * 8192.0f, 0.0f), 16383.0f);
+        const uint32_t face = 2u * (uint32_t)f + (major < 0.0f ? 1u : 0u);
+        keys[i] = (face << 28) | hilbert14(qx, qy);
         idx[i] = i;
     }
 }
@@ -133,23 +155,26 @@ radix_scatter_kernel(const uint32_t *__restrict__ keys_in, const uint32_t *__res
     }
 }
 
-// ------------------------------------------------------------------ gather + tile caps
-// One CTA per tile of kTile sorted points: writes the fp32 float4 records and the tile's bounding
-// cap {unit centre, cos(radius)} computed in fp64 from the fp64 vectors.
+// ------------------------------------------------------------------ gather + caps
+// One CTA per tile of kTile sorted points, one warp per group of kGroup points: writes the fp32 float4
+// records, the tile's bounding cap {unit centre, cos(radius)} and the kGroupsPerTile group caps, all
+// computed in fp64 from the fp64 vectors.
 __global__ void __launch_bounds__(256)
 gather_caps_kernel(const double *__restrict__ xyz, size_t stride, size_t off, const float *__restrict__ w,
                    const uint32_t *__restrict__ idx, uint32_t n, float4 *__restrict__ pts,
-                   uint32_t *__restrict__ perm, double4 *__restrict__ caps)
+                   uint32_t *__restrict__ perm, double4 *__restrict__ caps, GroupCap *__restrict__ gcaps)
 {
+    static_assert(kGroupsPerTile == 8 && kGroup == 128, "one warp of 256 threads per group");
     __shared__ double red[3][8];
     __shared__ double centre[3];
-    constexpr int kPer = kTile / 256;
-    const uint32_t base = blockIdx.x * kTile;
+    constexpr int kPer = kGroup / 32;
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t base = blockIdx.x * kTile + warp * kGroup;
     double px[kPer], py[kPer], pz[kPer];
-    double sx = 0, sy = 0, sz = 0;
+    double sx = 0, sy = 0, sz = 0, sw = 0;
 #pragma unroll
     for (int r = 0; r < kPer; ++r) {
-        const uint32_t s = base + r * 256 + threadIdx.x;
+        const uint32_t s = base + r * 32 + lane;
         if (s < n) {
             const uint32_t local = idx[s];
             const size_t g = off + local;
@@ -162,18 +187,52 @@ gather_caps_kernel(const double *__restrict__ xyz, size_t stride, size_t off, co
             sx += px[r];
             sy += py[r];
             sz += pz[r];
+            sw += (double)wi;
         } else {
             px[r] = py[r] = pz[r] = 0.0;
             pts[s] = make_float4(0.f, 0.f, 0.f, 0.f);  // padding up to the tile boundary, never paired
         }
     }
-    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
         sx += __shfl_xor_sync(0xffffffffu, sx, o);
         sy += __shfl_xor_sync(0xffffffffu, sy, o);
         sz += __shfl_xor_sync(0xffffffffu, sz, o);
+        sw += __shfl_xor_sync(0xffffffffu, sw, o);
     }
+    // ---- group cap (this warp's points)
+    {
+        double cx = 0.0, cy = 0.0, cz = 1.0;  // any centre is valid; the radius makes it a bound
+        const double nrm = sqrt(sx * sx + sy * sy + sz * sz);
+        if (nrm > 1e-9) {
+            cx = sx / nrm;
+            cy = sy / nrm;
+            cz = sz / nrm;
+        }
+        double mind = 2.0;
+#pragma unroll
+        for (int r = 0; r < kPer; ++r)
+            if (base + r * 32 + lane < n) mind = fmin(mind, cx * px[r] + cy * py[r] + cz * pz[r]);
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) mind = fmin(mind, __shfl_xor_sync(0xffffffffu, mind, o));
+        if (lane == 0) {
+            GroupCap gc;
+            gc.cx = cx;
+            gc.cy = cy;
+            gc.cz = cz;
+            if (base < n) {
+                // cos of the bounding radius, pushed outwards by far more than the rounding of the dots
+                gc.cos_r = fmax(-1.0, fmin(1.0, mind) - 1e-9);
+                gc.sin_r = sqrt(fmax(0.0, 1.0 - gc.cos_r * gc.cos_r));
+            } else {
+                gc.cos_r = 2.0;  // no points
+                gc.sin_r = 0.0;
+            }
+            gc.wsum = sw;
+            gcaps[(size_t)blockIdx.x * kGroupsPerTile + warp] = gc;
+        }
+    }
+    // ---- tile cap
     if (lane == 0) {
         red[0][warp] = sx;
         red[1][warp] = sy;
@@ -203,7 +262,7 @@ gather_caps_kernel(const double *__restrict__ xyz, size_t stride, size_t off, co
     double mind = 2.0;
 #pragma unroll
     for (int r = 0; r < kPer; ++r) {
-        const uint32_t s = base + r * 256 + threadIdx.x;
+        const uint32_t s = base + r * 32 + lane;
         if (s < n) mind = fmin(mind, cx * px[r] + cy * py[r] + cz * pz[r]);
     }
 #pragma unroll
@@ -213,7 +272,6 @@ gather_caps_kernel(const double *__restrict__ xyz, size_t stride, size_t off, co
     __syncthreads();
     if (threadIdx.x == 0) {
         for (int k = 1; k < 8; ++k) mind = fmin(mind, red[0][k]);
-        // cos of the bounding radius, pushed outwards by far more than the rounding of the dots
         caps[blockIdx.x] = make_double4(cx, cy, cz, fmax(-1.0, fmin(1.0, mind) - 1e-9));
     }
 }
@@ -309,12 +367,14 @@ int prepare_catalogue(acf_ctx *ctx, int slot, const double *xyz, size_t stride, 
     ACF_CUDA_TRY(ctx, ctx->s_pts[slot].reserve(sizeof(float4) * padded));
     ACF_CUDA_TRY(ctx, ctx->s_perm[slot].reserve(sizeof(uint32_t) * padded));
     ACF_CUDA_TRY(ctx, ctx->s_caps[slot].reserve(sizeof(double4) * (size_t)n_tiles));
+    ACF_CUDA_TRY(ctx, ctx->s_gcaps[slot].reserve(sizeof(GroupCap) * (size_t)n_tiles * kGroupsPerTile));
     ACF_CUDA_TRY(ctx, ctx->s_keys[slot].reserve(sizeof(uint32_t) * 4 * (size_t)n));  // keys x2, idx x2
     const uint32_t nblocks = (n + kSortBlockChunk - 1) / kSortBlockChunk;
     ACF_CUDA_TRY(ctx, ctx->s_misc.reserve(sizeof(uint32_t) * 256 * (size_t)nblocks));
     out->pts = ctx->s_pts[slot].as<float4>();
     out->perm = ctx->s_perm[slot].as<uint32_t>();
     out->caps = ctx->s_caps[slot].as<double4>();
+    out->gcaps = ctx->s_gcaps[slot].as<GroupCap>();
     uint32_t *k0 = ctx->s_keys[slot].as<uint32_t>(), *k1 = k0 + n, *i0 = k1 + n, *i1 = i0 + n;
     uint32_t *counts = ctx->s_misc.as<uint32_t>();
 
@@ -331,7 +391,7 @@ int prepare_catalogue(acf_ctx *ctx, int slot, const double *xyz, size_t stride, 
         uint32_t *t = k0; k0 = k1; k1 = t;
         t = i0; i0 = i1; i1 = t;
     }
-    gather_caps_kernel<<<n_tiles, 256, 0, st>>>(xyz, stride, off, w, i0, n, out->pts, out->perm, out->caps);
+    gather_caps_kernel<<<n_tiles, 256, 0, st>>>(xyz, stride, off, w, i0, n, out->pts, out->perm, out->caps, out->gcaps);
     ctx->last.kernel_launches++;
     ACF_CUDA_TRY(ctx, cudaGetLastError());
     return ACF_OK;
