@@ -49,6 +49,8 @@ constexpr float kGuard = kDelta + 0x1p-23f;
 constexpr int kExpLo = -19;  // t32 >= K - (1 + 1e-6) - kDelta > 2^-19
 constexpr int kExpHi = 2;    // t32 < 4
 constexpr int kMaxPrivateRows = 64;
+constexpr int kMaxStages = 8;      // j-tile buffers of the producer/consumer ring (at least 2)
+constexpr int kSmemHeader = 512;   // mbarriers + stage descriptors
 // Window path: |d32 - (e_m - c64)| <= 2^-25 [fp32(e_m)] + 2u(1+1e-6) [input rounding] + 3 * 2^-24
 // [three roundings of values of magnitude <= 2] = 3.3e-7.
 constexpr float kGuardWin = 4.5e-7f;
@@ -74,6 +76,7 @@ struct PairParams {
     unsigned long long *counters;
     int is_auto;
     int use_windows;
+    int n_stages;
 };
 
 __device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
@@ -85,6 +88,10 @@ __device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
 __device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
 {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
 {
@@ -274,10 +281,17 @@ __device__ __forceinline__ void window_group(const PairParams &p, Hist<kWeighted
 #pragma unroll
             for (int r = 0; r < kR; ++r) {
                 const float d = fmaf(nx[r], q.x, fmaf(ny[r], q.y, fmaf(nz[r], q.z, e32)));
-                const bool above = d > 0.f;
                 amb |= !(fabsf(d) > kGuardWin);
-                n_above += above ? 1.f : 0.f;
-                if constexpr (kWeighted) t_above[r] += above ? wj : 0.0;
+                // n_above += d > 0; t_above[r] += d > 0 ? w_j : 0 -- as predicated adds (one FSETP, no selects)
+                if constexpr (kWeighted)
+                    asm("{\n\t.reg .pred above;\n\tsetp.gt.f32 above, %2, 0f00000000;\n\t@above add.f32 %0, %0, 0f3F800000;\n\t"
+                        "@above add.f64 %1, %1, %3;\n\t}"
+                        : "+f"(n_above), "+d"(t_above[r])
+                        : "f"(d), "d"(wj));
+                else
+                    asm("{\n\t.reg .pred above;\n\tsetp.gt.f32 above, %1, 0f00000000;\n\t@above add.f32 %0, %0, 0f3F800000;\n\t}"
+                        : "+f"(n_above)
+                        : "f"(d));
             }
         }
         if (__any_sync(0xffffffffu, amb)) {
@@ -322,18 +336,32 @@ __device__ __forceinline__ void window_group(const PairParams &p, Hist<kWeighted
     }
 }
 
+// ---- the kernel ---------------------------------------------------------------------------------
+// kWarps consumer warps + one producer warp.  The producer pulls work items {i-tile, first j-tile,
+// number of j-tiles} from a global counter and streams their j-tiles through a ring of kStages
+// shared-memory buffers with TMA bulk copies (full/empty mbarriers per stage); each stage carries
+// {i-tile, j-tile, points}.  Every consumer warp walks the same stream at its own pace -- a warp whose
+// windows take the table path does not hold the others back until the ring is full -- holding its
+// kGroup i-points of the current i-tile in registers.
+struct StageMeta {
+    int ti, tj, jn, pad;
+};
+
 template <bool kWeighted, bool kPrivate>
-__global__ void __launch_bounds__(kThreads, kWeighted ? 1 : 2) pair_kernel(const PairParams p)
+__global__ void __launch_bounds__(kThreads + 32, kWeighted ? 1 : 2) pair_kernel(const PairParams p)
 {
     if (p.counters[kCtrBadInput] != 0) return;  // inputs failed validation: never index the LUT with garbage
     extern __shared__ __align__(128) unsigned char smem[];
     const int rows = p.nbins + 2;
-    // layout: [2 mbarriers][tile 0][tile 1][LUT][count rows][weighted rows]
-    uint64_t *bars = reinterpret_cast<uint64_t *>(smem);
-    float4 *tiles = reinterpret_cast<float4 *>(smem + 128);
-    uint2 *lut = reinterpret_cast<uint2 *>(smem + 128 + 2 * kTile * sizeof(float4));
-    const size_t cnt_words = kPrivate ? (size_t)kWarps * rows * 32 : (size_t)rows;
-    size_t off = 128 + 2 * kTile * sizeof(float4) + (size_t)p.lut_len * sizeof(uint2);
+    const int n_stages = p.n_stages;
+    // layout: [full bars | empty bars | stage meta] (512 B) [tiles][LUT][count rows][weighted rows]
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem);
+    uint64_t *empty = full + kMaxStages;
+    StageMeta *meta = reinterpret_cast<StageMeta *>(smem + 128);
+    float4 *tiles = reinterpret_cast<float4 *>(smem + kSmemHeader);
+    uint2 *lut = reinterpret_cast<uint2 *>(smem + kSmemHeader + (size_t)n_stages * kTile * sizeof(float4));
+    const size_t cnt_words = kPrivate ? (size_t)kWarps * rows * 32 : (size_t)kWarps * rows;
+    size_t off = kSmemHeader + (size_t)n_stages * kTile * sizeof(float4) + (size_t)p.lut_len * sizeof(uint2);
     off = (off + 15) & ~size_t(15);
     uint32_t *cnt_all = reinterpret_cast<uint32_t *>(smem + off);
     off += cnt_words * sizeof(uint32_t);
@@ -341,136 +369,174 @@ __global__ void __launch_bounds__(kThreads, kWeighted ? 1 : 2) pair_kernel(const
     double *ws_all = reinterpret_cast<double *>(smem + off);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    for (int i = tid; i < p.lut_len; i += kThreads) lut[i] = p.lut[i];
-    for (size_t i = tid; i < cnt_words; i += kThreads) cnt_all[i] = 0;
+    for (int i = tid; i < p.lut_len; i += blockDim.x) lut[i] = p.lut[i];
+    for (size_t i = tid; i < cnt_words; i += blockDim.x) cnt_all[i] = 0;
     if constexpr (kWeighted)
-        for (size_t i = tid; i < cnt_words; i += kThreads) ws_all[i] = 0.0;
+        for (size_t i = tid; i < cnt_words; i += blockDim.x) ws_all[i] = 0.0;
     if (tid == 0) {
-        mbar_init(&bars[0], 1);
-        mbar_init(&bars[1], 1);
+        for (int s = 0; s < n_stages; ++s) {
+            mbar_init(&full[s], 1);
+            mbar_init(&empty[s], kWarps);
+        }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
 
-    Hist<kWeighted, kPrivate> h;
-    h.cnt = kPrivate ? cnt_all + (size_t)warp * rows * 32 : cnt_all;
-    h.ws = kPrivate ? ws_all + (size_t)warp * rows * 32 : ws_all;
-    h.lane = lane;
-
     unsigned long long n_items = p.counters[kCtrWorkCount];
     if (n_items > p.capacity) n_items = p.capacity;
-    __shared__ unsigned int s_item;
-    uint32_t consumed = 0;  // j-tiles this CTA has staged so far: buffer = consumed & 1, parity = (consumed >> 1) & 1
-    unsigned long long n_fp64 = 0, n_eval = 0, n_win = 0;
 
-    while (true) {
-        if (tid == 0) s_item = (unsigned int)atomicAdd(&p.counters[kCtrWorkHead], 1ull);
-        __syncthreads();
-        const unsigned int item = s_item;
-        if (item >= n_items) break;
-        const int3 it = p.items[item];
-        const uint32_t i_base = (uint32_t)it.x * kTile;
-        float nx[kR], ny[kR], nz[kR], wi[kR];
-        uint32_t valid_mask = 0;
-#pragma unroll
-        for (int r = 0; r < kR; ++r) {
-            const uint32_t s = i_base + local_i(r);
-            const float4 v = p.pts_a[s];  // the array is padded to a whole tile
-            nx[r] = -v.x;
-            ny[r] = -v.y;
-            nz[r] = -v.z;
-            wi[r] = v.w;
-            valid_mask |= (s < p.n_a ? 1u : 0u) << r;
-        }
-        const bool i_full = i_base + kTile <= p.n_a;
-        const uint32_t n_i = i_full ? kTile : p.n_a - i_base;
-
-        auto tile_count = [&](int tj) -> uint32_t {
-            const uint32_t j0 = (uint32_t)tj * kTile;
-            return p.n_b - j0 < (uint32_t)kTile ? p.n_b - j0 : (uint32_t)kTile;
+    if (warp == kWarps) {
+        // ---------------- producer
+        if (lane != 0) return;
+        uint32_t produced = 0;  // stages filled so far: slot = produced % n_stages, round = produced / n_stages
+        auto acquire = [&]() -> int {
+            const int slot = (int)(produced % (uint32_t)n_stages);
+            const uint32_t round = produced / (uint32_t)n_stages;
+            mbar_wait(&empty[slot], (round & 1u) ^ 1u);  // round 0 passes at once: nothing to drain yet
+            return slot;
         };
-        if (tid == 0) {
-            const uint32_t bytes = tile_count(it.y) * sizeof(float4);
-            uint64_t *bar = &bars[consumed & 1];
-            mbar_expect_tx(bar, bytes);
-            bulk_load(tiles + (size_t)(consumed & 1) * kTile, p.pts_b + (size_t)it.y * kTile, bytes, bar);
-        }
-        for (int t = 0; t < it.z; ++t) {
-            const int tj = it.y + t;
-            if (tid == 0 && t + 1 < it.z) {  // prefetch the next tile into the other buffer (released by the sync below)
-                const uint32_t bytes = tile_count(tj + 1) * sizeof(float4);
-                uint64_t *bar = &bars[(consumed + 1) & 1];
-                mbar_expect_tx(bar, bytes);
-                bulk_load(tiles + (size_t)((consumed + 1) & 1) * kTile, p.pts_b + (size_t)(tj + 1) * kTile, bytes, bar);
+        while (true) {
+            const unsigned long long item = atomicAdd(&p.counters[kCtrWorkHead], 1ull);
+            if (item >= n_items) break;
+            const int3 it = p.items[item];
+            for (int t = 0; t < it.z; ++t) {
+                const int tj = it.y + t;
+                const uint32_t j0 = (uint32_t)tj * kTile;
+                const uint32_t jn = p.n_b - j0 < (uint32_t)kTile ? p.n_b - j0 : (uint32_t)kTile;
+                const int slot = acquire();
+                StageMeta m;
+                m.ti = it.x;
+                m.tj = tj;
+                m.jn = (int)jn;
+                m.pad = 0;
+                meta[slot] = m;
+                mbar_expect_tx(&full[slot], jn * (uint32_t)sizeof(float4));
+                bulk_load(tiles + (size_t)slot * kTile, p.pts_b + (size_t)j0, jn * (uint32_t)sizeof(float4), &full[slot]);
+                ++produced;
             }
-            mbar_wait(&bars[consumed & 1], (consumed >> 1) & 1);
-            const float4 *tile = tiles + (size_t)(consumed & 1) * kTile;
-            const int jn = (int)tile_count(tj);
-            const bool diag = p.is_auto && tj == it.x;
-            const uint32_t j_base = (uint32_t)tj * kTile;
-            if (diag || !i_full) {
-                process_tile<kWeighted, kPrivate, true>(p, h, tile, 0, jn, nx, ny, nz, wi, lut, i_base, j_base, diag, valid_mask, n_fp64);
-            } else if (!p.use_windows) {
-                process_tile<kWeighted, kPrivate, false>(p, h, tile, 0, jn, nx, ny, nz, wi, lut, i_base, j_base, false, valid_mask, n_fp64);
-            } else {
-                // lane g works out the window of this warp's i-group against j-group g of the tile
-                const int n_groups = (jn + kGroup - 1) / kGroup;
-                Window mine;
-                mine.edge = -1;
-                mine.e32 = 0.f;
-                mine.wsum = 0.0;
-                if (lane < n_groups && (lane + 1) * kGroup <= jn)
-                    mine = make_window(p.gcaps_a[(size_t)it.x * kGroupsPerTile + warp], p.gcaps_b[(size_t)tj * kGroupsPerTile + lane],
-                                       p.edges, p.nbins);
-                for (int g = 0; g < n_groups; ++g) {
-                    Window win;
-                    win.edge = __shfl_sync(0xffffffffu, mine.edge, g);
-                    win.e32 = __shfl_sync(0xffffffffu, mine.e32, g);
-                    win.wsum = __shfl_sync(0xffffffffu, mine.wsum, g);
-                    if (win.edge >= 0) {
-                        window_group<kWeighted, kPrivate>(p, h, tile + g * kGroup, nx, ny, nz, wi, win, i_base, j_base + g * kGroup, n_fp64);
-                        n_win += (unsigned long long)(kGroup * kR);
-                    } else {
-                        const int gn = jn - g * kGroup < kGroup ? jn - g * kGroup : kGroup;
-                        process_tile<kWeighted, kPrivate, false>(p, h, tile, g * kGroup, gn, nx, ny, nz, wi, lut, i_base, j_base, false, valid_mask, n_fp64);
-                    }
-                }
-            }
-            if (tid == 0) n_eval += diag ? (unsigned long long)n_i * (n_i - 1) / 2 : (unsigned long long)n_i * (unsigned)jn;
-            ++consumed;
-            __syncthreads();  // all reads of this buffer are done before it is refilled
         }
-        if constexpr (!kPrivate) {
-            // the CTA-wide u32 rows could overflow over a CTA's lifetime: flush per item (<= 2^23 pairs)
-            for (int row = 1 + tid; row <= p.nbins; row += kThreads) {
-                const uint32_t v = cnt_all[row];
-                if (v) atomicAdd(&p.counts[row - 1], (unsigned long long)v);
-                cnt_all[row] = 0;
-                if constexpr (kWeighted) {
-                    const double w = ws_all[row];
-                    if (w != 0.0) atomicAdd(&p.wsums[row - 1], w);
-                    ws_all[row] = 0.0;
-                }
-            }
-            __syncthreads();
-        }
+        const int slot = acquire();  // end of stream
+        StageMeta m;
+        m.ti = -1;
+        m.tj = m.jn = m.pad = 0;
+        meta[slot] = m;
+        mbar_arrive(&full[slot]);
+        return;
     }
 
-    if constexpr (kPrivate) {
-        // per-lane u32 counters: a thread sees < 2^32 pairs in any call this library accepts per CTA
-        // (n_a, n_b < 2^31 and >= 148 CTAs share the work), so one flush at the end suffices.
-        __syncwarp();
-        for (int row = 1; row <= p.nbins; ++row) {
-            const unsigned long long v = warp_sum_u64((unsigned long long)h.cnt[row * 32 + lane]);
-            if (lane == 0 && v) atomicAdd(&p.counts[row - 1], v);
-            if constexpr (kWeighted) {
-                double w = h.ws[row * 32 + lane];
+    // ---------------- consumers
+    Hist<kWeighted, kPrivate> h;
+    h.cnt = kPrivate ? cnt_all + (size_t)warp * rows * 32 : cnt_all + (size_t)warp * rows;
+    h.ws = kPrivate ? ws_all + (size_t)warp * rows * 32 : ws_all + (size_t)warp * rows;
+    h.lane = lane;
+
+    unsigned long long n_fp64 = 0, n_eval = 0, n_win = 0;
+    unsigned long long since_flush = 0;  // pairs this warp has tallied in its unflushed shared rows
+    float nx[kR], ny[kR], nz[kR], wi[kR];
 #pragma unroll
-                for (int o = 16; o > 0; o >>= 1) w += __shfl_xor_sync(0xffffffffu, w, o);
-                if (lane == 0 && w != 0.0) atomicAdd(&p.wsums[row - 1], w);
+    for (int r = 0; r < kR; ++r) nx[r] = ny[r] = nz[r] = wi[r] = 0.f;
+    uint32_t valid_mask = 0, i_base = 0, n_i = 0;
+    bool i_full = false;
+    int cur_ti = -1;
+
+    auto flush_rows = [&]() {
+        // this warp's rows -> global (u64 / f64 atomics); the rows restart from zero
+        __syncwarp();
+        if constexpr (kPrivate) {
+            for (int row = 1; row <= p.nbins; ++row) {
+                const unsigned long long v = warp_sum_u64((unsigned long long)h.cnt[row * 32 + lane]);
+                h.cnt[row * 32 + lane] = 0;
+                if (lane == 0 && v) atomicAdd(&p.counts[row - 1], v);
+                if constexpr (kWeighted) {
+                    double w = h.ws[row * 32 + lane];
+                    h.ws[row * 32 + lane] = 0.0;
+#pragma unroll
+                    for (int o = 16; o > 0; o >>= 1) w += __shfl_xor_sync(0xffffffffu, w, o);
+                    if (lane == 0 && w != 0.0) atomicAdd(&p.wsums[row - 1], w);
+                }
+            }
+            h.cnt[lane] = 0;  // the two out-of-range rows are tallied but never reported
+            h.cnt[(p.nbins + 1) * 32 + lane] = 0;
+        } else {
+            for (int row = lane; row < rows; row += 32) {
+                const uint32_t v = h.cnt[row];
+                h.cnt[row] = 0;
+                if (row >= 1 && row <= p.nbins && v) atomicAdd(&p.counts[row - 1], (unsigned long long)v);
+                if constexpr (kWeighted) {
+                    const double w = h.ws[row];
+                    h.ws[row] = 0.0;
+                    if (row >= 1 && row <= p.nbins && w != 0.0) atomicAdd(&p.wsums[row - 1], w);
+                }
             }
         }
+        __syncwarp();
+        since_flush = 0;
+    };
+
+    for (uint32_t consumed = 0;; ++consumed) {
+        const int slot = (int)(consumed % (uint32_t)n_stages);
+        mbar_wait(&full[slot], (consumed / (uint32_t)n_stages) & 1u);
+        const StageMeta m = meta[slot];
+        if (m.ti < 0) break;
+        if (m.ti != cur_ti) {
+            cur_ti = m.ti;
+            i_base = (uint32_t)m.ti * kTile;
+            valid_mask = 0;
+#pragma unroll
+            for (int r = 0; r < kR; ++r) {
+                const uint32_t s = i_base + local_i(r);
+                const float4 v = p.pts_a[s];  // the array is padded to a whole tile
+                nx[r] = -v.x;
+                ny[r] = -v.y;
+                nz[r] = -v.z;
+                wi[r] = v.w;
+                valid_mask |= (s < p.n_a ? 1u : 0u) << r;
+            }
+            i_full = i_base + kTile <= p.n_a;
+            n_i = i_full ? kTile : p.n_a - i_base;
+        }
+        const float4 *tile = tiles + (size_t)slot * kTile;
+        const int tj = m.tj, jn = m.jn;
+        const bool diag = p.is_auto && tj == m.ti;
+        const uint32_t j_base = (uint32_t)tj * kTile;
+        // u32 rows: flush before this warp's tallies could wrap (per lane when private, per row otherwise)
+        if (since_flush + (unsigned long long)kGroup * kTile > (kPrivate ? (32ull << 31) : (1ull << 31))) flush_rows();
+        since_flush += (unsigned long long)kGroup * (unsigned)jn;
+
+        if (diag || !i_full) {
+            process_tile<kWeighted, kPrivate, true>(p, h, tile, 0, jn, nx, ny, nz, wi, lut, i_base, j_base, diag, valid_mask, n_fp64);
+        } else if (!p.use_windows) {
+            process_tile<kWeighted, kPrivate, false>(p, h, tile, 0, jn, nx, ny, nz, wi, lut, i_base, j_base, false, valid_mask, n_fp64);
+        } else {
+            // lane g works out the window of this warp's i-group against j-group g of the tile
+            const int n_groups = (jn + kGroup - 1) / kGroup;
+            Window mine;
+            mine.edge = -1;
+            mine.e32 = 0.f;
+            mine.wsum = 0.0;
+            if (lane < n_groups && (lane + 1) * kGroup <= jn)
+                mine = make_window(p.gcaps_a[(size_t)m.ti * kGroupsPerTile + warp], p.gcaps_b[(size_t)tj * kGroupsPerTile + lane],
+                                   p.edges, p.nbins);
+            for (int g = 0; g < n_groups; ++g) {
+                Window win;
+                win.edge = __shfl_sync(0xffffffffu, mine.edge, g);
+                win.e32 = __shfl_sync(0xffffffffu, mine.e32, g);
+                win.wsum = __shfl_sync(0xffffffffu, mine.wsum, g);
+                if (win.edge >= 0) {
+                    window_group<kWeighted, kPrivate>(p, h, tile + g * kGroup, nx, ny, nz, wi, win, i_base, j_base + g * kGroup, n_fp64);
+                    n_win += (unsigned long long)(kGroup * kR);
+                } else {
+                    const int gn = jn - g * kGroup < kGroup ? jn - g * kGroup : kGroup;
+                    process_tile<kWeighted, kPrivate, false>(p, h, tile, g * kGroup, gn, nx, ny, nz, wi, lut, i_base, j_base, false, valid_mask, n_fp64);
+                }
+            }
+        }
+        if (tid == 0) n_eval += diag ? (unsigned long long)n_i * (n_i - 1) / 2 : (unsigned long long)n_i * (unsigned)jn;
+        __syncwarp();  // every lane has read the stage before it is handed back
+        if (lane == 0) mbar_arrive(&empty[slot]);
     }
+
+    flush_rows();
     n_fp64 = warp_sum_u64(n_fp64);
     if (lane == 0 && n_fp64) atomicAdd(&p.counters[kCtrPairsFp64], n_fp64);
     n_win = warp_sum_u64(n_win);
@@ -560,7 +626,7 @@ cudaError_t launch(acf_ctx *ctx, const PairParams &p, size_t smem, int grid)
     auto kern = pair_kernel<kWeighted, kPrivate>;
     cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    kern<<<grid, kThreads, smem, ctx->stream>>>(p);
+    kern<<<grid, kThreads + 32, smem, ctx->stream>>>(p);
     ctx->last.kernel_launches++;
     return cudaGetLastError();
 }
@@ -572,13 +638,24 @@ int count_prepared(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_au
     const bool weighted = d_wsums != nullptr;
     const int rows = nbins + 2;
     const bool priv = rows <= kMaxPrivateRows;
-    size_t smem = 128 + 2 * kTile * sizeof(float4) + L.cells.size() * sizeof(uint2);
-    smem = (smem + 15) & ~size_t(15);
-    const size_t cnt_words = priv ? (size_t)kWarps * rows * 32 : (size_t)rows;
-    smem += cnt_words * sizeof(uint32_t);
-    smem = (smem + 15) & ~size_t(15);
-    if (weighted) smem += cnt_words * sizeof(double);
-    if (smem > (size_t)ctx->max_smem_optin) return fail(ctx, ACF_EINVAL, "shared memory need %zu exceeds %d", smem, ctx->max_smem_optin);
+    // shared memory: header, LUT, histogram rows, and as many j-tile stages as fit (2 CTAs per SM when
+    // unweighted and small enough, else 1)
+    const size_t cnt_words = priv ? (size_t)kWarps * rows * 32 : (size_t)kWarps * rows;
+    auto smem_for = [&](int stages) {
+        size_t m = kSmemHeader + (size_t)stages * kTile * sizeof(float4) + L.cells.size() * sizeof(uint2);
+        m = (m + 15) & ~size_t(15);
+        m += cnt_words * sizeof(uint32_t);
+        m = (m + 15) & ~size_t(15);
+        if (weighted) m += cnt_words * sizeof(double);
+        return m;
+    };
+    const size_t per_sm = (size_t)ctx->max_smem_optin;            // per CTA limit; an SM has 1 KB more per resident CTA
+    int ctas_per_sm = (!weighted && smem_for(2) <= (per_sm - 1024) / 2) ? 2 : 1;
+    const size_t budget = ctas_per_sm == 2 ? (per_sm - 1024) / 2 : per_sm;
+    int n_stages = 2;
+    while (n_stages < 4 && smem_for(n_stages + 1) <= budget) ++n_stages;
+    const size_t smem = smem_for(n_stages);
+    if (smem > per_sm) return fail(ctx, ACF_EINVAL, "shared memory need %zu exceeds %d", smem, ctx->max_smem_optin);
 
     // i-tiles are handed out in batches so that the item buffer stays bounded
     // (worst case one item per surviving j-tile: survivors may alternate with pruned tiles)
@@ -616,8 +693,8 @@ int count_prepared(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_au
     p.wsums = d_wsums;
     p.counters = ctx->d_counters;
     p.is_auto = is_auto;
+    p.n_stages = n_stages;
 
-    const int ctas_per_sm = weighted ? 1 : (2 * smem <= (size_t)220 * 1024 ? 2 : 1);
     const int grid = ctx->num_sms * ctas_per_sm;
     for (int ti0 = 0; ti0 < a.n_tiles; ti0 += ti_per_batch) {
         const int ti1 = ti0 + ti_per_batch < a.n_tiles ? ti0 + ti_per_batch : a.n_tiles;
