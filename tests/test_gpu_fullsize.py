@@ -1,0 +1,139 @@
+"""GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times
+(acf_pair_count / acf_pair_count_weighted on whole catalogues):
+
+  * sampled outputs the oracle can compute one by one: the histogram of a few row blocks
+    (acf_pair_count_rows vs oracle rows), u64-equal;
+  * properties that hold at any size, on the full calls: the single-edge window path and the
+    table path (two different kernels paths) give identical u64 counts; DR(a, b) == DR(b, a);
+    row-block additivity; totals; the closed-form expectation on the uniform sphere.
+
+Run on the B200 box:  python -m pytest tests/test_gpu_fullsize.py -m gpu -x -q
+"""
+import numpy as np
+import pytest
+
+from workloads import make_config
+
+pytestmark = pytest.mark.gpu
+
+WSUM_RTOL = 1e-12
+
+
+@pytest.fixture(scope="module")
+def acf():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    import paper_1208_3658_b200 as P
+    return P
+
+
+@pytest.fixture(scope="module")
+def ctx(acf):
+    c = acf.acf_create(0)
+    yield c
+    acf.acf_destroy(c)
+
+
+class Dev:
+    """Device copies of one workload (uploaded once per test)."""
+
+    def __init__(self, acf, w):
+        import torch
+        self.w = w
+        self.h_xd, self.h_xr = acf.acf_radec_to_xyz(w.ra_d, w.dec_d), acf.acf_radec_to_xyz(w.ra_r, w.dec_r)
+        self.xd, self.xr = torch.from_numpy(self.h_xd).cuda(), torch.from_numpy(self.h_xr).cuda()
+        self.wd = torch.from_numpy(w.w_d).cuda() if w.w_d is not None else None
+        self.wr = torch.from_numpy(w.w_r).cuda() if w.w_r is not None else None
+
+
+def count(acf, ctx, d, which, rows=None, windows=1):
+    """-> (u64 counts, f64 sums or None, stats) of DD / DR / RD / RR on the device."""
+    import torch
+    a, wa, b, wb, auto = {"dd": (d.xd, d.wd, None, None, True), "dr": (d.xd, d.wd, d.xr, d.wr, False),
+                          "rd": (d.xr, d.wr, d.xd, d.wd, False), "rr": (d.xr, d.wr, None, None, True)}[which]
+    acf.acf_set_option(ctx, acf.ACF_OPT_WINDOWS, windows)
+    try:
+        n_a = a.numel() // 3
+        lo, hi = rows if rows is not None else (0, n_a)
+        out = acf.acf_pair_count_rows(ctx, a, wa, lo, hi, b, wb, d.w.cos_edges, auto)
+        torch.cuda.synchronize()
+        st = acf.acf_get_stats(ctx)
+    finally:
+        acf.acf_set_option(ctx, acf.ACF_OPT_WINDOWS, 1)
+    if wa is None:
+        return acf.counts_to_numpy(out), None, st
+    return acf.counts_to_numpy(out[0]), out[1].cpu().numpy(), st
+
+
+def oracle_rows(oracle, d, which, rows):
+    a, wa, b, wb, auto = {"dd": (d.h_xd, d.w.w_d, None, None, True), "dr": (d.h_xd, d.w.w_d, d.h_xr, d.w.w_r, False),
+                          "rr": (d.h_xr, d.w.w_r, None, None, True)}[which]
+    return oracle.pair_count(a, b, d.w.cos_edges, auto, w_a=wa, w_b=wb, rows=rows)
+
+
+def sample_blocks(n, width):
+    """Row blocks at the start, around the middle (straddling a tile boundary) and at the ragged end."""
+    mid = (n // 2 // 1024) * 1024
+    return [(0, width), (max(0, mid - width // 2), min(n, mid + width // 2)), (n - width, n)]
+
+
+@pytest.mark.parametrize("name,width", [("tiny", 256), ("clustered_patch", 192), ("survey_scale", 96),
+                                        ("full_sky", 96), ("pruning_stress", 48)])
+def test_fullsize_sampled_rows_and_properties(acf, ctx, oracle, name, width):
+    w = make_config(name, 1.0)
+    d = Dev(acf, w)
+    assert d.h_xd.tobytes() == oracle.radec_to_xyz(w.ra_d, w.dec_d).tobytes()
+    weighted = w.w_d is not None
+
+    # ---- sampled outputs: row blocks against the oracle, DD / DR / RR
+    for which, n in (("dd", w.n_d), ("dr", w.n_d), ("rr", w.n_r)):
+        for rows in sample_blocks(n, width):
+            got_c, got_w, _ = count(acf, ctx, d, which, rows=rows)
+            want = oracle_rows(oracle, d, which, rows)
+            if weighted:
+                assert got_c.tolist() == want[0].tolist(), (which, rows)
+                np.testing.assert_allclose(got_w, want[1], rtol=WSUM_RTOL, atol=0, err_msg="%s %s" % (which, rows))
+            else:
+                assert got_c.tolist() == want.tolist(), (which, rows)
+
+    # ---- the full calls, as bench.py makes them
+    full = {k: count(acf, ctx, d, k) for k in ("dd", "dr", "rr")}
+    for k, (c, s, st) in full.items():
+        n_a = w.n_d if k != "rr" else w.n_r
+        nominal = n_a * (n_a - 1) // 2 if k != "dr" else w.n_d * w.n_r
+        assert st["pairs_nominal"] == nominal and 0 < st["pairs_evaluated"] <= nominal
+        assert int(c.sum()) <= nominal
+    # window path == table path (independent classification code), bit for bit
+    for k in ("dd", "dr"):
+        c2, s2, st2 = count(acf, ctx, d, k, windows=0)
+        assert st2["pairs_window"] == 0
+        assert c2.tolist() == full[k][0].tolist(), k
+        if weighted:
+            np.testing.assert_allclose(s2, full[k][1], rtol=WSUM_RTOL, atol=0)
+    # swapping the catalogues of a cross count changes every tile, window and work item, not the result
+    c3, s3, _ = count(acf, ctx, d, "rd")
+    assert c3.tolist() == full["dr"][0].tolist()
+    if weighted:
+        np.testing.assert_allclose(s3, full["dr"][1], rtol=WSUM_RTOL, atol=0)
+    # additivity over row blocks
+    cut = (w.n_d // 3 // 1000) * 1000 + 17
+    parts = count(acf, ctx, d, "dd", rows=(0, cut))[0] + count(acf, ctx, d, "dd", rows=(cut, w.n_d))[0]
+    assert parts.tolist() == full["dd"][0].tolist()
+
+    if name == "full_sky":
+        # uniform sphere: cos(theta) is uniform on [-1, 1] => E[count_k] = N_pairs (e_k - e_k+1) / 2
+        e = w.cos_edges
+        for k, npairs in (("dd", w.n_d * (w.n_d - 1) // 2), ("dr", w.n_d * w.n_r)):
+            expect = npairs * (e[:-1] - e[1:]) / 2.0
+            assert np.all(np.abs(full[k][0].astype(np.float64) - expect) <= 6.0 * np.sqrt(expect) + 1.0)
+            # the range starts at 1 arcmin: the pairs closer than that are the only ones missing
+            assert npairs - int(full[k][0].sum()) <= 12 * npairs * (1.0 - e[0]) / 2.0 + 50
+        # weighted: E[w_i w_j] = exp(sigma^2) for independent lognormal(0, sigma) weights
+        ratio = full["dr"][1] / np.maximum(1, full["dr"][0])
+        big = full["dr"][0] > 10 ** 8
+        assert np.all(np.abs(ratio[big] / np.exp(0.09) - 1.0) < 5e-3)
+    # the estimator through the library and the oracle on the same counts
+    wt = acf.acf_wtheta(full["dd"][0], full["dr"][0], full["rr"][0], w.n_d, w.n_r)
+    wo = oracle.wtheta(full["dd"][0], full["dr"][0], full["rr"][0], w.n_d, w.n_r)
+    np.testing.assert_allclose(wt, wo, rtol=0, atol=1e-10, equal_nan=True)
