@@ -191,7 +191,7 @@ def main():
     flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device=dev)  # > 126 MB L2
     stream = torch.cuda.current_stream(dev)
 
-    stats_acc = {"launches": 0, "pair_ms": 0.0, "device_ms": 0.0, "evaluated": 0, "fp64": 0}
+    stats_acc = {"launches": 0, "pair_ms": 0.0, "device_ms": 0.0, "evaluated": 0, "fp64": 0, "window": 0}
 
     def step(collect: bool):
         calls = [(xd, wd, None, None, True, 0), (xd, wd, xr, wr, False, 1), (xr, wr, None, None, True, 2)]
@@ -207,6 +207,7 @@ def main():
                 stats_acc["device_ms"] += st["device_ms"]
                 stats_acc["evaluated"] += st["pairs_evaluated"]
                 stats_acc["fp64"] += st["pairs_fp64"]
+                stats_acc["window"] += st["pairs_window"]
 
     for _ in range(args.warmup):
         step(False)
@@ -312,7 +313,7 @@ def main():
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * args.steps, "roofline": roofline,
             "cpu_baseline": cpu_baseline,
             "detail": {"ms_steps": ms_steps, "wall_s_timed_region": t_wall, "pairs_fp64_per_step": stats_acc["fp64"],
-                       "pairs_evaluated_per_step": evaluated_per_step, "launches_per_step": launches_per_step,
+                       "pairs_evaluated_per_step": evaluated_per_step, "pairs_single_edge_window_per_step": stats_acc["window"], "launches_per_step": launches_per_step,
                        "version": P.acf_version()},
         }
         print(json.dumps(out), flush=True)
