@@ -85,6 +85,9 @@ extern "C" void acf_destroy(acf_ctx *ctx)
         ctx->s_keys[i].release();
         ctx->s_caps[i].release();
         ctx->s_gcaps[i].release();
+        ctx->s_pts2[i].release();
+        ctx->s_vj[i].release();
+        ctx->s_pack[i].release();
     }
     ctx->s_work.release();
     ctx->s_misc.release();

@@ -66,6 +66,15 @@ struct GroupCap {
     double cx, cy, cz, cos_r, sin_r, wsum;
 };
 
+// How the window path tallies a catalogue's weights when it is the j side (written on the device by
+// the gather kernel from the weight range).  vj[s] = C + w_s when packed (count and weight sum of the
+// pairs above an edge share one fp64 accumulator: sum = n * C + sum of w, exact while
+// exponent(w_max) - exponent(w_min > 0) <= 13), else vj[s] = w_s and the count is kept apart.
+struct PackInfo {
+    double C, inv_C;
+    int packed, pad;
+};
+
 // One catalogue prepared for the fast path (all device pointers live in ctx scratch).
 struct Prepared {
     const double *xyz = nullptr;  // caller's canonical fp64 SoA (not owned)
@@ -73,6 +82,9 @@ struct Prepared {
     size_t stride = 0;            // points in the caller's catalogue (SoA stride)
     size_t n = 0;                 // points prepared
     float4 *pts = nullptr;        // spatially sorted fp32 {x, y, z, w}; padded to a tile multiple
+    float *pts2 = nullptr;        // the same points, two by two: {x0, x1, y0, y1, z0, z1, w0, w1} (the staged j side)
+    double *vj = nullptr;         // per sorted point: C + w or w (see PackInfo); padded like pts
+    PackInfo *pack = nullptr;
     uint32_t *perm = nullptr;     // sorted position -> original index
     double4 *caps = nullptr;      // per tile: unit centre (x, y, z) and cos of the bounding radius
     GroupCap *gcaps = nullptr;    // per group of kGroup points (kGroupsPerTile per tile)
@@ -108,6 +120,9 @@ struct acf_ctx {
     acf::Scratch s_keys[2];          // sort keys (double-buffered inside)
     acf::Scratch s_caps[2];          // tile caps
     acf::Scratch s_gcaps[2];         // group caps
+    acf::Scratch s_pts2[2];          // paired layout of the sorted points
+    acf::Scratch s_vj[2];            // fp64 window-path weights
+    acf::Scratch s_pack[2];          // PackInfo + weight-range words
     acf::Scratch s_work;             // work list
     acf::Scratch s_misc;             // radix-sort histograms etc.
     acf::Scratch s_host_stage[6];    // acf_correlate_host: device copies of xyz / weights / outputs

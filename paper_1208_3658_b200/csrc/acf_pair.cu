@@ -55,11 +55,18 @@ constexpr int kSmemHeader = 512;   // mbarriers + stage descriptors
 // [three roundings of values of magnitude <= 2] = 3.3e-7.
 constexpr float kGuardWin = 4.5e-7f;
 constexpr int kWinUnroll = 4;  // j-points per guard-band vote
+// one staged j-tile: the paired fp32 records, then (weighted) the fp64 window-path weights
+constexpr size_t kTileBytes = (size_t)kTile * sizeof(float4);
+constexpr size_t kVjBytes = (size_t)kTile * sizeof(double);
+__host__ __device__ constexpr size_t stage_bytes(bool weighted) { return kTileBytes + (weighted ? kVjBytes : 0); }
 static_assert(kGroup == kR * 32, "a warp's i-points are one group");
 static_assert(kGroup % kWinUnroll == 0, "");
 
 struct PairParams {
-    const float4 *pts_a, *pts_b;
+    const float4 *pts_a;
+    const float *pts2_b;    // j side, two points per record {x0, x1, y0, y1, z0, z1, w0, w1}
+    const double *vj_b;     // j side window-path weights (PackInfo)
+    const PackInfo *pack_b;
     const uint32_t *perm_a, *perm_b;
     const GroupCap *gcaps_a, *gcaps_b;
     uint32_t n_a, n_b;
@@ -111,6 +118,24 @@ __device__ __forceinline__ void bulk_load(void *dst, const void *src, uint32_t b
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
                  "l"(src), "r"(bytes), "r"(smem_u32(bar))
                  : "memory");
+}
+
+__device__ __forceinline__ unsigned long long pack2(float lo, float hi)
+{
+    return ((unsigned long long)__float_as_uint(hi) << 32) | __float_as_uint(lo);
+}
+// two fp32 FMAs in one instruction (SASS FFMA2): each half is the IEEE fma of its operands
+__device__ __forceinline__ unsigned long long ffma2(unsigned long long a, unsigned long long b, unsigned long long c)
+{
+    unsigned long long d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+// point jj of a staged tile in the paired layout
+__device__ __forceinline__ float4 tile_point(const float *__restrict__ tile2, int jj)
+{
+    const float *pp = tile2 + (size_t)(jj >> 1) * 8 + (jj & 1);
+    return make_float4(pp[0], pp[2], pp[4], pp[6]);
 }
 
 // Exact histogram row of a pair: the definition of include/acf.h on the caller's doubles.
@@ -165,21 +190,22 @@ __device__ __forceinline__ uint32_t local_i(int r) { return (threadIdx.x >> 5) *
 
 // Table path: j-points [jj0, jj0 + jn) of the staged tile against the kR register-resident i-points.
 template <bool kWeighted, bool kPrivate, bool kMasked>
-__device__ __forceinline__ void process_tile(const PairParams &p, Hist<kWeighted, kPrivate> &h, const float4 *__restrict__ tile,
-                                             int jj0, int jn, const float (&nx)[kR], const float (&ny)[kR], const float (&nz)[kR],
+__device__ __forceinline__ void process_tile(const PairParams &p, Hist<kWeighted, kPrivate> &h, const float *__restrict__ tile2,
+                                             int jj0, int jn, const unsigned long long (&nx2)[kR], const unsigned long long (&ny2)[kR], const unsigned long long (&nz2)[kR],
                                              const float (&wi)[kR], const uint2 *__restrict__ lut, uint32_t i_base,
                                              uint32_t j_base, bool diag, uint32_t valid_mask, unsigned long long &n_fp64)
 {
     const int shift = p.shift, key0 = p.key0;
 #pragma unroll 2
     for (int jj = jj0; jj < jj0 + jn; ++jj) {
-        const float4 q = tile[jj];
+        const float4 q = tile_point(tile2, jj);
         bool amb_any = false;
         bool amb[kR];
         uint32_t row[kR];
 #pragma unroll
         for (int r = 0; r < kR; ++r) {
-            const float t = fmaf(nx[r], q.x, fmaf(ny[r], q.y, fmaf(nz[r], q.z, kK)));
+            const float t = fmaf(__uint_as_float((uint32_t)nx2[r]), q.x,
+                                 fmaf(__uint_as_float((uint32_t)ny2[r]), q.y, fmaf(__uint_as_float((uint32_t)nz2[r]), q.z, kK)));
             const uint2 e = lut[(int)(__float_as_uint(t) >> shift) - key0];
             const float thr = __uint_as_float(e.x);
             row[r] = e.y + (t > thr ? 1u : 0u);
@@ -258,52 +284,76 @@ __device__ __forceinline__ Window make_window(const GroupCap &a, const GroupCap 
 }
 
 // One group of kGroup staged j-points against this thread's kR i-points, every pair tested against
-// the single edge of the window.  Tallies stay in registers and are added to the histogram rows
-// `edge` and `edge + 1` at the end.
-template <bool kWeighted, bool kPrivate>
-__device__ __forceinline__ void window_group(const PairParams &p, Hist<kWeighted, kPrivate> &h, const float4 *__restrict__ grp,
-                                             const float (&nx)[kR], const float (&ny)[kR], const float (&nz)[kR],
-                                             const float (&wi)[kR], const Window win, uint32_t i_base, uint32_t j_first,
-                                             unsigned long long &n_fp64)
+// the single edge of the window.  Two j-points per step: d = e_m - c for both in three FFMA2.
+// Tallies stay in registers and are added to the histogram rows `edge` and `edge + 1` at the end:
+//   weighted: per i-point one fp64 accumulator t += ind * v_j, where ind = 2^-7 [d > 0] is the
+//             float 1.0f / 0.0f of the comparison read as the high word of a double, and
+//             v_j = C + w_j (packed: 128 t = n C + sum of w_j, both recovered exactly) or v_j = w_j
+//             (count kept in a float beside it);
+//   unweighted: the sign bits of d are shifted into a word per i-point and counted 32 at a time.
+// |d| <= G1 for any pair of a step of kWinUnroll j-points sends that step's pairs to the exact row.
+template <bool kWeighted, bool kPacked, bool kPrivate>
+__device__ __forceinline__ void window_group(const PairParams &p, Hist<kWeighted, kPrivate> &h, const float *__restrict__ grp2,
+                                             const double *__restrict__ vgrp, const unsigned long long (&nx2)[kR],
+                                             const unsigned long long (&ny2)[kR], const unsigned long long (&nz2)[kR],
+                                             const float (&wi)[kR], const Window win, const double packC, const double inv_packC,
+                                             uint32_t i_base, uint32_t j_first, unsigned long long &n_fp64)
 {
     const float e32 = win.e32;
-    float n_above = 0.f;  // exact: at most kGroup * kR = 512
-    double t_above[kR];   // per i-point: sum of w_j over its pairs above the edge
+    const unsigned long long e2 = pack2(e32, e32);
+    double t_above[kR];   // weighted: 2^-7 * sum of v_j over the pairs above the edge, per i-point
+    uint32_t sg[kR];      // unweighted: sign bits of d (1 = not above) of the last 32 j-points, per i-point
+    uint32_t n_below = 0; // unweighted
+    float n_above = 0.f;  // weighted, not packed: exact, at most kGroup * kR = 512
 #pragma unroll
-    for (int r = 0; r < kR; ++r) t_above[r] = 0.0;
+    for (int r = 0; r < kR; ++r) {
+        t_above[r] = 0.0;
+        sg[r] = 0u;
+    }
 #pragma unroll 1
     for (int jj = 0; jj < kGroup; jj += kWinUnroll) {
-        bool amb = false;
+        float mn = 1.0f;  // min |d| of the step
 #pragma unroll
-        for (int u = 0; u < kWinUnroll; ++u) {
-            const float4 q = grp[jj + u];
-            const double wj = (double)q.w;
+        for (int u = 0; u < kWinUnroll; u += 2) {
+            const ulonglong2 xy = *reinterpret_cast<const ulonglong2 *>(grp2 + (size_t)(jj + u) * 4);
+            const unsigned long long zz = *reinterpret_cast<const unsigned long long *>(grp2 + (size_t)(jj + u) * 4 + 4);
+            double v0 = 0.0, v1 = 0.0;
+            if constexpr (kWeighted) {
+                const double2 vv = *reinterpret_cast<const double2 *>(vgrp + jj + u);
+                v0 = vv.x;
+                v1 = vv.y;
+            }
 #pragma unroll
             for (int r = 0; r < kR; ++r) {
-                const float d = fmaf(nx[r], q.x, fmaf(ny[r], q.y, fmaf(nz[r], q.z, e32)));
-                amb |= !(fabsf(d) > kGuardWin);
-                // n_above += d > 0; t_above[r] += d > 0 ? w_j : 0 -- as predicated adds (one FSETP, no selects)
-                if constexpr (kWeighted)
-                    asm("{\n\t.reg .pred above;\n\tsetp.gt.f32 above, %2, 0f00000000;\n\t@above add.f32 %0, %0, 0f3F800000;\n\t"
-                        "@above add.f64 %1, %1, %3;\n\t}"
-                        : "+f"(n_above), "+d"(t_above[r])
-                        : "f"(d), "d"(wj));
-                else
-                    asm("{\n\t.reg .pred above;\n\tsetp.gt.f32 above, %1, 0f00000000;\n\t@above add.f32 %0, %0, 0f3F800000;\n\t}"
-                        : "+f"(n_above)
-                        : "f"(d));
+                const unsigned long long d2 = ffma2(nx2[r], xy.x, ffma2(ny2[r], xy.y, ffma2(nz2[r], zz, e2)));
+                const float d0 = __uint_as_float((uint32_t)d2), d1 = __uint_as_float((uint32_t)(d2 >> 32));
+                if constexpr (kWeighted) {
+                    float i0, i1;  // 1.0f if above else 0.0f (SASS FSET.BF)
+                    asm("set.gt.f32.f32 %0, %1, 0f00000000;" : "=f"(i0) : "f"(d0));
+                    asm("set.gt.f32.f32 %0, %1, 0f00000000;" : "=f"(i1) : "f"(d1));
+                    t_above[r] = fma(v0, __hiloint2double(__float_as_int(i0), 0), t_above[r]);
+                    t_above[r] = fma(v1, __hiloint2double(__float_as_int(i1), 0), t_above[r]);
+                    if constexpr (!kPacked) n_above += i0 + i1;
+                } else {
+                    asm("shf.l.wrap.b32 %0, %1, %0, 1;" : "+r"(sg[r]) : "r"(__float_as_uint(d0)));
+                    asm("shf.l.wrap.b32 %0, %1, %0, 1;" : "+r"(sg[r]) : "r"(__float_as_uint(d1)));
+                }
+                asm("min.f32 %0, %0, %1, %2;" : "+f"(mn) : "f"(fabsf(d0)), "f"(fabsf(d1)));
             }
         }
-        if (__any_sync(0xffffffffu, amb)) {
+        if (__any_sync(0xffffffffu, !(mn > kGuardWin))) {
             // some pair is within the guard band of the edge: replace its row by the exact one
 #pragma unroll 1
             for (int u = 0; u < kWinUnroll; ++u) {
-                const float4 q = grp[jj + u];
+                const float4 q = tile_point(grp2, jj + u);
 #pragma unroll
                 for (int r = 0; r < kR; ++r) {
-                    const float d = fmaf(nx[r], q.x, fmaf(ny[r], q.y, fmaf(nz[r], q.z, e32)));
+                    const float d = fmaf(__uint_as_float((uint32_t)nx2[r]), q.x,
+                                         fmaf(__uint_as_float((uint32_t)ny2[r]), q.y, fmaf(__uint_as_float((uint32_t)nz2[r]), q.z, e32)));
                     if (fabsf(d) > kGuardWin) continue;
-                    const uint32_t fast = (uint32_t)win.edge + (d > 0.f ? 1u : 0u);
+                    // what the loop above tallied for this pair
+                    const bool above = kWeighted ? d > 0.f : (__float_as_uint(d) >> 31) == 0u;
+                    const uint32_t fast = (uint32_t)win.edge + (above ? 1u : 0u);
                     const uint32_t exact = (uint32_t)exact_row(p.xyz_a, p.stride_a, p.perm_a[i_base + local_i(r)], p.xyz_b, p.stride_b,
                                                                p.perm_b[j_first + jj + u], p.edges, p.nbins);
                     if (exact != fast) {
@@ -318,22 +368,36 @@ __device__ __forceinline__ void window_group(const PairParams &p, Hist<kWeighted
                 }
             }
         }
+        if constexpr (!kWeighted) {
+            if ((jj & 31) == 32 - kWinUnroll) {
+#pragma unroll
+                for (int r = 0; r < kR; ++r) n_below += __popc(sg[r]);
+            }
+        }
     }
-    const uint32_t above = (uint32_t)n_above, total = (uint32_t)(kGroup * kR);
-    h.add_n((uint32_t)win.edge + 1u, above);
-    h.add_n((uint32_t)win.edge, total - above);
+    const uint32_t total = (uint32_t)(kGroup * kR);
+    uint32_t above = total - n_below;
     if constexpr (kWeighted) {
         // sum over this thread's pairs of w_i w_j = sum_r w_i[r] * (sum of w_j above / not above)
         double s_above = 0.0, s_below = 0.0;
+        above = kPacked ? 0u : (uint32_t)n_above;
 #pragma unroll
         for (int r = 0; r < kR; ++r) {
-            s_above = fma((double)wi[r], t_above[r], s_above);
-            s_below = fma((double)wi[r], win.wsum - t_above[r], s_below);
+            double sw = t_above[r] * 128.0;  // undo the 2^-7 of the indicator
+            if constexpr (kPacked) {
+                const double n = floor(sw * inv_packC);  // C is a power of two and sum of w < C: exact
+                sw -= n * packC;
+                above += (uint32_t)n;
+            }
+            s_above = fma((double)wi[r], sw, s_above);
+            s_below = fma((double)wi[r], win.wsum - sw, s_below);
         }
-        if (above == total) s_below = 0.0;  // nothing below: not even a rounding residue of wsum - t_above
+        if (above == total) s_below = 0.0;  // nothing below: not even a rounding residue of wsum - sw
         h.add_w((uint32_t)win.edge + 1u, s_above);
         h.add_w((uint32_t)win.edge, s_below);
     }
+    h.add_n((uint32_t)win.edge + 1u, above);
+    h.add_n((uint32_t)win.edge, total - above);
 }
 
 // ---- the kernel ---------------------------------------------------------------------------------
@@ -358,10 +422,11 @@ __global__ void __launch_bounds__(kThreads + 32, kWeighted ? 1 : 2) pair_kernel(
     uint64_t *full = reinterpret_cast<uint64_t *>(smem);
     uint64_t *empty = full + kMaxStages;
     StageMeta *meta = reinterpret_cast<StageMeta *>(smem + 128);
-    float4 *tiles = reinterpret_cast<float4 *>(smem + kSmemHeader);
-    uint2 *lut = reinterpret_cast<uint2 *>(smem + kSmemHeader + (size_t)n_stages * kTile * sizeof(float4));
+    unsigned char *stages = smem + kSmemHeader;
+    constexpr size_t kStage = stage_bytes(kWeighted);
+    uint2 *lut = reinterpret_cast<uint2 *>(smem + kSmemHeader + (size_t)n_stages * kStage);
     const size_t cnt_words = kPrivate ? (size_t)kWarps * rows * 32 : (size_t)kWarps * rows;
-    size_t off = kSmemHeader + (size_t)n_stages * kTile * sizeof(float4) + (size_t)p.lut_len * sizeof(uint2);
+    size_t off = kSmemHeader + (size_t)n_stages * kStage + (size_t)p.lut_len * sizeof(uint2);
     off = (off + 15) & ~size_t(15);
     uint32_t *cnt_all = reinterpret_cast<uint32_t *>(smem + off);
     off += cnt_words * sizeof(uint32_t);
@@ -410,8 +475,11 @@ __global__ void __launch_bounds__(kThreads + 32, kWeighted ? 1 : 2) pair_kernel(
                 m.jn = (int)jn;
                 m.pad = 0;
                 meta[slot] = m;
-                mbar_expect_tx(&full[slot], jn * (uint32_t)sizeof(float4));
-                bulk_load(tiles + (size_t)slot * kTile, p.pts_b + (size_t)j0, jn * (uint32_t)sizeof(float4), &full[slot]);
+                // the arrays are padded to whole tiles: always a full tile
+                mbar_expect_tx(&full[slot], (uint32_t)kStage);
+                bulk_load(stages + (size_t)slot * kStage, p.pts2_b + (size_t)j0 * 4, (uint32_t)kTileBytes, &full[slot]);
+                if constexpr (kWeighted)
+                    bulk_load(stages + (size_t)slot * kStage + kTileBytes, p.vj_b + (size_t)j0, (uint32_t)kVjBytes, &full[slot]);
                 ++produced;
             }
         }
@@ -432,9 +500,14 @@ __global__ void __launch_bounds__(kThreads + 32, kWeighted ? 1 : 2) pair_kernel(
 
     unsigned long long n_fp64 = 0, n_eval = 0, n_win = 0;
     unsigned long long since_flush = 0;  // pairs this warp has tallied in its unflushed shared rows
-    float nx[kR], ny[kR], nz[kR], wi[kR];
+    float wi[kR];
+    unsigned long long nx2[kR], ny2[kR], nz2[kR];  // {-x, -x} etc.: both halves of an FFMA2 see the same i-point
 #pragma unroll
-    for (int r = 0; r < kR; ++r) nx[r] = ny[r] = nz[r] = wi[r] = 0.f;
+    for (int r = 0; r < kR; ++r) {
+        wi[r] = 0.f;
+        nx2[r] = ny2[r] = nz2[r] = 0ull;
+    }
+    const PackInfo pack = *p.pack_b;
     uint32_t valid_mask = 0, i_base = 0, n_i = 0;
     bool i_full = false;
     int cur_ti = -1;
@@ -486,16 +559,17 @@ __global__ void __launch_bounds__(kThreads + 32, kWeighted ? 1 : 2) pair_kernel(
             for (int r = 0; r < kR; ++r) {
                 const uint32_t s = i_base + local_i(r);
                 const float4 v = p.pts_a[s];  // the array is padded to a whole tile
-                nx[r] = -v.x;
-                ny[r] = -v.y;
-                nz[r] = -v.z;
+                nx2[r] = pack2(-v.x, -v.x);
+                ny2[r] = pack2(-v.y, -v.y);
+                nz2[r] = pack2(-v.z, -v.z);
                 wi[r] = v.w;
                 valid_mask |= (s < p.n_a ? 1u : 0u) << r;
             }
             i_full = i_base + kTile <= p.n_a;
             n_i = i_full ? kTile : p.n_a - i_base;
         }
-        const float4 *tile = tiles + (size_t)slot * kTile;
+        const float *tile = reinterpret_cast<const float *>(stages + (size_t)slot * kStage);
+        const double *vtile = reinterpret_cast<const double *>(stages + (size_t)slot * kStage + kTileBytes);
         const int tj = m.tj, jn = m.jn;
         const bool diag = p.is_auto && tj == m.ti;
         const uint32_t j_base = (uint32_t)tj * kTile;
@@ -504,9 +578,9 @@ __global__ void __launch_bounds__(kThreads + 32, kWeighted ? 1 : 2) pair_kernel(
         since_flush += (unsigned long long)kGroup * (unsigned)jn;
 
         if (diag || !i_full) {
-            process_tile<kWeighted, kPrivate, true>(p, h, tile, 0, jn, nx, ny, nz, wi, lut, i_base, j_base, diag, valid_mask, n_fp64);
+            process_tile<kWeighted, kPrivate, true>(p, h, tile, 0, jn, nx2, ny2, nz2, wi, lut, i_base, j_base, diag, valid_mask, n_fp64);
         } else if (!p.use_windows) {
-            process_tile<kWeighted, kPrivate, false>(p, h, tile, 0, jn, nx, ny, nz, wi, lut, i_base, j_base, false, valid_mask, n_fp64);
+            process_tile<kWeighted, kPrivate, false>(p, h, tile, 0, jn, nx2, ny2, nz2, wi, lut, i_base, j_base, false, valid_mask, n_fp64);
         } else {
             // lane g works out the window of this warp's i-group against j-group g of the tile
             const int n_groups = (jn + kGroup - 1) / kGroup;
@@ -523,11 +597,16 @@ __global__ void __launch_bounds__(kThreads + 32, kWeighted ? 1 : 2) pair_kernel(
                 win.e32 = __shfl_sync(0xffffffffu, mine.e32, g);
                 win.wsum = __shfl_sync(0xffffffffu, mine.wsum, g);
                 if (win.edge >= 0) {
-                    window_group<kWeighted, kPrivate>(p, h, tile + g * kGroup, nx, ny, nz, wi, win, i_base, j_base + g * kGroup, n_fp64);
+                    if (!kWeighted || pack.packed)
+                        window_group<kWeighted, true, kPrivate>(p, h, tile + (size_t)g * kGroup * 4, vtile + g * kGroup, nx2, ny2, nz2, wi, win,
+                                                                pack.C, pack.inv_C, i_base, j_base + g * kGroup, n_fp64);
+                    else
+                        window_group<kWeighted, false, kPrivate>(p, h, tile + (size_t)g * kGroup * 4, vtile + g * kGroup, nx2, ny2, nz2, wi, win,
+                                                                 pack.C, pack.inv_C, i_base, j_base + g * kGroup, n_fp64);
                     n_win += (unsigned long long)(kGroup * kR);
                 } else {
                     const int gn = jn - g * kGroup < kGroup ? jn - g * kGroup : kGroup;
-                    process_tile<kWeighted, kPrivate, false>(p, h, tile, g * kGroup, gn, nx, ny, nz, wi, lut, i_base, j_base, false, valid_mask, n_fp64);
+                    process_tile<kWeighted, kPrivate, false>(p, h, tile, g * kGroup, gn, nx2, ny2, nz2, wi, lut, i_base, j_base, false, valid_mask, n_fp64);
                 }
             }
         }
@@ -642,7 +721,7 @@ int count_prepared(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_au
     // unweighted and small enough, else 1)
     const size_t cnt_words = priv ? (size_t)kWarps * rows * 32 : (size_t)kWarps * rows;
     auto smem_for = [&](int stages) {
-        size_t m = kSmemHeader + (size_t)stages * kTile * sizeof(float4) + L.cells.size() * sizeof(uint2);
+        size_t m = kSmemHeader + (size_t)stages * stage_bytes(weighted) + L.cells.size() * sizeof(uint2);
         m = (m + 15) & ~size_t(15);
         m += cnt_words * sizeof(uint32_t);
         m = (m + 15) & ~size_t(15);
@@ -669,7 +748,9 @@ int count_prepared(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_au
 
     PairParams p{};
     p.pts_a = a.pts;
-    p.pts_b = b.pts;
+    p.pts2_b = b.pts2;
+    p.vj_b = b.vj;
+    p.pack_b = b.pack;
     p.perm_a = a.perm;
     p.perm_b = b.perm;
     p.gcaps_a = a.gcaps;

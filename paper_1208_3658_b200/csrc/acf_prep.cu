@@ -155,6 +155,28 @@ radix_scatter_kernel(const uint32_t *__restrict__ keys_in, const uint32_t *__res
     }
 }
 
+// ------------------------------------------------------------------ weight range
+// range[0] = max of the weights' float bits, range[1] = max of ~bits over the non-zero weights (so that
+// both start from a zeroed buffer).  Weights are non-negative and finite (validate_kernel), so the
+// bit patterns order like the values.
+__global__ void __launch_bounds__(256) wrange_kernel(const float *__restrict__ w, size_t off, uint32_t n, uint32_t *__restrict__ range)
+{
+    uint32_t mx = 0u, inv_mn = 0u;
+    for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n; i += gridDim.x * blockDim.x) {
+        const uint32_t bits = __float_as_uint(w[off + i]) & 0x7fffffffu;
+        if (bits) {
+            mx = max(mx, bits);
+            inv_mn = max(inv_mn, ~bits);
+        }
+    }
+    mx = __reduce_max_sync(0xffffffffu, mx);
+    inv_mn = __reduce_max_sync(0xffffffffu, inv_mn);
+    if ((threadIdx.x & 31) == 0 && mx) {
+        atomicMax(&range[0], mx);
+        atomicMax(&range[1], inv_mn);
+    }
+}
+
 // ------------------------------------------------------------------ gather + caps
 // One CTA per tile of kTile sorted points, one warp per group of kGroup points: writes the fp32 float4
 // records, the tile's bounding cap {unit centre, cos(radius)} and the kGroupsPerTile group caps, all
@@ -162,7 +184,9 @@ radix_scatter_kernel(const uint32_t *__restrict__ keys_in, const uint32_t *__res
 __global__ void __launch_bounds__(256)
 gather_caps_kernel(const double *__restrict__ xyz, size_t stride, size_t off, const float *__restrict__ w,
                    const uint32_t *__restrict__ idx, uint32_t n, float4 *__restrict__ pts,
-                   uint32_t *__restrict__ perm, double4 *__restrict__ caps, GroupCap *__restrict__ gcaps)
+                   uint32_t *__restrict__ perm, double4 *__restrict__ caps, GroupCap *__restrict__ gcaps,
+                   float *__restrict__ pts2, double *__restrict__ vj, const uint32_t *__restrict__ range,
+                   PackInfo *__restrict__ pack)
 {
     static_assert(kGroupsPerTile == 8 && kGroup == 128, "one warp of 256 threads per group");
     __shared__ double red[3][8];
@@ -172,9 +196,23 @@ gather_caps_kernel(const double *__restrict__ xyz, size_t stride, size_t off, co
     const uint32_t base = blockIdx.x * kTile + warp * kGroup;
     double px[kPer], py[kPer], pz[kPer];
     double sx = 0, sy = 0, sz = 0, sw = 0;
+    // window-path weights (PackInfo): C = 2^(exponent(w_max) + 9) > 256 w_max, a power of two
+    const uint32_t mx_bits = w ? range[0] : 0x3f800000u, mn_bits = w ? ~range[1] : 0x3f800000u;
+    const int ex_max = (int)(mx_bits >> 23), ex_min = (int)(mn_bits >> 23);
+    const bool packed = mx_bits != 0u && ex_min >= 1 && ex_max - ex_min <= 13;
+    const double packC = __hiloint2double((ex_max - 127 + 9 + 1023) << 20, 0);
+    if (blockIdx.x == 0 && threadIdx.x == 0) {
+        PackInfo pi;
+        pi.C = packC;
+        pi.inv_C = __hiloint2double((127 - 9 - ex_max + 1023) << 20, 0);
+        pi.packed = packed ? 1 : 0;
+        pi.pad = 0;
+        *pack = pi;
+    }
 #pragma unroll
     for (int r = 0; r < kPer; ++r) {
         const uint32_t s = base + r * 32 + lane;
+        float *p2 = pts2 + (size_t)(s >> 1) * 8 + (s & 1u);
         if (s < n) {
             const uint32_t local = idx[s];
             const size_t g = off + local;
@@ -183,6 +221,11 @@ gather_caps_kernel(const double *__restrict__ xyz, size_t stride, size_t off, co
             pz[r] = xyz[2 * stride + g];
             const float wi = w ? w[g] : 1.0f;
             pts[s] = make_float4((float)px[r], (float)py[r], (float)pz[r], wi);
+            p2[0] = (float)px[r];
+            p2[2] = (float)py[r];
+            p2[4] = (float)pz[r];
+            p2[6] = wi;
+            vj[s] = packed ? packC + (double)wi : (double)wi;
             perm[s] = (uint32_t)g;  // index into the caller's catalogue
             sx += px[r];
             sy += py[r];
@@ -191,6 +234,8 @@ gather_caps_kernel(const double *__restrict__ xyz, size_t stride, size_t off, co
         } else {
             px[r] = py[r] = pz[r] = 0.0;
             pts[s] = make_float4(0.f, 0.f, 0.f, 0.f);  // padding up to the tile boundary, never paired
+            p2[0] = p2[2] = p2[4] = p2[6] = 0.f;
+            vj[s] = 0.0;
         }
     }
 #pragma unroll
@@ -369,12 +414,19 @@ int prepare_catalogue(acf_ctx *ctx, int slot, const double *xyz, size_t stride, 
     ACF_CUDA_TRY(ctx, ctx->s_caps[slot].reserve(sizeof(double4) * (size_t)n_tiles));
     ACF_CUDA_TRY(ctx, ctx->s_gcaps[slot].reserve(sizeof(GroupCap) * (size_t)n_tiles * kGroupsPerTile));
     ACF_CUDA_TRY(ctx, ctx->s_keys[slot].reserve(sizeof(uint32_t) * 4 * (size_t)n));  // keys x2, idx x2
+    ACF_CUDA_TRY(ctx, ctx->s_pts2[slot].reserve(sizeof(float4) * padded));
+    ACF_CUDA_TRY(ctx, ctx->s_vj[slot].reserve(sizeof(double) * padded));
+    ACF_CUDA_TRY(ctx, ctx->s_pack[slot].reserve(64));
     const uint32_t nblocks = (n + kSortBlockChunk - 1) / kSortBlockChunk;
     ACF_CUDA_TRY(ctx, ctx->s_misc.reserve(sizeof(uint32_t) * 256 * (size_t)nblocks));
     out->pts = ctx->s_pts[slot].as<float4>();
     out->perm = ctx->s_perm[slot].as<uint32_t>();
     out->caps = ctx->s_caps[slot].as<double4>();
     out->gcaps = ctx->s_gcaps[slot].as<GroupCap>();
+    out->pts2 = ctx->s_pts2[slot].as<float>();
+    out->vj = ctx->s_vj[slot].as<double>();
+    out->pack = ctx->s_pack[slot].as<PackInfo>();
+    uint32_t *range = reinterpret_cast<uint32_t *>(ctx->s_pack[slot].as<char>() + 32);
     uint32_t *k0 = ctx->s_keys[slot].as<uint32_t>(), *k1 = k0 + n, *i0 = k1 + n, *i1 = i0 + n;
     uint32_t *counts = ctx->s_misc.as<uint32_t>();
 
@@ -391,7 +443,13 @@ int prepare_catalogue(acf_ctx *ctx, int slot, const double *xyz, size_t stride, 
         uint32_t *t = k0; k0 = k1; k1 = t;
         t = i0; i0 = i1; i1 = t;
     }
-    gather_caps_kernel<<<n_tiles, 256, 0, st>>>(xyz, stride, off, w, i0, n, out->pts, out->perm, out->caps, out->gcaps);
+    if (w) {
+        ACF_CUDA_TRY(ctx, cudaMemsetAsync(range, 0, 2 * sizeof(uint32_t), st));
+        wrange_kernel<<<blocks, 256, 0, st>>>(w, off, n, range);
+        ctx->last.kernel_launches++;
+    }
+    gather_caps_kernel<<<n_tiles, 256, 0, st>>>(xyz, stride, off, w, i0, n, out->pts, out->perm, out->caps, out->gcaps, out->pts2,
+                                               out->vj, range, out->pack);
     ctx->last.kernel_launches++;
     ACF_CUDA_TRY(ctx, cudaGetLastError());
     return ACF_OK;
