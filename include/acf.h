@@ -57,9 +57,13 @@ typedef struct acf_ctx acf_ctx; /* opaque; library-owned */
 
 /* Options for acf_set_option. */
 enum {
-    /* Which pair kernel runs.  ACF_KERNEL_AUTO (default) = the fast fp32-certify path;
-     * ACF_KERNEL_FP64 = the reference kernel that evaluates the definition in double for
-     * every pair (slow; the arbiter the fast path defers to, kept callable for debugging). */
+    /* Which pair kernel runs.  ACF_KERNEL_AUTO (default) = the fast fp32-certify path, choosing
+     * between its two kernels; ACF_KERNEL_FP64 = the reference kernel that evaluates the definition
+     * in double for every pair (slow; the arbiter the fast path defers to, kept callable for
+     * debugging); ACF_KERNEL_TABLE = fast path, cell-table kernel (single-edge windows in registers,
+     * everything else through a bin table and per-lane shared-memory histograms);
+     * ACF_KERNEL_WINDOW = fast path, window kernel (every group of pairs classified in registers
+     * against the few edges its bounding caps allow).  All four give the same counts. */
     ACF_OPT_KERNEL = 1,
     /* 1 (default): tile pairs that provably hold no in-range pair are skipped
      * ("ignoring calculations that would fall outside the bin range");
@@ -73,7 +77,7 @@ enum {
      * The counts are the same either way. */
     ACF_OPT_WINDOWS = 4
 };
-enum { ACF_KERNEL_AUTO = 0, ACF_KERNEL_FP64 = 1 };
+enum { ACF_KERNEL_AUTO = 0, ACF_KERNEL_FP64 = 1, ACF_KERNEL_TABLE = 2, ACF_KERNEL_WINDOW = 3 };
 
 /* Counters of the most recent acf_pair_count* call on a context. */
 typedef struct acf_stats {

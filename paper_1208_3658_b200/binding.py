@@ -14,7 +14,7 @@ import numpy as np
 
 ACF_OK, ACF_EINVAL, ACF_ENOMEM, ACF_ECUDA = 0, -1, -2, -3
 ACF_OPT_KERNEL, ACF_OPT_PRUNE, ACF_OPT_STATS, ACF_OPT_WINDOWS = 1, 2, 3, 4
-ACF_KERNEL_AUTO, ACF_KERNEL_FP64 = 0, 1
+ACF_KERNEL_AUTO, ACF_KERNEL_FP64, ACF_KERNEL_TABLE, ACF_KERNEL_WINDOW = 0, 1, 2, 3
 ACF_MAX_BINS = 1024
 
 _PKG = os.path.dirname(os.path.abspath(__file__))

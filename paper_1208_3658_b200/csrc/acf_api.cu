@@ -110,7 +110,7 @@ extern "C" int acf_set_option(acf_ctx *ctx, int option, int64_t value)
     if (!ctx) return ACF_EINVAL;
     switch (option) {
     case ACF_OPT_KERNEL:
-        if (value != ACF_KERNEL_AUTO && value != ACF_KERNEL_FP64) return acf::fail(ctx, ACF_EINVAL, "unknown kernel %lld", (long long)value);
+        if (value < ACF_KERNEL_AUTO || value > ACF_KERNEL_WINDOW) return acf::fail(ctx, ACF_EINVAL, "unknown kernel %lld", (long long)value);
         ctx->opt_kernel = (int)value;
         return ACF_OK;
     case ACF_OPT_PRUNE:
@@ -181,7 +181,7 @@ extern "C" int acf_pair_count_rows(acf_ctx *ctx, const double *d_a, const float 
                                           sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
         ACF_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_flag, st));
 
-        if (ctx->opt_kernel == ACF_KERNEL_AUTO) {
+        if (ctx->opt_kernel != ACF_KERNEL_FP64) {
             int rc = acf::run_pair_count_fast(ctx, d_a, d_wa, n_a, i_begin, i_end, d_b, d_wb, n_b, cos_edges, nbins,
                                               is_auto, reinterpret_cast<unsigned long long *>(d_counts), d_wsums);
             if (rc != ACF_OK) return rc;

@@ -165,6 +165,10 @@ int run_pair_count_fast(acf_ctx *ctx, const double *d_a, const float *d_wa, size
                         size_t i_end, const double *d_b, const float *d_wb, size_t n_b, const double *h_edges,
                         int nbins, int is_auto, unsigned long long *d_counts, double *d_wsums);
 
+// ---- acf_pair_win.cu: the window kernel on the work items already in ctx->s_work (edges in ctx->s_edges).
+int launch_pair_win(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_auto, int nbins, uint32_t capacity,
+                    unsigned long long *d_counts, double *d_wsums);
+
 // ---- acf_prep.cu: sort + gather + caps of points [off, off+cnt) of a catalogue with `stride` points;
 // and the work list of (i-tile, j-tile run) items for i-tiles [ti_begin, ti_end).
 int prepare_catalogue(acf_ctx *ctx, int slot, const double *xyz, size_t stride, size_t off, size_t cnt,

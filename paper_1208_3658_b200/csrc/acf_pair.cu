@@ -33,6 +33,7 @@
 
 #include "acf_device.cuh"
 #include "acf_internal.h"
+#include "acf_pair_common.cuh"
 
 namespace acf {
 
@@ -49,16 +50,10 @@ constexpr float kGuard = kDelta + 0x1p-23f;
 constexpr int kExpLo = -19;  // t32 >= K - (1 + 1e-6) - kDelta > 2^-19
 constexpr int kExpHi = 2;    // t32 < 4
 constexpr int kMaxPrivateRows = 64;
-constexpr int kMaxStages = 8;      // j-tile buffers of the producer/consumer ring (at least 2)
-constexpr int kSmemHeader = 512;   // mbarriers + stage descriptors
 // Window path: |d32 - (e_m - c64)| <= 2^-25 [fp32(e_m)] + 2u(1+1e-6) [input rounding] + 3 * 2^-24
 // [three roundings of values of magnitude <= 2] = 3.3e-7.
 constexpr float kGuardWin = 4.5e-7f;
 constexpr int kWinUnroll = 4;  // j-points per guard-band vote
-// one staged j-tile: the paired fp32 records, then (weighted) the fp64 window-path weights
-constexpr size_t kTileBytes = (size_t)kTile * sizeof(float4);
-constexpr size_t kVjBytes = (size_t)kTile * sizeof(double);
-__host__ __device__ constexpr size_t stage_bytes(bool weighted) { return kTileBytes + (weighted ? kVjBytes : 0); }
 static_assert(kGroup == kR * 32, "a warp's i-points are one group");
 static_assert(kGroup % kWinUnroll == 0, "");
 
@@ -85,70 +80,6 @@ struct PairParams {
     int use_windows;
     int n_stages;
 };
-
-__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
-
-__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
-}
-__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
-{
-    asm volatile(
-        "{\n"
-        ".reg .pred p;\n"
-        "WAIT_LOOP:\n"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
-        "@p bra WAIT_DONE;\n"
-        "bra WAIT_LOOP;\n"
-        "WAIT_DONE:\n"
-        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
-}
-// TMA 1-D bulk copy global -> shared, completion signalled on an mbarrier (SASS: UBLKCP)
-__device__ __forceinline__ void bulk_load(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
-{
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
-                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
-                 : "memory");
-}
-
-__device__ __forceinline__ unsigned long long pack2(float lo, float hi)
-{
-    return ((unsigned long long)__float_as_uint(hi) << 32) | __float_as_uint(lo);
-}
-// two fp32 FMAs in one instruction (SASS FFMA2): each half is the IEEE fma of its operands
-__device__ __forceinline__ unsigned long long ffma2(unsigned long long a, unsigned long long b, unsigned long long c)
-{
-    unsigned long long d;
-    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
-    return d;
-}
-// point jj of a staged tile in the paired layout
-__device__ __forceinline__ float4 tile_point(const float *__restrict__ tile2, int jj)
-{
-    const float *pp = tile2 + (size_t)(jj >> 1) * 8 + (jj & 1);
-    return make_float4(pp[0], pp[2], pp[4], pp[6]);
-}
-
-// Exact histogram row of a pair: the definition of include/acf.h on the caller's doubles.
-__device__ __noinline__ int exact_row(const double *__restrict__ xyz_a, size_t stride_a, size_t gi,
-                                      const double *__restrict__ xyz_b, size_t stride_b, size_t gj,
-                                      const double *__restrict__ edges, int nbins)
-{
-    const double c = pair_cos_fp64(xyz_a[gi], xyz_a[stride_a + gi], xyz_a[2 * stride_a + gi], xyz_b[gj],
-                                   xyz_b[stride_b + gj], xyz_b[2 * stride_b + gj]);
-    const int k = bin_of_fp64(c, edges, nbins);
-    if (k >= 0) return k + 1;
-    return c > edges[0] ? 0 : nbins + 1;
-}
 
 template <bool kWeighted, bool kPrivate>
 struct Hist {
@@ -239,18 +170,6 @@ __device__ __forceinline__ void process_tile(const PairParams &p, Hist<kWeighted
 }
 
 // ---- window path --------------------------------------------------------------------------------
-// Histogram row of a cosine (the definition of include/acf.h): 0 if c > e[0]; nbins + 1 if c < e[nbins];
-// else 1 + its bin.  Equals #{m <= nbins - 1 : c <= e[m]} + [c < e[nbins]], non-increasing in c.
-__device__ __forceinline__ int row_of_cos(double c, const double *__restrict__ e, int nbins)
-{
-    int lo = 0, hi = nbins;  // c <= e[m] for m < lo; c > e[m] for m >= hi
-    while (lo < hi) {
-        const int mid = (lo + hi) >> 1;
-        if (c <= e[mid]) lo = mid + 1; else hi = mid;
-    }
-    return lo + ((lo == nbins && c < e[nbins]) ? 1 : 0);
-}
-
 struct Window {
     int edge;    // m: the one edge pairs of this window are tested against, or -1: take the table path
     float e32;   // fp32(e[m])
@@ -266,16 +185,8 @@ __device__ __forceinline__ Window make_window(const GroupCap &a, const GroupCap 
     w.edge = -1;
     w.e32 = 0.f;
     w.wsum = b.wsum;
-    if (a.cos_r > 1.5 || b.cos_r > 1.5) return w;  // an empty group
-    if (a.cos_r + b.cos_r <= 0.0) return w;         // radii sum to pi or more: no bound
-    const double d = fmin(1.0, fmax(-1.0, a.cx * b.cx + a.cy * b.cy + a.cz * b.cz));
-    const double C = a.cos_r * b.cos_r - a.sin_r * b.sin_r;  // cos(rho)
-    const double S = a.sin_r * b.cos_r + a.cos_r * b.sin_r;  // sin(rho) >= 0
-    const double sd = sqrt(fmax(0.0, 1.0 - d * d));
-    double c_hi = d >= C ? 1.0 : d * C + sd * S;
-    double c_lo = d <= -C ? -1.0 : d * C - sd * S;
-    c_hi = fmin(1.0, c_hi + 1e-9);  // rounding of the few operations above is ~1e-15
-    c_lo = fmax(-1.0, c_lo - 1e-9);
+    double c_lo, c_hi;
+    if (!cap_window(a, b, c_lo, c_hi)) return w;
     const int r_lo = row_of_cos(c_hi, edges, nbins), r_hi = row_of_cos(c_lo, edges, nbins);
     if (r_hi - r_lo > 1) return w;
     w.edge = r_lo <= nbins ? r_lo : nbins;  // rows edge (c > e[edge]) and edge + 1
@@ -407,9 +318,6 @@ __device__ __forceinline__ void window_group(const PairParams &p, Hist<kWeighted
 // {i-tile, j-tile, points}.  Every consumer warp walks the same stream at its own pace -- a warp whose
 // windows take the table path does not hold the others back until the ring is full -- holding its
 // kGroup i-points of the current i-tile in registers.
-struct StageMeta {
-    int ti, tj, jn, pad;
-};
 
 template <bool kWeighted, bool kPrivate>
 __global__ void __launch_bounds__(kThreads + 32, kWeighted ? 1 : 2) pair_kernel(const PairParams p)
@@ -787,9 +695,15 @@ int count_prepared(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_au
             ACF_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_k0, ctx->stream));
             ctx->pair_timed = true;
         }
-        if (weighted) e = priv ? launch<true, true>(ctx, p, smem, grid) : launch<true, false>(ctx, p, smem, grid);
-        else e = priv ? launch<false, true>(ctx, p, smem, grid) : launch<false, false>(ctx, p, smem, grid);
-        ACF_CUDA_TRY(ctx, e);
+        const bool use_win = ctx->opt_kernel == ACF_KERNEL_WINDOW || (ctx->opt_kernel == ACF_KERNEL_AUTO && weighted);
+        if (use_win) {
+            rc = launch_pair_win(ctx, a, b, is_auto, nbins, capacity, d_counts, d_wsums);
+            if (rc != ACF_OK) return rc;
+        } else {
+            if (weighted) e = priv ? launch<true, true>(ctx, p, smem, grid) : launch<true, false>(ctx, p, smem, grid);
+            else e = priv ? launch<false, true>(ctx, p, smem, grid) : launch<false, false>(ctx, p, smem, grid);
+            ACF_CUDA_TRY(ctx, e);
+        }
         ACF_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_k1, ctx->stream));
     }
     return ACF_OK;

@@ -1,0 +1,134 @@
+// acf_pair_common.cuh -- device helpers shared by the two pair kernels (acf_pair.cu: single-edge
+// windows + cell-table path; acf_pair_win.cu: windows of any number of edges).
+#pragma once
+
+#include <cuda_runtime.h>
+
+#include <cstdint>
+
+#include "acf_device.cuh"
+#include "acf_internal.h"
+
+namespace acf {
+
+constexpr int kMaxStages = 8;      // j-tile buffers of the producer/consumer ring (at least 2)
+constexpr int kSmemHeader = 512;   // mbarriers + stage descriptors
+// one staged j-tile: the paired fp32 records, then (weighted) the fp64 window-path weights
+constexpr size_t kTileBytes = (size_t)kTile * sizeof(float4);
+constexpr size_t kVjBytes = (size_t)kTile * sizeof(double);
+__host__ __device__ constexpr size_t stage_bytes(bool weighted) { return kTileBytes + (weighted ? kVjBytes : 0); }
+
+struct StageMeta {
+    int ti, tj, jn, pad;
+};
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p) { return (uint32_t)__cvta_generic_to_shared(p); }
+
+__device__ __forceinline__ void mbar_init(uint64_t *bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity)
+{
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_LOOP:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra WAIT_DONE;\n"
+        "bra WAIT_LOOP;\n"
+        "WAIT_DONE:\n"
+        "}\n" ::"r"(smem_u32(bar)), "r"(parity) : "memory");
+}
+// non-blocking: has the phase with this parity completed?
+__device__ __forceinline__ bool mbar_test(uint64_t *bar, uint32_t parity)
+{
+    uint32_t ok;
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "mbarrier.test_wait.parity.shared::cta.b64 p, [%1], %2;\n"
+        "selp.u32 %0, 1, 0, p;\n"
+        "}\n" : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
+    return ok != 0;
+}
+// TMA 1-D bulk copy global -> shared, completion signalled on an mbarrier (SASS: UBLKCP)
+__device__ __forceinline__ void bulk_load(void *dst, const void *src, uint32_t bytes, uint64_t *bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(dst)),
+                 "l"(src), "r"(bytes), "r"(smem_u32(bar))
+                 : "memory");
+}
+
+__device__ __forceinline__ unsigned long long pack2(float lo, float hi)
+{
+    return ((unsigned long long)__float_as_uint(hi) << 32) | __float_as_uint(lo);
+}
+// two fp32 FMAs in one instruction (SASS FFMA2): each half is the IEEE fma of its operands
+__device__ __forceinline__ unsigned long long ffma2(unsigned long long a, unsigned long long b, unsigned long long c)
+{
+    unsigned long long d;
+    asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(d) : "l"(a), "l"(b), "l"(c));
+    return d;
+}
+// point jj of a staged tile in the paired layout
+__device__ __forceinline__ float4 tile_point(const float *__restrict__ tile2, int jj)
+{
+    const float *pp = tile2 + (size_t)(jj >> 1) * 8 + (jj & 1);
+    return make_float4(pp[0], pp[2], pp[4], pp[6]);
+}
+
+// Exact histogram row of a pair: the definition of include/acf.h on the caller's doubles.
+static __device__ __noinline__ int exact_row(const double *__restrict__ xyz_a, size_t stride_a, size_t gi,
+                                      const double *__restrict__ xyz_b, size_t stride_b, size_t gj,
+                                      const double *__restrict__ edges, int nbins)
+{
+    const double c = pair_cos_fp64(xyz_a[gi], xyz_a[stride_a + gi], xyz_a[2 * stride_a + gi], xyz_b[gj],
+                                   xyz_b[stride_b + gj], xyz_b[2 * stride_b + gj]);
+    const int k = bin_of_fp64(c, edges, nbins);
+    if (k >= 0) return k + 1;
+    return c > edges[0] ? 0 : nbins + 1;
+}
+
+// Histogram row of a cosine (the definition of include/acf.h): 0 if c > e[0]; nbins + 1 if c < e[nbins];
+// else 1 + its bin.  Equals #{m <= nbins - 1 : c <= e[m]} + [c < e[nbins]], non-increasing in c.
+__device__ __forceinline__ int row_of_cos(double c, const double *__restrict__ e, int nbins)
+{
+    int lo = 0, hi = nbins;  // c <= e[m] for m < lo; c > e[m] for m >= hi
+    while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        if (c <= e[mid]) lo = mid + 1; else hi = mid;
+    }
+    return lo + ((lo == nbins && c < e[nbins]) ? 1 : 0);
+}
+
+
+// All pairs between points of caps a and b have c_lo <= cos(theta) <= c_hi (theta = angle between the
+// centres, rho = sum of the radii: cos(theta -+ rho) = cos(theta) cos(rho) +- sin(theta) sin(rho), clamped
+// at the poles, widened by 1e-9).  Returns false when the caps give no bound.
+__device__ __forceinline__ bool cap_window(const GroupCap &a, const GroupCap &b, double &c_lo, double &c_hi)
+{
+    c_lo = -1.0;
+    c_hi = 1.0;
+    if (a.cos_r > 1.5 || b.cos_r > 1.5) return false;  // an empty group
+    if (a.cos_r + b.cos_r <= 0.0) return false;         // radii sum to pi or more: no bound
+    const double d = fmin(1.0, fmax(-1.0, a.cx * b.cx + a.cy * b.cy + a.cz * b.cz));
+    const double C = a.cos_r * b.cos_r - a.sin_r * b.sin_r;  // cos(rho)
+    const double S = a.sin_r * b.cos_r + a.cos_r * b.sin_r;  // sin(rho) >= 0
+    const double sd = sqrt(fmax(0.0, 1.0 - d * d));
+    c_hi = d >= C ? 1.0 : d * C + sd * S;
+    c_lo = d <= -C ? -1.0 : d * C - sd * S;
+    c_hi = fmin(1.0, c_hi + 1e-9);  // rounding of the few operations above is ~1e-15
+    c_lo = fmax(-1.0, c_lo - 1e-9);
+    return true;
+}
+
+}  // namespace acf

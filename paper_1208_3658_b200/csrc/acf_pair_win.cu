@@ -1,0 +1,691 @@
+// acf_pair_win.cu -- the window kernel: every pair classified against the bin edges that can matter
+// for its window, tallies in registers, no per-pair shared-memory traffic.
+//
+// Points are sorted along a space-filling curve, so the kGroup i-points of a warp and a group of kGroup
+// staged j-points each sit in a small cap; the two caps bound the cosines of all their pairs to a window
+// [c_lo, c_hi] (fp64, rigorous), i.e. to the histogram rows r_lo .. r_hi and the k = r_hi - r_lo edges
+// e[r_lo] .. e[r_hi - 1] between them.  The edges are taken kChunk at a time.  Per pair and chunk:
+//   d_0 = e_m - (x_i x_j + y_i y_j + z_i z_j)      three fp32 FMAs seeded with fp32(e_m)  (two j-points per FFMA2)
+//   d_q = d_0 + fp32(e_{m+q} - e_m)                 one add per further edge of the chunk
+//   above_q = d_q > 0                               the pair lies in a row beyond edge m + q
+//   certified iff |d_q| > G for every q             else the exact fp64 row of include/acf.h decides
+// Per i-point and edge one fp64 accumulator takes t += [above_q] v_j (v_j = C + w_j packs the count and
+// the weight sum, see PackInfo; unweighted counts shift the sign bits of d_q into a word instead).
+// The accumulators are cumulative in q (above edge m + q implies above edge m + q - 1), so the rows get
+// the differences of consecutive edges; they are formed per i-point before anything is summed.
+// After a chunk the warp reduces its row tallies with shuffles and lane 0 adds them to the warp's rows in
+// shared memory; those go to global memory with u64 / f64 atomics (block histograms summed
+// into global memory -- here without a per-pair atomic, the 5-50 % serialisation the paper measures).
+// Ragged groups and the diagonal group of an auto-count (i < j) run the same loop with a per-pair mask.
+#include <cmath>
+#include <cstring>
+
+#include "acf_device.cuh"
+#include "acf_internal.h"
+#include "acf_pair_common.cuh"
+
+namespace acf {
+
+namespace {
+
+constexpr int kTeams = 2;              // teams of consumer warps: same i-points, alternate j-groups
+constexpr int kTeamWarps = kTile / kGroup;  // a team's warps hold the i-tile, kGroup points each
+constexpr int kWarps = kTeams * kTeamWarps;  // consumer warps
+constexpr int kThreads = 32 * kWarps;  // consumer threads
+constexpr int kR = kGroup / 32;        // i-points per thread
+#ifndef ACF_WIN_CHUNK
+#define ACF_WIN_CHUNK 3
+#endif
+constexpr int kChunk = ACF_WIN_CHUNK;  // edges per pass over a group
+constexpr int kStep = 4;               // j-points per guard-band vote
+// |d_0 - (e_m - c64)| <= 2^-25 [fp32(e_m)] + 2u(1+1e-6) [input rounding, u = 2^-24] + 3 * 2^-24 [three
+// roundings of values of magnitude <= 2] = 3.3e-7; d_q adds the rounding of the offset (<= 2^-24 * 2)
+// and of the sum (<= 2^-24 * 2): 5.7e-7.
+constexpr float kGuard1 = 4.5e-7f;
+constexpr float kGuardK = 7.0e-7f;
+static_assert(kGroup == kR * 32 && (kTeamWarps & (kTeamWarps - 1)) == 0, "a warp's i-points are one group");
+static_assert(kGroup % 32 == 0 && 32 % kStep == 0 && kStep % 2 == 0, "");
+
+struct WinParams {
+    const float4 *pts_a;
+    const float *pts2_b;
+    const double *vj_b;
+    const PackInfo *pack_b;
+    const uint32_t *perm_a, *perm_b;
+    const GroupCap *gcaps_a, *gcaps_b;
+    uint32_t n_a, n_b;
+    const double *xyz_a, *xyz_b;
+    size_t stride_a, stride_b;
+    const int3 *items;
+    uint32_t capacity;
+    const double *edges;
+    int nbins;
+    unsigned long long *counts;
+    double *wsums;
+    unsigned long long *counters;
+    int is_auto;
+    int n_stages;
+};
+
+__device__ __forceinline__ unsigned long long fadd2(unsigned long long a, unsigned long long b)
+{
+    unsigned long long d;
+    asm("add.rn.f32x2 %0, %1, %2;" : "=l"(d) : "l"(a), "l"(b));
+    return d;
+}
+__device__ __forceinline__ float lo32(unsigned long long v) { return __uint_as_float((uint32_t)v); }
+__device__ __forceinline__ float hi32(unsigned long long v) { return __uint_as_float((uint32_t)(v >> 32)); }
+// 1.0f if v > 0 else 0.0f (SASS FSET.BF); read as the high word of a double it is 2^-7 or 0
+__device__ __forceinline__ float ind_gt0(float v)
+{
+    float r;
+    asm("set.gt.f32.f32 %0, %1, 0f00000000;" : "=f"(r) : "f"(v));
+    return r;
+}
+
+// This warp's histogram rows in shared memory.  Lane 0 adds the reduced tallies; the rare exact
+// corrections come from any lane and are atomic.
+struct Rows {
+    uint32_t *cnt;
+    double *ws;
+};
+// per-CTA statistics kept in shared memory until the kernel ends
+enum { kStatFp64 = 0, kStatWindow = 1, kStatEvaluated = 2, kNumStats = 3 };
+// rows and weight of one window, parked in shared memory between its computation and its use
+struct WinRows {
+    int lo, hi;
+    double wsum;
+};
+
+__device__ __forceinline__ double warp_sum_f64(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+
+// Thread (warp, lane) holds the i-points (warp % kTeamWarps) * kGroup + r * 32 + lane of the i-tile, r < kR.
+__device__ __forceinline__ uint32_t local_i(int r)
+{
+    return ((threadIdx.x >> 5) & (kTeamWarps - 1)) * kGroup + r * 32 + (threadIdx.x & 31);
+}
+
+
+// Which pairs of a group count: ragged ends of the catalogues and the diagonal group of an auto-count.
+struct Mask {
+    uint32_t valid;  // bit r: i-point r of this thread exists
+    int jn;          // j-points of the group that exist
+    int j0;          // index in the tile of the group's first j-point
+    bool diag;       // count only pairs with (index in tile of j) > (index in tile of i)
+    __device__ __forceinline__ bool on(int r, int jj) const
+    {
+        return ((valid >> r) & 1u) && jj < jn && (!diag || (uint32_t)(j0 + jj) > local_i(r));
+    }
+};
+
+// Edges m_a .. m_a + K - 1 against one group of kGroup staged j-points and this thread's kR i-points.
+// The first chunk of a group (kFirst) fills rows m_a .. m_a + K - 1 (and m_a + K if it is also the last).
+// A later chunk starts with the previous chunk's last edge again, only to have the tallies above it
+// at hand, and fills rows m_a + 1 ..: no state is carried from chunk to chunk.
+template <int K, bool kWeighted, bool kPacked, bool kMasked, bool kFirst>
+__device__ __forceinline__ void window_chunk(const WinParams &p, const Rows rows, const float *__restrict__ grp2,
+                                             const double *__restrict__ vgrp, const float (&nx)[kR],
+                                             const float (&ny)[kR], const float (&nz)[kR],
+                                             const float (&wi)[kR], const int m_a, const bool last, const double wsum_j,
+                                             const Mask &mk, uint32_t i_base, uint32_t j_first, unsigned long long *stat)
+{
+    const int lane = threadIdx.x & 31;
+    const double e0 = p.edges[m_a];
+    const float e32 = (float)e0;
+    const unsigned long long e2 = pack2(e32, e32);
+    float dl[K];
+    unsigned long long dl2[K];
+    dl[0] = 0.f;
+    dl2[0] = 0ull;
+#pragma unroll
+    for (int q = 1; q < K; ++q) {
+        dl[q] = (float)(p.edges[m_a + q] - e0);
+        dl2[q] = pack2(dl[q], dl[q]);
+    }
+    const float G = K == 1 ? kGuard1 : kGuardK;
+
+    double t[K][kR];     // weighted: 2^-7 * sum of v_j over the pairs above edge q, per i-point
+    uint32_t sg[K][kR];  // unweighted: sign bits of d_q (1 = not above) of the last 32 j-points
+    uint32_t nb[K];      // unweighted: pairs not above edge q
+    float nf[K];         // weighted, not packed: pairs above edge q (exact: at most kGroup * kR)
+    double tall[kR];     // masked: 2^-7 * sum of v_j over the enabled pairs
+    uint32_t call = 0;   // masked: enabled pairs
+#pragma unroll
+    for (int q = 0; q < K; ++q) {
+        nb[q] = 0u;
+        nf[q] = 0.f;
+#pragma unroll
+        for (int r = 0; r < kR; ++r) {
+            t[q][r] = 0.0;
+            sg[q][r] = 0u;
+        }
+    }
+#pragma unroll
+    for (int r = 0; r < kR; ++r) tall[r] = 0.0;
+
+#pragma unroll 1
+    for (int jj = 0; jj < kGroup; jj += kStep) {
+        float mn = 1.0f;  // min |d_q| over the enabled pairs of the step
+#pragma unroll
+        for (int u = 0; u < kStep; u += 2) {
+            const ulonglong2 xy = *reinterpret_cast<const ulonglong2 *>(grp2 + (size_t)(jj + u) * 4);
+            const unsigned long long zz = *reinterpret_cast<const unsigned long long *>(grp2 + (size_t)(jj + u) * 4 + 4);
+            double v0 = 0.0, v1 = 0.0;
+            if constexpr (kWeighted) {
+                const double2 vv = *reinterpret_cast<const double2 *>(vgrp + jj + u);
+                v0 = vv.x;
+                v1 = vv.y;
+            }
+#pragma unroll
+            for (int r = 0; r < kR; ++r) {
+                // {n, n} packed at the use: the FFMA2 takes the one register for both halves
+                const unsigned long long d2 = ffma2(pack2(nx[r], nx[r]), xy.x,
+                                                    ffma2(pack2(ny[r], ny[r]), xy.y, ffma2(pack2(nz[r], nz[r]), zz, e2)));
+                bool on0 = true, on1 = true;
+                if constexpr (kMasked) {
+                    on0 = mk.on(r, jj + u);
+                    on1 = mk.on(r, jj + u + 1);
+                    call += (on0 ? 1u : 0u) + (on1 ? 1u : 0u);
+                    if constexpr (kWeighted) {
+                        tall[r] = fma(v0, __hiloint2double(on0 ? 0x3f800000 : 0, 0), tall[r]);
+                        tall[r] = fma(v1, __hiloint2double(on1 ? 0x3f800000 : 0, 0), tall[r]);
+                    }
+                }
+#pragma unroll
+                for (int q = 0; q < K; ++q) {
+                    const unsigned long long dq2 = q == 0 ? d2 : fadd2(d2, dl2[q]);
+                    const float a = lo32(dq2), b = hi32(dq2);
+                    if constexpr (kWeighted) {
+                        float i0 = ind_gt0(a), i1 = ind_gt0(b);
+                        if constexpr (kMasked) {
+                            i0 = on0 ? i0 : 0.f;
+                            i1 = on1 ? i1 : 0.f;
+                        }
+                        t[q][r] = fma(v0, __hiloint2double(__float_as_int(i0), 0), t[q][r]);
+                        t[q][r] = fma(v1, __hiloint2double(__float_as_int(i1), 0), t[q][r]);
+                        if constexpr (!kPacked) nf[q] += i0 + i1;
+                    } else {
+                        uint32_t ba = __float_as_uint(a), bb = __float_as_uint(b);
+                        if constexpr (kMasked) {
+                            ba = on0 ? ba : 0x80000000u;
+                            bb = on1 ? bb : 0x80000000u;
+                        }
+                        asm("shf.l.wrap.b32 %0, %1, %0, 1;" : "+r"(sg[q][r]) : "r"(ba));
+                        asm("shf.l.wrap.b32 %0, %1, %0, 1;" : "+r"(sg[q][r]) : "r"(bb));
+                    }
+                    float aa = fabsf(a), ab = fabsf(b);
+                    if constexpr (kMasked) {
+                        aa = on0 ? aa : 1.0f;
+                        ab = on1 ? ab : 1.0f;
+                    }
+                    asm("min.f32 %0, %0, %1, %2;" : "+f"(mn) : "f"(aa), "f"(ab));
+                }
+            }
+        }
+        if (__any_sync(0xffffffffu, !(mn > G))) {
+            // some pair is within the guard band of an edge: the exact row decides, edge by edge
+#pragma unroll 1
+            for (int u = 0; u < kStep; ++u) {
+                const float4 pj = tile_point(grp2, jj + u);
+#pragma unroll
+                for (int r = 0; r < kR; ++r) {  // unrolled: the register arrays must not be indexed at run time
+                    if (kMasked && !mk.on(r, jj + u)) continue;
+                    const float d0 = fmaf(nx[r], pj.x, fmaf(ny[r], pj.y, fmaf(nz[r], pj.z, e32)));
+                    bool amb = false;
+#pragma unroll
+                    for (int q = 0; q < K; ++q) amb |= !(fabsf(q == 0 ? d0 : __fadd_rn(d0, dl[q])) > G);
+                    if (!amb) continue;
+                    const int exact = exact_row(p.xyz_a, p.stride_a, p.perm_a[i_base + local_i(r)], p.xyz_b, p.stride_b,
+                                                p.perm_b[j_first + jj + u], p.edges, p.nbins);
+                    const double w = (double)wi[r] * (double)pj.w;
+#pragma unroll
+                    for (int q = 0; q < K; ++q) {
+                        const float dq = q == 0 ? d0 : __fadd_rn(d0, dl[q]);
+                        // what the loop above tallied for this pair and edge
+                        const bool fast_above = kWeighted ? dq > 0.f : (__float_as_uint(dq) >> 31) == 0u;
+                        const bool exact_above = exact > m_a + q;
+                        if (fast_above != exact_above) {
+                            // the tally above edge q is taken from row m_a + q and given to row m_a + q + 1
+                            const bool takes = q >= 1 || kFirst, gives = q < K - 1 || last;
+                            const uint32_t dn = fast_above ? 1u : 0xffffffffu;  // +1 / -1 for the lower row
+                            const double dw = fast_above ? w : -w;
+                            if (takes) {
+                                atomicAdd(&rows.cnt[m_a + q], dn);
+                                if constexpr (kWeighted) atomicAdd(&rows.ws[m_a + q], dw);
+                            }
+                            if (gives) {
+                                atomicAdd(&rows.cnt[m_a + q + 1], 0u - dn);
+                                if constexpr (kWeighted) atomicAdd(&rows.ws[m_a + q + 1], -dw);
+                            }
+                        }
+                    }
+                    atomicAdd(&stat[kStatFp64], 1ull);
+                }
+            }
+        }
+        if constexpr (!kWeighted) {
+            if ((jj & 31) == 32 - kStep) {
+#pragma unroll
+                for (int q = 0; q < K; ++q)
+#pragma unroll
+                    for (int r = 0; r < kR; ++r) nb[q] += __popc(sg[q][r]);
+            }
+        }
+    }
+
+    // ---- this thread's tallies -> row contributions -> the warp's rows
+    auto unpack = [&](double tt, uint32_t &n) -> double {  // 2^-7 (n C + sum of w) -> sum of w, n += count
+        double sw = tt * 128.0;
+        if constexpr (kPacked) {
+            const double nn = floor(sw * p.pack_b->inv_C);  // C is a power of two and the sum of w is below C: exact
+            sw -= nn * p.pack_b->C;
+            n += (uint32_t)nn;
+        }
+        return sw;
+    };
+    uint32_t c_prev = 0;  // this thread's pairs above the previous edge (all its pairs before the first)
+    double s_prev[kR];    // and, per i-point, the sum of their w_j
+    if constexpr (kFirst) {
+        if constexpr (kMasked) {
+            uint32_t n_unused = 0;
+            c_prev = call;
+#pragma unroll
+            for (int r = 0; r < kR; ++r) s_prev[r] = kWeighted ? unpack(tall[r], n_unused) : 0.0;
+        } else {
+            c_prev = (uint32_t)(kGroup * kR);
+#pragma unroll
+            for (int r = 0; r < kR; ++r) s_prev[r] = wsum_j;
+        }
+    }
+    __syncwarp();
+#pragma unroll
+    for (int q = 0; q <= K; ++q) {
+        if (q == K && !last) break;
+        uint32_t c_q = 0;  // pairs above edge q (q == K: nothing lies above the row after the last edge)
+        double rw = 0.0;   // weight of this thread's pairs in row m_a + q
+        if (q < K) {
+            if constexpr (kWeighted) {
+                c_q = kPacked ? 0u : (uint32_t)nf[q];
+#pragma unroll
+                for (int r = 0; r < kR; ++r) {
+                    const double sw = unpack(t[q][r], c_q);
+                    if (q > 0 || kFirst) rw = fma((double)wi[r], s_prev[r] - sw, rw);
+                    s_prev[r] = sw;
+                }
+            } else {
+                c_q = (uint32_t)(kGroup * kR) - nb[q];
+            }
+        } else if constexpr (kWeighted) {
+#pragma unroll
+            for (int r = 0; r < kR; ++r) rw = fma((double)wi[r], s_prev[r], rw);
+        }
+        const uint32_t rc = c_prev - c_q;
+        c_prev = c_q;
+        if (q == 0 && !kFirst) continue;  // the repeated edge: row m_a was filled by the previous chunk
+        if (rc == 0u) rw = 0.0;  // no pair of this thread in the row: not even a rounding residue
+        const uint32_t rc_warp = __reduce_add_sync(0xffffffffu, rc);
+        if constexpr (kWeighted) rw = warp_sum_f64(rw);
+        if (lane == 0) {
+            rows.cnt[m_a + q] += rc_warp;
+            if constexpr (kWeighted) rows.ws[m_a + q] += rw;
+        }
+    }
+    __syncwarp();
+}
+
+// One group: all edges r_lo .. r_hi - 1 of its window, kChunk at a time (masked groups one at a time).
+#define ACF_WIN_CHUNK_CALL(K, MASKED, FIRST, M, LAST) \
+    window_chunk<K, kWeighted, kPacked, MASKED, FIRST>(p, rows, grp2, vgrp, nx, ny, nz, wi, M, LAST, wsum_j, mk, i_base, j_first, stat)
+template <bool kWeighted, bool kPacked>
+__device__ __forceinline__ void window_group(const WinParams &p, const Rows rows, const float *__restrict__ grp2,
+                                             const double *__restrict__ vgrp, const float (&nx)[kR],
+                                             const float (&ny)[kR], const float (&nz)[kR],
+                                             const float (&wi)[kR], int r_lo, int r_hi, double wsum_j, bool masked, const Mask &mk,
+                                             uint32_t i_base, uint32_t j_first, unsigned long long *stat)
+{
+    static_assert(kChunk == 3, "the dispatch below spells the chunk sizes out");
+    if (r_hi == r_lo) {  // one row: still every pair is evaluated, against the edge that bounds the row
+        if (r_lo > p.nbins) r_lo = p.nbins;
+        r_hi = r_lo + 1;
+    }
+    // first chunk: edges r_lo .. ; later chunks repeat the last edge done and add up to kChunk - 1 new ones
+    int m = r_lo;  // edges below m are done
+    {
+        const int left = r_hi - m;
+        if (masked) {
+            ACF_WIN_CHUNK_CALL(1, true, true, m, left == 1);
+            m += 1;
+        } else if (left == 1) {
+            ACF_WIN_CHUNK_CALL(1, false, true, m, true);
+            m += 1;
+        } else if (left == 2) {
+            ACF_WIN_CHUNK_CALL(2, false, true, m, true);
+            m += 2;
+        } else {
+            ACF_WIN_CHUNK_CALL(3, false, true, m, left == 3);
+            m += 3;
+        }
+    }
+    while (m < r_hi) {
+        const int left = r_hi - m;
+        if (masked) {
+            ACF_WIN_CHUNK_CALL(2, true, false, m - 1, left == 1);
+            m += 1;
+        } else if (left == 1) {
+            ACF_WIN_CHUNK_CALL(2, false, false, m - 1, true);
+            m += 1;
+        } else {
+            ACF_WIN_CHUNK_CALL(3, false, false, m - 1, left == 2);
+            m += 2;
+        }
+    }
+}
+#undef ACF_WIN_CHUNK_CALL
+
+// ---- the kernel ---------------------------------------------------------------------------------
+// kWarps consumer warps and no producer warp (16 warps leave each thread 128 registers; a 17th would cost
+// 32 of them).  The j-tiles of the work items {i-tile, first j-tile, number of j-tiles} stream through a
+// ring of shared-memory stages filled by TMA bulk copies (full / empty mbarriers per stage).  Whichever
+// warp finds the ring's lock free refills the drained stages -- after it hands a stage back, and while it
+// waits for one -- pulling work items from a global counter.  Every warp walks the stream at its own
+// pace, holding its kGroup i-points of the current i-tile in registers.
+struct ProdState {
+    uint32_t lock;      // 0 free, 1 held
+    uint32_t produced;  // stages filled so far: slot = produced % n_stages, round = produced / n_stages
+    int ti, tj, left;   // the work item being streamed: its i-tile, next j-tile, j-tiles left
+    int done;           // the end-of-stream stage has been posted
+    unsigned long long n_items;
+};
+
+template <bool kWeighted>
+__device__ __forceinline__ void try_produce(const WinParams &p, volatile ProdState *ps, uint64_t *full, uint64_t *empty,
+                                            StageMeta *meta, unsigned char *stages, int n_stages)
+{
+    constexpr size_t kStage = stage_bytes(kWeighted);
+    if (ps->done || atomicCAS(const_cast<uint32_t *>(&ps->lock), 0u, 1u) != 0u) return;
+    while (!ps->done) {
+        const uint32_t produced = ps->produced;
+        const int slot = (int)(produced % (uint32_t)n_stages);
+        const uint32_t round = produced / (uint32_t)n_stages;
+        if (!mbar_test(&empty[slot], (round & 1u) ^ 1u)) break;  // not drained yet (round 0 passes at once)
+        if (ps->left == 0) {
+            const unsigned long long item = atomicAdd(&p.counters[kCtrWorkHead], 1ull);
+            if (item >= ps->n_items) {  // end of stream
+                StageMeta m;
+                m.ti = -1;
+                m.tj = m.jn = m.pad = 0;
+                meta[slot] = m;
+                ps->done = 1;
+                ps->produced = produced + 1;
+                mbar_arrive(&full[slot]);
+                break;
+            }
+            const int3 it = p.items[item];
+            ps->ti = it.x;
+            ps->tj = it.y;
+            ps->left = it.z;
+        }
+        const int tj = ps->tj;
+        const uint32_t j0 = (uint32_t)tj * kTile;
+        const uint32_t jn = p.n_b - j0 < (uint32_t)kTile ? p.n_b - j0 : (uint32_t)kTile;
+        StageMeta m;
+        m.ti = ps->ti;
+        m.tj = tj;
+        m.jn = (int)jn;
+        m.pad = 0;
+        meta[slot] = m;
+        ps->tj = tj + 1;
+        ps->left = ps->left - 1;
+        ps->produced = produced + 1;
+        // the arrays are padded to whole tiles: always a full tile
+        mbar_expect_tx(&full[slot], (uint32_t)kStage);
+        bulk_load(stages + (size_t)slot * kStage, p.pts2_b + (size_t)j0 * 4, (uint32_t)kTileBytes, &full[slot]);
+        if constexpr (kWeighted)
+            bulk_load(stages + (size_t)slot * kStage + kTileBytes, p.vj_b + (size_t)j0, (uint32_t)kVjBytes, &full[slot]);
+    }
+    __threadfence_block();
+    atomicExch(const_cast<uint32_t *>(&ps->lock), 0u);
+}
+
+template <bool kWeighted>
+__global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p)
+{
+    if (p.counters[kCtrBadInput] != 0) return;  // inputs failed validation
+    extern __shared__ __align__(128) unsigned char smem[];
+    const int rows_n = p.nbins + 2;
+    const int n_stages = p.n_stages;
+    constexpr size_t kStage = stage_bytes(kWeighted);
+    // layout: [full bars | empty bars | stage meta | producer state] (512 B) [stages][count rows per warp][weight rows per warp]
+    uint64_t *full = reinterpret_cast<uint64_t *>(smem);
+    uint64_t *empty = full + kMaxStages;
+    StageMeta *meta = reinterpret_cast<StageMeta *>(smem + 128);
+    volatile ProdState *ps = reinterpret_cast<volatile ProdState *>(smem + 128 + kMaxStages * sizeof(StageMeta));
+    unsigned long long *stat = reinterpret_cast<unsigned long long *>(smem + 128 + kMaxStages * sizeof(StageMeta) + sizeof(ProdState));
+    static_assert(sizeof(ProdState) % 8 == 0 && 128 + kMaxStages * sizeof(StageMeta) + sizeof(ProdState) + kNumStats * 8 <= kSmemHeader, "header");
+    unsigned char *stages = smem + kSmemHeader;
+    size_t off = kSmemHeader + (size_t)n_stages * kStage;
+    uint32_t *cnt_all = reinterpret_cast<uint32_t *>(smem + off);
+    off += (size_t)kWarps * rows_n * sizeof(uint32_t);
+    off = (off + 15) & ~size_t(15);
+    double *ws_all = reinterpret_cast<double *>(smem + off);
+    if constexpr (kWeighted) off += (size_t)kWarps * rows_n * sizeof(double);
+    WinRows *win_all = reinterpret_cast<WinRows *>(smem + off);
+
+    const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
+    const int igrp = warp & (kTeamWarps - 1), team = warp / kTeamWarps;
+    for (int i = tid; i < kWarps * rows_n; i += blockDim.x) {
+        cnt_all[i] = 0;
+        if constexpr (kWeighted) ws_all[i] = 0.0;
+    }
+    if (tid == 0) {
+        for (int s = 0; s < n_stages; ++s) {
+            mbar_init(&full[s], 1);
+            mbar_init(&empty[s], kWarps);
+        }
+        ps->lock = 0;
+        ps->produced = 0;
+        ps->ti = ps->tj = ps->left = 0;
+        ps->done = 0;
+        unsigned long long n_items = p.counters[kCtrWorkCount];
+        ps->n_items = n_items > p.capacity ? p.capacity : n_items;
+        for (int i = 0; i < kNumStats; ++i) stat[i] = 0ull;
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    if (tid == 0) try_produce<kWeighted>(p, ps, full, empty, meta, stages, n_stages);
+
+    // ---------------- consumers
+    Rows rows;
+    rows.cnt = cnt_all + (size_t)warp * rows_n;
+    rows.ws = ws_all + (size_t)warp * rows_n;
+    WinRows *win = win_all + (size_t)warp * kGroupsPerTile;
+    const bool packed = !kWeighted || p.pack_b->packed != 0;
+    uint32_t since_flush = 0;  // j-tiles this warp has tallied in its unflushed rows
+    float wi[kR];
+    float nx[kR], ny[kR], nz[kR];  // the i-points, negated
+#pragma unroll
+    for (int r = 0; r < kR; ++r) wi[r] = nx[r] = ny[r] = nz[r] = 0.f;
+    uint32_t valid_mask = 0, i_base = 0, n_i = 0;
+    bool warp_full = false, warp_any = false;
+    int cur_ti = -1;
+
+    auto flush_rows = [&]() {
+        // this warp's rows -> global (u64 / f64 atomics); the rows restart from zero
+        __syncwarp();
+        for (int row = lane; row < rows_n; row += 32) {
+            const uint32_t v = rows.cnt[row];
+            rows.cnt[row] = 0;
+            if (row >= 1 && row <= p.nbins && v) atomicAdd(&p.counts[row - 1], (unsigned long long)v);
+            if constexpr (kWeighted) {
+                const double w = rows.ws[row];
+                rows.ws[row] = 0.0;
+                if (row >= 1 && row <= p.nbins && w != 0.0) atomicAdd(&p.wsums[row - 1], w);
+            }
+        }
+        __syncwarp();
+        since_flush = 0;
+    };
+
+    for (uint32_t consumed = 0;; ++consumed) {
+        const int slot = (int)(consumed % (uint32_t)n_stages);
+        const uint32_t parity = (consumed / (uint32_t)n_stages) & 1u;
+        if (lane == 0)
+            while (!mbar_test(&full[slot], parity)) try_produce<kWeighted>(p, ps, full, empty, meta, stages, n_stages);
+        __syncwarp();
+        mbar_wait(&full[slot], parity);  // every lane observes the completed phase
+        const StageMeta m = meta[slot];
+        if (m.ti < 0) break;
+        if (m.ti != cur_ti) {
+            cur_ti = m.ti;
+            i_base = (uint32_t)m.ti * kTile;
+            valid_mask = 0;
+#pragma unroll
+            for (int r = 0; r < kR; ++r) {
+                const uint32_t s = i_base + local_i(r);
+                const float4 v = p.pts_a[s];  // the array is padded to a whole tile
+                nx[r] = -v.x;
+                ny[r] = -v.y;
+                nz[r] = -v.z;
+                wi[r] = v.w;
+                valid_mask |= (s < p.n_a ? 1u : 0u) << r;
+            }
+            n_i = i_base + kTile <= p.n_a ? kTile : p.n_a - i_base;
+            warp_full = (uint32_t)(igrp + 1) * kGroup <= n_i;
+            warp_any = (uint32_t)igrp * kGroup < n_i;
+        }
+        const float *tile = reinterpret_cast<const float *>(stages + (size_t)slot * kStage);
+        const double *vtile = reinterpret_cast<const double *>(stages + (size_t)slot * kStage + kTileBytes);
+        const int tj = m.tj, jn = m.jn;
+        const bool diag = p.is_auto && tj == m.ti;
+        const uint32_t j_base = (uint32_t)tj * kTile;
+        // u32 rows: flush before this warp's tallies could wrap
+        if (since_flush >= (1u << 31) / (uint32_t)(kGroup * kTile)) flush_rows();
+        ++since_flush;
+
+        if (warp_any) {
+            // lane g bounds the rows of this warp's i-group against j-group g of the tile
+            const int n_groups = (jn + kGroup - 1) / kGroup;
+            __syncwarp();
+            if (lane < n_groups) {
+                WinRows wr;
+                wr.lo = 0;
+                wr.hi = p.nbins + 1;
+                const GroupCap gb = p.gcaps_b[(size_t)tj * kGroupsPerTile + lane];
+                double c_lo, c_hi;
+                if (cap_window(p.gcaps_a[(size_t)m.ti * kGroupsPerTile + igrp], gb, c_lo, c_hi)) {
+                    wr.lo = row_of_cos(c_hi, p.edges, p.nbins);
+                    wr.hi = row_of_cos(c_lo, p.edges, p.nbins);
+                }
+                wr.wsum = gb.wsum;
+                win[lane] = wr;
+            }
+            __syncwarp();
+            for (int g = diag ? igrp : 0; g < n_groups; ++g) {
+                if ((g & (kTeams - 1)) != team) continue;  // the other team's group
+                const int r_lo = win[g].lo, r_hi = win[g].hi;
+                const double wsum_j = win[g].wsum;
+                Mask mk;
+                mk.valid = valid_mask;
+                mk.jn = jn - g * kGroup < kGroup ? jn - g * kGroup : kGroup;
+                mk.j0 = g * kGroup;
+                mk.diag = diag && g == igrp;
+                const bool masked = !warp_full || mk.jn < kGroup || mk.diag;
+                const float *grp2 = tile + (size_t)g * kGroup * 4;
+                const double *vgrp = vtile + g * kGroup;
+                if (packed)
+                    window_group<kWeighted, true>(p, rows, grp2, vgrp, nx, ny, nz, wi, r_lo, r_hi, wsum_j, masked, mk, i_base,
+                                                  j_base + g * kGroup, stat);
+                else
+                    window_group<kWeighted, false>(p, rows, grp2, vgrp, nx, ny, nz, wi, r_lo, r_hi, wsum_j, masked, mk, i_base,
+                                                   j_base + g * kGroup, stat);
+                if (lane == 0 && !masked && r_hi - r_lo <= 1) atomicAdd(&stat[kStatWindow], (unsigned long long)(kGroup * kGroup));
+            }
+        }
+        if (tid == 0) stat[kStatEvaluated] += diag ? (unsigned long long)n_i * (n_i - 1) / 2 : (unsigned long long)n_i * (unsigned)jn;
+        __syncwarp();  // every lane has read the stage before it is handed back
+        if (lane == 0) {
+            mbar_arrive(&empty[slot]);
+            try_produce<kWeighted>(p, ps, full, empty, meta, stages, n_stages);
+        }
+    }
+
+    flush_rows();
+    __syncthreads();
+    if (tid == 0) {
+        if (stat[kStatFp64]) atomicAdd(&p.counters[kCtrPairsFp64], stat[kStatFp64]);
+        if (stat[kStatWindow]) atomicAdd(&p.counters[kCtrPairsWindow], stat[kStatWindow]);
+        if (stat[kStatEvaluated]) atomicAdd(&p.counters[kCtrPairsEvaluated], stat[kStatEvaluated]);
+    }
+}
+
+}  // namespace
+
+// Launches the window kernel on the work items of the context's work list.
+int launch_pair_win(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_auto, int nbins, uint32_t capacity,
+                    unsigned long long *d_counts, double *d_wsums)
+{
+    const bool weighted = d_wsums != nullptr;
+    const int rows_n = nbins + 2;
+    auto smem_for = [&](int stages) {
+        size_t m = kSmemHeader + (size_t)stages * stage_bytes(weighted);
+        m += (size_t)kWarps * rows_n * sizeof(uint32_t);
+        m = (m + 15) & ~size_t(15);
+        if (weighted) m += (size_t)kWarps * rows_n * sizeof(double);
+        m += (size_t)kWarps * kGroupsPerTile * sizeof(WinRows);
+        return m;
+    };
+    // one CTA of 16 warps per SM: 128 registers a thread
+    const int ctas_per_sm = 1;
+    const size_t budget = (size_t)ctx->max_smem_optin;
+    if (smem_for(2) > budget) return fail(ctx, ACF_EINVAL, "too many bins for the window kernel (%d)", nbins);
+    int n_stages = 2;
+    while (n_stages < kMaxStages && smem_for(n_stages + 1) <= budget) ++n_stages;
+    const size_t smem = smem_for(n_stages);
+
+    WinParams p{};
+    p.pts_a = a.pts;
+    p.pts2_b = b.pts2;
+    p.vj_b = b.vj;
+    p.pack_b = b.pack;
+    p.perm_a = a.perm;
+    p.perm_b = b.perm;
+    p.gcaps_a = a.gcaps;
+    p.gcaps_b = b.gcaps;
+    p.n_a = (uint32_t)a.n;
+    p.n_b = (uint32_t)b.n;
+    p.xyz_a = a.xyz;
+    p.xyz_b = b.xyz;
+    p.stride_a = a.stride;
+    p.stride_b = b.stride;
+    p.items = ctx->s_work.as<int3>();
+    p.capacity = capacity;
+    p.edges = ctx->s_edges.as<double>();
+    p.nbins = nbins;
+    p.counts = d_counts;
+    p.wsums = d_wsums;
+    p.counters = ctx->d_counters;
+    p.is_auto = is_auto;
+    p.n_stages = n_stages;
+
+    const int grid = ctx->num_sms * ctas_per_sm;
+    cudaError_t e;
+    if (weighted) {
+        e = cudaFuncSetAttribute(pair_win_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) pair_win_kernel<true><<<grid, kThreads, smem, ctx->stream>>>(p);
+    } else {
+        e = cudaFuncSetAttribute(pair_win_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) pair_win_kernel<false><<<grid, kThreads, smem, ctx->stream>>>(p);
+    }
+    if (e == cudaSuccess) e = cudaGetLastError();
+    ACF_CUDA_TRY(ctx, e);
+    ctx->last.kernel_launches++;
+    return ACF_OK;
+}
+
+}  // namespace acf

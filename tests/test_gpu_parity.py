@@ -82,13 +82,13 @@ def test_canonical_vectors_bit_equal(acf, oracle):
     assert a.tobytes() == b.tobytes()
 
 
-@pytest.mark.parametrize("kernel", ["auto", "fp64"])
+@pytest.mark.parametrize("kernel", ["auto", "fp64", "table", "window"])
 @pytest.mark.parametrize("name,scale", [("tiny", 0.5), ("clustered_patch", 0.03), ("survey_scale", 0.006),
                                         ("full_sky", 0.008), ("pruning_stress", 0.0012)])
 def test_config_parity(acf, ctx, oracle, name, scale, kernel):
     """All five BASELINE configurations at a size the oracle finishes in seconds: several tiles
     and ragged tails on both catalogues; DD, DR, RR and the estimator."""
-    kern = acf.ACF_KERNEL_FP64 if kernel == "fp64" else acf.ACF_KERNEL_AUTO
+    kern = {"auto": acf.ACF_KERNEL_AUTO, "fp64": acf.ACF_KERNEL_FP64, "table": acf.ACF_KERNEL_TABLE, "window": acf.ACF_KERNEL_WINDOW}[kernel]
     w = make_config(name, scale)
     xd, xr = acf.acf_radec_to_xyz(w.ra_d, w.dec_d), acf.acf_radec_to_xyz(w.ra_r, w.dec_r)
     assert xd.tobytes() == oracle.radec_to_xyz(w.ra_d, w.dec_d).tobytes()
@@ -145,11 +145,11 @@ def test_polyhedra_and_full_range(acf, ctx, oracle):
     assert cb.tolist() == gpu_counts(acf, ctx, b, a, full, False).tolist()       # swap symmetry
 
 
-@pytest.mark.parametrize("kernel", ["auto", "fp64"])
+@pytest.mark.parametrize("kernel", ["auto", "fp64", "table", "window"])
 def test_edge_inclusivity_adversarial(acf, ctx, oracle, kernel):
     """Pairs whose cosine is exactly an edge, or one ulp either side, through the xyz entry point:
     a = (1,0,0), b = (c, sqrt(1-c^2), 0) makes the defined pair cosine equal c exactly."""
-    kern = acf.ACF_KERNEL_FP64 if kernel == "fp64" else acf.ACF_KERNEL_AUTO
+    kern = {"auto": acf.ACF_KERNEL_AUTO, "fp64": acf.ACF_KERNEL_FP64, "table": acf.ACF_KERNEL_TABLE, "window": acf.ACF_KERNEL_WINDOW}[kernel]
     edges = cos_edges_from_theta_deg(log_theta_edges_deg(0.05, 170.0, 12))
     cs = []
     for e in edges:
