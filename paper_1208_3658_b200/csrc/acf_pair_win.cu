@@ -38,10 +38,14 @@ constexpr int kR = kGroup / 32;        // i-points per thread
 #endif
 constexpr int kChunk = ACF_WIN_CHUNK;  // edges per pass over a group
 constexpr int kStep = 4;               // j-points per guard-band vote
-// |d_0 - (e_m - c64)| <= 2^-25 [fp32(e_m)] + 2u(1+1e-6) [input rounding, u = 2^-24] + 3 * 2^-24 [three
-// roundings of values of magnitude <= 2] = 3.3e-7; d_q adds the rounding of the offset (<= 2^-24 * 2)
-// and of the sum (<= 2^-24 * 2): 5.7e-7.
-constexpr float kGuard1 = 4.5e-7f;
+// Guard bands (u = 2^-24).  A wrong fp32 sign needs |d_0 - (e_m - c64)| >= |d_0|,
+// so only pairs with a small |d_0| matter; for those the partial sums of the chain are below 1 + 2e-6 in
+// magnitude (they differ from d_0 by products of coordinates whose absolute sum is at most 1 + 2e-6):
+//   2^-25 [fp32(e_m)] + 2u (1 + 1e-6) [the six rounded coordinates] + 2 * 2^-24 [the two inner FMAs]
+//   + 2^-24 |d_0| [the last FMA] + 4e-16 [c64 itself]  <=  2.69e-7.
+// d_q, q >= 1, is the sum of a d_0 that is not small and a rounded offset: partial sums below 4 (three
+// roundings of 2^-23), the offset (2^-24) and the six coordinates give 5.7e-7.
+constexpr float kGuard1 = 3.0e-7f;
 constexpr float kGuardK = 7.0e-7f;
 static_assert(kGroup == kR * 32 && (kTeamWarps & (kTeamWarps - 1)) == 0, "a warp's i-points are one group");
 static_assert(kGroup % 32 == 0 && 32 % kStep == 0 && kStep % 2 == 0, "");
@@ -81,6 +85,16 @@ __device__ __forceinline__ float ind_gt0(float v)
     float r;
     asm("set.gt.f32.f32 %0, %1, 0f00000000;" : "=f"(r) : "f"(v));
     return r;
+}
+
+// The same comparison written into the high word of a 64-bit register whose low word is and stays zero:
+// the register then reads as the double 2^-7 [v > 0] with no instruction spent on the low word.
+__device__ __forceinline__ double ind_gt0_f64(unsigned long long &reg, float v)
+{
+    asm("{\n\t.reg .b32 lo, hi;\n\tmov.b64 {lo, hi}, %0;\n\tset.gt.f32.f32 hi, %1, 0f00000000;\n\tmov.b64 %0, {lo, hi};\n\t}"
+        : "+l"(reg)
+        : "f"(v));
+    return __longlong_as_double((long long)reg);
 }
 
 // This warp's histogram rows in shared memory.  Lane 0 adds the reduced tallies; the rare exact
@@ -123,15 +137,108 @@ struct Mask {
     }
 };
 
+// The exact corrections of one chunk of a group, after its loop: amb_steps has a bit per step of kStep
+// j-points in which some pair came within the guard band of an edge.  Every pair of those steps is
+// re-derived exactly as the loop computed it; where the fp64 row of include/acf.h disagrees with what
+// the loop tallied, the rows are corrected (atomics: any lane may come here).  One copy for all chunk
+// shapes; it reloads the i-points rather than taking them in registers.
+template <bool kWeighted>
+__device__ __forceinline__ void fixup_body(const WinParams &p, const Rows rows, const float *__restrict__ grp2, uint32_t amb_steps,
+                                           int K, int m_a, bool first, bool last, bool masked, const Mask mk, uint32_t i_base,
+                                           uint32_t j_first, unsigned long long *stat, const float4 (&pi)[kR])
+{
+    const double e0 = p.edges[m_a];
+    const float e32 = (float)e0;
+    const float G = K == 1 ? kGuard1 : kGuardK;
+    float dl[kChunk];
+#pragma unroll
+    for (int q = 0; q < kChunk; ++q) dl[q] = q > 0 && q < K ? (float)(p.edges[m_a + q] - e0) : 0.f;
+    while (amb_steps) {
+        const int jj0 = (__ffs(amb_steps) - 1) * kStep;
+        amb_steps &= amb_steps - 1;
+        for (int u = 0; u < kStep; ++u) {
+            const float4 pj = tile_point(grp2, jj0 + u);
+#pragma unroll
+            for (int r = 0; r < kR; ++r) {
+                if (masked && !mk.on(r, jj0 + u)) continue;
+                const float d0 = fmaf(-pi[r].x, pj.x, fmaf(-pi[r].y, pj.y, fmaf(-pi[r].z, pj.z, e32)));
+                bool amb = false;
+#pragma unroll
+                for (int q = 0; q < kChunk; ++q) amb |= q < K && !(fabsf(q == 0 ? d0 : __fadd_rn(d0, dl[q])) > G);
+                if (!amb) continue;
+                const int exact = exact_row(p.xyz_a, p.stride_a, p.perm_a[i_base + local_i(r)], p.xyz_b, p.stride_b,
+                                            p.perm_b[j_first + jj0 + u], p.edges, p.nbins);
+                const double w = (double)pi[r].w * (double)pj.w;
+#pragma unroll
+                for (int q = 0; q < kChunk; ++q) {
+                    if (q >= K) break;
+                    const float dq = q == 0 ? d0 : __fadd_rn(d0, dl[q]);
+                    // what the loop tallied for this pair and edge
+                    const bool fast_above = kWeighted ? dq > 0.f : (__float_as_uint(dq) >> 31) == 0u;
+                    const bool exact_above = exact > m_a + q;
+                    if (fast_above != exact_above) {
+                        // the tally above edge q is taken from row m_a + q and given to row m_a + q + 1
+                        const bool takes = q >= 1 || first, gives = q < K - 1 || last;
+                        const uint32_t dn = fast_above ? 1u : 0xffffffffu;  // +1 / -1 for the lower row
+                        const double dw = fast_above ? w : -w;
+                        if (takes) {
+                            atomicAdd(&rows.cnt[m_a + q], dn);
+                            if constexpr (kWeighted) atomicAdd(&rows.ws[m_a + q], dw);
+                        }
+                        if (gives) {
+                            atomicAdd(&rows.cnt[m_a + q + 1], 0u - dn);
+                            if constexpr (kWeighted) atomicAdd(&rows.ws[m_a + q + 1], -dw);
+                        }
+                    }
+                }
+                atomicAdd(&stat[kStatFp64], 1ull);
+            }
+        }
+    }
+}
+
+template <bool kWeighted>
+__device__ __noinline__ void fixup_chunk(const WinParams &p, const Rows rows, const float *__restrict__ grp2, uint32_t amb_steps,
+                                         int K, int m_a, bool first, bool last, bool masked, const Mask mk, uint32_t i_base,
+                                         uint32_t j_first, unsigned long long *stat)
+{
+    float4 pi[kR];
+#pragma unroll
+    for (int r = 0; r < kR; ++r) pi[r] = p.pts_a[i_base + local_i(r)];  // the array is padded to a whole tile
+    fixup_body<kWeighted>(p, rows, grp2, amb_steps, K, m_a, first, last, masked, mk, i_base, j_first, stat, pi);
+}
+
+// The corrections of the single-edge groups of one staged tile, noted by the kernel's own loop
+// (one call per tile and warp instead of one per group).
+struct FixNote {
+    uint32_t amb_steps;
+    int m_edge;
+};
+template <bool kWeighted>
+__device__ __noinline__ void fixup_tile(const WinParams &p, const Rows rows, const float *__restrict__ tile, const FixNote *notes,
+                                        uint32_t i_base, uint32_t j_base, unsigned long long *stat)
+{
+    float4 pi[kR];
+#pragma unroll
+    for (int r = 0; r < kR; ++r) pi[r] = p.pts_a[i_base + local_i(r)];
+    Mask mk{};
+    for (int g = 0; g < kGroupsPerTile; ++g) {
+        const FixNote n = notes[g];
+        if (n.amb_steps)
+            fixup_body<kWeighted>(p, rows, tile + (size_t)g * kGroup * 4, n.amb_steps, 1, n.m_edge, true, true, false, mk, i_base,
+                                  j_base + g * kGroup, stat, pi);
+    }
+}
+
 // Edges m_a .. m_a + K - 1 against one group of kGroup staged j-points and this thread's kR i-points.
-// The first chunk of a group (kFirst) fills rows m_a .. m_a + K - 1 (and m_a + K if it is also the last).
+// The first chunk of a group (first) fills rows m_a .. m_a + K - 1 (and m_a + K if it is also the last).
 // A later chunk starts with the previous chunk's last edge again, only to have the tallies above it
 // at hand, and fills rows m_a + 1 ..: no state is carried from chunk to chunk.
-template <int K, bool kWeighted, bool kPacked, bool kMasked, bool kFirst>
-__device__ __forceinline__ void window_chunk(const WinParams &p, const Rows rows, const float *__restrict__ grp2,
+template <int K, bool kWeighted, bool kPacked, bool kMasked, bool kDeferFix = false>
+__device__ __forceinline__ uint32_t window_chunk(const WinParams &p, const Rows rows, const float *__restrict__ grp2,
                                              const double *__restrict__ vgrp, const float (&nx)[kR],
                                              const float (&ny)[kR], const float (&nz)[kR],
-                                             const float (&wi)[kR], const int m_a, const bool last, const double wsum_j,
+                                             const float (&wi)[kR], const int m_a, const bool first, const bool last, const double wsum_j,
                                              const Mask &mk, uint32_t i_base, uint32_t j_first, unsigned long long *stat)
 {
     const int lane = threadIdx.x & 31;
@@ -167,7 +274,13 @@ __device__ __forceinline__ void window_chunk(const WinParams &p, const Rows rows
     }
 #pragma unroll
     for (int r = 0; r < kR; ++r) tall[r] = 0.0;
+    constexpr int kInd = 2 * kR;  // indicator registers: low words zero for the whole loop
+    unsigned long long ind[kInd];
+#pragma unroll
+    for (int i = 0; i < kInd; ++i) ind[i] = 0ull;
 
+    uint32_t amb_steps = 0;  // warp-uniform
+    static_assert(kGroup / kStep <= 32, "one bit per step");
 #pragma unroll 1
     for (int jj = 0; jj < kGroup; jj += kStep) {
         float mn = 1.0f;  // min |d_q| over the enabled pairs of the step
@@ -200,12 +313,15 @@ __device__ __forceinline__ void window_chunk(const WinParams &p, const Rows rows
                 for (int q = 0; q < K; ++q) {
                     const unsigned long long dq2 = q == 0 ? d2 : fadd2(d2, dl2[q]);
                     const float a = lo32(dq2), b = hi32(dq2);
-                    if constexpr (kWeighted) {
+                    if constexpr (kWeighted && !kMasked) {
+                        unsigned long long &g0 = ind[(2 * r) % kInd], &g1 = ind[(2 * r + 1) % kInd];
+                        t[q][r] = fma(v0, ind_gt0_f64(g0, a), t[q][r]);
+                        t[q][r] = fma(v1, ind_gt0_f64(g1, b), t[q][r]);
+                        if constexpr (!kPacked) nf[q] += __uint_as_float((uint32_t)(g0 >> 32)) + __uint_as_float((uint32_t)(g1 >> 32));
+                    } else if constexpr (kWeighted) {
                         float i0 = ind_gt0(a), i1 = ind_gt0(b);
-                        if constexpr (kMasked) {
-                            i0 = on0 ? i0 : 0.f;
-                            i1 = on1 ? i1 : 0.f;
-                        }
+                        i0 = on0 ? i0 : 0.f;
+                        i1 = on1 ? i1 : 0.f;
                         t[q][r] = fma(v0, __hiloint2double(__float_as_int(i0), 0), t[q][r]);
                         t[q][r] = fma(v1, __hiloint2double(__float_as_int(i1), 0), t[q][r]);
                         if constexpr (!kPacked) nf[q] += i0 + i1;
@@ -227,47 +343,8 @@ __device__ __forceinline__ void window_chunk(const WinParams &p, const Rows rows
                 }
             }
         }
-        if (__any_sync(0xffffffffu, !(mn > G))) {
-            // some pair is within the guard band of an edge: the exact row decides, edge by edge
-#pragma unroll 1
-            for (int u = 0; u < kStep; ++u) {
-                const float4 pj = tile_point(grp2, jj + u);
-#pragma unroll
-                for (int r = 0; r < kR; ++r) {  // unrolled: the register arrays must not be indexed at run time
-                    if (kMasked && !mk.on(r, jj + u)) continue;
-                    const float d0 = fmaf(nx[r], pj.x, fmaf(ny[r], pj.y, fmaf(nz[r], pj.z, e32)));
-                    bool amb = false;
-#pragma unroll
-                    for (int q = 0; q < K; ++q) amb |= !(fabsf(q == 0 ? d0 : __fadd_rn(d0, dl[q])) > G);
-                    if (!amb) continue;
-                    const int exact = exact_row(p.xyz_a, p.stride_a, p.perm_a[i_base + local_i(r)], p.xyz_b, p.stride_b,
-                                                p.perm_b[j_first + jj + u], p.edges, p.nbins);
-                    const double w = (double)wi[r] * (double)pj.w;
-#pragma unroll
-                    for (int q = 0; q < K; ++q) {
-                        const float dq = q == 0 ? d0 : __fadd_rn(d0, dl[q]);
-                        // what the loop above tallied for this pair and edge
-                        const bool fast_above = kWeighted ? dq > 0.f : (__float_as_uint(dq) >> 31) == 0u;
-                        const bool exact_above = exact > m_a + q;
-                        if (fast_above != exact_above) {
-                            // the tally above edge q is taken from row m_a + q and given to row m_a + q + 1
-                            const bool takes = q >= 1 || kFirst, gives = q < K - 1 || last;
-                            const uint32_t dn = fast_above ? 1u : 0xffffffffu;  // +1 / -1 for the lower row
-                            const double dw = fast_above ? w : -w;
-                            if (takes) {
-                                atomicAdd(&rows.cnt[m_a + q], dn);
-                                if constexpr (kWeighted) atomicAdd(&rows.ws[m_a + q], dw);
-                            }
-                            if (gives) {
-                                atomicAdd(&rows.cnt[m_a + q + 1], 0u - dn);
-                                if constexpr (kWeighted) atomicAdd(&rows.ws[m_a + q + 1], -dw);
-                            }
-                        }
-                    }
-                    atomicAdd(&stat[kStatFp64], 1ull);
-                }
-            }
-        }
+        // a pair within the guard band of an edge: the step is noted and redone exactly after the loop
+        if (__any_sync(0xffffffffu, !(mn > G))) amb_steps |= 1u << (jj / kStep);
         if constexpr (!kWeighted) {
             if ((jj & 31) == 32 - kStep) {
 #pragma unroll
@@ -290,7 +367,9 @@ __device__ __forceinline__ void window_chunk(const WinParams &p, const Rows rows
     };
     uint32_t c_prev = 0;  // this thread's pairs above the previous edge (all its pairs before the first)
     double s_prev[kR];    // and, per i-point, the sum of their w_j
-    if constexpr (kFirst) {
+#pragma unroll
+    for (int r = 0; r < kR; ++r) s_prev[r] = 0.0;
+    if (first) {
         if constexpr (kMasked) {
             uint32_t n_unused = 0;
             c_prev = call;
@@ -314,7 +393,7 @@ __device__ __forceinline__ void window_chunk(const WinParams &p, const Rows rows
 #pragma unroll
                 for (int r = 0; r < kR; ++r) {
                     const double sw = unpack(t[q][r], c_q);
-                    if (q > 0 || kFirst) rw = fma((double)wi[r], s_prev[r] - sw, rw);
+                    if (q > 0 || first) rw = fma((double)wi[r], s_prev[r] - sw, rw);
                     s_prev[r] = sw;
                 }
             } else {
@@ -326,7 +405,7 @@ __device__ __forceinline__ void window_chunk(const WinParams &p, const Rows rows
         }
         const uint32_t rc = c_prev - c_q;
         c_prev = c_q;
-        if (q == 0 && !kFirst) continue;  // the repeated edge: row m_a was filled by the previous chunk
+        if (q == 0 && !first) continue;  // the repeated edge: row m_a was filled by the previous chunk
         if (rc == 0u) rw = 0.0;  // no pair of this thread in the row: not even a rounding residue
         const uint32_t rc_warp = __reduce_add_sync(0xffffffffu, rc);
         if constexpr (kWeighted) rw = warp_sum_f64(rw);
@@ -336,18 +415,31 @@ __device__ __forceinline__ void window_chunk(const WinParams &p, const Rows rows
         }
     }
     __syncwarp();
+    if constexpr (kDeferFix) return amb_steps;  // the caller sees to the corrections
+    if (amb_steps) fixup_chunk<kWeighted>(p, rows, grp2, amb_steps, K, m_a, first, last, kMasked, mk, i_base, j_first, stat);
+    return 0u;
 }
 
 // One group: all edges r_lo .. r_hi - 1 of its window, kChunk at a time (masked groups one at a time).
 #define ACF_WIN_CHUNK_CALL(K, MASKED, FIRST, M, LAST) \
-    window_chunk<K, kWeighted, kPacked, MASKED, FIRST>(p, rows, grp2, vgrp, nx, ny, nz, wi, M, LAST, wsum_j, mk, i_base, j_first, stat)
+    window_chunk<K, kWeighted, kPacked, MASKED>(p, rows, grp2, vgrp, nx, ny, nz, wi, M, FIRST, LAST, wsum_j, mk, i_base, j_first, stat)
+// Not inlined: only the common case (one edge, nothing masked) lives in the kernel's own loop, so that
+// the register allocation of that loop is not set by the rare variants.  It reloads the i-points.
 template <bool kWeighted, bool kPacked>
-__device__ __forceinline__ void window_group(const WinParams &p, const Rows rows, const float *__restrict__ grp2,
-                                             const double *__restrict__ vgrp, const float (&nx)[kR],
-                                             const float (&ny)[kR], const float (&nz)[kR],
-                                             const float (&wi)[kR], int r_lo, int r_hi, double wsum_j, bool masked, const Mask &mk,
-                                             uint32_t i_base, uint32_t j_first, unsigned long long *stat)
+__device__ __noinline__ void window_group(const WinParams &p, const Rows rows, const float *__restrict__ grp2,
+                                          const double *__restrict__ vgrp, int r_lo, int r_hi,
+                                          double wsum_j, bool masked, const Mask mk, uint32_t i_base, uint32_t j_first,
+                                          unsigned long long *stat)
 {
+    float nx[kR], ny[kR], nz[kR], wi[kR];
+#pragma unroll
+    for (int r = 0; r < kR; ++r) {
+        const float4 v = p.pts_a[i_base + local_i(r)];  // the array is padded to a whole tile
+        nx[r] = -v.x;
+        ny[r] = -v.y;
+        nz[r] = -v.z;
+        wi[r] = v.w;
+    }
     static_assert(kChunk == 3, "the dispatch below spells the chunk sizes out");
     if (r_hi == r_lo) {  // one row: still every pair is evaluated, against the edge that bounds the row
         if (r_lo > p.nbins) r_lo = p.nbins;
@@ -452,10 +544,13 @@ __device__ __forceinline__ void try_produce(const WinParams &p, volatile ProdSta
     atomicExch(const_cast<uint32_t *>(&ps->lock), 0u);
 }
 
-template <bool kWeighted>
+// kPacked: the variant for j-side weights that pack with the count (PackInfo); the host launches both
+// variants of a weighted count and the one that does not match the catalogue returns at once.
+template <bool kWeighted, bool kPacked>
 __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p)
 {
     if (p.counters[kCtrBadInput] != 0) return;  // inputs failed validation
+    if (kWeighted && (p.pack_b->packed != 0) != kPacked) return;
     extern __shared__ __align__(128) unsigned char smem[];
     const int rows_n = p.nbins + 2;
     const int n_stages = p.n_stages;
@@ -475,6 +570,8 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p
     double *ws_all = reinterpret_cast<double *>(smem + off);
     if constexpr (kWeighted) off += (size_t)kWarps * rows_n * sizeof(double);
     WinRows *win_all = reinterpret_cast<WinRows *>(smem + off);
+    off += (size_t)kWarps * kGroupsPerTile * sizeof(WinRows);
+    FixNote *notes_all = reinterpret_cast<FixNote *>(smem + off);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int igrp = warp & (kTeamWarps - 1), team = warp / kTeamWarps;
@@ -505,7 +602,7 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p
     rows.cnt = cnt_all + (size_t)warp * rows_n;
     rows.ws = ws_all + (size_t)warp * rows_n;
     WinRows *win = win_all + (size_t)warp * kGroupsPerTile;
-    const bool packed = !kWeighted || p.pack_b->packed != 0;
+    FixNote *notes = notes_all + (size_t)warp * kGroupsPerTile;
     uint32_t since_flush = 0;  // j-tiles this warp has tallied in its unflushed rows
     float wi[kR];
     float nx[kR], ny[kR], nz[kR];  // the i-points, negated
@@ -536,7 +633,10 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p
         const int slot = (int)(consumed % (uint32_t)n_stages);
         const uint32_t parity = (consumed / (uint32_t)n_stages) & 1u;
         if (lane == 0)
-            while (!mbar_test(&full[slot], parity)) try_produce<kWeighted>(p, ps, full, empty, meta, stages, n_stages);
+            while (!mbar_test(&full[slot], parity)) {
+                try_produce<kWeighted>(p, ps, full, empty, meta, stages, n_stages);
+                if (!mbar_test(&full[slot], parity)) __nanosleep(100);  // leave the issue slots to the warps that have work
+            }
         __syncwarp();
         mbar_wait(&full[slot], parity);  // every lane observes the completed phase
         const StageMeta m = meta[slot];
@@ -586,25 +686,59 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p
                 win[lane] = wr;
             }
             __syncwarp();
+            // pass 1: the common groups (one edge, nothing masked), inline; the others are noted in slow_groups
+            uint32_t slow_groups = 0;
+            bool any_amb = false;
+            if (lane < kGroupsPerTile) notes[lane].amb_steps = 0u;
+            __syncwarp();
             for (int g = diag ? igrp : 0; g < n_groups; ++g) {
                 if ((g & (kTeams - 1)) != team) continue;  // the other team's group
                 const int r_lo = win[g].lo, r_hi = win[g].hi;
-                const double wsum_j = win[g].wsum;
-                Mask mk;
-                mk.valid = valid_mask;
-                mk.jn = jn - g * kGroup < kGroup ? jn - g * kGroup : kGroup;
-                mk.j0 = g * kGroup;
-                mk.diag = diag && g == igrp;
-                const bool masked = !warp_full || mk.jn < kGroup || mk.diag;
-                const float *grp2 = tile + (size_t)g * kGroup * 4;
-                const double *vgrp = vtile + g * kGroup;
-                if (packed)
-                    window_group<kWeighted, true>(p, rows, grp2, vgrp, nx, ny, nz, wi, r_lo, r_hi, wsum_j, masked, mk, i_base,
-                                                  j_base + g * kGroup, stat);
-                else
-                    window_group<kWeighted, false>(p, rows, grp2, vgrp, nx, ny, nz, wi, r_lo, r_hi, wsum_j, masked, mk, i_base,
-                                                   j_base + g * kGroup, stat);
-                if (lane == 0 && !masked && r_hi - r_lo <= 1) atomicAdd(&stat[kStatWindow], (unsigned long long)(kGroup * kGroup));
+                const bool masked = !warp_full || jn - g * kGroup < kGroup || (diag && g == igrp);
+                if (masked || r_hi - r_lo > 1) {
+                    slow_groups |= 1u << g;
+                    continue;
+                }
+                // a window inside one row is tested against the edge that bounds the row
+                const int m_edge = r_hi > r_lo ? r_lo : (r_lo > p.nbins ? p.nbins : r_lo);
+                Mask mk{};
+                const uint32_t amb = window_chunk<1, kWeighted, kPacked, false, true>(p, rows, tile + (size_t)g * kGroup * 4, vtile + g * kGroup,
+                                                                                      nx, ny, nz, wi, m_edge, true, true, win[g].wsum, mk,
+                                                                                      i_base, j_base + g * kGroup, stat);
+                if (lane == 0) {
+                    atomicAdd(&stat[kStatWindow], (unsigned long long)(kGroup * kGroup));
+                    notes[g].amb_steps = amb;
+                    notes[g].m_edge = m_edge;
+                }
+                any_amb |= amb != 0u;
+            }
+            __syncwarp();
+            if (any_amb) slow_groups |= 0x80000000u;  // corrections to make: also a call, also followed by the reload
+            // pass 2: the rest through the function; it reloads the i-points, and so does this loop afterwards
+            // (they are not kept in registers across the calls)
+            if (slow_groups) {
+                if (any_amb) fixup_tile<kWeighted>(p, rows, tile, notes, i_base, j_base, stat);
+                for (int g = 0; g < n_groups; ++g) {
+                    if (!((slow_groups >> g) & 1u)) continue;
+                    const int r_lo = win[g].lo, r_hi = win[g].hi;
+                    Mask mk;
+                    mk.valid = valid_mask;
+                    mk.jn = jn - g * kGroup < kGroup ? jn - g * kGroup : kGroup;
+                    mk.j0 = g * kGroup;
+                    mk.diag = diag && g == igrp;
+                    const bool masked = !warp_full || mk.jn < kGroup || mk.diag;
+                    window_group<kWeighted, kPacked>(p, rows, tile + (size_t)g * kGroup * 4, vtile + g * kGroup, r_lo, r_hi, win[g].wsum,
+                                                     masked, mk, i_base, j_base + g * kGroup, stat);
+                    if (lane == 0 && !masked && r_hi - r_lo <= 1) atomicAdd(&stat[kStatWindow], (unsigned long long)(kGroup * kGroup));
+                }
+#pragma unroll
+                for (int r = 0; r < kR; ++r) {
+                    const float4 v = p.pts_a[i_base + local_i(r)];
+                    nx[r] = -v.x;
+                    ny[r] = -v.y;
+                    nz[r] = -v.z;
+                    wi[r] = v.w;
+                }
             }
         }
         if (tid == 0) stat[kStatEvaluated] += diag ? (unsigned long long)n_i * (n_i - 1) / 2 : (unsigned long long)n_i * (unsigned)jn;
@@ -637,7 +771,7 @@ int launch_pair_win(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_a
         m += (size_t)kWarps * rows_n * sizeof(uint32_t);
         m = (m + 15) & ~size_t(15);
         if (weighted) m += (size_t)kWarps * rows_n * sizeof(double);
-        m += (size_t)kWarps * kGroupsPerTile * sizeof(WinRows);
+        m += (size_t)kWarps * kGroupsPerTile * (sizeof(WinRows) + sizeof(FixNote));
         return m;
     };
     // one CTA of 16 warps per SM: 128 registers a thread
@@ -674,17 +808,21 @@ int launch_pair_win(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_a
     p.n_stages = n_stages;
 
     const int grid = ctx->num_sms * ctas_per_sm;
-    cudaError_t e;
+    cudaError_t e = cudaSuccess;
+    auto launch = [&](auto kern) {
+        if (e != cudaSuccess) return;
+        e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (e == cudaSuccess) kern<<<grid, kThreads, smem, ctx->stream>>>(p);
+        ctx->last.kernel_launches++;
+    };
     if (weighted) {
-        e = cudaFuncSetAttribute(pair_win_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e == cudaSuccess) pair_win_kernel<true><<<grid, kThreads, smem, ctx->stream>>>(p);
+        launch(pair_win_kernel<true, true>);
+        launch(pair_win_kernel<true, false>);  // one of the two returns at once (PackInfo of the j side)
     } else {
-        e = cudaFuncSetAttribute(pair_win_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-        if (e == cudaSuccess) pair_win_kernel<false><<<grid, kThreads, smem, ctx->stream>>>(p);
+        launch(pair_win_kernel<false, true>);
     }
     if (e == cudaSuccess) e = cudaGetLastError();
     ACF_CUDA_TRY(ctx, e);
-    ctx->last.kernel_launches++;
     return ACF_OK;
 }
 
