@@ -44,6 +44,7 @@ def parse_args():
     ap.add_argument("--workload", default="full_sky")
     ap.add_argument("--scale", type=float, default=1.0)
     ap.add_argument("--cpu-rows", type=int, default=0, help="rows of the oracle sample (0 = auto)")
+    ap.add_argument("--kernel", default="auto", choices=["auto", "table", "window"], help="pair kernel (ACF_OPT_KERNEL)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -178,6 +179,7 @@ def main():
     w = make_config(args.workload, args.scale, seed_offset=1000 * rank)
     weighted = w.w_d is not None
     ctx = P.acf_create(local_rank)
+    P.acf_set_option(ctx, P.ACF_OPT_KERNEL, {"auto": P.ACF_KERNEL_AUTO, "table": P.ACF_KERNEL_TABLE, "window": P.ACF_KERNEL_WINDOW}[args.kernel])
     dev = torch.device("cuda", local_rank)
     h_xd = P.acf_radec_to_xyz(w.ra_d, w.dec_d)
     h_xr = P.acf_radec_to_xyz(w.ra_r, w.dec_r)

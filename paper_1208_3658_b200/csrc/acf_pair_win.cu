@@ -230,6 +230,13 @@ __device__ __noinline__ void fixup_tile(const WinParams &p, const Rows rows, con
     }
 }
 
+// One thread's tallies of the two rows around an edge, kept in registers over consecutive groups that
+// are tested against the same edge (the common single-edge groups of the kernel's own loop).
+struct LaneTally {
+    uint32_t c_lo, c_hi;  // pairs in row m / row m + 1
+    double w_lo, w_hi;    // and their weight
+};
+
 // Edges m_a .. m_a + K - 1 against one group of kGroup staged j-points and this thread's kR i-points.
 // The first chunk of a group (first) fills rows m_a .. m_a + K - 1 (and m_a + K if it is also the last).
 // A later chunk starts with the previous chunk's last edge again, only to have the tallies above it
@@ -239,7 +246,8 @@ __device__ __forceinline__ uint32_t window_chunk(const WinParams &p, const Rows 
                                              const double *__restrict__ vgrp, const float (&nx)[kR],
                                              const float (&ny)[kR], const float (&nz)[kR],
                                              const float (&wi)[kR], const int m_a, const bool first, const bool last, const double wsum_j,
-                                             const Mask &mk, uint32_t i_base, uint32_t j_first, unsigned long long *stat)
+                                             const Mask &mk, uint32_t i_base, uint32_t j_first, unsigned long long *stat,
+                                             LaneTally *tally = nullptr)
 {
     const int lane = threadIdx.x & 31;
     const double e0 = p.edges[m_a];
@@ -274,7 +282,7 @@ __device__ __forceinline__ uint32_t window_chunk(const WinParams &p, const Rows 
     }
 #pragma unroll
     for (int r = 0; r < kR; ++r) tall[r] = 0.0;
-    constexpr int kInd = 2 * kR;  // indicator registers: low words zero for the whole loop
+    constexpr int kInd = (K == 1 ? kStep : 2) * kR;  // indicator registers: low words zero for the whole loop
     unsigned long long ind[kInd];
 #pragma unroll
     for (int i = 0; i < kInd; ++i) ind[i] = 0ull;
@@ -314,7 +322,7 @@ __device__ __forceinline__ uint32_t window_chunk(const WinParams &p, const Rows 
                     const unsigned long long dq2 = q == 0 ? d2 : fadd2(d2, dl2[q]);
                     const float a = lo32(dq2), b = hi32(dq2);
                     if constexpr (kWeighted && !kMasked) {
-                        unsigned long long &g0 = ind[(2 * r) % kInd], &g1 = ind[(2 * r + 1) % kInd];
+                        unsigned long long &g0 = ind[(u * kR + 2 * r) % kInd], &g1 = ind[(u * kR + 2 * r + 1) % kInd];
                         t[q][r] = fma(v0, ind_gt0_f64(g0, a), t[q][r]);
                         t[q][r] = fma(v1, ind_gt0_f64(g1, b), t[q][r]);
                         if constexpr (!kPacked) nf[q] += __uint_as_float((uint32_t)(g0 >> 32)) + __uint_as_float((uint32_t)(g1 >> 32));
@@ -365,6 +373,26 @@ __device__ __forceinline__ uint32_t window_chunk(const WinParams &p, const Rows 
         }
         return sw;
     };
+    if constexpr (kDeferFix) {
+        // the kernel's own loop: one edge, nothing masked; the two rows' tallies stay with the thread
+        static_assert(K == 1 && !kMasked, "");
+        uint32_t c_hi = kWeighted ? (kPacked ? 0u : (uint32_t)nf[0]) : (uint32_t)(kGroup * kR) - nb[0];
+        double w_lo = 0.0, w_hi = 0.0;
+        if constexpr (kWeighted) {
+#pragma unroll
+            for (int r = 0; r < kR; ++r) {
+                const double sw = unpack(t[0][r], c_hi);
+                w_lo = fma((double)wi[r], wsum_j - sw, w_lo);
+                w_hi = fma((double)wi[r], sw, w_hi);
+            }
+        }
+        const uint32_t c_lo = (uint32_t)(kGroup * kR) - c_hi;
+        tally->c_lo += c_lo;
+        tally->c_hi += c_hi;
+        if (c_lo != 0u) tally->w_lo += w_lo;  // no pair of this thread in the row: not even a rounding residue
+        if (c_hi != 0u) tally->w_hi += w_hi;
+        return amb_steps;  // the caller sees to the corrections
+    }
     uint32_t c_prev = 0;  // this thread's pairs above the previous edge (all its pairs before the first)
     double s_prev[kR];    // and, per i-point, the sum of their w_j
 #pragma unroll
@@ -415,7 +443,6 @@ __device__ __forceinline__ uint32_t window_chunk(const WinParams &p, const Rows 
         }
     }
     __syncwarp();
-    if constexpr (kDeferFix) return amb_steps;  // the caller sees to the corrections
     if (amb_steps) fixup_chunk<kWeighted>(p, rows, grp2, amb_steps, K, m_a, first, last, kMasked, mk, i_base, j_first, stat);
     return 0u;
 }
@@ -612,8 +639,32 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p
     bool warp_full = false, warp_any = false;
     int cur_ti = -1;
 
+    LaneTally tally{0u, 0u, 0.0, 0.0};
+    int tally_m = -1;  // the edge the tally belongs to (warp-uniform)
+    auto flush_tally = [&]() {
+        // the threads' tallies of rows tally_m and tally_m + 1 -> the warp's rows
+        if (tally_m >= 0) {
+            const uint32_t c_lo = __reduce_add_sync(0xffffffffu, tally.c_lo), c_hi = __reduce_add_sync(0xffffffffu, tally.c_hi);
+            double w_lo = 0.0, w_hi = 0.0;
+            if constexpr (kWeighted) {
+                w_lo = warp_sum_f64(tally.w_lo);
+                w_hi = warp_sum_f64(tally.w_hi);
+            }
+            if (lane == 0) {
+                rows.cnt[tally_m] += c_lo;
+                rows.cnt[tally_m + 1] += c_hi;
+                if constexpr (kWeighted) {
+                    rows.ws[tally_m] += w_lo;
+                    rows.ws[tally_m + 1] += w_hi;
+                }
+            }
+            tally = LaneTally{0u, 0u, 0.0, 0.0};
+            tally_m = -1;
+        }
+    };
     auto flush_rows = [&]() {
         // this warp's rows -> global (u64 / f64 atomics); the rows restart from zero
+        flush_tally();
         __syncwarp();
         for (int row = lane; row < rows_n; row += 32) {
             const uint32_t v = rows.cnt[row];
@@ -702,9 +753,13 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p
                 // a window inside one row is tested against the edge that bounds the row
                 const int m_edge = r_hi > r_lo ? r_lo : (r_lo > p.nbins ? p.nbins : r_lo);
                 Mask mk{};
+                if (m_edge != tally_m) {
+                    flush_tally();
+                    tally_m = m_edge;
+                }
                 const uint32_t amb = window_chunk<1, kWeighted, kPacked, false, true>(p, rows, tile + (size_t)g * kGroup * 4, vtile + g * kGroup,
                                                                                       nx, ny, nz, wi, m_edge, true, true, win[g].wsum, mk,
-                                                                                      i_base, j_base + g * kGroup, stat);
+                                                                                      i_base, j_base + g * kGroup, stat, &tally);
                 if (lane == 0) {
                     atomicAdd(&stat[kStatWindow], (unsigned long long)(kGroup * kGroup));
                     notes[g].amb_steps = amb;
