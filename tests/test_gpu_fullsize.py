@@ -47,12 +47,13 @@ class Dev:
         self.wr = torch.from_numpy(w.w_r).cuda() if w.w_r is not None else None
 
 
-def count(acf, ctx, d, which, rows=None, windows=1):
+def count(acf, ctx, d, which, rows=None, windows=1, kernel=None):
     """-> (u64 counts, f64 sums or None, stats) of DD / DR / RD / RR on the device."""
     import torch
     a, wa, b, wb, auto = {"dd": (d.xd, d.wd, None, None, True), "dr": (d.xd, d.wd, d.xr, d.wr, False),
                           "rd": (d.xr, d.wr, d.xd, d.wd, False), "rr": (d.xr, d.wr, None, None, True)}[which]
     acf.acf_set_option(ctx, acf.ACF_OPT_WINDOWS, windows)
+    acf.acf_set_option(ctx, acf.ACF_OPT_KERNEL, acf.ACF_KERNEL_AUTO if kernel is None else kernel)
     try:
         n_a = a.numel() // 3
         lo, hi = rows if rows is not None else (0, n_a)
@@ -61,6 +62,7 @@ def count(acf, ctx, d, which, rows=None, windows=1):
         st = acf.acf_get_stats(ctx)
     finally:
         acf.acf_set_option(ctx, acf.ACF_OPT_WINDOWS, 1)
+        acf.acf_set_option(ctx, acf.ACF_OPT_KERNEL, acf.ACF_KERNEL_AUTO)
     if wa is None:
         return acf.counts_to_numpy(out), None, st
     return acf.counts_to_numpy(out[0]), out[1].cpu().numpy(), st
@@ -104,13 +106,16 @@ def test_fullsize_sampled_rows_and_properties(acf, ctx, oracle, name, width):
         nominal = n_a * (n_a - 1) // 2 if k != "dr" else w.n_d * w.n_r
         assert st["pairs_nominal"] == nominal and 0 < st["pairs_evaluated"] <= nominal
         assert int(c.sum()) <= nominal
-    # window path == table path (independent classification code), bit for bit
+    # three independent classification codes, bit for bit: the window kernel (edges of a window against
+    # register tallies), the table kernel with its single-edge windows, and the table kernel's cell table alone
     for k in ("dd", "dr"):
-        c2, s2, st2 = count(acf, ctx, d, k, windows=0)
-        assert st2["pairs_window"] == 0
-        assert c2.tolist() == full[k][0].tolist(), k
-        if weighted:
-            np.testing.assert_allclose(s2, full[k][1], rtol=WSUM_RTOL, atol=0)
+        for kern, windows in ((acf.ACF_KERNEL_WINDOW, 1), (acf.ACF_KERNEL_TABLE, 1), (acf.ACF_KERNEL_TABLE, 0)):
+            c2, s2, st2 = count(acf, ctx, d, k, windows=windows, kernel=kern)
+            assert windows == 1 or st2["pairs_window"] == 0
+            assert st2["pairs_evaluated"] == full[k][2]["pairs_evaluated"]
+            assert c2.tolist() == full[k][0].tolist(), (k, kern, windows)
+            if weighted:
+                np.testing.assert_allclose(s2, full[k][1], rtol=WSUM_RTOL, atol=0)
     # swapping the catalogues of a cross count changes every tile, window and work item, not the result
     c3, s3, _ = count(acf, ctx, d, "rd")
     assert c3.tolist() == full["dr"][0].tolist()

@@ -197,17 +197,19 @@ def test_degenerate_sizes(acf, ctx):
     assert gpu_counts(acf, ctx, two, None, edges, True, rows=(1, 1)).tolist() == [0, 0]
 
 
-def test_row_ranges_add_up(acf, ctx, oracle):
+@pytest.mark.parametrize("kernel", ["table", "window"])
+def test_row_ranges_add_up(acf, ctx, oracle, kernel):
     # the pair matrix cut into sub-matrices; counts are additive over row ranges
+    kern = {"table": acf.ACF_KERNEL_TABLE, "window": acf.ACF_KERNEL_WINDOW}[kernel]
     w = make_config("clustered_patch", 0.02)
     xd, xr = acf.acf_radec_to_xyz(w.ra_d, w.dec_d), acf.acf_radec_to_xyz(w.ra_r, w.dec_r)
     n = w.n_d
     cuts = [0, 1, 777, 1024, 2049, n]
     for b, auto in ((None, True), (xr, False)):
-        whole = gpu_counts(acf, ctx, xd, b, w.cos_edges, auto)
+        whole = gpu_counts(acf, ctx, xd, b, w.cos_edges, auto, kernel=kern)
         parts = np.zeros_like(whole)
         for lo, hi in zip(cuts[:-1], cuts[1:]):
-            p = gpu_counts(acf, ctx, xd, b, w.cos_edges, auto, rows=(lo, hi))
+            p = gpu_counts(acf, ctx, xd, b, w.cos_edges, auto, rows=(lo, hi), kernel=kern)
             assert p.tolist() == oracle.pair_count(xd, b, w.cos_edges, auto, rows=(lo, hi)).tolist()
             parts += p
         assert parts.tolist() == whole.tolist()
@@ -219,7 +221,35 @@ def test_linear_bins_many(acf, ctx, oracle):
     a = acf.acf_radec_to_xyz(ra, dec)
     for theta in (linear_theta_edges_deg(0.0, 120.0, 254), log_theta_edges_deg(0.01, 100.0, 254)):
         edges = cos_edges_from_theta_deg(theta)
-        assert gpu_counts(acf, ctx, a, None, edges, True).tolist() == oracle.pair_count(a, None, edges, True).tolist()
+        want = oracle.pair_count(a, None, edges, True).tolist()
+        for kern in (acf.ACF_KERNEL_TABLE, acf.ACF_KERNEL_WINDOW):
+            assert gpu_counts(acf, ctx, a, None, edges, True, kernel=kern).tolist() == want
+    acf.acf_set_option(ctx, acf.ACF_OPT_KERNEL, acf.ACF_KERNEL_AUTO)
+
+
+@pytest.mark.parametrize("kernel", ["table", "window"])
+def test_weights_wide_range_and_zero(acf, ctx, oracle, kernel):
+    """Weights that cannot share an fp64 accumulator with the count (range far above 2^13, zeros among them):
+    the window kernel must take its unpacked variant; narrow-range weights take the packed one.  Both
+    against the oracle, counts exact and sums to 1e-12."""
+    kern = {"table": acf.ACF_KERNEL_TABLE, "window": acf.ACF_KERNEL_WINDOW}[kernel]
+    ra, dec = full_sky(5000, 61)
+    rb, db = full_sky(4100, 62)
+    a, b = acf.acf_radec_to_xyz(ra, dec), acf.acf_radec_to_xyz(rb, db)
+    rng = np.random.default_rng(63)
+    edges = cos_edges_from_theta_deg(log_theta_edges_deg(0.5, 180.0, 24))
+    for lo, hi, zeros in ((-20.0, 10.0, True), (-1.0, 1.0, False), (-6.0, 7.0, False)):
+        wa = np.exp(rng.uniform(lo, hi, 5000)).astype(np.float32)
+        wb = np.exp(rng.uniform(lo, hi, 4100)).astype(np.float32)
+        if zeros:
+            wa[::7] = 0.0
+            wb[::5] = 0.0
+        for xb, w_b, auto in ((None, None, True), (b, wb, False)):
+            got = gpu_counts(acf, ctx, a, xb, edges, auto, wa=wa, wb=w_b, kernel=kern)
+            want = oracle.pair_count(a, xb, edges, auto, w_a=wa, w_b=w_b)
+            assert got[0].tolist() == want[0].tolist()
+            np.testing.assert_allclose(got[1], want[1], rtol=WSUM_RTOL, atol=0)
+    acf.acf_set_option(ctx, acf.ACF_OPT_KERNEL, acf.ACF_KERNEL_AUTO)
 
 
 def test_weighted_dyadic_exact(acf, ctx):
