@@ -33,6 +33,10 @@ UNIT = "Gpairs/s"
 # SURVEY.md 8(d) / DESIGN.md "Roofline": algorithmic thread-instructions per pair
 I_ALG_UNWEIGHTED = 11
 I_ALG_WEIGHTED = 14
+# From the committed ncu capture of the dominant kernel on the default workload (one launch: the weighted DR
+# count, 1.0e12 pairs); not measured by this script.  See profiles/r1_v5_pair_win_kernel_ncu.md.
+NCU_FULL_SKY = {"profile": "profiles/r1_v5_pair_win_kernel_ncu.md", "launch": "weighted DR count, 1.0e12 pairs",
+                "dram_bytes": 991470592, "sass_thread_inst_per_pair": 7.41, "issue_active_pct": 58.6}
 
 
 def parse_args():
@@ -285,8 +289,11 @@ def main():
     pair_s = pair_ms_per_step * 1e-3
     achieved = evaluated_per_step * i_alg / pair_s / 1e12 if pair_s > 0 else 0.0
     roofline = {
-        "bound": "alu", "kernel": "pair_kernel", "achieved": achieved, "peak": peak_tinst, "unit": "Tinst/s",
-        "frac": achieved / peak_tinst, "traffic": None,
+        "bound": "alu", "kernel": "pair_win_kernel" if (weighted or args.kernel == "window") and args.kernel != "table" else "pair_kernel", "achieved": achieved, "peak": peak_tinst, "unit": "Tinst/s",
+        "frac": achieved / peak_tinst,
+        "traffic": NCU_FULL_SKY["dram_bytes"] if (args.workload == "full_sky" and args.scale == 1.0 and args.kernel == "auto") else None,
+        "traffic_is": "dram__bytes_read.sum + dram__bytes_write.sum of one launch (%s), %s" % (NCU_FULL_SKY["launch"], NCU_FULL_SKY["profile"]),
+        "ncu": NCU_FULL_SKY if (args.workload == "full_sky" and args.scale == 1.0 and args.kernel == "auto") else None,
         "algorithmic_inst_per_pair": i_alg, "pairs_per_step": evaluated_per_step, "kernel_ms_per_step": pair_ms_per_step,
         "kernel_share_of_step": pair_kernel_share,
         "peak_is": "%d SMs x 4 schedulers x 32 lanes x %.0f MHz (max SM clock, MEASURED_PEAKS.json / fallback 1965)"
