@@ -720,21 +720,25 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p
         ++since_flush;
 
         if (warp_any) {
-            // lane g bounds the rows of this warp's i-group against j-group g of the tile
+            // lane l bounds the rows of this warp's i-group against the team's l-th j-group of the tile
             const int n_groups = (jn + kGroup - 1) / kGroup;
             __syncwarp();
-            if (lane < n_groups) {
+            const int my_g = lane * kTeams + team;
+            if (lane < kGroupsPerTile / kTeams && my_g < n_groups) {
                 WinRows wr;
                 wr.lo = 0;
                 wr.hi = p.nbins + 1;
-                const GroupCap gb = p.gcaps_b[(size_t)tj * kGroupsPerTile + lane];
+                const GroupCap gb = p.gcaps_b[(size_t)tj * kGroupsPerTile + my_g];
                 double c_lo, c_hi;
                 if (cap_window(p.gcaps_a[(size_t)m.ti * kGroupsPerTile + igrp], gb, c_lo, c_hi)) {
-                    wr.lo = row_of_cos(c_hi, p.edges, p.nbins);
-                    wr.hi = row_of_cos(c_lo, p.edges, p.nbins);
+                    // rows of the two ends; the far end is a few rows on at most: walk there
+                    int hi = wr.lo = row_of_cos(c_hi, p.edges, p.nbins);
+                    while (hi < p.nbins && c_lo <= p.edges[hi]) ++hi;
+                    if (hi == p.nbins && c_lo < p.edges[p.nbins]) ++hi;
+                    wr.hi = hi;
                 }
                 wr.wsum = gb.wsum;
-                win[lane] = wr;
+                win[my_g] = wr;
             }
             __syncwarp();
             // pass 1: the common groups (one edge, nothing masked), inline; the others are noted in slow_groups
