@@ -179,11 +179,15 @@ def test_duplicates_and_clamp(acf, ctx, oracle):
     a = acf.acf_radec_to_xyz(ra, dec)
     for edges in (cos_edges_from_theta_deg(np.array([0.0, 1.0, 90.0, 180.0])),
                   cos_edges_from_theta_deg(np.array([1e-6, 1.0, 90.0, 180.0]))):
-        assert gpu_counts(acf, ctx, a, None, edges, True).tolist() == oracle.pair_count(a, None, edges, True).tolist()
+        want = oracle.pair_count(a, None, edges, True).tolist()
+        for kern in (acf.ACF_KERNEL_TABLE, acf.ACF_KERNEL_WINDOW):
+            assert gpu_counts(acf, ctx, a, None, edges, True, kernel=kern).tolist() == want
 
 
-def test_degenerate_sizes(acf, ctx):
+@pytest.mark.parametrize("kernel", ["table", "window"])
+def test_degenerate_sizes(acf, ctx, kernel):
     import torch
+    acf.acf_set_option(ctx, acf.ACF_OPT_KERNEL, {"table": acf.ACF_KERNEL_TABLE, "window": acf.ACF_KERNEL_WINDOW}[kernel])
     edges = np.array([1.0, 0.0, -1.0])
     one = soa([(0.0, 0.0, 1.0)])
     two = soa([(0.0, 0.0, 1.0), (0.0, 1.0, 0.0)])
@@ -195,6 +199,10 @@ def test_degenerate_sizes(acf, ctx):
     torch.cuda.synchronize()
     assert out.cpu().tolist() == [0, 0]
     assert gpu_counts(acf, ctx, two, None, edges, True, rows=(1, 1)).tolist() == [0, 0]
+    ones = np.ones(2, np.float32)
+    c, ws = gpu_counts(acf, ctx, two, None, edges, True, wa=ones)                   # weighted, one pair
+    assert c.tolist() == [0, 1] and ws.tolist() == [0.0, 1.0]
+    acf.acf_set_option(ctx, acf.ACF_OPT_KERNEL, acf.ACF_KERNEL_AUTO)
 
 
 @pytest.mark.parametrize("kernel", ["table", "window"])
