@@ -63,7 +63,9 @@ enum {
      * debugging); ACF_KERNEL_TABLE = fast path, cell-table kernel (single-edge windows in registers,
      * everything else through a bin table and per-lane shared-memory histograms);
      * ACF_KERNEL_WINDOW = fast path, window kernel (every group of pairs classified in registers
-     * against the few edges its bounding caps allow).  All four give the same counts. */
+     * against the few edges its bounding caps allow).  All four give the same counts.  With very many
+     * bins a kernel's shared-memory histograms may not fit: AUTO then takes the other fast kernel, an
+     * explicit choice returns ACF_EINVAL. */
     ACF_OPT_KERNEL = 1,
     /* 1 (default): tile pairs that provably hold no in-range pair are skipped
      * ("ignoring calculations that would fall outside the bin range");

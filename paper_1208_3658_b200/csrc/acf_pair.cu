@@ -642,7 +642,13 @@ int count_prepared(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_au
     int n_stages = 2;
     while (n_stages < 4 && smem_for(n_stages + 1) <= budget) ++n_stages;
     const size_t smem = smem_for(n_stages);
-    if (smem > per_sm) return fail(ctx, ACF_EINVAL, "shared memory need %zu exceeds %d", smem, ctx->max_smem_optin);
+    // which kernel: the window kernel for weighted counts, the table kernel for unweighted ones;
+    // with very many bins the table kernel's rows may not fit beside its table: the window kernel then takes over
+    bool use_win = ctx->opt_kernel == ACF_KERNEL_WINDOW || (ctx->opt_kernel == ACF_KERNEL_AUTO && weighted);
+    if (!use_win && smem > per_sm) {
+        if (ctx->opt_kernel != ACF_KERNEL_AUTO) return fail(ctx, ACF_EINVAL, "shared memory need %zu exceeds %d", smem, ctx->max_smem_optin);
+        use_win = true;
+    }
 
     // i-tiles are handed out in batches so that the item buffer stays bounded
     // (worst case one item per surviving j-tile: survivors may alternate with pruned tiles)
@@ -695,7 +701,6 @@ int count_prepared(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_au
             ACF_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_k0, ctx->stream));
             ctx->pair_timed = true;
         }
-        const bool use_win = ctx->opt_kernel == ACF_KERNEL_WINDOW || (ctx->opt_kernel == ACF_KERNEL_AUTO && weighted);
         if (use_win) {
             rc = launch_pair_win(ctx, a, b, is_auto, nbins, capacity, d_counts, d_wsums);
             if (rc != ACF_OK) return rc;

@@ -69,6 +69,7 @@ struct WinParams {
     unsigned long long *counters;
     int is_auto;
     int n_stages;
+    int shared_rows;  // 1: one set of histogram rows per CTA instead of one per warp
 };
 
 __device__ __forceinline__ unsigned long long fadd2(unsigned long long a, unsigned long long b)
@@ -102,6 +103,19 @@ __device__ __forceinline__ double ind_gt0_f64(unsigned long long &reg, float v)
 struct Rows {
     uint32_t *cnt;
     double *ws;
+    bool shared;  // one set of rows for the whole CTA (many bins): every update is atomic
+    template <bool kWeighted>
+    __device__ __forceinline__ void add(int row, uint32_t c, double w) const
+    {
+        if (shared) {
+            if (c) atomicAdd(&cnt[row], c);
+            if constexpr (kWeighted)
+                if (w != 0.0) atomicAdd(&ws[row], w);
+        } else {
+            cnt[row] += c;
+            if constexpr (kWeighted) ws[row] += w;
+        }
+    }
 };
 // per-CTA statistics kept in shared memory until the kernel ends
 enum { kStatFp64 = 0, kStatWindow = 1, kStatEvaluated = 2, kNumStats = 3 };
@@ -438,8 +452,7 @@ __device__ __forceinline__ uint32_t window_chunk(const WinParams &p, const Rows 
         const uint32_t rc_warp = __reduce_add_sync(0xffffffffu, rc);
         if constexpr (kWeighted) rw = warp_sum_f64(rw);
         if (lane == 0) {
-            rows.cnt[m_a + q] += rc_warp;
-            if constexpr (kWeighted) rows.ws[m_a + q] += rw;
+            rows.template add<kWeighted>(m_a + q, rc_warp, rw);
         }
     }
     __syncwarp();
@@ -592,17 +605,18 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p
     unsigned char *stages = smem + kSmemHeader;
     size_t off = kSmemHeader + (size_t)n_stages * kStage;
     uint32_t *cnt_all = reinterpret_cast<uint32_t *>(smem + off);
-    off += (size_t)kWarps * rows_n * sizeof(uint32_t);
+    const int row_sets = p.shared_rows ? 1 : kWarps;
+    off += (size_t)row_sets * rows_n * sizeof(uint32_t);
     off = (off + 15) & ~size_t(15);
     double *ws_all = reinterpret_cast<double *>(smem + off);
-    if constexpr (kWeighted) off += (size_t)kWarps * rows_n * sizeof(double);
+    if constexpr (kWeighted) off += (size_t)row_sets * rows_n * sizeof(double);
     WinRows *win_all = reinterpret_cast<WinRows *>(smem + off);
     off += (size_t)kWarps * kGroupsPerTile * sizeof(WinRows);
     FixNote *notes_all = reinterpret_cast<FixNote *>(smem + off);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int igrp = warp & (kTeamWarps - 1), team = warp / kTeamWarps;
-    for (int i = tid; i < kWarps * rows_n; i += blockDim.x) {
+    for (int i = tid; i < row_sets * rows_n; i += blockDim.x) {
         cnt_all[i] = 0;
         if constexpr (kWeighted) ws_all[i] = 0.0;
     }
@@ -626,11 +640,14 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p
 
     // ---------------- consumers
     Rows rows;
-    rows.cnt = cnt_all + (size_t)warp * rows_n;
-    rows.ws = ws_all + (size_t)warp * rows_n;
+    rows.shared = p.shared_rows != 0;
+    rows.cnt = cnt_all + (rows.shared ? 0 : (size_t)warp * rows_n);
+    rows.ws = ws_all + (rows.shared ? 0 : (size_t)warp * rows_n);
     WinRows *win = win_all + (size_t)warp * kGroupsPerTile;
     FixNote *notes = notes_all + (size_t)warp * kGroupsPerTile;
     uint32_t since_flush = 0;  // j-tiles this warp has tallied in its unflushed rows
+    // u32 rows: flush before the tallies could wrap (shared rows take the pairs of all the CTA's warps)
+    const uint32_t flush_every = (1u << 31) / (uint32_t)(kGroup * kTile) / (rows.shared ? (uint32_t)kWarps : 1u);
     float wi[kR];
     float nx[kR], ny[kR], nz[kR];  // the i-points, negated
 #pragma unroll
@@ -651,12 +668,8 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p
                 w_hi = warp_sum_f64(tally.w_hi);
             }
             if (lane == 0) {
-                rows.cnt[tally_m] += c_lo;
-                rows.cnt[tally_m + 1] += c_hi;
-                if constexpr (kWeighted) {
-                    rows.ws[tally_m] += w_lo;
-                    rows.ws[tally_m + 1] += w_hi;
-                }
+                rows.template add<kWeighted>(tally_m, c_lo, w_lo);
+                rows.template add<kWeighted>(tally_m + 1, c_hi, w_hi);
             }
             tally = LaneTally{0u, 0u, 0.0, 0.0};
             tally_m = -1;
@@ -667,12 +680,14 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p
         flush_tally();
         __syncwarp();
         for (int row = lane; row < rows_n; row += 32) {
-            const uint32_t v = rows.cnt[row];
-            rows.cnt[row] = 0;
+            // (shared rows: other warps add while this one takes the value and leaves zero)
+            const uint32_t v = rows.shared ? atomicExch(&rows.cnt[row], 0u) : rows.cnt[row];
+            if (!rows.shared) rows.cnt[row] = 0;
             if (row >= 1 && row <= p.nbins && v) atomicAdd(&p.counts[row - 1], (unsigned long long)v);
             if constexpr (kWeighted) {
-                const double w = rows.ws[row];
-                rows.ws[row] = 0.0;
+                const double w = rows.shared ? __longlong_as_double((long long)atomicExch(reinterpret_cast<unsigned long long *>(&rows.ws[row]), 0ull))
+                                             : rows.ws[row];
+                if (!rows.shared) rows.ws[row] = 0.0;
                 if (row >= 1 && row <= p.nbins && w != 0.0) atomicAdd(&p.wsums[row - 1], w);
             }
         }
@@ -716,7 +731,7 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p
         const bool diag = p.is_auto && tj == m.ti;
         const uint32_t j_base = (uint32_t)tj * kTile;
         // u32 rows: flush before this warp's tallies could wrap
-        if (since_flush >= (1u << 31) / (uint32_t)(kGroup * kTile)) flush_rows();
+        if (since_flush >= flush_every) flush_rows();
         ++since_flush;
 
         if (warp_any) {
@@ -825,17 +840,19 @@ int launch_pair_win(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_a
 {
     const bool weighted = d_wsums != nullptr;
     const int rows_n = nbins + 2;
+    int row_sets = kWarps;  // a set of rows per warp, or one per CTA when that leaves no room for the ring
     auto smem_for = [&](int stages) {
         size_t m = kSmemHeader + (size_t)stages * stage_bytes(weighted);
-        m += (size_t)kWarps * rows_n * sizeof(uint32_t);
+        m += (size_t)row_sets * rows_n * sizeof(uint32_t);
         m = (m + 15) & ~size_t(15);
-        if (weighted) m += (size_t)kWarps * rows_n * sizeof(double);
+        if (weighted) m += (size_t)row_sets * rows_n * sizeof(double);
         m += (size_t)kWarps * kGroupsPerTile * (sizeof(WinRows) + sizeof(FixNote));
         return m;
     };
     // one CTA of 16 warps per SM: 128 registers a thread
     const int ctas_per_sm = 1;
     const size_t budget = (size_t)ctx->max_smem_optin;
+    if (smem_for(4) > budget) row_sets = 1;
     if (smem_for(2) > budget) return fail(ctx, ACF_EINVAL, "too many bins for the window kernel (%d)", nbins);
     int n_stages = 2;
     while (n_stages < kMaxStages && smem_for(n_stages + 1) <= budget) ++n_stages;
@@ -865,6 +882,7 @@ int launch_pair_win(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_a
     p.counters = ctx->d_counters;
     p.is_auto = is_auto;
     p.n_stages = n_stages;
+    p.shared_rows = row_sets == 1 ? 1 : 0;
 
     const int grid = ctx->num_sms * ctas_per_sm;
     cudaError_t e = cudaSuccess;

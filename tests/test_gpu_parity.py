@@ -235,6 +235,22 @@ def test_linear_bins_many(acf, ctx, oracle):
     acf.acf_set_option(ctx, acf.ACF_OPT_KERNEL, acf.ACF_KERNEL_AUTO)
 
 
+@pytest.mark.parametrize("kernel", ["auto", "window"])
+def test_maximum_number_of_bins(acf, ctx, oracle, kernel):
+    """ACF_MAX_BINS bins, unweighted and weighted: the window kernel then keeps one set of histogram rows per
+    CTA instead of one per warp; AUTO must find a kernel whose shared memory fits."""
+    kern = {"auto": acf.ACF_KERNEL_AUTO, "window": acf.ACF_KERNEL_WINDOW}[kernel]
+    ra, dec = full_sky(3000, 7)
+    a = acf.acf_radec_to_xyz(ra, dec)
+    wa = np.random.default_rng(8).uniform(0.5, 2.0, 3000).astype(np.float32)
+    edges = cos_edges_from_theta_deg(linear_theta_edges_deg(0.0, 180.0, 1024))
+    assert gpu_counts(acf, ctx, a, None, edges, True, kernel=kern).tolist() == oracle.pair_count(a, None, edges, True).tolist()
+    got = gpu_counts(acf, ctx, a, None, edges, True, wa=wa, kernel=kern)
+    want = oracle.pair_count(a, None, edges, True, w_a=wa)
+    assert got[0].tolist() == want[0].tolist()
+    np.testing.assert_allclose(got[1], want[1], rtol=WSUM_RTOL, atol=0)
+
+
 @pytest.mark.parametrize("kernel", ["table", "window"])
 def test_weights_wide_range_and_zero(acf, ctx, oracle, kernel):
     """Weights that cannot share an fp64 accumulator with the count (range far above 2^13, zeros among them):
