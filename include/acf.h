@@ -170,6 +170,33 @@ int acf_wtheta_weighted(const double *wdd, const double *wdr, const double *wrr,
                         size_t n_d, const float *w_r, size_t n_r, int nbins, double *w_host);
 
 /*
+ * Other estimators on the same three histograms ("allows the user to easily experiment
+ * with other estimators"), pure host, O(nbins).  With dd, dr, rr the pair-normalised counts of acf_wtheta:
+ *   ACF_EST_LANDY_SZALAY  (dd - 2 dr + rr) / rr     (Eq. 2; the same values as acf_wtheta)
+ *   ACF_EST_NATURAL       dd / rr - 1               (Peebles & Hauser)
+ *   ACF_EST_DAVIS_PEEBLES dd / dr - 1
+ *   ACF_EST_HAMILTON      dd rr / dr^2 - 1
+ * NaN where the estimator's denominator is zero.  ACF_EINVAL for an unknown kind.
+ */
+enum { ACF_EST_LANDY_SZALAY = 0, ACF_EST_NATURAL = 1, ACF_EST_DAVIS_PEEBLES = 2, ACF_EST_HAMILTON = 3 };
+int acf_estimator(int kind, const uint64_t *dd, const uint64_t *dr, const uint64_t *rr, uint64_t n_d,
+                  uint64_t n_r, int nbins, double *w_host);
+
+/*
+ * The paper's bin presets (a low and a high limit and "evenly spaced, natural log or
+ * log base 10" bins), pure host.  theta_deg_host: HOST, nbins + 1 doubles, overwritten, ascending:
+ *   ACF_BINS_EVEN   theta_k = lo + (hi - lo) k / nbins
+ *   ACF_BINS_LOG    theta_k = lo (hi / lo)^(k / nbins)   (lo > 0; natural log and log10 spacing are the
+ *   ACF_BINS_LOG10                                        same edges, both names are accepted)
+ * with theta_0 = lo and theta_nbins = hi exactly; 0 <= lo < hi <= 180.
+ * acf_cos_edges turns angle edges (degrees, ascending within [0, 180]) into the descending cosine edges
+ * the pair counts take: cos(theta pi/180) by libm, exactly 1 and -1 at 0 and 180 degrees.
+ */
+enum { ACF_BINS_EVEN = 0, ACF_BINS_LOG = 1, ACF_BINS_LOG10 = 2 };
+int acf_theta_edges(int mode, double lo_deg, double hi_deg, int nbins, double *theta_deg_host);
+int acf_cos_edges(const double *theta_deg, int n_edges, double *cos_edges_host);
+
+/*
  * The whole job from HOST buffers: canonicalise both catalogues (acf_radec_to_xyz), copy them
  * to the device, count DD, DR, RR, copy the histograms back and apply Eq. 2.  Synchronous.
  *   ra_*, dec_* : HOST doubles (degrees);  w_d, w_r : HOST floats or both NULL (unweighted)

@@ -401,3 +401,60 @@ int oracle_wtheta_weighted(const double *dd, const double *dr, const double *rr,
     }
     return ORACLE_OK;
 }
+
+/*
+ * "allows the user to easily experiment with other estimators".  The usual ones on the
+ * pair-normalised counts dd, dr, rr of O7 (kind 0 is O7 itself):
+ *   1 natural (Peebles-Hauser)  dd / rr - 1
+ *   2 Davis-Peebles             dd / dr - 1
+ *   3 Hamilton                  dd rr / dr^2 - 1
+ * NaN where the denominator is zero.
+ */
+int oracle_estimator(int kind, const uint64_t *dd, const uint64_t *dr, const uint64_t *rr, uint64_t n_d,
+                     uint64_t n_r, int nbins, double *w)
+{
+    if (kind == 0) return oracle_wtheta(dd, dr, rr, n_d, n_r, nbins, w);
+    if (!dd || !dr || !rr || !w || nbins < 1 || kind < 0 || kind > 3) return ORACLE_EINVAL;
+    double ndd = (double)n_d * ((double)n_d - 1.0) / 2.0;
+    double ndr = (double)n_d * (double)n_r;
+    double nrr = (double)n_r * ((double)n_r - 1.0) / 2.0;
+    for (int k = 0; k < nbins; ++k) {
+        w[k] = NAN;
+        if (nrr <= 0.0 || ndd <= 0.0 || ndr <= 0.0) continue;
+        double fdd = (double)dd[k] / ndd;
+        double fdr = (double)dr[k] / ndr;
+        double frr = (double)rr[k] / nrr;
+        if (kind == 1 && rr[k] != 0) w[k] = fdd / frr - 1.0;
+        if (kind == 2 && dr[k] != 0) w[k] = fdd / fdr - 1.0;
+        if (kind == 3 && dr[k] != 0) w[k] = fdd * frr / (fdr * fdr) - 1.0;
+    }
+    return ORACLE_OK;
+}
+
+/*
+ * bins between a low and a high limit, "evenly spaced, natural log or log base 10".
+ * mode 0: theta_k = lo + (hi - lo) k / n;  mode 1, 2: theta_k = lo (hi / lo)^(k / n) (the two logarithms
+ * give the same edges: reading R5).  The end edges are lo and hi exactly.
+ */
+int oracle_theta_edges(int mode, double lo, double hi, int nbins, double *theta)
+{
+    if (!theta || nbins < 1 || !(lo >= 0.0) || !(hi > lo) || !(hi <= 180.0)) return ORACLE_EINVAL;
+    if (mode != 0 && !(lo > 0.0)) return ORACLE_EINVAL;
+    if (mode < 0 || mode > 2) return ORACLE_EINVAL;
+    for (int k = 0; k <= nbins; ++k) {
+        double f = (double)k / (double)nbins;
+        theta[k] = mode == 0 ? lo + (hi - lo) * f : lo * pow(hi / lo, f);
+    }
+    theta[0] = lo;
+    theta[nbins] = hi;
+    return ORACLE_OK;
+}
+
+/* Cosine edges of angle edges in degrees (reading R5): cos(theta pi/180), 1 and -1 exactly at 0 and 180. */
+int oracle_cos_edges(const double *theta, int n, double *e)
+{
+    if (!theta || !e || n < 2) return ORACLE_EINVAL;
+    for (int k = 0; k < n; ++k)
+        e[k] = theta[k] == 0.0 ? 1.0 : (theta[k] == 180.0 ? -1.0 : cos(theta[k] * 0.017453292519943295));
+    return ORACLE_OK;
+}

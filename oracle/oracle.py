@@ -62,6 +62,10 @@ def _load():
                 ctypes.c_int, ctypes.c_double, c_u64_p, c_u64_p, c_u64_p, sz]
             lib.oracle_wtheta.argtypes = [c_u64_p, c_u64_p, c_u64_p, ctypes.c_uint64, ctypes.c_uint64,
                                           ctypes.c_int, c_double_p]
+            lib.oracle_estimator.argtypes = [ctypes.c_int, c_u64_p, c_u64_p, c_u64_p, ctypes.c_uint64, ctypes.c_uint64,
+                                             ctypes.c_int, c_double_p]
+            lib.oracle_theta_edges.argtypes = [ctypes.c_int, ctypes.c_double, ctypes.c_double, ctypes.c_int, c_double_p]
+            lib.oracle_cos_edges.argtypes = [c_double_p, ctypes.c_int, c_double_p]
             lib.oracle_wtheta_weighted.argtypes = [c_double_p, c_double_p, c_double_p, c_float_p, sz,
                                                    c_float_p, sz, ctypes.c_int, c_double_p]
             _lib = lib
@@ -194,6 +198,31 @@ def wtheta(dd, dr, rr, n_d: int, n_r: int) -> np.ndarray:
     w = np.empty(dd.size, dtype=np.float64)
     _check(_load().oracle_wtheta(pdd, pdr, prr, int(n_d), int(n_r), dd.size, w.ctypes.data_as(c_double_p)), "wtheta")
     return w
+
+
+def estimator(kind: int, dd, dr, rr, n_d: int, n_r: int) -> np.ndarray:
+    """0 Landy-Szalay (O7), 1 natural, 2 Davis-Peebles, 3 Hamilton."""
+    dd, pdd = _u64(dd)
+    dr, pdr = _u64(dr)
+    rr, prr = _u64(rr)
+    w = np.empty(dd.size, dtype=np.float64)
+    _check(_load().oracle_estimator(int(kind), pdd, pdr, prr, int(n_d), int(n_r), dd.size, w.ctypes.data_as(c_double_p)), "estimator")
+    return w
+
+
+def theta_edges(mode: int, lo_deg: float, hi_deg: float, nbins: int) -> np.ndarray:
+    """0 even, 1 natural log, 2 log10 (the two give the same edges)."""
+    theta = np.empty(int(nbins) + 1, dtype=np.float64)
+    _check(_load().oracle_theta_edges(int(mode), ctypes.c_double(lo_deg), ctypes.c_double(hi_deg), int(nbins),
+                                      theta.ctypes.data_as(c_double_p)), "theta_edges")
+    return theta
+
+
+def cos_edges(theta_deg) -> np.ndarray:
+    theta, pt = _f64(theta_deg)
+    e = np.empty(theta.size, dtype=np.float64)
+    _check(_load().oracle_cos_edges(pt, theta.size, e.ctypes.data_as(c_double_p)), "cos_edges")
+    return e
 
 
 def wtheta_weighted(dd, dr, rr, w_d, w_r) -> np.ndarray:

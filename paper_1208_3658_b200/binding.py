@@ -16,6 +16,8 @@ ACF_OK, ACF_EINVAL, ACF_ENOMEM, ACF_ECUDA = 0, -1, -2, -3
 ACF_OPT_KERNEL, ACF_OPT_PRUNE, ACF_OPT_STATS, ACF_OPT_WINDOWS = 1, 2, 3, 4
 ACF_KERNEL_AUTO, ACF_KERNEL_FP64, ACF_KERNEL_TABLE, ACF_KERNEL_WINDOW = 0, 1, 2, 3
 ACF_MAX_BINS = 1024
+ACF_EST_LANDY_SZALAY, ACF_EST_NATURAL, ACF_EST_DAVIS_PEEBLES, ACF_EST_HAMILTON = 0, 1, 2, 3
+ACF_BINS_EVEN, ACF_BINS_LOG, ACF_BINS_LOG10 = 0, 1, 2
 
 _PKG = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_PKG, "libacf.so")
@@ -23,7 +25,7 @@ LIB_PATH = os.path.join(_PKG, "libacf.so")
 EXPORTS = [
     "acf_create", "acf_destroy", "acf_last_error", "acf_set_option", "acf_set_stream", "acf_radec_to_xyz",
     "acf_pair_count", "acf_pair_count_weighted", "acf_pair_count_rows", "acf_wtheta", "acf_wtheta_weighted",
-    "acf_correlate_host", "acf_get_stats", "acf_version",
+    "acf_estimator", "acf_theta_edges", "acf_cos_edges", "acf_correlate_host", "acf_get_stats", "acf_version",
 ]
 
 
@@ -73,6 +75,9 @@ def load_library(build_if_missing: bool = True):
     lib.acf_pair_count_rows.argtypes = [vp, vp, vp, sz, sz, sz, vp, vp, sz, vp, i32, i32, vp, vp]
     lib.acf_wtheta.argtypes = [vp, vp, vp, u64, u64, i32, vp]
     lib.acf_wtheta_weighted.argtypes = [vp, vp, vp, vp, sz, vp, sz, i32, vp]
+    lib.acf_estimator.argtypes = [i32, vp, vp, vp, u64, u64, i32, vp]
+    lib.acf_theta_edges.argtypes = [i32, ctypes.c_double, ctypes.c_double, i32, vp]
+    lib.acf_cos_edges.argtypes = [vp, i32, vp]
     lib.acf_correlate_host.argtypes = [vp, vp, vp, vp, sz, vp, vp, vp, sz, vp, i32, vp, vp, vp, vp, vp, vp, vp]
     lib.acf_get_stats.argtypes = [vp, ctypes.POINTER(acf_stats)]
     lib.acf_version.restype = ctypes.c_char_p
@@ -232,6 +237,34 @@ def acf_wtheta(dd, dr, rr, n_d: int, n_r: int) -> np.ndarray:
     if rc != ACF_OK:
         raise AcfError(rc, "acf_wtheta")
     return w
+
+
+def acf_estimator(kind: int, dd, dr, rr, n_d: int, n_r: int) -> np.ndarray:
+    dd, pdd = _host(dd, np.uint64)
+    dr, pdr = _host(dr, np.uint64)
+    rr, prr = _host(rr, np.uint64)
+    w = np.empty(dd.size, dtype=np.float64)
+    rc = load_library().acf_estimator(int(kind), pdd, pdr, prr, int(n_d), int(n_r), dd.size, w.ctypes.data)
+    if rc != ACF_OK:
+        raise AcfError(rc, "acf_estimator")
+    return w
+
+
+def acf_theta_edges(mode: int, lo_deg: float, hi_deg: float, nbins: int) -> np.ndarray:
+    theta = np.empty(max(0, int(nbins)) + 1, dtype=np.float64)
+    rc = load_library().acf_theta_edges(int(mode), float(lo_deg), float(hi_deg), int(nbins), theta.ctypes.data)
+    if rc != ACF_OK:
+        raise AcfError(rc, "acf_theta_edges")
+    return theta
+
+
+def acf_cos_edges(theta_deg) -> np.ndarray:
+    theta, pt = _host(theta_deg, np.float64)
+    out = np.empty(theta.size, dtype=np.float64)
+    rc = load_library().acf_cos_edges(pt, theta.size, out.ctypes.data)
+    if rc != ACF_OK:
+        raise AcfError(rc, "acf_cos_edges")
+    return out
 
 
 def acf_wtheta_weighted(wdd, wdr, wrr, w_d, w_r) -> np.ndarray:

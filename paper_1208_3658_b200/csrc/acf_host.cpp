@@ -69,3 +69,63 @@ extern "C" int acf_wtheta_weighted(const double *wdd, const double *wdr, const d
     for (int k = 0; k < nbins; ++k) w_host[k] = landy_szalay(wdd[k], wdr[k], wrr[k], ndd, ndr, nrr);
     return ACF_OK;
 }
+
+// other estimators on the same pair-normalised counts.
+extern "C" int acf_estimator(int kind, const uint64_t *dd, const uint64_t *dr, const uint64_t *rr, uint64_t n_d,
+                             uint64_t n_r, int nbins, double *w_host)
+{
+    if (!dd || !dr || !rr || !w_host || nbins < 1) return ACF_EINVAL;
+    if (kind < ACF_EST_LANDY_SZALAY || kind > ACF_EST_HAMILTON) return ACF_EINVAL;
+    const double nan = std::numeric_limits<double>::quiet_NaN();
+    const double nd = (double)n_d, nr = (double)n_r;
+    const double ndd = nd * (nd - 1.0) / 2.0, ndr = nd * nr, nrr = nr * (nr - 1.0) / 2.0;
+    for (int k = 0; k < nbins; ++k) {
+        if (kind == ACF_EST_LANDY_SZALAY) {
+            w_host[k] = landy_szalay((double)dd[k], (double)dr[k], (double)rr[k], ndd, ndr, nrr);
+            continue;
+        }
+        if (!(ndd > 0.0) || !(ndr > 0.0) || !(nrr > 0.0)) {
+            w_host[k] = nan;
+            continue;
+        }
+        const double fdd = (double)dd[k] / ndd, fdr = (double)dr[k] / ndr, frr = (double)rr[k] / nrr;
+        if (kind == ACF_EST_NATURAL) w_host[k] = frr > 0.0 ? fdd / frr - 1.0 : nan;
+        else if (kind == ACF_EST_DAVIS_PEEBLES) w_host[k] = fdr > 0.0 ? fdd / fdr - 1.0 : nan;
+        else w_host[k] = fdr > 0.0 ? fdd * frr / (fdr * fdr) - 1.0 : nan;
+    }
+    return ACF_OK;
+}
+
+// the bin presets.
+extern "C" int acf_theta_edges(int mode, double lo_deg, double hi_deg, int nbins, double *theta_deg_host)
+{
+    if (!theta_deg_host || nbins < 1 || nbins > ACF_MAX_BINS) return ACF_EINVAL;
+    if (!(lo_deg >= 0.0) || !(hi_deg > lo_deg) || !(hi_deg <= 180.0)) return ACF_EINVAL;
+    if (mode == ACF_BINS_EVEN) {
+        for (int k = 0; k <= nbins; ++k) theta_deg_host[k] = lo_deg + (hi_deg - lo_deg) * ((double)k / (double)nbins);
+    } else if (mode == ACF_BINS_LOG || mode == ACF_BINS_LOG10) {
+        if (!(lo_deg > 0.0)) return ACF_EINVAL;
+        const double ratio = hi_deg / lo_deg;
+        for (int k = 0; k <= nbins; ++k) theta_deg_host[k] = lo_deg * std::pow(ratio, (double)k / (double)nbins);
+    } else {
+        return ACF_EINVAL;
+    }
+    theta_deg_host[0] = lo_deg;
+    theta_deg_host[nbins] = hi_deg;
+    for (int k = 0; k < nbins; ++k)
+        if (!(theta_deg_host[k + 1] > theta_deg_host[k])) return ACF_EINVAL;  // bins too fine for doubles
+    return ACF_OK;
+}
+
+extern "C" int acf_cos_edges(const double *theta_deg, int n_edges, double *cos_edges_host)
+{
+    if (!theta_deg || !cos_edges_host || n_edges < 2) return ACF_EINVAL;
+    for (int k = 0; k < n_edges; ++k) {
+        const double t = theta_deg[k];
+        if (!(t >= 0.0) || !(t <= 180.0) || (k > 0 && !(t > theta_deg[k - 1]))) return ACF_EINVAL;
+        cos_edges_host[k] = t == 0.0 ? 1.0 : (t == 180.0 ? -1.0 : std::cos(t * kDegToRad));
+    }
+    for (int k = 1; k < n_edges; ++k)
+        if (!(cos_edges_host[k] < cos_edges_host[k - 1])) return ACF_EINVAL;  // edges closer than a double resolves
+    return ACF_OK;
+}

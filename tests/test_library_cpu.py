@@ -74,6 +74,40 @@ def test_wtheta_golden_and_oracle(acf, oracle):
                                rtol=0, atol=1e-10)
 
 
+def test_estimators_and_bin_presets_against_golden_and_oracle(acf, oracle):
+    # PAPER.md:65 (other estimators) and PAPER.md:103 (bin presets): pure host entry points
+    for r in read_golden("estimator_examples.txt"):
+        n_d, n_r, dd, dr, rr = (int(v) for v in r[:5])
+        for kind in range(4):
+            w = acf.acf_estimator(kind, [dd], [dr], [rr], n_d, n_r)[0]
+            want = float("nan") if r[5 + kind] == "nan" else float(r[5 + kind])
+            assert (math.isnan(w) and math.isnan(want)) or abs(w - want) < 1e-15, (r, kind, w)
+    rng = np.random.default_rng(4)
+    dd, dr, rr = (rng.integers(0, 10 ** 9, size=50).astype(np.uint64) for _ in range(3))
+    rr[5] = 0
+    dr[7] = 0
+    for kind in range(4):
+        np.testing.assert_allclose(acf.acf_estimator(kind, dd, dr, rr, 123456, 234567), oracle.estimator(kind, dd, dr, rr, 123456, 234567),
+                                   rtol=0, atol=1e-10, equal_nan=True)
+    assert acf.acf_estimator(0, dd, dr, rr, 123456, 234567).tobytes() == acf.acf_wtheta(dd, dr, rr, 123456, 234567).tobytes()
+    for mode, lo, hi, nb in ((acf.ACF_BINS_EVEN, 0.0, 120.0, 254), (acf.ACF_BINS_LOG, 1 / 60, 180.0, 40), (acf.ACF_BINS_LOG10, 0.1 / 60, 3.0, 30)):
+        theta = acf.acf_theta_edges(mode, lo, hi, nb)
+        assert theta.tobytes() == oracle.theta_edges(mode, lo, hi, nb).tobytes()    # same libm, same operations
+        assert acf.acf_cos_edges(theta).tobytes() == oracle.cos_edges(theta).tobytes()
+        e = acf.acf_cos_edges(theta)
+        assert np.all(np.diff(e) < 0) and (hi < 180.0 or e[-1] == -1.0) and (lo > 0.0 or e[0] == 1.0)
+    for r in read_golden("bin_presets.txt"):
+        if r[0] != "cos":
+            mode = {"even": acf.ACF_BINS_EVEN, "log": acf.ACF_BINS_LOG, "log10": acf.ACF_BINS_LOG10}[r[0]]
+            np.testing.assert_allclose(acf.acf_theta_edges(mode, float(r[1]), float(r[2]), int(r[3])), [float(v) for v in r[4:]], rtol=4e-16)
+    lib = acf.load_library()
+    buf = (ctypes.c_double * 8)()
+    assert lib.acf_theta_edges(acf.ACF_BINS_LOG, 0.0, 10.0, 4, buf) == -1      # log bins from 0
+    assert lib.acf_theta_edges(acf.ACF_BINS_EVEN, 5.0, 5.0, 4, buf) == -1      # empty range
+    assert lib.acf_theta_edges(7, 1.0, 5.0, 4, buf) == -1                      # unknown preset
+    assert lib.acf_estimator(9, buf, buf, buf, 1, 1, 1, buf) == -1
+
+
 def test_host_argument_errors(acf):
     lib = acf.load_library()
     assert lib.acf_wtheta(None, None, None, 1, 1, 3, None) == -1

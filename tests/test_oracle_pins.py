@@ -237,6 +237,65 @@ def test_O7_estimator_golden(oracle):
             assert abs(w - float(r[5])) < 1e-15
 
 
+def _num(v):
+    return float("nan") if v == "nan" else float(v)
+
+
+def test_other_estimators_golden(oracle):
+    # PAPER.md:65 "other estimators": hand-computed values, and kind 0 is Eq. 2 itself
+    for r in read_golden("estimator_examples.txt"):
+        n_d, n_r, dd, dr, rr = (int(v) for v in r[:5])
+        for kind in range(4):
+            w = oracle.estimator(kind, [dd], [dr], [rr], n_d, n_r)[0]
+            want = _num(r[5 + kind])
+            assert (math.isnan(w) and math.isnan(want)) or abs(w - want) < 1e-15, (r, kind, w)
+        ls = oracle.wtheta([dd], [dr], [rr], n_d, n_r)[0]
+        assert (math.isnan(ls) and r[5] == "nan") or ls == oracle.estimator(0, [dd], [dr], [rr], n_d, n_r)[0]
+
+
+def test_other_estimators_identities(oracle):
+    # (1 + natural) = (1 + DP) * dr/rr and (1 + Hamilton) = (1 + natural) / (1 + DP)^2 * ... : all four are
+    # functions of the two ratios a = dd/rr, b = dr/rr:  LS = a - 2b + 1, nat = a - 1, DP = a/b - 1, Ham = a/b^2 - 1
+    rng = np.random.default_rng(5)
+    n_d, n_r = 1000, 1700
+    dd = rng.integers(1, 10 ** 5, 30).astype(np.uint64)
+    dr = rng.integers(1, 10 ** 5, 30).astype(np.uint64)
+    rr = rng.integers(1, 10 ** 5, 30).astype(np.uint64)
+    f = lambda c, n: c.astype(np.float64) / n
+    a = f(dd, n_d * (n_d - 1) / 2) / f(rr, n_r * (n_r - 1) / 2)
+    b = f(dr, n_d * n_r) / f(rr, n_r * (n_r - 1) / 2)
+    est = [oracle.estimator(k, dd, dr, rr, n_d, n_r) for k in range(4)]
+    np.testing.assert_allclose(est[0], a - 2 * b + 1, rtol=0, atol=1e-11)
+    np.testing.assert_allclose(est[1], a - 1, rtol=1e-13)
+    np.testing.assert_allclose(est[2], a / b - 1, rtol=0, atol=1e-11)
+    np.testing.assert_allclose(est[3], a / b ** 2 - 1, rtol=0, atol=1e-10)
+
+
+def test_bin_presets_golden(oracle):
+    modes = {"even": 0, "log": 1, "log10": 2}
+    for r in read_golden("bin_presets.txt"):
+        if r[0] == "cos":
+            n = (len(r) - 1) // 2
+            theta = [float(v) for v in r[1:1 + n]]
+            want = np.array([float(v) for v in r[1 + n:]])
+            e = oracle.cos_edges(theta)
+            # the radian argument is rounded twice (the constant pi/180 and the product): up to ~2 ulp of pi
+            np.testing.assert_allclose(e, want, rtol=0, atol=5e-16)
+            assert e[0] == 1.0 and e[-1] == -1.0
+            continue
+        lo, hi, nb = float(r[1]), float(r[2]), int(r[3])
+        want = np.array([float(v) for v in r[4:]])
+        theta = oracle.theta_edges(modes[r[0]], lo, hi, nb)
+        np.testing.assert_allclose(theta, want, rtol=4e-16, atol=0)
+        assert theta[0] == lo and theta[-1] == hi
+    # natural-log and log10 spacing are the same edges (reading R5); the workload generator agrees
+    assert oracle.theta_edges(1, 0.5 / 60, 10.0, 25).tolist() == oracle.theta_edges(2, 0.5 / 60, 10.0, 25).tolist()
+    from workloads import log_theta_edges_deg, cos_edges_from_theta_deg
+    np.testing.assert_allclose(oracle.theta_edges(1, 1 / 60, 180.0, 40), log_theta_edges_deg(1 / 60, 180.0, 40), rtol=1e-14)
+    np.testing.assert_allclose(oracle.cos_edges(log_theta_edges_deg(1 / 60, 180.0, 40)),
+                               cos_edges_from_theta_deg(log_theta_edges_deg(1 / 60, 180.0, 40)), rtol=0, atol=2e-16)
+
+
 def test_O7_unclustered_is_zero_within_noise(oracle):
     # north_star: w(theta) ~ 0 within Poisson noise for an unclustered uniform catalogue
     w = make_config("tiny", scale=0.4)
