@@ -24,7 +24,7 @@ NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
     "-Xcompiler", "-fPIC,-O2,-fno-fast-math,-ffp-contract=off", "--fmad=true",
 ]
-HOST_FLAGS = ["-O2", "-std=c++17", "-fPIC", "-fno-fast-math", "-ffp-contract=off"]
+HOST_FLAGS = ["-O2", "-std=c++17", "-fPIC", "-pthread", "-fno-fast-math", "-ffp-contract=off"]
 
 
 def _nvcc() -> str:
@@ -71,7 +71,7 @@ def build_lib(force: bool = False, verbose: bool = False) -> str:
         # static cudart: the library carries its own runtime and shares the primary context with
         # whatever allocated the caller's buffers (PyTorch), exchanging raw pointers and streams
         cmd = [_nvcc(), "-gencode", "arch=compute_100a,code=sm_100a", "-shared", "-o", tmp, *objs, "-cudart", "static",
-               "-Xlinker", "--no-undefined"]
+               "-Xcompiler", "-pthread", "-Xlinker", "--no-undefined"]
         if verbose:
             print(" ".join(cmd), flush=True)
         subprocess.run(cmd, check=True)

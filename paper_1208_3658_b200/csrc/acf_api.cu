@@ -276,8 +276,9 @@ extern "C" int acf_correlate_host(acf_ctx *ctx, const double *ra_d, const double
     double *h_xyz_d = static_cast<double *>(ctx->h_stage), *h_xyz_r = h_xyz_d + 3 * n_d;
     uint64_t *h_cnt = reinterpret_cast<uint64_t *>(h_xyz_r + 3 * n_r);
     double *h_ws = reinterpret_cast<double *>(h_cnt + 3 * (size_t)nbins);
+    // the randoms are canonicalised on the host while the device counts DD (PAPER.md:128 names the
+    // overlap of transfers and kernels as the step its own code did not take)
     acf_radec_to_xyz(ra_d, dec_d, n_d, h_xyz_d);
-    acf_radec_to_xyz(ra_r, dec_r, n_r, h_xyz_r);
 
     ACF_CUDA_TRY(ctx, ctx->s_host_stage[0].reserve(sizeof(double) * 3 * (n_d ? n_d : 1)));
     ACF_CUDA_TRY(ctx, ctx->s_host_stage[1].reserve(sizeof(double) * 3 * (n_r ? n_r : 1)));
@@ -290,13 +291,14 @@ extern "C" int acf_correlate_host(acf_ctx *ctx, const double *ra_d, const double
     uint64_t *d_cnt = ctx->s_host_stage[4].as<uint64_t>();
     double *d_ws = weighted ? ctx->s_host_stage[5].as<double>() : nullptr;
     if (n_d) ACF_CUDA_TRY(ctx, cudaMemcpyAsync(d_xd, h_xyz_d, sizeof(double) * 3 * n_d, cudaMemcpyHostToDevice, st));
-    if (n_r) ACF_CUDA_TRY(ctx, cudaMemcpyAsync(d_xr, h_xyz_r, sizeof(double) * 3 * n_r, cudaMemcpyHostToDevice, st));
     if (weighted && n_d) ACF_CUDA_TRY(ctx, cudaMemcpyAsync(d_wd, w_d, sizeof(float) * n_d, cudaMemcpyHostToDevice, st));
-    if (weighted && n_r) ACF_CUDA_TRY(ctx, cudaMemcpyAsync(d_wr, w_r, sizeof(float) * n_r, cudaMemcpyHostToDevice, st));
 
     int rc;
     rc = acf_pair_count_rows(ctx, d_xd, d_wd, n_d, 0, n_d, d_xd, d_wd, n_d, cos_edges, nbins, 1, d_cnt, d_ws);
     if (rc != ACF_OK) return rc;
+    acf_radec_to_xyz(ra_r, dec_r, n_r, h_xyz_r);
+    if (n_r) ACF_CUDA_TRY(ctx, cudaMemcpyAsync(d_xr, h_xyz_r, sizeof(double) * 3 * n_r, cudaMemcpyHostToDevice, st));
+    if (weighted && n_r) ACF_CUDA_TRY(ctx, cudaMemcpyAsync(d_wr, w_r, sizeof(float) * n_r, cudaMemcpyHostToDevice, st));
     rc = acf_pair_count_rows(ctx, d_xd, d_wd, n_d, 0, n_d, d_xr, d_wr, n_r, cos_edges, nbins, 0, d_cnt + nbins, d_ws ? d_ws + nbins : nullptr);
     if (rc != ACF_OK) return rc;
     rc = acf_pair_count_rows(ctx, d_xr, d_wr, n_r, 0, n_r, d_xr, d_wr, n_r, cos_edges, nbins, 1, d_cnt + 2 * nbins, d_ws ? d_ws + 2 * nbins : nullptr);

@@ -6,6 +6,8 @@
 #include <cstddef>
 #include <cstdint>
 #include <limits>
+#include <thread>
+#include <vector>
 
 #include "acf.h"
 
@@ -19,14 +21,33 @@ extern "C" int acf_radec_to_xyz(const double *ra_deg, const double *dec_deg, siz
     if (n == 0) return ACF_OK;
     if (!ra_deg || !dec_deg || !xyz_host) return ACF_EINVAL;
     double *x = xyz_host, *y = xyz_host + n, *z = xyz_host + 2 * n;
-    for (size_t i = 0; i < n; ++i) {
-        const double alpha = ra_deg[i] * kDegToRad;
-        const double delta = dec_deg[i] * kDegToRad;
-        const double cos_delta = std::cos(delta);
-        x[i] = cos_delta * std::cos(alpha);
-        y[i] = cos_delta * std::sin(alpha);
-        z[i] = std::sin(delta);
+    auto range = [=](size_t lo, size_t hi) {
+        for (size_t i = lo; i < hi; ++i) {
+            const double alpha = ra_deg[i] * kDegToRad;
+            const double delta = dec_deg[i] * kDegToRad;
+            const double cos_delta = std::cos(delta);
+            x[i] = cos_delta * std::cos(alpha);
+            y[i] = cos_delta * std::sin(alpha);
+            z[i] = std::sin(delta);
+        }
+    };
+    // every point is independent, so splitting the index range over threads changes no bit of the result
+    unsigned n_thr = std::thread::hardware_concurrency();
+    if (n_thr > 16) n_thr = 16;
+    if (n < (size_t(1) << 16) || n_thr < 2) {
+        range(0, n);
+        return ACF_OK;
     }
+    std::vector<std::thread> pool;
+    try {
+        for (unsigned t = 1; t < n_thr; ++t) pool.emplace_back(range, n * t / n_thr, n * (t + 1) / n_thr);
+    } catch (...) {
+        // no more threads to be had: the caller's thread does what is left
+        const size_t done = pool.size() + 1;
+        range(n * done / n_thr, n);
+    }
+    range(0, n / n_thr);
+    for (auto &th : pool) th.join();
     return ACF_OK;
 }
 
