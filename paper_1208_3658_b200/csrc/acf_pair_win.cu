@@ -158,8 +158,8 @@ struct Mask {
 // shapes; it reloads the i-points rather than taking them in registers.
 template <bool kWeighted>
 __device__ __forceinline__ void fixup_body(const WinParams &p, const Rows rows, const float *__restrict__ grp2, uint32_t amb_steps,
-                                           int K, int m_a, bool first, bool last, bool masked, const Mask mk, uint32_t i_base,
-                                           uint32_t j_first, unsigned long long *stat, const float4 (&pi)[kR])
+                                           int K, int m_a, bool masked, const Mask mk, uint32_t i_base, uint32_t j_first,
+                                           unsigned long long *stat, const float4 (&pi)[kR])
 {
     const double e0 = p.edges[m_a];
     const float e32 = (float)e0;
@@ -192,16 +192,14 @@ __device__ __forceinline__ void fixup_body(const WinParams &p, const Rows rows, 
                     const bool exact_above = exact > m_a + q;
                     if (fast_above != exact_above) {
                         // the tally above edge q is taken from row m_a + q and given to row m_a + q + 1
-                        const bool takes = q >= 1 || first, gives = q < K - 1 || last;
+                        // (by this chunk or, carried, by the next): the pair moves between the two
                         const uint32_t dn = fast_above ? 1u : 0xffffffffu;  // +1 / -1 for the lower row
                         const double dw = fast_above ? w : -w;
-                        if (takes) {
-                            atomicAdd(&rows.cnt[m_a + q], dn);
-                            if constexpr (kWeighted) atomicAdd(&rows.ws[m_a + q], dw);
-                        }
-                        if (gives) {
-                            atomicAdd(&rows.cnt[m_a + q + 1], 0u - dn);
-                            if constexpr (kWeighted) atomicAdd(&rows.ws[m_a + q + 1], -dw);
+                        atomicAdd(&rows.cnt[m_a + q], dn);
+                        atomicAdd(&rows.cnt[m_a + q + 1], 0u - dn);
+                        if constexpr (kWeighted) {
+                            atomicAdd(&rows.ws[m_a + q], dw);
+                            atomicAdd(&rows.ws[m_a + q + 1], -dw);
                         }
                     }
                 }
@@ -213,13 +211,13 @@ __device__ __forceinline__ void fixup_body(const WinParams &p, const Rows rows, 
 
 template <bool kWeighted>
 __device__ __noinline__ void fixup_chunk(const WinParams &p, const Rows rows, const float *__restrict__ grp2, uint32_t amb_steps,
-                                         int K, int m_a, bool first, bool last, bool masked, const Mask mk, uint32_t i_base,
-                                         uint32_t j_first, unsigned long long *stat)
+                                         int K, int m_a, bool masked, const Mask mk, uint32_t i_base, uint32_t j_first,
+                                         unsigned long long *stat)
 {
     float4 pi[kR];
 #pragma unroll
     for (int r = 0; r < kR; ++r) pi[r] = p.pts_a[i_base + local_i(r)];  // the array is padded to a whole tile
-    fixup_body<kWeighted>(p, rows, grp2, amb_steps, K, m_a, first, last, masked, mk, i_base, j_first, stat, pi);
+    fixup_body<kWeighted>(p, rows, grp2, amb_steps, K, m_a, masked, mk, i_base, j_first, stat, pi);
 }
 
 // The corrections of the single-edge groups of one staged tile, noted by the kernel's own loop
@@ -239,10 +237,17 @@ __device__ __noinline__ void fixup_tile(const WinParams &p, const Rows rows, con
     for (int g = 0; g < kGroupsPerTile; ++g) {
         const FixNote n = notes[g];
         if (n.amb_steps)
-            fixup_body<kWeighted>(p, rows, tile + (size_t)g * kGroup * 4, n.amb_steps, 1, n.m_edge, true, true, false, mk, i_base,
+            fixup_body<kWeighted>(p, rows, tile + (size_t)g * kGroup * 4, n.amb_steps, 1, n.m_edge, false, mk, i_base,
                                   j_base + g * kGroup, stat, pi);
     }
 }
+
+// What a thread carries from one chunk of a group's edges to the next (registers of window_group): its
+// pairs above the last edge done and, per i-point, the sum of their w_j.
+struct Carry {
+    uint32_t c;
+    double s[kGroup / 32];
+};
 
 // One thread's tallies of the two rows around an edge, kept in registers over consecutive groups that
 // are tested against the same edge (the common single-edge groups of the kernel's own loop).
@@ -252,16 +257,15 @@ struct LaneTally {
 };
 
 // Edges m_a .. m_a + K - 1 against one group of kGroup staged j-points and this thread's kR i-points.
-// The first chunk of a group (first) fills rows m_a .. m_a + K - 1 (and m_a + K if it is also the last).
-// A later chunk starts with the previous chunk's last edge again, only to have the tallies above it
-// at hand, and fills rows m_a + 1 ..: no state is carried from chunk to chunk.
+// A chunk fills rows m_a .. m_a + K - 1 (and m_a + K if it is the last of its group); the tallies above
+// its last edge go to the next chunk through `carry`.
 template <int K, bool kWeighted, bool kPacked, bool kMasked, bool kDeferFix = false>
 __device__ __forceinline__ uint32_t window_chunk(const WinParams &p, const Rows rows, const float *__restrict__ grp2,
                                              const double *__restrict__ vgrp, const float (&nx)[kR],
                                              const float (&ny)[kR], const float (&nz)[kR],
                                              const float (&wi)[kR], const int m_a, const bool first, const bool last, const double wsum_j,
                                              const Mask &mk, uint32_t i_base, uint32_t j_first, unsigned long long *stat,
-                                             LaneTally *tally = nullptr)
+                                             LaneTally *tally = nullptr, Carry *carry = nullptr)
 {
     const int lane = threadIdx.x & 31;
     const double e0 = p.edges[m_a];
@@ -409,8 +413,6 @@ __device__ __forceinline__ uint32_t window_chunk(const WinParams &p, const Rows 
     }
     uint32_t c_prev = 0;  // this thread's pairs above the previous edge (all its pairs before the first)
     double s_prev[kR];    // and, per i-point, the sum of their w_j
-#pragma unroll
-    for (int r = 0; r < kR; ++r) s_prev[r] = 0.0;
     if (first) {
         if constexpr (kMasked) {
             uint32_t n_unused = 0;
@@ -422,6 +424,10 @@ __device__ __forceinline__ uint32_t window_chunk(const WinParams &p, const Rows 
 #pragma unroll
             for (int r = 0; r < kR; ++r) s_prev[r] = wsum_j;
         }
+    } else {
+        c_prev = carry->c;
+#pragma unroll
+        for (int r = 0; r < kR; ++r) s_prev[r] = carry->s[r];
     }
     __syncwarp();
 #pragma unroll
@@ -435,7 +441,7 @@ __device__ __forceinline__ uint32_t window_chunk(const WinParams &p, const Rows 
 #pragma unroll
                 for (int r = 0; r < kR; ++r) {
                     const double sw = unpack(t[q][r], c_q);
-                    if (q > 0 || first) rw = fma((double)wi[r], s_prev[r] - sw, rw);
+                    rw = fma((double)wi[r], s_prev[r] - sw, rw);
                     s_prev[r] = sw;
                 }
             } else {
@@ -447,7 +453,6 @@ __device__ __forceinline__ uint32_t window_chunk(const WinParams &p, const Rows 
         }
         const uint32_t rc = c_prev - c_q;
         c_prev = c_q;
-        if (q == 0 && !first) continue;  // the repeated edge: row m_a was filled by the previous chunk
         if (rc == 0u) rw = 0.0;  // no pair of this thread in the row: not even a rounding residue
         const uint32_t rc_warp = __reduce_add_sync(0xffffffffu, rc);
         if constexpr (kWeighted) rw = warp_sum_f64(rw);
@@ -455,14 +460,20 @@ __device__ __forceinline__ uint32_t window_chunk(const WinParams &p, const Rows 
             rows.template add<kWeighted>(m_a + q, rc_warp, rw);
         }
     }
+    if (!last) {
+        carry->c = c_prev;
+#pragma unroll
+        for (int r = 0; r < kR; ++r) carry->s[r] = s_prev[r];
+    }
     __syncwarp();
-    if (amb_steps) fixup_chunk<kWeighted>(p, rows, grp2, amb_steps, K, m_a, first, last, kMasked, mk, i_base, j_first, stat);
+    if (amb_steps) fixup_chunk<kWeighted>(p, rows, grp2, amb_steps, K, m_a, kMasked, mk, i_base, j_first, stat);
     return 0u;
 }
 
-// One group: all edges r_lo .. r_hi - 1 of its window, kChunk at a time (masked groups one at a time).
-#define ACF_WIN_CHUNK_CALL(K, MASKED, FIRST, M, LAST) \
-    window_chunk<K, kWeighted, kPacked, MASKED>(p, rows, grp2, vgrp, nx, ny, nz, wi, M, FIRST, LAST, wsum_j, mk, i_base, j_first, stat)
+// One group: all edges r_lo .. r_hi - 1 of its window, kChunk at a time.
+#define ACF_WIN_CHUNK_CALL(K, MASKED) \
+    window_chunk<K, kWeighted, kPacked, MASKED>(p, rows, grp2, vgrp, nx, ny, nz, wi, m, m == r_lo, left <= K, wsum_j, mk, i_base, j_first, stat, \
+                                                nullptr, &carry)
 // Not inlined: only the common case (one edge, nothing masked) lives in the kernel's own loop, so that
 // the register allocation of that loop is not set by the rare variants.  It reloads the i-points.
 template <bool kWeighted, bool kPacked>
@@ -485,36 +496,23 @@ __device__ __noinline__ void window_group(const WinParams &p, const Rows rows, c
         if (r_lo > p.nbins) r_lo = p.nbins;
         r_hi = r_lo + 1;
     }
-    // first chunk: edges r_lo .. ; later chunks repeat the last edge done and add up to kChunk - 1 new ones
+    Carry carry;
+    carry.c = 0u;
+#pragma unroll
+    for (int r = 0; r < kR; ++r) carry.s[r] = 0.0;
     int m = r_lo;  // edges below m are done
-    {
-        const int left = r_hi - m;
-        if (masked) {
-            ACF_WIN_CHUNK_CALL(1, true, true, m, left == 1);
-            m += 1;
-        } else if (left == 1) {
-            ACF_WIN_CHUNK_CALL(1, false, true, m, true);
-            m += 1;
-        } else if (left == 2) {
-            ACF_WIN_CHUNK_CALL(2, false, true, m, true);
-            m += 2;
-        } else {
-            ACF_WIN_CHUNK_CALL(3, false, true, m, left == 3);
-            m += 3;
-        }
-    }
     while (m < r_hi) {
         const int left = r_hi - m;
         if (masked) {
-            ACF_WIN_CHUNK_CALL(2, true, false, m - 1, left == 1);
-            m += 1;
-        } else if (left == 1) {
-            ACF_WIN_CHUNK_CALL(2, false, false, m - 1, true);
-            m += 1;
+            if (left == 1) ACF_WIN_CHUNK_CALL(1, true);
+            else if (left == 2) ACF_WIN_CHUNK_CALL(2, true);
+            else ACF_WIN_CHUNK_CALL(3, true);
         } else {
-            ACF_WIN_CHUNK_CALL(3, false, false, m - 1, left == 2);
-            m += 2;
+            if (left == 1) ACF_WIN_CHUNK_CALL(1, false);
+            else if (left == 2) ACF_WIN_CHUNK_CALL(2, false);
+            else ACF_WIN_CHUNK_CALL(3, false);
         }
+        m += left < kChunk ? left : kChunk;
     }
 }
 #undef ACF_WIN_CHUNK_CALL
