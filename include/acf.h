@@ -92,6 +92,7 @@ typedef struct acf_stats {
     uint64_t kernel_launches;    /* CUDA kernels launched by the call */
     double device_ms;            /* device time of the call, CUDA events on the ctx stream */
     double pair_kernel_ms;       /* of which: first to last pair-kernel launch (the dominant kernel) */
+    uint64_t pairs_chord;        /* pairs the fp32 cosine left open and the fp32 chord length decided (not in pairs_fp64) */
 } acf_stats;
 
 /* Create a context on CUDA device `device`.  cuda_stream: a cudaStream_t (as void*) all

@@ -41,6 +41,7 @@ class acf_stats(ctypes.Structure):
         ("pairs_window", ctypes.c_uint64),
         ("tile_pairs_total", ctypes.c_uint64), ("tile_pairs_pruned", ctypes.c_uint64),
         ("kernel_launches", ctypes.c_uint64), ("device_ms", ctypes.c_double), ("pair_kernel_ms", ctypes.c_double),
+        ("pairs_chord", ctypes.c_uint64),
     ]
 
     def as_dict(self):

@@ -239,6 +239,7 @@ extern "C" int acf_get_stats(acf_ctx *ctx, acf_stats *out)
         ctx->last.pairs_evaluated = ctx->h_counters[acf::kCtrPairsEvaluated];
         ctx->last.pairs_fp64 = ctx->h_counters[acf::kCtrPairsFp64];
         ctx->last.pairs_window = ctx->h_counters[acf::kCtrPairsWindow];
+        ctx->last.pairs_chord = ctx->h_counters[acf::kCtrPairsChord];
         ctx->last.tile_pairs_total = ctx->h_counters[acf::kCtrTilePairsTotal];
         ctx->last.tile_pairs_pruned = ctx->h_counters[acf::kCtrTilePairsPruned];
         ctx->stats_pending = false;

@@ -51,7 +51,9 @@ enum Counter : int {
     kCtrWorkHead = 5,   // persistent-kernel work counter
     kCtrWorkCount = 6,  // number of work items produced on the device
     kCtrPairsWindow = 7,  // pairs classified by the single-edge window path
-    kNumCounters = 8
+    kCtrNormDev = 8,      // max over the validated points of |x^2 + y^2 + z^2 - 1|, as the bits of a double
+    kCtrPairsChord = 9,   // pairs the fp32 cosine left open and the fp32 chord length decided
+    kNumCounters = 10
 };
 
 constexpr int kTile = 1024;      // points per tile (both the register-resident i side and the staged j side)
@@ -115,6 +117,7 @@ struct acf_ctx {
 
     // scratch, grown lazily
     acf::Scratch s_edges;            // device copy of cos_edges (+ fp32 tables of the fast path)
+    const float *d_sedges = nullptr; // inside s_edges: the edges as squared chord lengths (chord tier)
     acf::Scratch s_pts[2];           // sorted float4 points of catalogue a / b
     acf::Scratch s_perm[2];          // permutations
     acf::Scratch s_keys[2];          // sort keys (double-buffered inside)

@@ -98,10 +98,12 @@ __global__ void validate_kernel(const double *__restrict__ xyz, const float *__r
                                 unsigned long long *__restrict__ counters)
 {
     unsigned int bad = 0;
+    double dev = 0.0;  // largest |r^2 - 1| seen: the chord tier of the pair kernels needs it (acf_pair_common.cuh)
     for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
         const double x = xyz[i], y = xyz[n + i], z = xyz[2 * n + i];
         const double r2 = x * x + y * y + z * z;
         bool ok = isfinite(x) && isfinite(y) && isfinite(z) && fabs(r2 - 1.0) <= 1e-6;
+        if (ok) dev = fmax(dev, fabs(r2 - 1.0));
         if (w) {
             const float wi = w[i];
             ok = ok && isfinite(wi) && wi >= 0.0f;
@@ -110,6 +112,10 @@ __global__ void validate_kernel(const double *__restrict__ xyz, const float *__r
     }
     bad = __reduce_add_sync(0xffffffffu, bad);
     if ((threadIdx.x & 31) == 0 && bad) atomicAdd(&counters[kCtrBadInput], (unsigned long long)bad);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) dev = fmax(dev, __shfl_xor_sync(0xffffffffu, dev, o));
+    // non-negative doubles order like their bit patterns
+    if ((threadIdx.x & 31) == 0 && dev > 0.0) atomicMax(&counters[kCtrNormDev], (unsigned long long)__double_as_longlong(dev));
 }
 
 }  // namespace

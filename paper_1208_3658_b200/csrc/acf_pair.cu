@@ -29,6 +29,7 @@
 // each thread holds kR i-points in registers.  Auto-correlations visit the upper triangle only.
 #include <cmath>
 #include <cstring>
+#include <limits>
 #include <vector>
 
 #include "acf_device.cuh"
@@ -72,6 +73,8 @@ struct PairParams {
     const uint2 *lut;
     int lut_len, key0, shift;
     const double *edges;
+    const float *sedges;   // the edges as squared chord lengths (chord_row)
+    float chord_margin;    // filled in by the kernel from the validation result
     int nbins;
     unsigned long long *counts;
     double *wsums;
@@ -158,11 +161,18 @@ __device__ __forceinline__ void process_tile(const PairParams &p, Hist<kWeighted
 #pragma unroll
             for (int r = 0; r < kR; ++r) {
                 if (amb[r]) {
-                    const int exact = exact_row(p.xyz_a, p.stride_a, p.perm_a[i_base + local_i(r)], p.xyz_b,
-                                                p.stride_b, p.perm_b[j_base + jj], p.edges, p.nbins);
+                    // the chord length decides where the cosine could not; what it leaves open, the definition
+                    int exact = chord_row(-__uint_as_float((uint32_t)nx2[r]), -__uint_as_float((uint32_t)ny2[r]),
+                                          -__uint_as_float((uint32_t)nz2[r]), q.x, q.y, q.z, p.sedges, p.nbins, p.chord_margin);
+                    if (exact < 0) {
+                        exact = exact_row(p.xyz_a, p.stride_a, p.perm_a[i_base + local_i(r)], p.xyz_b, p.stride_b,
+                                          p.perm_b[j_base + jj], p.edges, p.nbins);
+                        ++n_fp64;
+                    } else {
+                        n_fp64 += 1ull << 32;  // high word: pairs the chord tier decided
+                    }
                     if ((uint32_t)exact != row[r]) h.move(row[r], (uint32_t)exact);
                     if constexpr (kWeighted) h.add_w((uint32_t)exact, (double)wi[r] * (double)q.w);
-                    ++n_fp64;
                 }
             }
         }
@@ -265,8 +275,16 @@ __device__ __forceinline__ void window_group(const PairParams &p, Hist<kWeighted
                     // what the loop above tallied for this pair
                     const bool above = kWeighted ? d > 0.f : (__float_as_uint(d) >> 31) == 0u;
                     const uint32_t fast = (uint32_t)win.edge + (above ? 1u : 0u);
-                    const uint32_t exact = (uint32_t)exact_row(p.xyz_a, p.stride_a, p.perm_a[i_base + local_i(r)], p.xyz_b, p.stride_b,
-                                                               p.perm_b[j_first + jj + u], p.edges, p.nbins);
+                    int ex = chord_row(-__uint_as_float((uint32_t)nx2[r]), -__uint_as_float((uint32_t)ny2[r]),
+                                       -__uint_as_float((uint32_t)nz2[r]), q.x, q.y, q.z, p.sedges, p.nbins, p.chord_margin);
+                    if (ex < 0) {
+                        ex = exact_row(p.xyz_a, p.stride_a, p.perm_a[i_base + local_i(r)], p.xyz_b, p.stride_b,
+                                       p.perm_b[j_first + jj + u], p.edges, p.nbins);
+                        ++n_fp64;
+                    } else {
+                        n_fp64 += 1ull << 32;
+                    }
+                    const uint32_t exact = (uint32_t)ex;
                     if (exact != fast) {
                         h.move(fast, exact);
                         if constexpr (kWeighted) {
@@ -275,7 +293,6 @@ __device__ __forceinline__ void window_group(const PairParams &p, Hist<kWeighted
                             h.add_w(exact, w);
                         }
                     }
-                    ++n_fp64;
                 }
             }
         }
@@ -320,9 +337,11 @@ __device__ __forceinline__ void window_group(const PairParams &p, Hist<kWeighted
 // kGroup i-points of the current i-tile in registers.
 
 template <bool kWeighted, bool kPrivate>
-__global__ void __launch_bounds__(kThreads + 32, kWeighted ? 1 : 2) pair_kernel(const PairParams p)
+__global__ void __launch_bounds__(kThreads + 32, kWeighted ? 1 : 2) pair_kernel(const PairParams p_in)
 {
-    if (p.counters[kCtrBadInput] != 0) return;  // inputs failed validation: never index the LUT with garbage
+    if (p_in.counters[kCtrBadInput] != 0) return;  // inputs failed validation: never index the LUT with garbage
+    PairParams p = p_in;
+    p.chord_margin = chord_margin(p_in.counters);
     extern __shared__ __align__(128) unsigned char smem[];
     const int rows = p.nbins + 2;
     const int n_stages = p.n_stages;
@@ -524,8 +543,9 @@ __global__ void __launch_bounds__(kThreads + 32, kWeighted ? 1 : 2) pair_kernel(
     }
 
     flush_rows();
-    n_fp64 = warp_sum_u64(n_fp64);
-    if (lane == 0 && n_fp64) atomicAdd(&p.counters[kCtrPairsFp64], n_fp64);
+    n_fp64 = warp_sum_u64(n_fp64);  // low word: re-evaluated in fp64; high word: decided by the chord tier
+    if (lane == 0 && (n_fp64 & 0xffffffffull)) atomicAdd(&p.counters[kCtrPairsFp64], n_fp64 & 0xffffffffull);
+    if (lane == 0 && (n_fp64 >> 32)) atomicAdd(&p.counters[kCtrPairsChord], n_fp64 >> 32);
     n_win = warp_sum_u64(n_win);
     if (lane == 0 && n_win) atomicAdd(&p.counters[kCtrPairsWindow], n_win);
     if (tid == 0 && n_eval) atomicAdd(&p.counters[kCtrPairsEvaluated], n_eval);
@@ -683,6 +703,7 @@ int count_prepared(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_au
     p.key0 = L.key0;
     p.shift = L.shift;
     p.edges = ctx->s_edges.as<double>();
+    p.sedges = ctx->d_sedges;
     p.nbins = nbins;
     p.counts = d_counts;
     p.wsums = d_wsums;
@@ -723,10 +744,19 @@ int run_pair_count_fast(acf_ctx *ctx, const double *d_a, const float *d_wa, size
     // cell table: the coarsest resolution that leaves no resolvable cell crowded
     Lut L = build_lut(h_edges, nbins, 6);
     for (int m = 7; m <= 9 && crowded_resolvable(L) > 0; ++m) L = build_lut(h_edges, nbins, m);
+    // device tables: the edges (fp64), the edges as squared chord lengths (fp32, chord tier), the cell table
     const size_t edge_bytes = (sizeof(double) * (size_t)(nbins + 1) + 15) & ~size_t(15);
-    ACF_CUDA_TRY(ctx, ctx->s_edges.reserve(edge_bytes + L.cells.size() * sizeof(uint2)));
+    const size_t sed_bytes = (sizeof(float) * (size_t)(nbins + 1) + 15) & ~size_t(15);
+    std::vector<float> sed((size_t)nbins + 1);
+    for (int k = 0; k <= nbins; ++k) sed[(size_t)k] = (float)(2.0 * (1.0 - h_edges[k]));
+    if (h_edges[0] >= 1.0) sed[0] = -1.0f;                                 // c is clamped: nothing lies beyond a pole
+    if (h_edges[nbins] <= -1.0) sed[(size_t)nbins] = std::numeric_limits<float>::infinity();
+    ACF_CUDA_TRY(ctx, ctx->s_edges.reserve(edge_bytes + sed_bytes + L.cells.size() * sizeof(uint2)));
     ACF_CUDA_TRY(ctx, cudaMemcpyAsync(ctx->s_edges.ptr, h_edges, sizeof(double) * (size_t)(nbins + 1), cudaMemcpyHostToDevice, ctx->stream));
-    uint2 *d_lut = reinterpret_cast<uint2 *>(static_cast<char *>(ctx->s_edges.ptr) + edge_bytes);
+    float *d_sed = reinterpret_cast<float *>(static_cast<char *>(ctx->s_edges.ptr) + edge_bytes);
+    ACF_CUDA_TRY(ctx, cudaMemcpyAsync(d_sed, sed.data(), sizeof(float) * sed.size(), cudaMemcpyHostToDevice, ctx->stream));
+    ctx->d_sedges = d_sed;
+    uint2 *d_lut = reinterpret_cast<uint2 *>(static_cast<char *>(ctx->s_edges.ptr) + edge_bytes + sed_bytes);
     ACF_CUDA_TRY(ctx, cudaMemcpyAsync(d_lut, L.cells.data(), L.cells.size() * sizeof(uint2), cudaMemcpyHostToDevice, ctx->stream));
 
     Prepared a, b;

@@ -111,6 +111,49 @@ __device__ __forceinline__ int row_of_cos(double c, const double *__restrict__ e
 }
 
 
+// ---- chord tier ---------------------------------------------------------------------------------------
+// Below a few arc minutes 1 - cos(theta) is smaller than the fp32 error of the cosine (3e-7), so the
+// cosine test leaves every such pair open.  The squared chord length s = |u_i - u_j|^2 does not cancel:
+// c = (|u_i|^2 + |u_j|^2 - s) / 2, and in fp32 from the fp32 coordinates
+//   |s32 - s| <= 2.4e-7 sqrt(s) + 3.1e-7 s + 6e-14
+// (coordinates rounded to 2^-24 relative: an error vector of at most 1.19e-7 + 2^-24 sqrt(s); three
+// roundings of the sum of squares).  With eps = max |u|^2 - 1 over the validated points and the 4e-16
+// of the fp64 chain, c64 <= e_k holds iff s >= s_k + eta, s_k = 2 (1 - e_k), |eta| <= 2 eps + 8e-16.
+// sed[m] = fp32(s_m) ascending (a pole edge e_0 = 1 is stored as -1: always passed; e_n = -1 as +inf:
+// never passed).  Returns the histogram row (0 .. nbins + 1) if s32 clears both neighbouring edges by
+// the bound (with the rounding of sed and of this arithmetic folded in), else -1: the fp64 definition
+// decides.  (xi, yi, zi) and (xj, yj, zj) are the fp32 coordinates the kernels hold.
+__device__ __forceinline__ int chord_row(float xi, float yi, float zi, float xj, float yj, float zj,
+                                         const float *__restrict__ sed, int nbins, float margin)
+{
+    const float dx = __fsub_rn(xi, xj), dy = __fsub_rn(yi, yj), dz = __fsub_rn(zi, zj);
+    const float s = fmaf(dx, dx, fmaf(dy, dy, __fmul_rn(dz, dz)));
+    int lo = 0, hi = nbins + 1;  // s >= sed[m] for m < lo; s < sed[m] for m >= hi
+    while (lo < hi) {
+        const int mid = (lo + hi) >> 1;
+        if (s >= sed[mid]) lo = mid + 1; else hi = mid;
+    }
+    auto cleared = [&](float se, float gap) {
+        const float sm = se + margin;  // G is taken at the far end of the uncertainty of the edge
+        return gap > 1.02f * (2.5e-7f * sqrtf(sm) + 4.0e-7f * sm + 1.0e-13f) + margin;
+    };
+    if (lo >= 1) {
+        const float se = sed[lo - 1];
+        if (se >= 0.f && !cleared(se, s - se)) return -1;
+    }
+    if (lo <= nbins) {
+        const float se = sed[lo];
+        if (se < 3.0e38f && !cleared(se, se - s)) return -1;
+    }
+    return lo;
+}
+// margin of chord_row from the validation's largest | |u|^2 - 1 |
+__device__ __forceinline__ float chord_margin(const unsigned long long *counters)
+{
+    const double eps = __longlong_as_double((long long)counters[kCtrNormDev]);
+    return (float)(2.02 * eps + 1.0e-15) * 1.0001f;
+}
+
 // All pairs between points of caps a and b have c_lo <= cos(theta) <= c_hi (theta = angle between the
 // centres, rho = sum of the radii: cos(theta -+ rho) = cos(theta) cos(rho) +- sin(theta) sin(rho), clamped
 // at the poles, widened by 1e-9).  Returns false when the caps give no bound.

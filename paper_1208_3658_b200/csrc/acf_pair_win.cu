@@ -63,6 +63,7 @@ struct WinParams {
     const int3 *items;
     uint32_t capacity;
     const double *edges;
+    const float *sedges;  // the edges as squared chord lengths (chord_row)
     int nbins;
     unsigned long long *counts;
     double *wsums;
@@ -118,7 +119,7 @@ struct Rows {
     }
 };
 // per-CTA statistics kept in shared memory until the kernel ends
-enum { kStatFp64 = 0, kStatWindow = 1, kStatEvaluated = 2, kNumStats = 3 };
+enum { kStatFp64 = 0, kStatWindow = 1, kStatEvaluated = 2, kStatChord = 3, kNumStats = 4 };
 // rows and weight of one window, parked in shared memory between its computation and its use
 struct WinRows {
     int lo, hi;
@@ -180,8 +181,15 @@ __device__ __forceinline__ void fixup_body(const WinParams &p, const Rows rows, 
 #pragma unroll
                 for (int q = 0; q < kChunk; ++q) amb |= q < K && !(fabsf(q == 0 ? d0 : __fadd_rn(d0, dl[q])) > G);
                 if (!amb) continue;
-                const int exact = exact_row(p.xyz_a, p.stride_a, p.perm_a[i_base + local_i(r)], p.xyz_b, p.stride_b,
-                                            p.perm_b[j_first + jj0 + u], p.edges, p.nbins);
+                // the chord length decides where the cosine could not; what it leaves open, the definition
+                int exact = chord_row(pi[r].x, pi[r].y, pi[r].z, pj.x, pj.y, pj.z, p.sedges, p.nbins, chord_margin(p.counters));
+                if (exact < 0) {
+                    exact = exact_row(p.xyz_a, p.stride_a, p.perm_a[i_base + local_i(r)], p.xyz_b, p.stride_b,
+                                      p.perm_b[j_first + jj0 + u], p.edges, p.nbins);
+                    atomicAdd(&stat[kStatFp64], 1ull);
+                } else {
+                    atomicAdd(&stat[kStatChord], 1ull);
+                }
                 const double w = (double)pi[r].w * (double)pj.w;
 #pragma unroll
                 for (int q = 0; q < kChunk; ++q) {
@@ -203,7 +211,6 @@ __device__ __forceinline__ void fixup_body(const WinParams &p, const Rows rows, 
                         }
                     }
                 }
-                atomicAdd(&stat[kStatFp64], 1ull);
             }
         }
     }
@@ -827,6 +834,7 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p
         if (stat[kStatFp64]) atomicAdd(&p.counters[kCtrPairsFp64], stat[kStatFp64]);
         if (stat[kStatWindow]) atomicAdd(&p.counters[kCtrPairsWindow], stat[kStatWindow]);
         if (stat[kStatEvaluated]) atomicAdd(&p.counters[kCtrPairsEvaluated], stat[kStatEvaluated]);
+        if (stat[kStatChord]) atomicAdd(&p.counters[kCtrPairsChord], stat[kStatChord]);
     }
 }
 
@@ -874,6 +882,7 @@ int launch_pair_win(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_a
     p.items = ctx->s_work.as<int3>();
     p.capacity = capacity;
     p.edges = ctx->s_edges.as<double>();
+    p.sedges = ctx->d_sedges;
     p.nbins = nbins;
     p.counts = d_counts;
     p.wsums = d_wsums;

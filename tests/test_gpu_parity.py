@@ -235,6 +235,32 @@ def test_linear_bins_many(acf, ctx, oracle):
     acf.acf_set_option(ctx, acf.ACF_OPT_KERNEL, acf.ACF_KERNEL_AUTO)
 
 
+@pytest.mark.parametrize("kernel", ["table", "window"])
+def test_small_angles_chord_tier_and_inexact_norms(acf, ctx, oracle, kernel):
+    """Bins far below the fp32 resolution of 1 - cos(theta) (0.02 arcsec to 2 arcmin): the fp32 chord
+    length must decide most of what the cosine leaves open, and exactly.  Then the same points with
+    norms off by up to 4e-7 (accepted by the validation): c = (|u|^2 + |v|^2 - s) / 2 moves every pair
+    across several of these bins and the chord tier must step aside instead of trusting s."""
+    kern = {"table": acf.ACF_KERNEL_TABLE, "window": acf.ACF_KERNEL_WINDOW}[kernel]
+    rng = np.random.default_rng(71)
+    # 300 tight clumps of 24 points (sigma = 10 arcsec) so that thousands of pairs fall into the bins
+    ra0, dec0 = full_sky(300, 72)
+    ra = (np.repeat(ra0, 24) + rng.normal(0, 10 / 3600, 7200) / np.maximum(0.05, np.cos(np.radians(np.repeat(dec0, 24))))) % 360.0
+    dec = np.clip(np.repeat(dec0, 24) + rng.normal(0, 10 / 3600, 7200), -89.9, 89.9)
+    a = acf.acf_radec_to_xyz(ra, dec)
+    edges = cos_edges_from_theta_deg(log_theta_edges_deg(0.02 / 3600, 2.0 / 60, 36))
+    want = oracle.pair_count(a, None, edges, True)
+    got = gpu_counts(acf, ctx, a, None, edges, True, kernel=kern)
+    st = acf.acf_get_stats(ctx)
+    assert got.tolist() == want.tolist() and int(want.sum()) > 20000
+    assert st["pairs_chord"] > 10 * st["pairs_fp64"] > 0, st
+    scale = 1.0 + rng.uniform(-2e-7, 2e-7, 7200)
+    b = (a.reshape(3, -1) * scale).reshape(-1)
+    want = oracle.pair_count(b, None, edges, True)
+    got = gpu_counts(acf, ctx, b, None, edges, True, kernel=kern)
+    assert got.tolist() == want.tolist()
+
+
 @pytest.mark.parametrize("kernel", ["auto", "window"])
 def test_maximum_number_of_bins(acf, ctx, oracle, kernel):
     """ACF_MAX_BINS bins, unweighted and weighted: the window kernel then keeps one set of histogram rows per
