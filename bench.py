@@ -110,6 +110,12 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
+def workload_label(args, w) -> str:
+    """The same workload name on both arms."""
+    return "%s x%g: %d data + %d random, %d log bins, %s; DD+DR+RR per step" % (
+        args.workload, args.scale, w.n_d, w.n_r, w.nbins, "weighted (u64 counts + f64 sums)" if w.w_d is not None else "unweighted")
+
+
 # --------------------------------------------------------------------------- oracle legs
 def oracle_sample(w, n_rows: int):
     """Times the CPU oracle on DR rows [0, n_rows) x all randoms (weighted when the workload is).
@@ -147,8 +153,8 @@ def run_reference(args):
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * secs / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-        "config": {"workload": "%s x%g" % (args.workload, args.scale), "n_data": w.n_d, "n_random": w.n_r, "nbins": w.nbins,
-                   "weighted": w.w_d is not None},
+        "config": {"workload": workload_label(args, w), "pairs_per_step": w.nominal_pairs,
+                   "reference_step": "a bounded sample of the workload: " + sample},
         "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
         "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
@@ -315,9 +321,7 @@ def main():
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
-            "config": {"workload": "%s x%g: %d data + %d random, %d log bins, %s; DD+DR+RR per step" % (
-                args.workload, args.scale, w.n_d, w.n_r, nb, "weighted (u64 counts + f64 sums)" if weighted else "unweighted"),
-                "pairs_per_step": pairs_per_step, "l2": "flushed between timed steps (256 MB write)",
+            "config": {"workload": workload_label(args, w), "pairs_per_step": pairs_per_step, "l2": "flushed between timed steps (256 MB write)",
                 "per_rank": "independent realisation per rank (seeds + 1000*rank)"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * args.steps, "roofline": roofline,
             "cpu_baseline": cpu_baseline,
