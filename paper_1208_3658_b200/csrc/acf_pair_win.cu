@@ -124,6 +124,8 @@ enum { kStatFp64 = 0, kStatWindow = 1, kStatEvaluated = 2, kStatChord = 3, kNumS
 struct WinRows {
     int lo, hi;
     double wsum;
+    float e32;  // fp32 of the edge a window with at most one edge is tested against
+    int pad;
 };
 
 __device__ __forceinline__ double warp_sum_f64(double v)
@@ -272,11 +274,11 @@ __device__ __forceinline__ uint32_t window_chunk(const WinParams &p, const Rows 
                                              const float (&ny)[kR], const float (&nz)[kR],
                                              const float (&wi)[kR], const int m_a, const bool first, const bool last, const double wsum_j,
                                              const Mask &mk, uint32_t i_base, uint32_t j_first, unsigned long long *stat,
-                                             LaneTally *tally = nullptr, Carry *carry = nullptr)
+                                             LaneTally *tally = nullptr, Carry *carry = nullptr, float e32_known = 0.f)
 {
     const int lane = threadIdx.x & 31;
-    const double e0 = p.edges[m_a];
-    const float e32 = (float)e0;
+    const double e0 = kDeferFix ? 0.0 : p.edges[m_a];               // (the kernel's own loop has the edge at hand)
+    const float e32 = kDeferFix ? e32_known : (float)e0;
     const unsigned long long e2 = pack2(e32, e32);
     float dl[K];
     unsigned long long dl2[K];
@@ -757,6 +759,9 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p
                     if (hi == p.nbins && c_lo < p.edges[p.nbins]) ++hi;
                     wr.hi = hi;
                 }
+                const int m_one = wr.hi > wr.lo ? wr.lo : (wr.lo > p.nbins ? p.nbins : wr.lo);
+                wr.e32 = (float)p.edges[m_one];
+                wr.pad = 0;
                 wr.wsum = gb.wsum;
                 win[my_g] = wr;
             }
@@ -783,7 +788,8 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p
                 }
                 const uint32_t amb = window_chunk<1, kWeighted, kPacked, false, true>(p, rows, tile + (size_t)g * kGroup * 4, vtile + g * kGroup,
                                                                                       nx, ny, nz, wi, m_edge, true, true, win[g].wsum, mk,
-                                                                                      i_base, j_base + g * kGroup, stat, &tally);
+                                                                                      i_base, j_base + g * kGroup, stat, &tally, nullptr,
+                                                                                      win[g].e32);
                 if (lane == 0) {
                     atomicAdd(&stat[kStatWindow], (unsigned long long)(kGroup * kGroup));
                     notes[g].amb_steps = amb;
