@@ -198,6 +198,26 @@ int acf_theta_edges(int mode, double lo_deg, double hi_deg, int nbins, double *t
 int acf_cos_edges(const double *theta_deg, int n_edges, double *cos_edges_host);
 
 /*
+ * Delete-one jackknife of an estimator over n_regions regions of the sky (PAPER.md:201 names "a full
+ * MC-based calculation of the errors" as what the speed-up makes affordable; resampling the catalogues
+ * by region is its usual form).  For every region k the histograms are recounted without the points of
+ * region k -- as DD - (pairs with a point in k), each such set counted by acf_pair_count_rows calls on the
+ * device -- and the estimator of the remaining points is formed; cov is the jackknife covariance
+ *   cov[a][b] = (N - 1)/N  sum_k (w_k[a] - mean[a]) (w_k[b] - mean[b]),   mean = (1/N) sum_k w_k.
+ *   d_xyz_d, d_xyz_r : DEVICE canonical vectors (SoA, 3 n doubles), points ORDERED BY REGION: region k is
+ *                      rows [off[k], off[k+1]) (a region may be empty)
+ *   off_d, off_r     : HOST, n_regions + 1 offsets, off[0] = 0, off[n_regions] = n, non-decreasing
+ *   estimator        : ACF_EST_*
+ *   w_full           : HOST, nbins doubles: the estimator of the full catalogues
+ *   w_jk             : HOST, n_regions x nbins doubles, row k = the estimator without region k
+ *   cov              : HOST, nbins x nbins doubles, or NULL
+ * Unweighted.  Synchronous.  2 <= n_regions.  ACF_EINVAL for bad offsets or arguments.
+ */
+int acf_jackknife(acf_ctx *ctx, const double *d_xyz_d, size_t n_d, const size_t *off_d, const double *d_xyz_r,
+                  size_t n_r, const size_t *off_r, int n_regions, const double *cos_edges, int nbins,
+                  int estimator, double *w_full, double *w_jk, double *cov);
+
+/*
  * The whole job from HOST buffers: canonicalise both catalogues (acf_radec_to_xyz), copy them
  * to the device, count DD, DR, RR, copy the histograms back and apply Eq. 2.  Synchronous.
  *   ra_*, dec_* : HOST doubles (degrees);  w_d, w_r : HOST floats or both NULL (unweighted)

@@ -225,6 +225,35 @@ def cos_edges(theta_deg) -> np.ndarray:
     return e
 
 
+def jackknife_cov(w_jk) -> np.ndarray:
+    """Delete-one jackknife covariance of N resampled estimates (rows of w_jk):
+    cov = (N - 1)/N sum_k (w_k - mean)(w_k - mean)^T, mean = (1/N) sum_k w_k."""
+    w_jk = np.asarray(w_jk, dtype=np.float64)
+    n = w_jk.shape[0]
+    dev = w_jk - w_jk.mean(axis=0)
+    return (n - 1) / n * (dev.T @ dev)
+
+
+def jackknife(xyz_d, region_d, xyz_r, region_r, n_regions: int, cos_edges, kind: int = 0):
+    """PAPER.md:201 (resampling errors), by the definition: for every region k the points of region k are
+    removed from both catalogues, DD, DR, RR are counted afresh and the estimator is formed.
+    region_*: the region index of every point.  -> (w_full, w_jk, cov)."""
+    xd = np.asarray(xyz_d, dtype=np.float64).reshape(3, -1)
+    xr = np.asarray(xyz_r, dtype=np.float64).reshape(3, -1)
+    region_d, region_r = np.asarray(region_d), np.asarray(region_r)
+
+    def est(a, b):
+        a, b = np.ascontiguousarray(a).reshape(-1), np.ascontiguousarray(b).reshape(-1)
+        dd = pair_count(a, None, cos_edges, True)
+        dr = pair_count(a, b, cos_edges, False)
+        rr = pair_count(b, None, cos_edges, True)
+        return estimator(kind, dd, dr, rr, a.size // 3, b.size // 3)
+
+    w_full = est(xd, xr)
+    w_jk = np.stack([est(xd[:, region_d != k], xr[:, region_r != k]) for k in range(n_regions)])
+    return w_full, w_jk, jackknife_cov(w_jk)
+
+
 def wtheta_weighted(dd, dr, rr, w_d, w_r) -> np.ndarray:
     dd, pdd = _f64(dd)
     dr, pdr = _f64(dr)

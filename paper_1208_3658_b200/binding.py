@@ -25,7 +25,7 @@ LIB_PATH = os.path.join(_PKG, "libacf.so")
 EXPORTS = [
     "acf_create", "acf_destroy", "acf_last_error", "acf_set_option", "acf_set_stream", "acf_radec_to_xyz",
     "acf_pair_count", "acf_pair_count_weighted", "acf_pair_count_rows", "acf_wtheta", "acf_wtheta_weighted",
-    "acf_estimator", "acf_theta_edges", "acf_cos_edges", "acf_correlate_host", "acf_get_stats", "acf_version",
+    "acf_estimator", "acf_theta_edges", "acf_cos_edges", "acf_jackknife", "acf_correlate_host", "acf_get_stats", "acf_version",
 ]
 
 
@@ -79,6 +79,7 @@ def load_library(build_if_missing: bool = True):
     lib.acf_estimator.argtypes = [i32, vp, vp, vp, u64, u64, i32, vp]
     lib.acf_theta_edges.argtypes = [i32, ctypes.c_double, ctypes.c_double, i32, vp]
     lib.acf_cos_edges.argtypes = [vp, i32, vp]
+    lib.acf_jackknife.argtypes = [vp, vp, sz, vp, vp, sz, vp, i32, vp, i32, i32, vp, vp, vp]
     lib.acf_correlate_host.argtypes = [vp, vp, vp, vp, sz, vp, vp, vp, sz, vp, i32, vp, vp, vp, vp, vp, vp, vp]
     lib.acf_get_stats.argtypes = [vp, ctypes.POINTER(acf_stats)]
     lib.acf_version.restype = ctypes.c_char_p
@@ -266,6 +267,26 @@ def acf_cos_edges(theta_deg) -> np.ndarray:
     if rc != ACF_OK:
         raise AcfError(rc, "acf_cos_edges")
     return out
+
+
+def acf_jackknife(ctx, d_xyz_d, off_d, d_xyz_r, off_r, cos_edges, estimator: int = ACF_EST_LANDY_SZALAY) -> dict:
+    """Delete-one jackknife over regions; the catalogues (device tensors) are ordered by region and
+    off_d / off_r give each region's row range.  -> {"w": ..., "w_jk": (regions, nbins), "cov": (nbins, nbins)}."""
+    off_d = np.ascontiguousarray(off_d, dtype=np.uint64)
+    off_r = np.ascontiguousarray(off_r, dtype=np.uint64)
+    edges, pe = _host(cos_edges, np.float64)
+    nbins, n_regions = edges.size - 1, off_d.size - 1
+    if off_r.size != off_d.size:
+        raise ValueError("off_d and off_r must name the same regions")
+    w = np.empty(nbins, dtype=np.float64)
+    w_jk = np.empty((n_regions, nbins), dtype=np.float64)
+    cov = np.empty((nbins, nbins), dtype=np.float64)
+    rc = load_library().acf_jackknife(ctx, d_xyz_d.data_ptr(), _n_points(d_xyz_d), off_d.ctypes.data, d_xyz_r.data_ptr(),
+                                      _n_points(d_xyz_r), off_r.ctypes.data, n_regions, pe, nbins, int(estimator),
+                                      w.ctypes.data, w_jk.ctypes.data, cov.ctypes.data)
+    if rc != ACF_OK:
+        raise AcfError(rc, acf_last_error(ctx))
+    return {"w": w, "w_jk": w_jk, "cov": cov}
 
 
 def acf_wtheta_weighted(wdd, wdr, wrr, w_d, w_r) -> np.ndarray:

@@ -248,6 +248,98 @@ extern "C" int acf_get_stats(acf_ctx *ctx, acf_stats *out)
     return ACF_OK;
 }
 
+// Delete-one jackknife (include/acf.h).  Pairs with a point in region k, for a catalogue ordered by region:
+// rows k of the auto-count (pairs inside k and from k to the regions after it) plus the rows before k
+// against region k.  The cross-count loses D_k x R, D x R_k and gets D_k x R_k back.
+extern "C" int acf_jackknife(acf_ctx *ctx, const double *d_xyz_d, size_t n_d, const size_t *off_d, const double *d_xyz_r,
+                             size_t n_r, const size_t *off_r, int n_regions, const double *cos_edges, int nbins,
+                             int estimator, double *w_full, double *w_jk, double *cov)
+{
+    if (!ctx) return ACF_EINVAL;
+    ctx->err[0] = 0;
+    if (const char *why = check_edges(cos_edges, nbins)) return acf::fail(ctx, ACF_EINVAL, "%s", why);
+    if (!d_xyz_d || !d_xyz_r || !off_d || !off_r || !w_full || !w_jk) return acf::fail(ctx, ACF_EINVAL, "NULL argument");
+    if (n_regions < 2) return acf::fail(ctx, ACF_EINVAL, "n_regions must be at least 2");
+    if (estimator < ACF_EST_LANDY_SZALAY || estimator > ACF_EST_HAMILTON) return acf::fail(ctx, ACF_EINVAL, "unknown estimator");
+    size_t max_d = 0, max_r = 0;
+    for (int k = 0; k < n_regions; ++k) {
+        if (off_d[k + 1] < off_d[k] || off_r[k + 1] < off_r[k]) return acf::fail(ctx, ACF_EINVAL, "region offsets must not decrease");
+        if (off_d[k + 1] - off_d[k] > max_d) max_d = off_d[k + 1] - off_d[k];
+        if (off_r[k + 1] - off_r[k] > max_r) max_r = off_r[k + 1] - off_r[k];
+    }
+    if (off_d[0] != 0 || off_r[0] != 0 || off_d[n_regions] != n_d || off_r[n_regions] != n_r)
+        return acf::fail(ctx, ACF_EINVAL, "region offsets must run from 0 to n");
+    ACF_CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t st = ctx->stream;
+    const size_t nb = (size_t)nbins;
+    // scratch: the points of region k of either catalogue as catalogues of their own, and 8 histograms
+    ACF_CUDA_TRY(ctx, ctx->s_host_stage[0].reserve(sizeof(double) * 3 * (max_d ? max_d : 1)));
+    ACF_CUDA_TRY(ctx, ctx->s_host_stage[1].reserve(sizeof(double) * 3 * (max_r ? max_r : 1)));
+    ACF_CUDA_TRY(ctx, ctx->s_host_stage[4].reserve(sizeof(uint64_t) * 8 * nb));
+    double *d_dk = ctx->s_host_stage[0].as<double>(), *d_rk = ctx->s_host_stage[1].as<double>();
+    uint64_t *d_cnt = ctx->s_host_stage[4].as<uint64_t>();
+    std::vector<uint64_t> h((size_t)8 * nb), tot((size_t)3 * nb), dd(nb), dr(nb), rr(nb);
+
+    int rc;
+    auto count = [&](const double *a, size_t na, size_t i0, size_t i1, const double *b, size_t nbp, int is_auto, int slot) -> int {
+        return acf_pair_count_rows(ctx, a, nullptr, na, i0, i1, b, nullptr, nbp, cos_edges, nbins, is_auto, d_cnt + (size_t)slot * nb, nullptr);
+    };
+    auto fetch = [&](int slots) -> int {
+        ACF_CUDA_TRY(ctx, cudaMemcpyAsync(h.data(), d_cnt, sizeof(uint64_t) * (size_t)slots * nb, cudaMemcpyDeviceToHost, st));
+        ACF_CUDA_TRY(ctx, cudaStreamSynchronize(st));
+        return ACF_OK;
+    };
+    auto subset = [&](const double *src, size_t n, size_t lo, size_t cnt, double *dst) -> int {
+        for (int c = 0; c < 3 && cnt; ++c)
+            ACF_CUDA_TRY(ctx, cudaMemcpyAsync(dst + (size_t)c * cnt, src + (size_t)c * n + lo, sizeof(double) * cnt, cudaMemcpyDeviceToDevice, st));
+        return ACF_OK;
+    };
+    if ((rc = count(d_xyz_d, n_d, 0, n_d, d_xyz_d, n_d, 1, 0)) != ACF_OK) return rc;
+    if ((rc = count(d_xyz_d, n_d, 0, n_d, d_xyz_r, n_r, 0, 1)) != ACF_OK) return rc;
+    if ((rc = count(d_xyz_r, n_r, 0, n_r, d_xyz_r, n_r, 1, 2)) != ACF_OK) return rc;
+    if ((rc = fetch(3)) != ACF_OK) return rc;
+    tot.assign(h.begin(), h.begin() + 3 * (long)nb);
+    if ((rc = acf_estimator(estimator, tot.data(), tot.data() + nb, tot.data() + 2 * nb, n_d, n_r, nbins, w_full)) != ACF_OK) return rc;
+
+    for (int k = 0; k < n_regions; ++k) {
+        const size_t d0 = off_d[k], d1 = off_d[k + 1], r0 = off_r[k], r1 = off_r[k + 1];
+        const size_t ndk = d1 - d0, nrk = r1 - r0;
+        if ((rc = subset(d_xyz_d, n_d, d0, ndk, d_dk)) != ACF_OK) return rc;
+        if ((rc = subset(d_xyz_r, n_r, r0, nrk, d_rk)) != ACF_OK) return rc;
+        // slots: 0 DD rows k, 1 DD rows before k x D_k, 2 RR rows k, 3 RR rows before k x R_k,
+        //        4 D_k x R, 5 D x R_k, 6 D_k x R_k
+        if ((rc = count(d_xyz_d, n_d, d0, d1, d_xyz_d, n_d, 1, 0)) != ACF_OK) return rc;
+        if ((rc = count(d_xyz_d, n_d, 0, d0, d_dk, ndk, 0, 1)) != ACF_OK) return rc;
+        if ((rc = count(d_xyz_r, n_r, r0, r1, d_xyz_r, n_r, 1, 2)) != ACF_OK) return rc;
+        if ((rc = count(d_xyz_r, n_r, 0, r0, d_rk, nrk, 0, 3)) != ACF_OK) return rc;
+        if ((rc = count(d_xyz_d, n_d, d0, d1, d_xyz_r, n_r, 0, 4)) != ACF_OK) return rc;
+        if ((rc = count(d_xyz_d, n_d, 0, n_d, d_rk, nrk, 0, 5)) != ACF_OK) return rc;
+        if ((rc = count(d_dk, ndk, 0, ndk, d_rk, nrk, 0, 6)) != ACF_OK) return rc;
+        if ((rc = fetch(7)) != ACF_OK) return rc;
+        for (size_t b = 0; b < nb; ++b) {
+            dd[b] = tot[b] - h[b] - h[nb + b];
+            rr[b] = tot[2 * nb + b] - h[2 * nb + b] - h[3 * nb + b];
+            dr[b] = tot[nb + b] - h[4 * nb + b] - h[5 * nb + b] + h[6 * nb + b];
+        }
+        if ((rc = acf_estimator(estimator, dd.data(), dr.data(), rr.data(), n_d - ndk, n_r - nrk, nbins, w_jk + (size_t)k * nb)) != ACF_OK)
+            return rc;
+    }
+    if (cov) {
+        std::vector<double> mean(nb, 0.0);
+        for (int k = 0; k < n_regions; ++k)
+            for (size_t b = 0; b < nb; ++b) mean[b] += w_jk[(size_t)k * nb + b];
+        for (size_t b = 0; b < nb; ++b) mean[b] /= (double)n_regions;
+        const double f = (double)(n_regions - 1) / (double)n_regions;
+        for (size_t a = 0; a < nb; ++a)
+            for (size_t b = 0; b < nb; ++b) {
+                double sum = 0.0;
+                for (int k = 0; k < n_regions; ++k) sum += (w_jk[(size_t)k * nb + a] - mean[a]) * (w_jk[(size_t)k * nb + b] - mean[b]);
+                cov[a * nb + b] = f * sum;
+            }
+    }
+    return ACF_OK;
+}
+
 extern "C" int acf_correlate_host(acf_ctx *ctx, const double *ra_d, const double *dec_d, const float *w_d, size_t n_d,
                                   const double *ra_r, const double *dec_r, const float *w_r, size_t n_r,
                                   const double *cos_edges, int nbins, uint64_t *dd, uint64_t *dr, uint64_t *rr,

@@ -342,6 +342,33 @@ def test_invalid_arguments(acf, ctx):
     assert int(out.sum()) == 100 * 99 // 2
 
 
+@pytest.mark.parametrize("est", [0, 3])
+def test_jackknife_against_recount(acf, ctx, oracle, est):
+    """acf_jackknife (counts without region k as total minus the pairs touching k, all on the device)
+    against the oracle's definition (remove the region, count afresh): same integers, so the same
+    estimates; regions of unequal size, one of them empty in the randoms."""
+    import torch
+    w = make_config("clustered_patch", 0.012)
+    n_reg = 6
+    reg_d = np.minimum((w.ra_d / 20.0 * n_reg).astype(int), n_reg - 1)
+    reg_r = np.minimum((w.ra_r / 20.0 * n_reg).astype(int), n_reg - 1)
+    reg_r[reg_r == 4] = 5                                   # region 4 has no randoms
+    od, orr = np.argsort(reg_d, kind="stable"), np.argsort(reg_r, kind="stable")
+    ra_d, dec_d, reg_d = w.ra_d[od], w.dec_d[od], reg_d[od]
+    ra_r, dec_r, reg_r = w.ra_r[orr], w.dec_r[orr], reg_r[orr]
+    off_d = np.searchsorted(reg_d, np.arange(n_reg + 1))
+    off_r = np.searchsorted(reg_r, np.arange(n_reg + 1))
+    xd, xr = acf.acf_radec_to_xyz(ra_d, dec_d), acf.acf_radec_to_xyz(ra_r, dec_r)
+    got = acf.acf_jackknife(ctx, torch.from_numpy(xd).cuda(), off_d, torch.from_numpy(xr).cuda(), off_r, w.cos_edges, est)
+    w_full, w_jk, cov = oracle.jackknife(xd, reg_d, xr, reg_r, n_reg, w.cos_edges, est)
+    np.testing.assert_allclose(got["w"], w_full, rtol=0, atol=WTHETA_ATOL, equal_nan=True)
+    np.testing.assert_allclose(got["w_jk"], w_jk, rtol=0, atol=WTHETA_ATOL, equal_nan=True)
+    ok = ~np.isnan(cov)
+    assert np.array_equal(np.isnan(got["cov"]), np.isnan(cov))
+    np.testing.assert_allclose(got["cov"][ok], cov[ok], rtol=1e-9, atol=1e-12)
+    assert np.isfinite(w_jk).any()
+
+
 def test_correlate_host_end_to_end(acf, ctx, oracle):
     w = make_config("full_sky", 0.004)
     res = acf.acf_correlate_host(ctx, w.ra_d, w.dec_d, w.w_d, w.ra_r, w.dec_r, w.w_r, w.cos_edges)

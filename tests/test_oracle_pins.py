@@ -296,6 +296,32 @@ def test_bin_presets_golden(oracle):
                                cos_edges_from_theta_deg(log_theta_edges_deg(1 / 60, 180.0, 40)), rtol=0, atol=2e-16)
 
 
+def test_jackknife_pins(oracle):
+    # covariance formula on a hand example: rows (1,2),(3,4),(5,6): mean (3,4), deviations (-2,-2),(0,0),(2,2),
+    # sum of outer products 8 everywhere, times (N-1)/N = 2/3
+    np.testing.assert_allclose(oracle.jackknife_cov([[1, 2], [3, 4], [5, 6]]), np.full((2, 2), 16.0 / 3.0), rtol=1e-15)
+    # a constant estimate has no variance; one varying bin leaves the others' rows and columns zero
+    assert np.all(oracle.jackknife_cov(np.ones((7, 3))) == 0)
+    c = oracle.jackknife_cov([[0, 1], [2, 1], [4, 1], [6, 1]])
+    assert c[0, 0] == pytest.approx(0.75 * 20.0) and c[1, 1] == 0 and c[0, 1] == 0
+    # delete-one counts: a pair between two regions is missing from two of the resampled counts, a pair inside
+    # a region from one: sum_k (DD - DD_(-k)) = 2 DD - sum_k DD(inside k)
+    w = make_config("tiny", scale=0.06)
+    xd = oracle.radec_to_xyz(w.ra_d, w.dec_d).reshape(3, -1)
+    reg = np.minimum((w.ra_d / 10.0 * 5).astype(int), 4)
+    dd = oracle.pair_count(xd.reshape(-1), None, w.cos_edges, True)
+    gone = sum(dd - oracle.pair_count(np.ascontiguousarray(xd[:, reg != k]).reshape(-1), None, w.cos_edges, True) for k in range(5))
+    inside = sum(oracle.pair_count(np.ascontiguousarray(xd[:, reg == k]).reshape(-1), None, w.cos_edges, True) for k in range(5))
+    assert gone.tolist() == (2 * dd - inside).tolist()
+    # the resampled estimates of an unclustered catalogue scatter around the full one
+    xr = oracle.radec_to_xyz(w.ra_r, w.dec_r)
+    regr = np.minimum((w.ra_r / 10.0 * 5).astype(int), 4)
+    w_full, w_jk, cov = oracle.jackknife(xd.reshape(-1), reg, xr, regr, 5, w.cos_edges, 0)
+    ok = ~np.isnan(w_full) & ~np.isnan(w_jk).any(axis=0)
+    assert w_jk.shape == (5, w.nbins) and np.all(np.abs(w_jk[:, ok].mean(axis=0) - w_full[ok]) < 0.5 * np.abs(w_full[ok]) + 0.2)
+    assert np.all(np.diag(cov)[ok] >= 0)
+
+
 def test_O7_unclustered_is_zero_within_noise(oracle):
     # north_star: w(theta) ~ 0 within Poisson noise for an unclustered uniform catalogue
     w = make_config("tiny", scale=0.4)
