@@ -67,9 +67,9 @@ enum {
      * bins a kernel's shared-memory histograms may not fit: AUTO then takes the other fast kernel, an
      * explicit choice returns ACF_EINVAL. */
     ACF_OPT_KERNEL = 1,
-    /* 1 (default): tile pairs that provably hold no in-range pair are skipped
-     * ("ignoring calculations that would fall outside the bin range");
-     * 0: every tile pair is evaluated. */
+    /* 1 (default): tile pairs -- and, inside the tile pairs that remain, pairs of groups of 128 points --
+     * that provably hold no in-range pair are skipped ("ignoring calculations that would
+     * fall outside the bin range"); 0: every pair is evaluated. */
     ACF_OPT_PRUNE = 2,
     /* 1: collect acf_stats device counters (pairs evaluated, fp64 re-checks); default 1. */
     ACF_OPT_STATS = 3,

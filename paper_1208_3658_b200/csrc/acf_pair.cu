@@ -81,6 +81,7 @@ struct PairParams {
     unsigned long long *counters;
     int is_auto;
     int use_windows;
+    int prune;
     int n_stages;
 };
 
@@ -181,7 +182,8 @@ __device__ __forceinline__ void process_tile(const PairParams &p, Hist<kWeighted
 
 // ---- window path --------------------------------------------------------------------------------
 struct Window {
-    int edge;    // m: the one edge pairs of this window are tested against, or -1: take the table path
+    int edge;    // m: the one edge pairs of this window are tested against; -1: take the table path;
+                 // -2: every pair of the window is out of range: nothing to evaluate
     float e32;   // fp32(e[m])
     double wsum; // sum of the j-group's weights
 };
@@ -189,7 +191,8 @@ struct Window {
 // All pairs between points of cap a and cap b have c_lo <= cos(theta) <= c_hi; the window is usable
 // when rows(c_lo) - rows(c_hi) <= 1.  theta = angle between the centres, rho = sum of the radii:
 // cos(theta -+ rho) = cos(theta) cos(rho) +- sin(theta) sin(rho), clamped at the poles.
-__device__ __forceinline__ Window make_window(const GroupCap &a, const GroupCap &b, const double *__restrict__ edges, int nbins)
+__device__ __forceinline__ Window make_window(const GroupCap &a, const GroupCap &b, const double *__restrict__ edges, int nbins,
+                                              bool prune)
 {
     Window w;
     w.edge = -1;
@@ -199,6 +202,10 @@ __device__ __forceinline__ Window make_window(const GroupCap &a, const GroupCap 
     if (!cap_window(a, b, c_lo, c_hi)) return w;
     const int r_lo = row_of_cos(c_hi, edges, nbins), r_hi = row_of_cos(c_lo, edges, nbins);
     if (r_hi - r_lo > 1) return w;
+    if (prune && r_hi == r_lo && (r_lo == 0 || r_lo == nbins + 1)) {  // all closer than theta_min or all beyond theta_max
+        w.edge = -2;
+        return w;
+    }
     w.edge = r_lo <= nbins ? r_lo : nbins;  // rows edge (c > e[edge]) and edge + 1
     w.e32 = (float)edges[w.edge];
     return w;
@@ -425,7 +432,7 @@ __global__ void __launch_bounds__(kThreads + 32, kWeighted ? 1 : 2) pair_kernel(
     h.ws = kPrivate ? ws_all + (size_t)warp * rows * 32 : ws_all + (size_t)warp * rows;
     h.lane = lane;
 
-    unsigned long long n_fp64 = 0, n_eval = 0, n_win = 0;
+    unsigned long long n_fp64 = 0, n_eval = 0, n_win = 0, n_skip = 0;
     unsigned long long since_flush = 0;  // pairs this warp has tallied in its unflushed shared rows
     float wi[kR];
     unsigned long long nx2[kR], ny2[kR], nz2[kR];  // {-x, -x} etc.: both halves of an FFMA2 see the same i-point
@@ -517,12 +524,16 @@ __global__ void __launch_bounds__(kThreads + 32, kWeighted ? 1 : 2) pair_kernel(
             mine.wsum = 0.0;
             if (lane < n_groups && (lane + 1) * kGroup <= jn)
                 mine = make_window(p.gcaps_a[(size_t)m.ti * kGroupsPerTile + warp], p.gcaps_b[(size_t)tj * kGroupsPerTile + lane],
-                                   p.edges, p.nbins);
+                                   p.edges, p.nbins, p.prune != 0);
             for (int g = 0; g < n_groups; ++g) {
                 Window win;
                 win.edge = __shfl_sync(0xffffffffu, mine.edge, g);
                 win.e32 = __shfl_sync(0xffffffffu, mine.e32, g);
                 win.wsum = __shfl_sync(0xffffffffu, mine.wsum, g);
+                if (win.edge == -2) {  // pruned at the level of groups, like whole tiles in the work list
+                    n_skip += (unsigned long long)(kGroup * kR);
+                    continue;
+                }
                 if (win.edge >= 0) {
                     if (!kWeighted || pack.packed)
                         window_group<kWeighted, true, kPrivate>(p, h, tile + (size_t)g * kGroup * 4, vtile + g * kGroup, nx2, ny2, nz2, wi, win,
@@ -549,6 +560,8 @@ __global__ void __launch_bounds__(kThreads + 32, kWeighted ? 1 : 2) pair_kernel(
     n_win = warp_sum_u64(n_win);
     if (lane == 0 && n_win) atomicAdd(&p.counters[kCtrPairsWindow], n_win);
     if (tid == 0 && n_eval) atomicAdd(&p.counters[kCtrPairsEvaluated], n_eval);
+    n_skip = warp_sum_u64(n_skip);  // counted in n_eval with their tile, never evaluated
+    if (lane == 0 && n_skip) atomicAdd(&p.counters[kCtrPairsEvaluated], 0ull - n_skip);
 }
 
 // ---- host: the cell table -------------------------------------------------------------------
@@ -690,6 +703,7 @@ int count_prepared(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_au
     p.gcaps_a = a.gcaps;
     p.gcaps_b = b.gcaps;
     p.use_windows = ctx->opt_windows;
+    p.prune = ctx->opt_prune;
     p.n_a = (uint32_t)a.n;
     p.n_b = (uint32_t)b.n;
     p.xyz_a = a.xyz;

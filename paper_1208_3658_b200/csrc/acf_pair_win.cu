@@ -71,6 +71,7 @@ struct WinParams {
     int is_auto;
     int n_stages;
     int shared_rows;  // 1: one set of histogram rows per CTA instead of one per warp
+    int prune;        // 1: groups whose window lies wholly out of range are not evaluated
 };
 
 __device__ __forceinline__ unsigned long long fadd2(unsigned long long a, unsigned long long b)
@@ -759,7 +760,16 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p
                     if (hi == p.nbins && c_lo < p.edges[p.nbins]) ++hi;
                     wr.hi = hi;
                 }
-                const int m_one = wr.hi > wr.lo ? wr.lo : (wr.lo > p.nbins ? p.nbins : wr.lo);
+                if (p.prune && wr.hi == wr.lo && (wr.lo == 0 || wr.lo > p.nbins) && !(diag && my_g < igrp)) {
+                    // all closer than theta_min or all beyond theta_max: pruned at the level of groups, like whole
+                    // tiles in the work list; the tile's pair count in the statistics loses them
+                    const uint32_t gi = n_i - (uint32_t)igrp * kGroup < (uint32_t)kGroup ? n_i - (uint32_t)igrp * kGroup : (uint32_t)kGroup;
+                    const uint32_t gj = (uint32_t)(jn - my_g * kGroup < kGroup ? jn - my_g * kGroup : kGroup);
+                    const unsigned long long gone = diag && my_g == igrp ? (unsigned long long)gi * (gi - 1) / 2 : (unsigned long long)gi * gj;
+                    atomicAdd(&stat[kStatEvaluated], 0ull - gone);
+                    wr.lo = wr.hi = -1;
+                }
+                const int m_one = wr.hi > wr.lo ? wr.lo : (wr.lo > p.nbins ? p.nbins : (wr.lo < 0 ? 0 : wr.lo));
                 wr.e32 = (float)p.edges[m_one];
                 wr.pad = 0;
                 wr.wsum = gb.wsum;
@@ -774,6 +784,7 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p
             for (int g = diag ? igrp : 0; g < n_groups; ++g) {
                 if ((g & (kTeams - 1)) != team) continue;  // the other team's group
                 const int r_lo = win[g].lo, r_hi = win[g].hi;
+                if (r_lo < 0) continue;  // pruned (see where the windows are bounded)
                 const bool masked = !warp_full || jn - g * kGroup < kGroup || (diag && g == igrp);
                 if (masked || r_hi - r_lo > 1) {
                     slow_groups |= 1u << g;
@@ -826,7 +837,7 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p
                 }
             }
         }
-        if (tid == 0) stat[kStatEvaluated] += diag ? (unsigned long long)n_i * (n_i - 1) / 2 : (unsigned long long)n_i * (unsigned)jn;
+        if (tid == 0) atomicAdd(&stat[kStatEvaluated], diag ? (unsigned long long)n_i * (n_i - 1) / 2 : (unsigned long long)n_i * (unsigned)jn);
         __syncwarp();  // every lane has read the stage before it is handed back
         if (lane == 0) {
             mbar_arrive(&empty[slot]);
@@ -896,6 +907,7 @@ int launch_pair_win(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_a
     p.is_auto = is_auto;
     p.n_stages = n_stages;
     p.shared_rows = row_sets == 1 ? 1 : 0;
+    p.prune = ctx->opt_prune;
 
     const int grid = ctx->num_sms * ctas_per_sm;
     cudaError_t e = cudaSuccess;

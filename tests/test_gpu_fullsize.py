@@ -112,7 +112,8 @@ def test_fullsize_sampled_rows_and_properties(acf, ctx, oracle, name, width):
         for kern, windows in ((acf.ACF_KERNEL_WINDOW, 1), (acf.ACF_KERNEL_TABLE, 1), (acf.ACF_KERNEL_TABLE, 0)):
             c2, s2, st2 = count(acf, ctx, d, k, windows=windows, kernel=kern)
             assert windows == 1 or st2["pairs_window"] == 0
-            assert st2["pairs_evaluated"] == full[k][2]["pairs_evaluated"]
+            nominal = w.n_d * (w.n_d - 1) // 2 if k == "dd" else w.n_d * w.n_r
+            assert 0 < st2["pairs_evaluated"] <= nominal    # (the kernels prune groups of points to different depths)
             assert c2.tolist() == full[k][0].tolist(), (k, kern, windows)
             if weighted:
                 np.testing.assert_allclose(s2, full[k][1], rtol=WSUM_RTOL, atol=0)
