@@ -143,3 +143,25 @@ def test_fullsize_sampled_rows_and_properties(acf, ctx, oracle, name, width):
     wt = acf.acf_wtheta(full["dd"][0], full["dr"][0], full["rr"][0], w.n_d, w.n_r)
     wo = oracle.wtheta(full["dd"][0], full["dr"][0], full["rr"][0], w.n_d, w.n_r)
     np.testing.assert_allclose(wt, wo, rtol=0, atol=1e-10, equal_nan=True)
+
+
+def test_two_million_points_mid_kernel_flush(acf, ctx):
+    """2M x 2M weighted DR (4e12 pairs): every CTA walks more j-tiles than a u32 histogram row may take,
+    so the rows are flushed to global memory in mid-kernel.  The two fast kernels (independent codes) must
+    agree bit for bit; the counts must follow the uniform-sphere law and add up to all pairs beyond 1'."""
+    import torch
+    w = make_config("full_sky", 2.0)
+    d = Dev(acf, w)
+    res = {}
+    for kern in (acf.ACF_KERNEL_WINDOW, acf.ACF_KERNEL_TABLE):
+        res[kern] = count(acf, ctx, d, "dr", kernel=kern)
+    c, s, st = res[acf.ACF_KERNEL_WINDOW]
+    c2, s2, _ = res[acf.ACF_KERNEL_TABLE]
+    assert c.tolist() == c2.tolist()
+    np.testing.assert_allclose(s, s2, rtol=WSUM_RTOL, atol=0)
+    npairs = w.n_d * w.n_r
+    e = w.cos_edges
+    expect = npairs * (e[:-1] - e[1:]) / 2.0
+    assert np.all(np.abs(c.astype(np.float64) - expect) <= 6.0 * np.sqrt(expect) + 1.0)
+    assert 0 <= npairs - int(c.sum()) <= 12 * npairs * (1.0 - e[0]) / 2.0 + 50
+    assert st["pairs_evaluated"] == npairs
