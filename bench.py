@@ -49,6 +49,7 @@ def parse_args():
     ap.add_argument("--scale", type=float, default=1.0)
     ap.add_argument("--cpu-rows", type=int, default=0, help="rows of the oracle sample (0 = auto)")
     ap.add_argument("--kernel", default="auto", choices=["auto", "table", "window"], help="pair kernel (ACF_OPT_KERNEL)")
+    ap.add_argument("--bulk", action="store_true", help="ACF_OPT_BULK: count single-bin groups of points as a whole (not the default path)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -190,6 +191,8 @@ def main():
     weighted = w.w_d is not None
     ctx = P.acf_create(local_rank)
     P.acf_set_option(ctx, P.ACF_OPT_KERNEL, {"auto": P.ACF_KERNEL_AUTO, "table": P.ACF_KERNEL_TABLE, "window": P.ACF_KERNEL_WINDOW}[args.kernel])
+    if args.bulk:
+        P.acf_set_option(ctx, P.ACF_OPT_BULK, 1)
     dev = torch.device("cuda", local_rank)
     h_xd = P.acf_radec_to_xyz(w.ra_d, w.dec_d)
     h_xr = P.acf_radec_to_xyz(w.ra_r, w.dec_r)
@@ -322,7 +325,8 @@ def main():
             "ms_per_step": ms_total / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": workload_label(args, w), "pairs_per_step": pairs_per_step, "l2": "flushed between timed steps (256 MB write)",
-                "per_rank": "independent realisation per rank (seeds + 1000*rank)"},
+                "per_rank": "independent realisation per rank (seeds + 1000*rank)",
+                "bulk_windows": bool(args.bulk)},
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches_per_step * args.steps, "roofline": roofline,
             "cpu_baseline": cpu_baseline,
             "detail": {"ms_steps": ms_steps, "wall_s_timed_region": t_wall, "pairs_fp64_per_step": stats_acc["fp64"],

@@ -77,7 +77,14 @@ enum {
      * at most one bin edge can separate their pairs, every pair is tested against that one edge and
      * tallied in registers; 0: every pair goes through the bin table and the shared-memory histogram.
      * The counts are the same either way. */
-    ACF_OPT_WINDOWS = 4
+    ACF_OPT_WINDOWS = 4,
+    /* 0 (default): every in-range pair is evaluated on its own, as the paper's method does;
+     * 1: where the bounding caps of two groups of 128 points prove that all their pairs fall into one
+     * and the same bin, the window kernel adds the group's pair count and weight product to that bin
+     * without visiting the pairs (the counterpart, inside the range, of skipping what lies outside it;
+     * still exact: the proof is the same fp64 bound that picks the edges of a window).  Such pairs are
+     * reported in acf_stats.pairs_bulk and not in pairs_evaluated. */
+    ACF_OPT_BULK = 5
 };
 enum { ACF_KERNEL_AUTO = 0, ACF_KERNEL_FP64 = 1, ACF_KERNEL_TABLE = 2, ACF_KERNEL_WINDOW = 3 };
 
@@ -93,6 +100,7 @@ typedef struct acf_stats {
     double device_ms;            /* device time of the call, CUDA events on the ctx stream */
     double pair_kernel_ms;       /* of which: first to last pair-kernel launch (the dominant kernel) */
     uint64_t pairs_chord;        /* pairs the fp32 cosine left open and the fp32 chord length decided (not in pairs_fp64) */
+    uint64_t pairs_bulk;         /* pairs counted group by group without being evaluated (ACF_OPT_BULK) */
 } acf_stats;
 
 /* Create a context on CUDA device `device`.  cuda_stream: a cudaStream_t (as void*) all

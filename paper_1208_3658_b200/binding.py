@@ -13,7 +13,7 @@ import os
 import numpy as np
 
 ACF_OK, ACF_EINVAL, ACF_ENOMEM, ACF_ECUDA = 0, -1, -2, -3
-ACF_OPT_KERNEL, ACF_OPT_PRUNE, ACF_OPT_STATS, ACF_OPT_WINDOWS = 1, 2, 3, 4
+ACF_OPT_KERNEL, ACF_OPT_PRUNE, ACF_OPT_STATS, ACF_OPT_WINDOWS, ACF_OPT_BULK = 1, 2, 3, 4, 5
 ACF_KERNEL_AUTO, ACF_KERNEL_FP64, ACF_KERNEL_TABLE, ACF_KERNEL_WINDOW = 0, 1, 2, 3
 ACF_MAX_BINS = 1024
 ACF_EST_LANDY_SZALAY, ACF_EST_NATURAL, ACF_EST_DAVIS_PEEBLES, ACF_EST_HAMILTON = 0, 1, 2, 3
@@ -41,7 +41,7 @@ class acf_stats(ctypes.Structure):
         ("pairs_window", ctypes.c_uint64),
         ("tile_pairs_total", ctypes.c_uint64), ("tile_pairs_pruned", ctypes.c_uint64),
         ("kernel_launches", ctypes.c_uint64), ("device_ms", ctypes.c_double), ("pair_kernel_ms", ctypes.c_double),
-        ("pairs_chord", ctypes.c_uint64),
+        ("pairs_chord", ctypes.c_uint64), ("pairs_bulk", ctypes.c_uint64),
     ]
 
     def as_dict(self):

@@ -122,6 +122,9 @@ extern "C" int acf_set_option(acf_ctx *ctx, int option, int64_t value)
     case ACF_OPT_WINDOWS:
         ctx->opt_windows = value != 0;
         return ACF_OK;
+    case ACF_OPT_BULK:
+        ctx->opt_bulk = value != 0;
+        return ACF_OK;
     default:
         return acf::fail(ctx, ACF_EINVAL, "unknown option %d", option);
     }
@@ -240,6 +243,7 @@ extern "C" int acf_get_stats(acf_ctx *ctx, acf_stats *out)
         ctx->last.pairs_fp64 = ctx->h_counters[acf::kCtrPairsFp64];
         ctx->last.pairs_window = ctx->h_counters[acf::kCtrPairsWindow];
         ctx->last.pairs_chord = ctx->h_counters[acf::kCtrPairsChord];
+        ctx->last.pairs_bulk = ctx->h_counters[acf::kCtrPairsBulk];
         ctx->last.tile_pairs_total = ctx->h_counters[acf::kCtrTilePairsTotal];
         ctx->last.tile_pairs_pruned = ctx->h_counters[acf::kCtrTilePairsPruned];
         ctx->stats_pending = false;

@@ -53,7 +53,8 @@ enum Counter : int {
     kCtrPairsWindow = 7,  // pairs classified by the single-edge window path
     kCtrNormDev = 8,      // max over the validated points of |x^2 + y^2 + z^2 - 1|, as the bits of a double
     kCtrPairsChord = 9,   // pairs the fp32 cosine left open and the fp32 chord length decided
-    kNumCounters = 10
+    kCtrPairsBulk = 10,   // pairs counted per group of points, not one by one (ACF_OPT_BULK)
+    kNumCounters = 11
 };
 
 constexpr int kTile = 1024;      // points per tile (both the register-resident i side and the staged j side)
@@ -106,6 +107,7 @@ struct acf_ctx {
     int opt_prune = 1;
     int opt_stats = 1;
     int opt_windows = 1;
+    int opt_bulk = 0;
 
     cudaEvent_t ev_start = nullptr, ev_stop = nullptr, ev_flag = nullptr;
     cudaEvent_t ev_k0 = nullptr, ev_k1 = nullptr;  // around the pair kernel(s) of the last call

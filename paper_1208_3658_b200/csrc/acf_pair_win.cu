@@ -72,6 +72,7 @@ struct WinParams {
     int n_stages;
     int shared_rows;  // 1: one set of histogram rows per CTA instead of one per warp
     int prune;        // 1: groups whose window lies wholly out of range are not evaluated
+    int bulk;         // 1: groups whose window lies wholly inside one bin are counted as a whole (ACF_OPT_BULK)
 };
 
 __device__ __forceinline__ unsigned long long fadd2(unsigned long long a, unsigned long long b)
@@ -107,7 +108,13 @@ struct Rows {
     double *ws;
     bool shared;  // one set of rows for the whole CTA (many bins): every update is atomic
     template <bool kWeighted>
-    __device__ __forceinline__ void add(int row, uint32_t c, double w) const
+    __device__ __forceinline__ void add_atomic(int row, uint32_t c, double w) const  // from any lane
+    {
+        atomicAdd(&cnt[row], c);
+        if constexpr (kWeighted) atomicAdd(&ws[row], w);
+    }
+    template <bool kWeighted>
+    __device__ __forceinline__ void add(int row, uint32_t c, double w) const  // lane 0 of the rows' warp
     {
         if (shared) {
             if (c) atomicAdd(&cnt[row], c);
@@ -120,7 +127,7 @@ struct Rows {
     }
 };
 // per-CTA statistics kept in shared memory until the kernel ends
-enum { kStatFp64 = 0, kStatWindow = 1, kStatEvaluated = 2, kStatChord = 3, kNumStats = 4 };
+enum { kStatFp64 = 0, kStatWindow = 1, kStatEvaluated = 2, kStatChord = 3, kStatBulk = 4, kNumStats = 5 };
 // rows and weight of one window, parked in shared memory between its computation and its use
 struct WinRows {
     int lo, hi;
@@ -769,6 +776,15 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p
                     atomicAdd(&stat[kStatEvaluated], 0ull - gone);
                     wr.lo = wr.hi = -1;
                 }
+                if (p.bulk && wr.lo >= 0 && wr.hi == wr.lo && warp_full && jn - my_g * kGroup >= kGroup && !(diag && my_g <= igrp)) {
+                    // all pairs of two full groups in one bin: the bin gets the groups' pair count and the product of
+                    // their weight sums, and nothing is evaluated (ACF_OPT_BULK)
+                    const unsigned long long all = (unsigned long long)kGroup * kGroup;
+                    rows.template add_atomic<kWeighted>(wr.lo, (uint32_t)all, p.gcaps_a[(size_t)m.ti * kGroupsPerTile + igrp].wsum * gb.wsum);
+                    atomicAdd(&stat[kStatEvaluated], 0ull - all);
+                    atomicAdd(&stat[kStatBulk], all);
+                    wr.lo = wr.hi = -1;
+                }
                 const int m_one = wr.hi > wr.lo ? wr.lo : (wr.lo > p.nbins ? p.nbins : (wr.lo < 0 ? 0 : wr.lo));
                 wr.e32 = (float)p.edges[m_one];
                 wr.pad = 0;
@@ -852,6 +868,7 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p
         if (stat[kStatWindow]) atomicAdd(&p.counters[kCtrPairsWindow], stat[kStatWindow]);
         if (stat[kStatEvaluated]) atomicAdd(&p.counters[kCtrPairsEvaluated], stat[kStatEvaluated]);
         if (stat[kStatChord]) atomicAdd(&p.counters[kCtrPairsChord], stat[kStatChord]);
+        if (stat[kStatBulk]) atomicAdd(&p.counters[kCtrPairsBulk], stat[kStatBulk]);
     }
 }
 
@@ -908,6 +925,7 @@ int launch_pair_win(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_a
     p.n_stages = n_stages;
     p.shared_rows = row_sets == 1 ? 1 : 0;
     p.prune = ctx->opt_prune;
+    p.bulk = ctx->opt_bulk;
 
     const int grid = ctx->num_sms * ctas_per_sm;
     cudaError_t e = cudaSuccess;

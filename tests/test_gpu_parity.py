@@ -342,6 +342,29 @@ def test_invalid_arguments(acf, ctx):
     assert int(out.sum()) == 100 * 99 // 2
 
 
+def test_bulk_windows_option(acf, ctx, oracle):
+    """ACF_OPT_BULK: groups of points whose bounding caps put all their pairs into one bin are counted as
+    a whole.  Same integers as the oracle, weighted sums to 1e-12, and the statistics say how many pairs
+    were never evaluated."""
+    w = make_config("full_sky", 0.02)
+    xd, xr = acf.acf_radec_to_xyz(w.ra_d, w.dec_d), acf.acf_radec_to_xyz(w.ra_r, w.dec_r)
+    acf.acf_set_option(ctx, acf.ACF_OPT_BULK, 1)
+    try:
+        for a, b, auto, wa, wb in ((xd, None, True, w.w_d, None), (xd, xr, False, w.w_d, w.w_r)):
+            want = oracle.pair_count(a, b, w.cos_edges, auto, w_a=wa, w_b=wb)
+            got = gpu_counts(acf, ctx, a, b, w.cos_edges, auto, wa=wa, wb=wb, kernel=acf.ACF_KERNEL_WINDOW)
+            st = acf.acf_get_stats(ctx)
+            assert got[0].tolist() == want[0].tolist()
+            np.testing.assert_allclose(got[1], want[1], rtol=WSUM_RTOL, atol=0)
+            assert st["pairs_bulk"] > 0 and st["pairs_bulk"] + st["pairs_evaluated"] == st["pairs_nominal"]
+            want_u = oracle.pair_count(a, b, w.cos_edges, auto)
+            assert gpu_counts(acf, ctx, a, b, w.cos_edges, auto, kernel=acf.ACF_KERNEL_WINDOW).tolist() == want_u.tolist()
+    finally:
+        acf.acf_set_option(ctx, acf.ACF_OPT_BULK, 0)
+    gpu_counts(acf, ctx, xd, xr, w.cos_edges, False, wa=w.w_d, wb=w.w_r, kernel=acf.ACF_KERNEL_WINDOW)
+    assert acf.acf_get_stats(ctx)["pairs_bulk"] == 0
+
+
 @pytest.mark.parametrize("est", [0, 3])
 def test_jackknife_against_recount(acf, ctx, oracle, est):
     """acf_jackknife (counts without region k as total minus the pairs touching k, all on the device)
