@@ -106,6 +106,7 @@ __device__ __forceinline__ double ind_gt0_f64(unsigned long long &reg, float v)
 struct Rows {
     uint32_t *cnt;
     double *ws;
+    const PackInfo *pack;  // the j side's PackInfo, copied to shared memory
     bool shared;  // one set of rows for the whole CTA (many bins): every update is atomic
     template <bool kWeighted>
     __device__ __forceinline__ void add_atomic(int row, uint32_t c, double w) const  // from any lane
@@ -402,8 +403,8 @@ __device__ __forceinline__ uint32_t window_chunk(const WinParams &p, const Rows 
     auto unpack = [&](double tt, uint32_t &n) -> double {  // 2^-7 (n C + sum of w) -> sum of w, n += count
         double sw = tt * 128.0;
         if constexpr (kPacked) {
-            const double nn = floor(sw * p.pack_b->inv_C);  // C is a power of two and the sum of w is below C: exact
-            sw -= nn * p.pack_b->C;
+            const double nn = floor(sw * rows.pack->inv_C);  // C is a power of two and the sum of w is below C: exact
+            sw -= nn * rows.pack->C;
             n += (uint32_t)nn;
         }
         return sw;
@@ -616,7 +617,10 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p
     StageMeta *meta = reinterpret_cast<StageMeta *>(smem + 128);
     volatile ProdState *ps = reinterpret_cast<volatile ProdState *>(smem + 128 + kMaxStages * sizeof(StageMeta));
     unsigned long long *stat = reinterpret_cast<unsigned long long *>(smem + 128 + kMaxStages * sizeof(StageMeta) + sizeof(ProdState));
-    static_assert(sizeof(ProdState) % 8 == 0 && 128 + kMaxStages * sizeof(StageMeta) + sizeof(ProdState) + kNumStats * 8 <= kSmemHeader, "header");
+    PackInfo *pack_sm = reinterpret_cast<PackInfo *>(stat + kNumStats);
+    static_assert(sizeof(ProdState) % 8 == 0 &&
+                      128 + kMaxStages * sizeof(StageMeta) + sizeof(ProdState) + kNumStats * 8 + sizeof(PackInfo) <= kSmemHeader,
+                  "header");
     unsigned char *stages = smem + kSmemHeader;
     size_t off = kSmemHeader + (size_t)n_stages * kStage;
     uint32_t *cnt_all = reinterpret_cast<uint32_t *>(smem + off);
@@ -647,6 +651,7 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p
         unsigned long long n_items = p.counters[kCtrWorkCount];
         ps->n_items = n_items > p.capacity ? p.capacity : n_items;
         for (int i = 0; i < kNumStats; ++i) stat[i] = 0ull;
+        *pack_sm = *p.pack_b;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -656,13 +661,15 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p
     // ---------------- consumers
     Rows rows;
     rows.shared = p.shared_rows != 0;
+    rows.pack = pack_sm;
     rows.cnt = cnt_all + (rows.shared ? 0 : (size_t)warp * rows_n);
     rows.ws = ws_all + (rows.shared ? 0 : (size_t)warp * rows_n);
     WinRows *win = win_all + (size_t)warp * kGroupsPerTile;
     FixNote *notes = notes_all + (size_t)warp * kGroupsPerTile;
     uint32_t since_flush = 0;  // j-tiles this warp has tallied in its unflushed rows
     // u32 rows: flush before the tallies could wrap (shared rows take the pairs of all the CTA's warps)
-    const uint32_t flush_every = (1u << 31) / (uint32_t)(kGroup * kTile) / (rows.shared ? (uint32_t)kWarps : 1u);
+    // (the rows are read as signed 32-bit numbers when flushed: half the range)
+    const uint32_t flush_every = (1u << 30) / (uint32_t)(kGroup * kTile) / (rows.shared ? (uint32_t)kWarps : 1u);
     float wi[kR];
     float nx[kR], ny[kR], nz[kR];  // the i-points, negated
 #pragma unroll
@@ -698,7 +705,9 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p
             // (shared rows: other warps add while this one takes the value and leaves zero)
             const uint32_t v = rows.shared ? atomicExch(&rows.cnt[row], 0u) : rows.cnt[row];
             if (!rows.shared) rows.cnt[row] = 0;
-            if (row >= 1 && row <= p.nbins && v) atomicAdd(&p.counts[row - 1], (unsigned long long)v);
+            // read as signed: with shared rows another warp's exact correction (-1 now, its tally later) may be
+            // caught in between; the two's-complement sum in global memory comes out the same
+            if (row >= 1 && row <= p.nbins && v) atomicAdd(&p.counts[row - 1], (unsigned long long)(long long)(int32_t)v);
             if constexpr (kWeighted) {
                 const double w = rows.shared ? __longlong_as_double((long long)atomicExch(reinterpret_cast<unsigned long long *>(&rows.ws[row]), 0ull))
                                              : rows.ws[row];
