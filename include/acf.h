@@ -63,7 +63,8 @@ enum {
      * debugging); ACF_KERNEL_TABLE = fast path, cell-table kernel (single-edge windows in registers,
      * everything else through a bin table and per-lane shared-memory histograms);
      * ACF_KERNEL_WINDOW = fast path, window kernel (every group of pairs classified in registers
-     * against the few edges its bounding caps allow).  All four give the same counts.  With very many
+     * against the few edges its bounding caps allow; weights whose range exceeds 2^13 are handed to the
+     * table kernel's per-pair path, whatever the choice).  All four give the same counts.  With very many
      * bins a kernel's shared-memory histograms may not fit: AUTO then takes the other fast kernel, an
      * explicit choice returns ACF_EINVAL. */
     ACF_OPT_KERNEL = 1,

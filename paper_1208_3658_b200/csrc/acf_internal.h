@@ -70,9 +70,12 @@ struct GroupCap {
 };
 
 // How the window path tallies a catalogue's weights when it is the j side (written on the device by
-// the gather kernel from the weight range).  vj[s] = C + w_s when packed (count and weight sum of the
-// pairs above an edge share one fp64 accumulator: sum = n * C + sum of w, exact while
-// exponent(w_max) - exponent(w_min > 0) <= 13), else vj[s] = w_s and the count is kept apart.
+// the gather kernel from the weight range).  vj[s] = C + w_s when packed: count and weight sum of the
+// pairs above an edge share one fp64 accumulator, sum = n * C + sum of w, exact while
+// exponent(w_max) - exponent(w_min > 0) <= 13.  Rows are then differences of exact cumulative sums.
+// Weights of a wider range do not pack (vj[s] = w_s): their cumulative sums would round at the size of
+// the largest weights and a sparsely filled row would inherit that error, so such calls take the table
+// path for every pair, which adds each w_i w_j to its row directly (acf_pair.cu).
 struct PackInfo {
     double C, inv_C;
     int packed, pad;

@@ -81,6 +81,7 @@ struct PairParams {
     unsigned long long *counters;
     int is_auto;
     int use_windows;
+    int only_unpackable;  // 1: run only if the j side's weights do not pack (the window kernel ran otherwise)
     int prune;
     int n_stages;
 };
@@ -349,6 +350,14 @@ __global__ void __launch_bounds__(kThreads + 32, kWeighted ? 1 : 2) pair_kernel(
     if (p_in.counters[kCtrBadInput] != 0) return;  // inputs failed validation: never index the LUT with garbage
     PairParams p = p_in;
     p.chord_margin = chord_margin(p_in.counters);
+    if (kWeighted) {
+        // Weights that do not pack with the count (PackInfo: range above 2^13) take the table path for every pair:
+        // it adds each product w_i w_j to its row directly, where the window tallies would form small rows as
+        // differences of large cumulative sums.
+        const bool packed = p_in.pack_b->packed != 0;
+        if (p_in.only_unpackable && packed) return;
+        if (!packed) p.use_windows = 0;
+    }
     extern __shared__ __align__(128) unsigned char smem[];
     const int rows = p.nbins + 2;
     const int n_stages = p.n_stages;
@@ -535,12 +544,8 @@ __global__ void __launch_bounds__(kThreads + 32, kWeighted ? 1 : 2) pair_kernel(
                     continue;
                 }
                 if (win.edge >= 0) {
-                    if (!kWeighted || pack.packed)
-                        window_group<kWeighted, true, kPrivate>(p, h, tile + (size_t)g * kGroup * 4, vtile + g * kGroup, nx2, ny2, nz2, wi, win,
-                                                                pack.C, pack.inv_C, i_base, j_base + g * kGroup, n_fp64);
-                    else
-                        window_group<kWeighted, false, kPrivate>(p, h, tile + (size_t)g * kGroup * 4, vtile + g * kGroup, nx2, ny2, nz2, wi, win,
-                                                                 pack.C, pack.inv_C, i_base, j_base + g * kGroup, n_fp64);
+                    window_group<kWeighted, true, kPrivate>(p, h, tile + (size_t)g * kGroup * 4, vtile + g * kGroup, nx2, ny2, nz2, wi, win,
+                                                            pack.C, pack.inv_C, i_base, j_base + g * kGroup, n_fp64);
                     n_win += (unsigned long long)(kGroup * kR);
                 } else {
                     const int gn = jn - g * kGroup < kGroup ? jn - g * kGroup : kGroup;
@@ -678,9 +683,20 @@ int count_prepared(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_au
     // which kernel: the window kernel for weighted counts, the table kernel for unweighted ones;
     // with very many bins the table kernel's rows may not fit beside its table: the window kernel then takes over
     bool use_win = ctx->opt_kernel == ACF_KERNEL_WINDOW || (ctx->opt_kernel == ACF_KERNEL_AUTO && weighted);
-    if (!use_win && smem > per_sm) {
+    const bool table_fits = smem <= per_sm;
+    if (!use_win && !table_fits) {
         if (ctx->opt_kernel != ACF_KERNEL_AUTO) return fail(ctx, ACF_EINVAL, "shared memory need %zu exceeds %d", smem, ctx->max_smem_optin);
         use_win = true;
+    }
+    // The window kernel tallies weights only when they pack with the count (PackInfo, decided on the device from the
+    // weight range); otherwise it returns at once and the table kernel, launched behind it, does the call.  Where the
+    // table kernel's histograms do not fit either, the verdict is fetched and the call refused.
+    if (use_win && weighted && !table_fits) {
+        int packed = 0;
+        ACF_CUDA_TRY(ctx, cudaMemcpyAsync(&packed, &b.pack->packed, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+        ACF_CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
+        if (!packed && ctx->h_counters[kCtrBadInput] == 0)
+            return fail(ctx, ACF_EINVAL, "weights ranging over more than 2^13 cannot be tallied with %d bins (at most about 600)", nbins);
     }
 
     // i-tiles are handed out in batches so that the item buffer stays bounded
@@ -739,6 +755,13 @@ int count_prepared(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_au
         if (use_win) {
             rc = launch_pair_win(ctx, a, b, is_auto, nbins, capacity, d_counts, d_wsums);
             if (rc != ACF_OK) return rc;
+            if (weighted && table_fits) {  // the same work list again, for weights that do not pack
+                ACF_CUDA_TRY(ctx, cudaMemsetAsync(&ctx->d_counters[kCtrWorkHead], 0, sizeof(unsigned long long), ctx->stream));
+                PairParams q = p;
+                q.only_unpackable = 1;
+                e = priv ? launch<true, true>(ctx, q, smem, grid) : launch<true, false>(ctx, q, smem, grid);
+                ACF_CUDA_TRY(ctx, e);
+            }
         } else {
             if (weighted) e = priv ? launch<true, true>(ctx, p, smem, grid) : launch<true, false>(ctx, p, smem, grid);
             else e = priv ? launch<false, true>(ctx, p, smem, grid) : launch<false, false>(ctx, p, smem, grid);
@@ -758,6 +781,15 @@ int run_pair_count_fast(acf_ctx *ctx, const double *d_a, const float *d_wa, size
     // cell table: the coarsest resolution that leaves no resolvable cell crowded
     Lut L = build_lut(h_edges, nbins, 6);
     for (int m = 7; m <= 9 && crowded_resolvable(L) > 0; ++m) L = build_lut(h_edges, nbins, m);
+    {   // with very many bins a coarser table (more cells left to the re-checks) may be what lets the kernel fit
+        const bool weighted = d_wsums != nullptr;
+        const int rows = nbins + 2;
+        const size_t words = rows <= kMaxPrivateRows ? (size_t)kWarps * rows * 32 : (size_t)kWarps * rows;
+        auto need = [&](const Lut &t) {
+            return kSmemHeader + 2 * stage_bytes(weighted) + t.cells.size() * sizeof(uint2) + words * (weighted ? 12 : 4) + 32;
+        };
+        while (L.m > 6 && need(L) > (size_t)ctx->max_smem_optin) L = build_lut(h_edges, nbins, L.m - 1);
+    }
     // device tables: the edges (fp64), the edges as squared chord lengths (fp32, chord tier), the cell table
     const size_t edge_bytes = (sizeof(double) * (size_t)(nbins + 1) + 15) & ~size_t(15);
     const size_t sed_bytes = (sizeof(float) * (size_t)(nbins + 1) + 15) & ~size_t(15);

@@ -606,7 +606,7 @@ template <bool kWeighted, bool kPacked>
 __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p)
 {
     if (p.counters[kCtrBadInput] != 0) return;  // inputs failed validation
-    if (kWeighted && (p.pack_b->packed != 0) != kPacked) return;
+    if (kWeighted && p.pack_b->packed == 0) return;  // weights that do not pack: the table kernel does the call
     extern __shared__ __align__(128) unsigned char smem[];
     const int rows_n = p.nbins + 2;
     const int n_stages = p.n_stages;
@@ -945,8 +945,7 @@ int launch_pair_win(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_a
         ctx->last.kernel_launches++;
     };
     if (weighted) {
-        launch(pair_win_kernel<true, true>);
-        launch(pair_win_kernel<true, false>);  // one of the two returns at once (PackInfo of the j side)
+        launch(pair_win_kernel<true, true>);  // returns at once if the j side's weights do not pack (acf_pair.cu)
     } else {
         launch(pair_win_kernel<false, true>);
     }

@@ -1,0 +1,110 @@
+"""Seeded random cases through every fast kernel against the oracle (-m gpu): catalogue sizes around the
+tile and group boundaries, few to 1024 bins of both presets over random ranges, auto and cross counts,
+unweighted and weighted (narrow and wide weight ranges, zeros), clustered and uniform points, row ranges.
+Each case is small; the point is the variety of paths (masked groups, many-edge windows, shared rows,
+packed and unpacked accumulators, pruning, the chord tier)."""
+import numpy as np
+import pytest
+
+from workloads import cos_edges_from_theta_deg, full_sky, linear_theta_edges_deg, log_theta_edges_deg
+
+pytestmark = pytest.mark.gpu
+
+WSUM_RTOL = 1e-12
+
+
+@pytest.fixture(scope="module")
+def acf():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    import paper_1208_3658_b200 as P
+    P.load_library()
+    return P
+
+
+@pytest.fixture(scope="module")
+def oracle():
+    from oracle import oracle as O
+    O.build()
+    return O
+
+
+def make_points(rng, n, clustered):
+    ra, dec = full_sky(n, int(rng.integers(1, 1 << 30)))
+    if clustered:  # pull the points into a few clumps so that small separations are populated
+        k = max(1, n // 40)
+        ra = (ra[rng.integers(0, k, n)] + rng.normal(0, 0.05, n)) % 360.0
+        dec = np.clip(dec[rng.integers(0, k, n)] + rng.normal(0, 0.05, n), -89.0, 89.0)
+    return ra, dec
+
+
+def random_case(rng):
+    n_a = int(rng.choice([1, 2, 31, 127, 128, 129, 700, 1023, 1024, 1025, 2500, 5000]))
+    n_b = int(rng.choice([1, 33, 128, 640, 1024, 1100, 3000]))
+    auto = bool(rng.integers(0, 2))
+    nbins = int(rng.choice([1, 2, 7, 40, 254, 1024]))
+    lo = float(rng.choice([0.0, 1e-4, 0.01, 0.5]))
+    hi = float(rng.choice([0.2, 5.0, 60.0, 180.0]))
+    if hi <= lo:
+        hi = 180.0
+    if rng.integers(0, 2) and lo > 0:
+        theta = log_theta_edges_deg(lo, hi, nbins)
+    else:
+        theta = linear_theta_edges_deg(lo, hi, nbins)
+    weights = int(rng.integers(0, 4))  # 0 none, 1 narrow, 2 wide, 3 with zeros
+    return n_a, n_b, auto, cos_edges_from_theta_deg(theta), weights, bool(rng.integers(0, 2))
+
+
+def draw_weights(rng, n, kind):
+    if kind == 0:
+        return None
+    w = np.exp(rng.uniform(-1, 1, n) if kind == 1 else rng.uniform(-12, 12, n)).astype(np.float32)
+    if kind == 3:
+        w[rng.integers(0, 3, n) == 0] = 0.0
+    return w
+
+
+@pytest.mark.parametrize("seed", range(48))
+def test_random_cases_all_kernels(acf, oracle, seed):
+    import torch
+    rng = np.random.default_rng(1000 + seed)
+    n_a, n_b, auto, edges, wk, clustered = random_case(rng)
+    ra, dec = make_points(rng, n_a, clustered)
+    a = acf.acf_radec_to_xyz(ra, dec)
+    b = None
+    if not auto:
+        rb, db = make_points(rng, n_b, clustered)
+        b = acf.acf_radec_to_xyz(rb, db)
+    wa = draw_weights(rng, n_a, wk)
+    wb = None if (auto or wa is None) else draw_weights(rng, n_b, wk)
+    rows = None
+    if rng.integers(0, 3) == 0 and n_a > 2:
+        i0 = int(rng.integers(0, n_a - 1))
+        rows = (i0, int(rng.integers(i0 + 1, n_a + 1)))
+    want = oracle.pair_count(a, b, edges, auto, w_a=wa, w_b=wb, rows=rows)
+    ctx = acf.acf_create(0)
+    try:
+        for kern in (acf.ACF_KERNEL_WINDOW, acf.ACF_KERNEL_TABLE, acf.ACF_KERNEL_AUTO):
+            for bulk in (0, 1):
+                acf.acf_set_option(ctx, acf.ACF_OPT_KERNEL, kern)
+                acf.acf_set_option(ctx, acf.ACF_OPT_BULK, bulk)
+                da = torch.from_numpy(a).cuda()
+                db_ = None if auto else torch.from_numpy(b).cuda()
+                dwa = None if wa is None else torch.from_numpy(wa).cuda()
+                dwb = None if wb is None else torch.from_numpy(wb).cuda()
+                i0, i1 = rows if rows is not None else (0, n_a)
+                try:
+                    out = acf.acf_pair_count_rows(ctx, da, dwa, i0, i1, db_, dwb, edges, auto)
+                except acf.AcfError as e:
+                    # an explicit kernel choice may not fit its histograms into shared memory (include/acf.h)
+                    assert kern != acf.ACF_KERNEL_AUTO and edges.size > 600, str(e)
+                    continue
+                torch.cuda.synchronize()
+                if wa is None:
+                    assert acf.counts_to_numpy(out).tolist() == want.tolist(), (seed, kern, bulk)
+                else:
+                    assert acf.counts_to_numpy(out[0]).tolist() == want[0].tolist(), (seed, kern, bulk)
+                    np.testing.assert_allclose(out[1].cpu().numpy(), want[1], rtol=WSUM_RTOL, atol=0, err_msg=str((seed, kern, bulk)))
+    finally:
+        acf.acf_destroy(ctx)
