@@ -356,7 +356,10 @@ __global__ void __launch_bounds__(kThreads + 32, kWeighted ? 1 : 2) pair_kernel(
         // differences of large cumulative sums.
         const bool packed = p_in.pack_b->packed != 0;
         if (p_in.only_unpackable && packed) return;
-        if (!packed) p.use_windows = 0;
+        // This kernel's windows correct a mis-tallied pair by adding its weight to one row and subtracting it from
+        // another; a row left with much smaller weights keeps the rounding of the larger one.  Counts are integers and
+        // do not mind; weighted sums go pair by pair here (the window kernel corrects its exact accumulators instead).
+        p.use_windows = 0;
     }
     extern __shared__ __align__(128) unsigned char smem[];
     const int rows = p.nbins + 2;

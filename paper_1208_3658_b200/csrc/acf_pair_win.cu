@@ -163,19 +163,30 @@ struct Mask {
     }
 };
 
-// The exact corrections of one chunk of a group, after its loop: amb_steps has a bit per step of kStep
-// j-points in which some pair came within the guard band of an edge.  Every pair of those steps is
-// re-derived exactly as the loop computed it; where the fp64 row of include/acf.h disagrees with what
-// the loop tallied, the rows are corrected (atomics: any lane may come here).  One copy for all chunk
-// shapes; it reloads the i-points rather than taking them in registers.
+// The exact corrections of one chunk of a group, after its loop and before its tallies are read:
+// amb_steps has a bit per step of kStep j-points in which some pair came within the guard band of an
+// edge.  Every pair of those steps is re-derived bit for bit as the loop computed it; a pair within a
+// guard band gets its row from the chord tier or the fp64 definition of include/acf.h, and where that
+// disagrees with what the loop tallied, the correction of this thread's accumulators comes back:
+//   dt[q * kR + r]  to add to t[q][r]: 2^-7 v_j for a pair that is above edge q after all, minus that for
+//                   one that is not (the accumulators are exact sums, so the corrected tally is exactly the
+//                   tally of the exact classification: no row ever sees a wrong pair added and taken back);
+//   dn[q]           to add to nb[q] (unweighted: pairs not above edge q).
+// One copy for all chunk shapes; it reloads the i-points rather than taking them in registers.
 template <bool kWeighted>
-__device__ __forceinline__ void fixup_body(const WinParams &p, const Rows rows, const float *__restrict__ grp2, uint32_t amb_steps,
-                                           int K, int m_a, bool masked, const Mask mk, uint32_t i_base, uint32_t j_first,
-                                           unsigned long long *stat, const float4 (&pi)[kR])
+__device__ __noinline__ void fixup_chunk(const WinParams &p, const float *__restrict__ grp2, const double *__restrict__ vgrp,
+                                         uint32_t amb_steps, int K, int m_a, bool masked, const Mask mk, uint32_t i_base,
+                                         uint32_t j_first, unsigned long long *stat, double *__restrict__ dt, int *__restrict__ dn)
 {
+    float4 pi[kR];
+#pragma unroll
+    for (int r = 0; r < kR; ++r) pi[r] = p.pts_a[i_base + local_i(r)];  // the array is padded to a whole tile
+    for (int i = 0; i < kChunk * kR; ++i) dt[i] = 0.0;
+    for (int i = 0; i < kChunk; ++i) dn[i] = 0;
     const double e0 = p.edges[m_a];
     const float e32 = (float)e0;
     const float G = K == 1 ? kGuard1 : kGuardK;
+    const float margin = chord_margin(p.counters);
     float dl[kChunk];
 #pragma unroll
     for (int q = 0; q < kChunk; ++q) dl[q] = q > 0 && q < K ? (float)(p.edges[m_a + q] - e0) : 0.f;
@@ -193,7 +204,7 @@ __device__ __forceinline__ void fixup_body(const WinParams &p, const Rows rows, 
                 for (int q = 0; q < kChunk; ++q) amb |= q < K && !(fabsf(q == 0 ? d0 : __fadd_rn(d0, dl[q])) > G);
                 if (!amb) continue;
                 // the chord length decides where the cosine could not; what it leaves open, the definition
-                int exact = chord_row(pi[r].x, pi[r].y, pi[r].z, pj.x, pj.y, pj.z, p.sedges, p.nbins, chord_margin(p.counters));
+                int exact = chord_row(pi[r].x, pi[r].y, pi[r].z, pj.x, pj.y, pj.z, p.sedges, p.nbins, margin);
                 if (exact < 0) {
                     exact = exact_row(p.xyz_a, p.stride_a, p.perm_a[i_base + local_i(r)], p.xyz_b, p.stride_b,
                                       p.perm_b[j_first + jj0 + u], p.edges, p.nbins);
@@ -201,7 +212,6 @@ __device__ __forceinline__ void fixup_body(const WinParams &p, const Rows rows, 
                 } else {
                     atomicAdd(&stat[kStatChord], 1ull);
                 }
-                const double w = (double)pi[r].w * (double)pj.w;
 #pragma unroll
                 for (int q = 0; q < kChunk; ++q) {
                     if (q >= K) break;
@@ -210,53 +220,12 @@ __device__ __forceinline__ void fixup_body(const WinParams &p, const Rows rows, 
                     const bool fast_above = kWeighted ? dq > 0.f : (__float_as_uint(dq) >> 31) == 0u;
                     const bool exact_above = exact > m_a + q;
                     if (fast_above != exact_above) {
-                        // the tally above edge q is taken from row m_a + q and given to row m_a + q + 1
-                        // (by this chunk or, carried, by the next): the pair moves between the two
-                        const uint32_t dn = fast_above ? 1u : 0xffffffffu;  // +1 / -1 for the lower row
-                        const double dw = fast_above ? w : -w;
-                        atomicAdd(&rows.cnt[m_a + q], dn);
-                        atomicAdd(&rows.cnt[m_a + q + 1], 0u - dn);
-                        if constexpr (kWeighted) {
-                            atomicAdd(&rows.ws[m_a + q], dw);
-                            atomicAdd(&rows.ws[m_a + q + 1], -dw);
-                        }
+                        if constexpr (kWeighted) dt[q * kR + r] += (exact_above ? 0.0078125 : -0.0078125) * vgrp[jj0 + u];
+                        else dn[q] += exact_above ? -1 : 1;
                     }
                 }
             }
         }
-    }
-}
-
-template <bool kWeighted>
-__device__ __noinline__ void fixup_chunk(const WinParams &p, const Rows rows, const float *__restrict__ grp2, uint32_t amb_steps,
-                                         int K, int m_a, bool masked, const Mask mk, uint32_t i_base, uint32_t j_first,
-                                         unsigned long long *stat)
-{
-    float4 pi[kR];
-#pragma unroll
-    for (int r = 0; r < kR; ++r) pi[r] = p.pts_a[i_base + local_i(r)];  // the array is padded to a whole tile
-    fixup_body<kWeighted>(p, rows, grp2, amb_steps, K, m_a, masked, mk, i_base, j_first, stat, pi);
-}
-
-// The corrections of the single-edge groups of one staged tile, noted by the kernel's own loop
-// (one call per tile and warp instead of one per group).
-struct FixNote {
-    uint32_t amb_steps;
-    int m_edge;
-};
-template <bool kWeighted>
-__device__ __noinline__ void fixup_tile(const WinParams &p, const Rows rows, const float *__restrict__ tile, const FixNote *notes,
-                                        uint32_t i_base, uint32_t j_base, unsigned long long *stat)
-{
-    float4 pi[kR];
-#pragma unroll
-    for (int r = 0; r < kR; ++r) pi[r] = p.pts_a[i_base + local_i(r)];
-    Mask mk{};
-    for (int g = 0; g < kGroupsPerTile; ++g) {
-        const FixNote n = notes[g];
-        if (n.amb_steps)
-            fixup_body<kWeighted>(p, rows, tile + (size_t)g * kGroup * 4, n.amb_steps, 1, n.m_edge, false, mk, i_base,
-                                  j_base + g * kGroup, stat, pi);
     }
 }
 
@@ -399,6 +368,21 @@ __device__ __forceinline__ uint32_t window_chunk(const WinParams &p, const Rows 
         }
     }
 
+    if (amb_steps) {
+        // exact corrections, applied to the (exact) accumulators before anything is read from them
+        double dt[kChunk * kR];
+        int dn[kChunk];
+        fixup_chunk<kWeighted>(p, grp2, vgrp, amb_steps, K, m_a, kMasked, mk, i_base, j_first, stat, dt, dn);
+#pragma unroll
+        for (int q = 0; q < K; ++q) {
+            if constexpr (kWeighted) {
+#pragma unroll
+                for (int r = 0; r < kR; ++r) t[q][r] += dt[q * kR + r];
+            } else {
+                nb[q] += (uint32_t)dn[q];
+            }
+        }
+    }
     // ---- this thread's tallies -> row contributions -> the warp's rows
     auto unpack = [&](double tt, uint32_t &n) -> double {  // 2^-7 (n C + sum of w) -> sum of w, n += count
         double sw = tt * 128.0;
@@ -427,7 +411,7 @@ __device__ __forceinline__ uint32_t window_chunk(const WinParams &p, const Rows 
         tally->c_hi += c_hi;
         if (c_lo != 0u) tally->w_lo += w_lo;  // no pair of this thread in the row: not even a rounding residue
         if (c_hi != 0u) tally->w_hi += w_hi;
-        return amb_steps;  // the caller sees to the corrections
+        return 0u;
     }
     uint32_t c_prev = 0;  // this thread's pairs above the previous edge (all its pairs before the first)
     double s_prev[kR];    // and, per i-point, the sum of their w_j
@@ -484,7 +468,6 @@ __device__ __forceinline__ uint32_t window_chunk(const WinParams &p, const Rows 
         for (int r = 0; r < kR; ++r) carry->s[r] = s_prev[r];
     }
     __syncwarp();
-    if (amb_steps) fixup_chunk<kWeighted>(p, rows, grp2, amb_steps, K, m_a, kMasked, mk, i_base, j_first, stat);
     return 0u;
 }
 
@@ -630,8 +613,6 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p
     double *ws_all = reinterpret_cast<double *>(smem + off);
     if constexpr (kWeighted) off += (size_t)row_sets * rows_n * sizeof(double);
     WinRows *win_all = reinterpret_cast<WinRows *>(smem + off);
-    off += (size_t)kWarps * kGroupsPerTile * sizeof(WinRows);
-    FixNote *notes_all = reinterpret_cast<FixNote *>(smem + off);
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int igrp = warp & (kTeamWarps - 1), team = warp / kTeamWarps;
@@ -665,7 +646,6 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p
     rows.cnt = cnt_all + (rows.shared ? 0 : (size_t)warp * rows_n);
     rows.ws = ws_all + (rows.shared ? 0 : (size_t)warp * rows_n);
     WinRows *win = win_all + (size_t)warp * kGroupsPerTile;
-    FixNote *notes = notes_all + (size_t)warp * kGroupsPerTile;
     uint32_t since_flush = 0;  // j-tiles this warp has tallied in its unflushed rows
     // u32 rows: flush before the tallies could wrap (shared rows take the pairs of all the CTA's warps)
     // (the rows are read as signed 32-bit numbers when flushed: half the range)
@@ -803,9 +783,6 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p
             __syncwarp();
             // pass 1: the common groups (one edge, nothing masked), inline; the others are noted in slow_groups
             uint32_t slow_groups = 0;
-            bool any_amb = false;
-            if (lane < kGroupsPerTile) notes[lane].amb_steps = 0u;
-            __syncwarp();
             for (int g = diag ? igrp : 0; g < n_groups; ++g) {
                 if ((g & (kTeams - 1)) != team) continue;  // the other team's group
                 const int r_lo = win[g].lo, r_hi = win[g].hi;
@@ -822,23 +799,15 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p
                     flush_tally();
                     tally_m = m_edge;
                 }
-                const uint32_t amb = window_chunk<1, kWeighted, kPacked, false, true>(p, rows, tile + (size_t)g * kGroup * 4, vtile + g * kGroup,
+                window_chunk<1, kWeighted, kPacked, false, true>(p, rows, tile + (size_t)g * kGroup * 4, vtile + g * kGroup,
                                                                                       nx, ny, nz, wi, m_edge, true, true, win[g].wsum, mk,
                                                                                       i_base, j_base + g * kGroup, stat, &tally, nullptr,
                                                                                       win[g].e32);
-                if (lane == 0) {
-                    atomicAdd(&stat[kStatWindow], (unsigned long long)(kGroup * kGroup));
-                    notes[g].amb_steps = amb;
-                    notes[g].m_edge = m_edge;
-                }
-                any_amb |= amb != 0u;
+                if (lane == 0) atomicAdd(&stat[kStatWindow], (unsigned long long)(kGroup * kGroup));
             }
-            __syncwarp();
-            if (any_amb) slow_groups |= 0x80000000u;  // corrections to make: also a call, also followed by the reload
             // pass 2: the rest through the function; it reloads the i-points, and so does this loop afterwards
             // (they are not kept in registers across the calls)
             if (slow_groups) {
-                if (any_amb) fixup_tile<kWeighted>(p, rows, tile, notes, i_base, j_base, stat);
                 for (int g = 0; g < n_groups; ++g) {
                     if (!((slow_groups >> g) & 1u)) continue;
                     const int r_lo = win[g].lo, r_hi = win[g].hi;
@@ -895,7 +864,7 @@ int launch_pair_win(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_a
         m += (size_t)row_sets * rows_n * sizeof(uint32_t);
         m = (m + 15) & ~size_t(15);
         if (weighted) m += (size_t)row_sets * rows_n * sizeof(double);
-        m += (size_t)kWarps * kGroupsPerTile * (sizeof(WinRows) + sizeof(FixNote));
+        m += (size_t)kWarps * kGroupsPerTile * sizeof(WinRows);
         return m;
     };
     // one CTA of 16 warps per SM: 128 registers a thread

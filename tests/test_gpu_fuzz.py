@@ -3,6 +3,8 @@ tile and group boundaries, few to 1024 bins of both presets over random ranges, 
 unweighted and weighted (narrow and wide weight ranges, zeros), clustered and uniform points, row ranges.
 Each case is small; the point is the variety of paths (masked groups, many-edge windows, shared rows,
 packed and unpacked accumulators, pruning, the chord tier)."""
+import os
+
 import numpy as np
 import pytest
 
@@ -65,7 +67,10 @@ def draw_weights(rng, n, kind):
     return w
 
 
-@pytest.mark.parametrize("seed", range(48))
+N_SEEDS = int(os.environ.get("ACF_FUZZ_SEEDS", "48"))  # more seeds for a longer hunt
+
+
+@pytest.mark.parametrize("seed", range(N_SEEDS))
 def test_random_cases_all_kernels(acf, oracle, seed):
     import torch
     rng = np.random.default_rng(1000 + seed)
