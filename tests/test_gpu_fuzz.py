@@ -42,8 +42,9 @@ def make_points(rng, n, clustered):
 
 
 def random_case(rng):
-    n_a = int(rng.choice([1, 2, 31, 127, 128, 129, 700, 1023, 1024, 1025, 2500, 5000]))
-    n_b = int(rng.choice([1, 33, 128, 640, 1024, 1100, 3000]))
+    big = [9000, 20000] if os.environ.get("ACF_FUZZ_BIG") else []
+    n_a = int(rng.choice([1, 2, 31, 127, 128, 129, 700, 1023, 1024, 1025, 2500, 5000] + big))
+    n_b = int(rng.choice([1, 33, 128, 640, 1024, 1100, 3000] + big))
     auto = bool(rng.integers(0, 2))
     nbins = int(rng.choice([1, 2, 7, 40, 254, 1024]))
     lo = float(rng.choice([0.0, 1e-4, 0.01, 0.5]))
