@@ -36,7 +36,7 @@ I_ALG_WEIGHTED = 14
 # From the committed ncu capture of the dominant kernel on the default workload (one launch: the weighted DR
 # count, 1.0e12 pairs); not measured by this script.  See profiles/r1_v5_pair_win_kernel_ncu.md.
 NCU_FULL_SKY = {"profile": "profiles/r1_v5_pair_win_kernel_ncu.md", "launch": "weighted DR count, 1.0e12 pairs",
-                "dram_bytes": 1174507096, "sass_thread_inst_per_pair": 7.08, "issue_active_pct": 58.6}
+                "dram_bytes": 2298431496, "sass_thread_inst_per_pair": 7.23, "issue_active_pct": 60.8}
 
 
 def parse_args():
