@@ -10,7 +10,8 @@
 //   above_q = d_q > 0                               the pair lies in a row beyond edge m + q
 //   certified iff |d_q| > G for every q             else the exact fp64 row of include/acf.h decides
 // Per i-point and edge one fp64 accumulator takes t += [above_q] v_j (v_j = C + w_j packs the count and
-// the weight sum, see PackInfo; unweighted counts shift the sign bits of d_q into a word instead).
+// the weight sum, see PackInfo: exact sums; weights of too wide a range for that are not tallied here
+// but pair by pair in acf_pair.cu; unweighted counts shift the sign bits of d_q into a word instead).
 // The accumulators are cumulative in q (above edge m + q implies above edge m + q - 1), so the rows get
 // the differences of consecutive edges; they are formed per i-point before anything is summed.
 // After a chunk the warp reduces its row tallies with shuffles and lane 0 adds them to the warp's rows in
@@ -246,7 +247,7 @@ struct LaneTally {
 // Edges m_a .. m_a + K - 1 against one group of kGroup staged j-points and this thread's kR i-points.
 // A chunk fills rows m_a .. m_a + K - 1 (and m_a + K if it is the last of its group); the tallies above
 // its last edge go to the next chunk through `carry`.
-template <int K, bool kWeighted, bool kPacked, bool kMasked, bool kDeferFix = false>
+template <int K, bool kWeighted, bool kMasked, bool kDeferFix = false>
 __device__ __forceinline__ uint32_t window_chunk(const WinParams &p, const Rows rows, const float *__restrict__ grp2,
                                              const double *__restrict__ vgrp, const float (&nx)[kR],
                                              const float (&ny)[kR], const float (&nz)[kR],
@@ -272,13 +273,11 @@ __device__ __forceinline__ uint32_t window_chunk(const WinParams &p, const Rows 
     double t[K][kR];     // weighted: 2^-7 * sum of v_j over the pairs above edge q, per i-point
     uint32_t sg[K][kR];  // unweighted: sign bits of d_q (1 = not above) of the last 32 j-points
     uint32_t nb[K];      // unweighted: pairs not above edge q
-    float nf[K];         // weighted, not packed: pairs above edge q (exact: at most kGroup * kR)
     double tall[kR];     // masked: 2^-7 * sum of v_j over the enabled pairs
     uint32_t call = 0;   // masked: enabled pairs
 #pragma unroll
     for (int q = 0; q < K; ++q) {
         nb[q] = 0u;
-        nf[q] = 0.f;
 #pragma unroll
         for (int r = 0; r < kR; ++r) {
             t[q][r] = 0.0;
@@ -330,14 +329,12 @@ __device__ __forceinline__ uint32_t window_chunk(const WinParams &p, const Rows 
                         unsigned long long &g0 = ind[(u * kR + 2 * r) % kInd], &g1 = ind[(u * kR + 2 * r + 1) % kInd];
                         t[q][r] = fma(v0, ind_gt0_f64(g0, a), t[q][r]);
                         t[q][r] = fma(v1, ind_gt0_f64(g1, b), t[q][r]);
-                        if constexpr (!kPacked) nf[q] += __uint_as_float((uint32_t)(g0 >> 32)) + __uint_as_float((uint32_t)(g1 >> 32));
                     } else if constexpr (kWeighted) {
                         float i0 = ind_gt0(a), i1 = ind_gt0(b);
                         i0 = on0 ? i0 : 0.f;
                         i1 = on1 ? i1 : 0.f;
                         t[q][r] = fma(v0, __hiloint2double(__float_as_int(i0), 0), t[q][r]);
                         t[q][r] = fma(v1, __hiloint2double(__float_as_int(i1), 0), t[q][r]);
-                        if constexpr (!kPacked) nf[q] += i0 + i1;
                     } else {
                         uint32_t ba = __float_as_uint(a), bb = __float_as_uint(b);
                         if constexpr (kMasked) {
@@ -386,7 +383,7 @@ __device__ __forceinline__ uint32_t window_chunk(const WinParams &p, const Rows 
     // ---- this thread's tallies -> row contributions -> the warp's rows
     auto unpack = [&](double tt, uint32_t &n) -> double {  // 2^-7 (n C + sum of w) -> sum of w, n += count
         double sw = tt * 128.0;
-        if constexpr (kPacked) {
+        if constexpr (kWeighted) {
             const double nn = floor(sw * rows.pack->inv_C);  // C is a power of two and the sum of w is below C: exact
             sw -= nn * rows.pack->C;
             n += (uint32_t)nn;
@@ -396,7 +393,7 @@ __device__ __forceinline__ uint32_t window_chunk(const WinParams &p, const Rows 
     if constexpr (kDeferFix) {
         // the kernel's own loop: one edge, nothing masked; the two rows' tallies stay with the thread
         static_assert(K == 1 && !kMasked, "");
-        uint32_t c_hi = kWeighted ? (kPacked ? 0u : (uint32_t)nf[0]) : (uint32_t)(kGroup * kR) - nb[0];
+        uint32_t c_hi = kWeighted ? 0u : (uint32_t)(kGroup * kR) - nb[0];
         double w_lo = 0.0, w_hi = 0.0;
         if constexpr (kWeighted) {
 #pragma unroll
@@ -439,7 +436,7 @@ __device__ __forceinline__ uint32_t window_chunk(const WinParams &p, const Rows 
         double rw = 0.0;   // weight of this thread's pairs in row m_a + q
         if (q < K) {
             if constexpr (kWeighted) {
-                c_q = kPacked ? 0u : (uint32_t)nf[q];
+                c_q = 0u;
 #pragma unroll
                 for (int r = 0; r < kR; ++r) {
                     const double sw = unpack(t[q][r], c_q);
@@ -473,11 +470,11 @@ __device__ __forceinline__ uint32_t window_chunk(const WinParams &p, const Rows 
 
 // One group: all edges r_lo .. r_hi - 1 of its window, kChunk at a time.
 #define ACF_WIN_CHUNK_CALL(K, MASKED) \
-    window_chunk<K, kWeighted, kPacked, MASKED>(p, rows, grp2, vgrp, nx, ny, nz, wi, m, m == r_lo, left <= K, wsum_j, mk, i_base, j_first, stat, \
+    window_chunk<K, kWeighted, MASKED>(p, rows, grp2, vgrp, nx, ny, nz, wi, m, m == r_lo, left <= K, wsum_j, mk, i_base, j_first, stat, \
                                                 nullptr, &carry)
 // Not inlined: only the common case (one edge, nothing masked) lives in the kernel's own loop, so that
 // the register allocation of that loop is not set by the rare variants.  It reloads the i-points.
-template <bool kWeighted, bool kPacked>
+template <bool kWeighted>
 __device__ __noinline__ void window_group(const WinParams &p, const Rows rows, const float *__restrict__ grp2,
                                           const double *__restrict__ vgrp, int r_lo, int r_hi,
                                           double wsum_j, bool masked, const Mask mk, uint32_t i_base, uint32_t j_first,
@@ -583,9 +580,7 @@ __device__ __forceinline__ void try_produce(const WinParams &p, volatile ProdSta
     atomicExch(const_cast<uint32_t *>(&ps->lock), 0u);
 }
 
-// kPacked: the variant for j-side weights that pack with the count (PackInfo); the host launches both
-// variants of a weighted count and the one that does not match the catalogue returns at once.
-template <bool kWeighted, bool kPacked>
+template <bool kWeighted>
 __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p)
 {
     if (p.counters[kCtrBadInput] != 0) return;  // inputs failed validation
@@ -799,7 +794,7 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p
                     flush_tally();
                     tally_m = m_edge;
                 }
-                window_chunk<1, kWeighted, kPacked, false, true>(p, rows, tile + (size_t)g * kGroup * 4, vtile + g * kGroup,
+                window_chunk<1, kWeighted, false, true>(p, rows, tile + (size_t)g * kGroup * 4, vtile + g * kGroup,
                                                                                       nx, ny, nz, wi, m_edge, true, true, win[g].wsum, mk,
                                                                                       i_base, j_base + g * kGroup, stat, &tally, nullptr,
                                                                                       win[g].e32);
@@ -817,7 +812,7 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p
                     mk.j0 = g * kGroup;
                     mk.diag = diag && g == igrp;
                     const bool masked = !warp_full || mk.jn < kGroup || mk.diag;
-                    window_group<kWeighted, kPacked>(p, rows, tile + (size_t)g * kGroup * 4, vtile + g * kGroup, r_lo, r_hi, win[g].wsum,
+                    window_group<kWeighted>(p, rows, tile + (size_t)g * kGroup * 4, vtile + g * kGroup, r_lo, r_hi, win[g].wsum,
                                                      masked, mk, i_base, j_base + g * kGroup, stat);
                     if (lane == 0 && !masked && r_hi - r_lo <= 1) atomicAdd(&stat[kStatWindow], (unsigned long long)(kGroup * kGroup));
                 }
@@ -914,9 +909,9 @@ int launch_pair_win(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_a
         ctx->last.kernel_launches++;
     };
     if (weighted) {
-        launch(pair_win_kernel<true, true>);  // returns at once if the j side's weights do not pack (acf_pair.cu)
+        launch(pair_win_kernel<true>);  // returns at once if the j side's weights do not pack (acf_pair.cu)
     } else {
-        launch(pair_win_kernel<false, true>);
+        launch(pair_win_kernel<false>);
     }
     if (e == cudaSuccess) e = cudaGetLastError();
     ACF_CUDA_TRY(ctx, e);
