@@ -303,7 +303,11 @@ def main():
         "traffic": NCU_FULL_SKY["dram_bytes"] if (args.workload == "full_sky" and args.scale == 1.0 and args.kernel == "auto") else None,
         "traffic_is": "dram__bytes_read.sum + dram__bytes_write.sum of one launch (%s), %s" % (NCU_FULL_SKY["launch"], NCU_FULL_SKY["profile"]),
         "ncu": NCU_FULL_SKY if (args.workload == "full_sky" and args.scale == 1.0 and args.kernel == "auto") else None,
-        "algorithmic_inst_per_pair": i_alg, "pairs_per_step": evaluated_per_step, "kernel_ms_per_step": pair_ms_per_step,
+        "algorithmic_inst_per_pair": i_alg,
+        "algorithmic_inst_is": "SURVEY.md 8(d): 3 cosine + ~5 locate + 2 certify + 1 update (+3 weighted); the window kernel's "
+                               "single-edge loop issues 5.5 per weighted pair, so frac may exceed 1: see ncu.issue_active_pct for the "
+                               "issue-slot utilisation itself",
+        "frac_of_fma_floor": (evaluated_per_step * 3 / pair_s / 1e12 / peak_tinst) if pair_s > 0 else 0.0, "pairs_per_step": evaluated_per_step, "kernel_ms_per_step": pair_ms_per_step,
         "kernel_share_of_step": pair_kernel_share,
         "peak_is": "%d SMs x 4 schedulers x 32 lanes x %.0f MHz (max SM clock, MEASURED_PEAKS.json / fallback 1965)"
                    % (props.multi_processor_count, sm_max_mhz),
