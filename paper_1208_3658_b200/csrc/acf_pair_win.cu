@@ -608,6 +608,8 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p
     double *ws_all = reinterpret_cast<double *>(smem + off);
     if constexpr (kWeighted) off += (size_t)row_sets * rows_n * sizeof(double);
     WinRows *win_all = reinterpret_cast<WinRows *>(smem + off);
+    off += (size_t)kWarps * kGroupsPerTile * sizeof(WinRows);
+    double *edges_sm = reinterpret_cast<double *>(smem + off);  // the edges, for the windows' row searches
 
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
     const int igrp = warp & (kTeamWarps - 1), team = warp / kTeamWarps;
@@ -615,6 +617,7 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p
         cnt_all[i] = 0;
         if constexpr (kWeighted) ws_all[i] = 0.0;
     }
+    for (int i = tid; i <= p.nbins; i += blockDim.x) edges_sm[i] = p.edges[i];
     if (tid == 0) {
         for (int s = 0; s < n_stages; ++s) {
             mbar_init(&full[s], 1);
@@ -746,9 +749,9 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p
                 double c_lo, c_hi;
                 if (cap_window(p.gcaps_a[(size_t)m.ti * kGroupsPerTile + igrp], gb, c_lo, c_hi)) {
                     // rows of the two ends; the far end is a few rows on at most: walk there
-                    int hi = wr.lo = row_of_cos(c_hi, p.edges, p.nbins);
-                    while (hi < p.nbins && c_lo <= p.edges[hi]) ++hi;
-                    if (hi == p.nbins && c_lo < p.edges[p.nbins]) ++hi;
+                    int hi = wr.lo = row_of_cos(c_hi, edges_sm, p.nbins);
+                    while (hi < p.nbins && c_lo <= edges_sm[hi]) ++hi;
+                    if (hi == p.nbins && c_lo < edges_sm[p.nbins]) ++hi;
                     wr.hi = hi;
                 }
                 if (p.prune && wr.hi == wr.lo && (wr.lo == 0 || wr.lo > p.nbins) && !(diag && my_g < igrp)) {
@@ -770,7 +773,7 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p
                     wr.lo = wr.hi = -1;
                 }
                 const int m_one = wr.hi > wr.lo ? wr.lo : (wr.lo > p.nbins ? p.nbins : (wr.lo < 0 ? 0 : wr.lo));
-                wr.e32 = (float)p.edges[m_one];
+                wr.e32 = (float)edges_sm[m_one];
                 wr.pad = 0;
                 wr.wsum = gb.wsum;
                 win[my_g] = wr;
@@ -860,6 +863,7 @@ int launch_pair_win(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_a
         m = (m + 15) & ~size_t(15);
         if (weighted) m += (size_t)row_sets * rows_n * sizeof(double);
         m += (size_t)kWarps * kGroupsPerTile * sizeof(WinRows);
+        m += sizeof(double) * (size_t)(nbins + 1);
         return m;
     };
     // one CTA of 16 warps per SM: 128 registers a thread
