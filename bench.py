@@ -122,6 +122,8 @@ def oracle_sample(w, n_rows: int):
     """Times the CPU oracle on DR rows [0, n_rows) x all randoms (weighted when the workload is).
     Returns (pairs, seconds, cores)."""
     from oracle import oracle as O
+    # all the box's cores, also under torchrun (which sets OMP_NUM_THREADS=1 for its workers)
+    O.set_num_threads(len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1))
     xd = O.radec_to_xyz(w.ra_d, w.dec_d)
     xr = O.radec_to_xyz(w.ra_r, w.dec_r)
     n_rows = min(n_rows, w.n_d)
@@ -138,6 +140,7 @@ def run_reference(args):
         return 0
     w = make_config(args.workload, args.scale)
     from oracle import oracle as O
+    O.set_num_threads(len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1))
     cores = O.num_threads()
     # ~2 s of work per step at ~25 Mpairs/s/core
     n_rows = args.cpu_rows or max(1, min(w.n_d, int(2.0 * 25e6 * cores / max(1, w.n_r))))
@@ -317,6 +320,7 @@ def main():
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         from oracle import oracle as O
+        O.set_num_threads(len(os.sched_getaffinity(0)) if hasattr(os, "sched_getaffinity") else (os.cpu_count() or 1))
         cores = O.num_threads()
         n_rows = args.cpu_rows or max(1, min(w.n_d, int(12.0 * 25e6 * cores / max(1, w.n_r))))
         pairs, dt, cores = oracle_sample(w, n_rows)
