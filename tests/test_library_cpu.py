@@ -47,6 +47,26 @@ def test_no_gpu_means_error_not_fallback(acf):
     assert b"no CUDA device" in lib.acf_last_error(None)
 
 
+def test_binding_constants_match_header(acf):
+    """Every enumerator and #define of include/acf.h that the binding repeats has the header's value."""
+    header = open(os.path.join(ROOT, "include", "acf.h")).read()
+    header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
+    values = {m.group(1): int(m.group(2)) for m in re.finditer(r"\b(ACF_[A-Z0-9_]+)\s*=\s*(-?\d+)", header)}
+    values.update({m.group(1): int(m.group(2)) for m in re.finditer(r"#define\s+(ACF_[A-Z0-9_]+)\s+\(?(-?\d+)\)?", header)})
+    assert {"ACF_OPT_KERNEL", "ACF_KERNEL_WINDOW", "ACF_EST_HAMILTON", "ACF_BINS_LOG10", "ACF_OPT_BULK", "ACF_MAX_BINS"} <= set(values)
+    import paper_1208_3658_b200.binding as B
+    checked = 0
+    for name, val in values.items():
+        if hasattr(B, name):
+            assert getattr(B, name) == val, name
+            checked += 1
+    assert checked >= 20
+    # the statistics structure: same fields, same order as the header
+    fields = re.search(r"typedef struct acf_stats \{(.*?)\} acf_stats;", header, flags=re.S).group(1)
+    names = re.findall(r"(?:uint64_t|double)\s+(\w+);", fields)
+    assert names == [f for f, _ in B.acf_stats._fields_]
+
+
 def test_radec_to_xyz_matches_oracle_bitwise(acf, oracle):
     ra, dec = full_sky(50000, 77)
     assert acf.acf_radec_to_xyz(ra, dec).tobytes() == oracle.radec_to_xyz(ra, dec).tobytes()
