@@ -47,13 +47,14 @@ class Dev:
         self.wr = torch.from_numpy(w.w_r).cuda() if w.w_r is not None else None
 
 
-def count(acf, ctx, d, which, rows=None, windows=1, kernel=None):
+def count(acf, ctx, d, which, rows=None, windows=1, kernel=None, bulk=0):
     """-> (u64 counts, f64 sums or None, stats) of DD / DR / RD / RR on the device."""
     import torch
     a, wa, b, wb, auto = {"dd": (d.xd, d.wd, None, None, True), "dr": (d.xd, d.wd, d.xr, d.wr, False),
                           "rd": (d.xr, d.wr, d.xd, d.wd, False), "rr": (d.xr, d.wr, None, None, True)}[which]
     acf.acf_set_option(ctx, acf.ACF_OPT_WINDOWS, windows)
     acf.acf_set_option(ctx, acf.ACF_OPT_KERNEL, acf.ACF_KERNEL_AUTO if kernel is None else kernel)
+    acf.acf_set_option(ctx, acf.ACF_OPT_BULK, bulk)
     try:
         n_a = a.numel() // 3
         lo, hi = rows if rows is not None else (0, n_a)
@@ -63,6 +64,7 @@ def count(acf, ctx, d, which, rows=None, windows=1, kernel=None):
     finally:
         acf.acf_set_option(ctx, acf.ACF_OPT_WINDOWS, 1)
         acf.acf_set_option(ctx, acf.ACF_OPT_KERNEL, acf.ACF_KERNEL_AUTO)
+        acf.acf_set_option(ctx, acf.ACF_OPT_BULK, 0)
     if wa is None:
         return acf.counts_to_numpy(out), None, st
     return acf.counts_to_numpy(out[0]), out[1].cpu().numpy(), st
@@ -128,6 +130,11 @@ def test_fullsize_sampled_rows_and_properties(acf, ctx, oracle, name, width):
     assert parts.tolist() == full["dd"][0].tolist()
 
     if name == "full_sky":
+        # groups of points counted as a whole where their caps allow it (ACF_OPT_BULK): the same histograms
+        cb, sb, stb = count(acf, ctx, d, "dr", kernel=acf.ACF_KERNEL_WINDOW, bulk=1)
+        assert cb.tolist() == full["dr"][0].tolist()
+        np.testing.assert_allclose(sb, full["dr"][1], rtol=WSUM_RTOL, atol=0)
+        assert stb["pairs_bulk"] > 0.3 * stb["pairs_nominal"] and stb["pairs_bulk"] + stb["pairs_evaluated"] == stb["pairs_nominal"]
         # uniform sphere: cos(theta) is uniform on [-1, 1] => E[count_k] = N_pairs (e_k - e_k+1) / 2
         e = w.cos_edges
         for k, npairs in (("dd", w.n_d * (w.n_d - 1) // 2), ("dr", w.n_d * w.n_r)):
