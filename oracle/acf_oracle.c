@@ -292,6 +292,166 @@ int oracle_pair_count_decwindow(const double *xyz_a, const double *dec_a_deg, si
 }
 
 /*
+ * Dec + RA window variant, for a small theta_max on a wide footprint (BASELINE configs 3 and 5: the Dec
+ * window alone still visits 14-22 % of the pair matrix, 1.8e13 pairs on config 5).  Identical O1-O6 pair
+ * by pair; row i visits only the j whose Dec lies in the band of row i or a neighbouring band (bands of
+ * height W_dec = theta_max + margin) and whose RA lies within W_ra(i) of ra_i (modulo 360).  Both
+ * windows are supersets of the counted set:
+ *   theta >= |d2 - d1|                                             (as in oracle_pair_count_decwindow)
+ *   hav(theta) = hav(d2 - d1) + cos d1 cos d2 hav(a2 - a1),  hav(x) = sin^2(x/2)   (haversine formula,
+ *     equivalent to the C term of PAPER.md:215)   =>   sin^2((a2 - a1)/2) <= hav(theta) / (cos d1 cos d2);
+ *   a visited j has |d2| <= |d1| + 2 W_dec (own or neighbouring band), so cos d2 >= cos(min(90 deg,
+ *   |d1| + 2 W_dec)) =: cmin, and a pair with theta <= theta_max has
+ *     |a2 - a1| <= 2 asin( sqrt( hav(theta_max) / (cos d1 * cmin) ) ) =: W_ra(i)
+ *   (no RA bound at all, W_ra = 180 deg, when that ratio reaches 1: rows near a pole).
+ * Every skipped pair therefore has theta > theta_max, i.e. c < e[nbins], and O3 would have dropped it.
+ * Tests check it equals oracle_pair_count exactly wherever both can run (patches, RA wrap-around,
+ * points at the poles, theta_max up to 180 deg).  Unweighted.  Rows [i0, i1) of A.
+ */
+typedef struct {
+    int band;
+    double ra; /* in [0, 360) */
+    size_t idx;
+} cell_key;
+
+static int cell_key_cmp(const void *pa, const void *pb)
+{
+    const cell_key *a = (const cell_key *)pa, *b = (const cell_key *)pb;
+    if (a->band != b->band) return a->band < b->band ? -1 : 1;
+    if (a->ra < b->ra) return -1;
+    if (a->ra > b->ra) return 1;
+    return (a->idx > b->idx) - (a->idx < b->idx);
+}
+
+static double wrap360(double ra)
+{
+    double r = fmod(ra, 360.0);
+    if (r < 0.0) r += 360.0;
+    if (r >= 360.0) r = 0.0;
+    return r;
+}
+
+/* first key of [l, r) with ra >= v */
+static size_t cell_lower(const cell_key *k, size_t l, size_t r, double v)
+{
+    while (l < r) {
+        size_t m = l + (r - l) / 2;
+        if (k[m].ra < v) l = m + 1; else r = m;
+    }
+    return l;
+}
+
+int oracle_pair_count_cellwindow(const double *xyz_a, const double *ra_a_deg, const double *dec_a_deg, size_t n_a,
+                                 size_t i0, size_t i1, const double *xyz_b, const double *ra_b_deg,
+                                 const double *dec_b_deg, size_t n_b, const double *cos_edges, int nbins,
+                                 int is_auto, uint64_t *counts)
+{
+    if (!counts || !edges_ok(cos_edges, nbins)) return ORACLE_EINVAL;
+    if ((n_a && (!xyz_a || !ra_a_deg || !dec_a_deg)) || (n_b && (!xyz_b || !ra_b_deg || !dec_b_deg))) return ORACLE_EINVAL;
+    if (i0 > i1 || i1 > n_a) return ORACLE_EINVAL;
+    if (is_auto && (xyz_a != xyz_b || n_a != n_b)) return ORACLE_EINVAL;
+
+    const double theta_max = acos(cos_edges[nbins]);            /* radians */
+    const double w_dec = theta_max * RAD2DEG + 1e-6;            /* degrees; the margin dwarfs every rounding here */
+    const double hav_max = sin(0.5 * theta_max) * sin(0.5 * theta_max) * (1.0 + 1e-9);
+    const int n_bands = (int)floor(180.0 / w_dec) + 1;
+    memset(counts, 0, sizeof(uint64_t) * (size_t)nbins);
+
+    cell_key *keys = (cell_key *)malloc(sizeof(cell_key) * (n_b ? n_b : 1));
+    size_t *start = (size_t *)calloc((size_t)n_bands + 1, sizeof(size_t));
+    if (!keys || !start) {
+        free(keys);
+        free(start);
+        return ORACLE_ENOMEM;
+    }
+    for (size_t j = 0; j < n_b; ++j) {
+        int band = (int)floor((dec_b_deg[j] + 90.0) / w_dec);
+        if (band < 0) band = 0;
+        if (band >= n_bands) band = n_bands - 1;
+        keys[j].band = band;
+        keys[j].ra = wrap360(ra_b_deg[j]);
+        keys[j].idx = j;
+        start[band + 1] += 1;
+    }
+    for (int b = 0; b < n_bands; ++b) start[b + 1] += start[b];
+    qsort(keys, n_b, sizeof(cell_key), cell_key_cmp);
+
+    const double *xa = xyz_a, *ya = xyz_a + n_a, *za = xyz_a + 2 * n_a;
+    const double *xb = xyz_b, *yb = xyz_b + n_b, *zb = xyz_b + 2 * n_b;
+    int failed = 0;
+
+#pragma omp parallel
+    {
+        uint64_t *cnt = (uint64_t *)calloc((size_t)nbins, sizeof(uint64_t));
+        if (!cnt) {
+#pragma omp atomic write
+            failed = 1;
+        } else {
+#pragma omp for schedule(dynamic, 64)
+            for (long long ii = (long long)i0; ii < (long long)i1; ++ii) {
+                size_t i = (size_t)ii;
+                double di = dec_a_deg[i], ai = wrap360(ra_a_deg[i]);
+                int band = (int)floor((di + 90.0) / w_dec);
+                if (band < 0) band = 0;
+                if (band >= n_bands) band = n_bands - 1;
+                /* RA half-width of row i, degrees */
+                double far = fabs(di) + 2.0 * w_dec;
+                double cmin = far >= 90.0 ? 0.0 : cos(far * DEG2RAD);
+                double den = cos(di * DEG2RAD) * cmin;
+                double w_ra = 180.0;
+                if (den > 0.0 && hav_max < den) w_ra = 2.0 * asin(sqrt(hav_max / den)) * RAD2DEG + 1e-6;
+                double xi = xa[i], yi = ya[i], zi = za[i];
+                for (int b = band - 1; b <= band + 1; ++b) {
+                    if (b < 0 || b >= n_bands) continue;
+                    size_t l = start[b], r = start[b + 1];
+                    /* up to two RA runs of the band: [lo, hi], wrapped at 0 / 360 */
+                    size_t run_l[2], run_r[2];
+                    int n_runs = 1;
+                    if (w_ra >= 180.0) {
+                        run_l[0] = l;
+                        run_r[0] = r;
+                    } else {
+                        double lo = ai - w_ra, hi = ai + w_ra;
+                        if (lo < 0.0) {
+                            run_l[0] = l;
+                            run_r[0] = cell_lower(keys, l, r, nextafter(hi, 1e300));
+                            run_l[1] = cell_lower(keys, l, r, lo + 360.0);
+                            run_r[1] = r;
+                            n_runs = 2;
+                        } else if (hi >= 360.0) {
+                            run_l[0] = l;
+                            run_r[0] = cell_lower(keys, l, r, nextafter(hi - 360.0, 1e300));
+                            run_l[1] = cell_lower(keys, l, r, lo);
+                            run_r[1] = r;
+                            n_runs = 2;
+                        } else {
+                            run_l[0] = cell_lower(keys, l, r, lo);
+                            run_r[0] = cell_lower(keys, l, r, nextafter(hi, 1e300));
+                        }
+                        /* two runs that meet or overlap (w_ra close to 180): visit nothing twice */
+                        if (n_runs == 2 && run_l[1] < run_r[0]) run_l[1] = run_r[0];
+                    }
+                    for (int t = 0; t < n_runs; ++t)
+                        for (size_t s = run_l[t]; s < run_r[t]; ++s) {
+                            size_t j = keys[s].idx;
+                            if (is_auto && j <= i) continue; /* O6: unordered pairs i<j once */
+                            double c = pair_cos(xi, yi, zi, xb[j], yb[j], zb[j]);
+                            int k = bin_of(c, cos_edges, nbins);
+                            if (k >= 0) cnt[k] += 1;
+                        }
+                }
+            }
+#pragma omp critical
+            for (int k = 0; k < nbins; ++k) counts[k] += cnt[k];
+        }
+        free(cnt);
+    }
+    free(keys);
+    free(start);
+    return failed ? ORACLE_ENOMEM : ORACLE_OK;
+}
+
+/*
  * O8 -- the paper's own separation formula, PAPER.md:207-219 (Appendix A), with
  * atan2 in place of arctan(./C) so that theta lands in [0, 180] deg (reading R6):
  *   da = a2 - a1

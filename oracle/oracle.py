@@ -2,9 +2,11 @@
 
 Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
 legs may import this module.  It builds the C oracle with gcc on first use (or when
-the source is newer than the shared object) and marshals numpy arrays; it holds no
-arithmetic of its own.  See acf_oracle.c for the definition (O1-O8) and citations
-into PAPER.md (arXiv 1208.3658 sect. 2, Eq. 2, Appendix A).
+the source is newer than the shared object) and marshals numpy arrays.  The definition
+(O1-O8) lives in acf_oracle.c, with citations into PAPER.md (arXiv 1208.3658 sect. 2, Eq. 2,
+Appendix A); the only arithmetic written here is the delete-one jackknife at the end of
+the file (`jackknife`, `jackknife_cov`: remove a region, recount with the C functions,
+numpy mean and outer products), pinned on a hand example in tests/test_oracle_pins.py.
 """
 from __future__ import annotations
 
@@ -57,6 +59,9 @@ def _load():
             lib.oracle_pair_count_decwindow.argtypes = [
                 c_double_p, c_double_p, sz, c_double_p, c_double_p, sz, c_double_p, ctypes.c_int,
                 ctypes.c_int, c_u64_p]
+            lib.oracle_pair_count_cellwindow.argtypes = [
+                c_double_p, c_double_p, c_double_p, sz, sz, sz, c_double_p, c_double_p, c_double_p, sz,
+                c_double_p, ctypes.c_int, ctypes.c_int, c_u64_p]
             lib.oracle_pair_count_theta.argtypes = [
                 c_double_p, c_double_p, sz, c_double_p, c_double_p, sz, c_double_p, ctypes.c_int,
                 ctypes.c_int, ctypes.c_double, c_u64_p, c_u64_p, c_u64_p, sz]
@@ -165,6 +170,29 @@ def pair_count_decwindow(xyz_a, dec_a_deg, xyz_b, dec_b_deg, cos_edges, is_auto:
     rc = _load().oracle_pair_count_decwindow(pa, pda, _n_of(a), pb, pdb, _n_of(b), pe, nbins,
                                              int(bool(is_auto)), counts.ctypes.data_as(c_u64_p))
     _check(rc, "pair_count_decwindow")
+    return counts
+
+
+def pair_count_cellwindow(xyz_a, ra_a_deg, dec_a_deg, xyz_b, ra_b_deg, dec_b_deg, cos_edges, is_auto: bool, rows=None):
+    """O2-O6 with the Dec + RA window of acf_oracle.c (a superset of the counted pairs): configs 3 and 5."""
+    a, pa = _f64(xyz_a)
+    ra, pra = _f64(ra_a_deg)
+    da, pda = _f64(dec_a_deg)
+    if is_auto:
+        b, pb, rb, prb, db, pdb = a, pa, ra, pra, da, pda
+    else:
+        b, pb = _f64(xyz_b)
+        rb, prb = _f64(ra_b_deg)
+        db, pdb = _f64(dec_b_deg)
+    if ra.size != _n_of(a) or da.size != _n_of(a) or rb.size != _n_of(b) or db.size != _n_of(b):
+        raise ValueError("ra/dec length mismatch")
+    e, pe = _f64(cos_edges)
+    nbins = e.size - 1
+    counts = np.zeros(max(nbins, 1), dtype=np.uint64)
+    i0, i1 = (0, _n_of(a)) if rows is None else rows
+    rc = _load().oracle_pair_count_cellwindow(pa, pra, pda, _n_of(a), i0, i1, pb, prb, pdb, _n_of(b), pe, nbins,
+                                              int(bool(is_auto)), counts.ctypes.data_as(c_u64_p))
+    _check(rc, "pair_count_cellwindow")
     return counts
 
 

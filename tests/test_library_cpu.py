@@ -94,6 +94,22 @@ def test_wtheta_golden_and_oracle(acf, oracle):
                                rtol=0, atol=1e-10)
 
 
+def test_wtheta_weighted_golden_non_unit_weights(acf):
+    # the same hand-computed fixture that pins the oracle's weighted estimator (sum w^2 != sum w != n)
+    n = 0
+    for r in read_golden("wtheta_weighted_examples.txt"):
+        n_d = int(r[0])
+        w_d = np.array([float(v) for v in r[1:1 + n_d]], dtype=np.float32)
+        n_r = int(r[1 + n_d])
+        w_r = np.array([float(v) for v in r[2 + n_d:2 + n_d + n_r]], dtype=np.float32)
+        wdd, wdr, wrr = (float(v) for v in r[2 + n_d + n_r:5 + n_d + n_r])
+        want = r[5 + n_d + n_r]
+        got = acf.acf_wtheta_weighted([wdd], [wdr], [wrr], w_d, w_r)[0]
+        assert math.isnan(got) if want == "nan" else abs(got - float(want)) < 1e-15, (r, got)
+        n += 1
+    assert n >= 6
+
+
 def test_estimators_and_bin_presets_against_golden_and_oracle(acf, oracle):
     # PAPER.md:65 (other estimators) and PAPER.md:103 (bin presets): pure host entry points
     for r in read_golden("estimator_examples.txt"):

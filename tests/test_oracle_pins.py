@@ -383,6 +383,82 @@ def test_decwindow_equals_plain(oracle):
         oracle.pair_count_decwindow(xd, w.dec_d, None, None, e0, True).tolist()
 
 
+def _weighted_golden():
+    for r in read_golden("wtheta_weighted_examples.txt"):
+        n_d = int(r[0])
+        w_d = np.array([float(v) for v in r[1:1 + n_d]], dtype=np.float32)
+        n_r = int(r[1 + n_d])
+        w_r = np.array([float(v) for v in r[2 + n_d:2 + n_d + n_r]], dtype=np.float32)
+        wdd, wdr, wrr = (float(v) for v in r[2 + n_d + n_r:5 + n_d + n_r])
+        yield w_d, w_r, wdd, wdr, wrr, _num(r[5 + n_d + n_r])
+
+
+def test_O7_weighted_estimator_golden_non_unit_weights(oracle):
+    # hand-computed values with weights for which sum w^2 != sum w != n (tests/golden/wtheta_weighted_examples.txt)
+    n = 0
+    for w_d, w_r, wdd, wdr, wrr, want in _weighted_golden():
+        assert not np.all(w_d == 1) and not np.all(w_r == 1)
+        got = oracle.wtheta_weighted([wdd], [wdr], [wrr], w_d, w_r)[0]
+        assert (math.isnan(got) and math.isnan(want)) or abs(got - want) < 1e-15, (w_d, w_r, got, want)
+        n += 1
+    assert n >= 6
+    # the normalisers are the weighted pair totals: the weighted sums of ALL pairs of a catalogue, counted by
+    # O2-O6 over the whole range, divided by them give fdd = fdr = frr = 1 and w = 0 (ties O7 to O5)
+    a, _, _ = _random_xyz(oracle, 300, 41)
+    b, _, _ = _random_xyz(oracle, 200, 42)
+    wa, wb = lognormal_weights(300, 43), lognormal_weights(200, 44)
+    everything = np.array([1.0, -1.0])
+    _, sdd = oracle.pair_count(a, None, everything, True, w_a=wa)
+    _, sdr = oracle.pair_count(a, b, everything, False, w_a=wa, w_b=wb)
+    _, srr = oracle.pair_count(b, None, everything, True, w_a=wb)
+    assert abs(oracle.wtheta_weighted(sdd, sdr, srr, wa, wb)[0]) < 1e-12
+
+
+def test_cellwindow_equals_plain(oracle):
+    # the Dec + RA window variant visits a superset of the counted pairs: same u64 histograms as the plain loop
+    # on the small-angle configurations ...
+    for name, scale in (("survey_scale", 0.004), ("pruning_stress", 0.002), ("clustered_patch", 0.01)):
+        w = make_config(name, scale)
+        xd, xr = oracle.radec_to_xyz(w.ra_d, w.dec_d), oracle.radec_to_xyz(w.ra_r, w.dec_r)
+        for (a, ra, da, b, rb, db, auto) in [(xd, w.ra_d, w.dec_d, None, None, None, True),
+                                             (xd, w.ra_d, w.dec_d, xr, w.ra_r, w.dec_r, False),
+                                             (xr, w.ra_r, w.dec_r, None, None, None, True)]:
+            plain = oracle.pair_count(a, b, w.cos_edges, auto)
+            assert oracle.pair_count_cellwindow(a, ra, da, b, rb, db, w.cos_edges, auto).tolist() == plain.tolist()
+            assert int(plain.sum()) > 0
+    # ... and where the windows are stressed: the whole sphere with points at and near both poles (no RA bound
+    # there), RA given outside [0, 360), pairs across RA = 0, theta_max from half a degree to 180 degrees
+    # (bands wider than the sphere), row ranges
+    rng = np.random.default_rng(91)
+    ra, dec = full_sky(2500, 92)
+    ra = np.concatenate([ra, rng.uniform(0, 360, 300), rng.uniform(-3, 3, 300), [0.0, 123.0, 359.999999, 10.0]])
+    dec = np.concatenate([dec, np.where(rng.integers(0, 2, 300) == 0, -1, 1) * (90.0 - np.abs(rng.normal(0, 1.5, 300))),
+                          rng.uniform(-4, 4, 300), [90.0, -90.0, 89.9999, -89.9999]])
+    dec = np.clip(dec, -90.0, 90.0)
+    ra[100:200] += 360.0     # the same directions, RA outside [0, 360)
+    ra[200:300] -= 720.0
+    rb, db = full_sky(1500, 93)
+    a, b = oracle.radec_to_xyz(ra, dec), oracle.radec_to_xyz(rb, db)
+    n_pairs_seen = 0
+    for theta_max, nb in ((0.5, 5), (5.0, 9), (60.0, 6), (179.0, 4), (180.0, 3)):
+        edges = cos_edges_from_theta_deg(log_theta_edges_deg(0.01, theta_max, nb))
+        for (bb, rbb, dbb, auto) in ((None, None, None, True), (b, rb, db, False)):
+            plain = oracle.pair_count(a, bb, edges, auto)
+            assert oracle.pair_count_cellwindow(a, ra, dec, bb, rbb, dbb, edges, auto).tolist() == plain.tolist(), (theta_max, auto)
+            n_pairs_seen += int(plain.sum())
+        rows = (700, 1900)
+        assert oracle.pair_count_cellwindow(a, ra, dec, None, None, None, edges, True, rows=rows).tolist() == \
+            oracle.pair_count(a, None, edges, True, rows=rows).tolist()
+    assert n_pairs_seen > 10 ** 6
+    # near the poles a pair a fraction of a degree apart can be 180 degrees apart in RA: counted all the same
+    pr = np.array([0.0, 180.0, 90.0, 270.0])
+    pd = np.array([89.9, 89.9, -89.95, -89.95])
+    px = oracle.radec_to_xyz(pr, pd)
+    e = cos_edges_from_theta_deg(np.array([0.05, 0.15, 0.25]))
+    assert oracle.pair_count_cellwindow(px, pr, pd, None, None, None, e, True).tolist() == [1, 1] == \
+        oracle.pair_count(px, None, e, True).tolist()
+
+
 def test_weighted_dyadic_exact(oracle):
     # weights that are small powers of two: every product and every partial sum is exact in fp64,
     # so the expected value can be computed in integer arithmetic
