@@ -1,17 +1,26 @@
 """GPU parity at BASELINE.json's full sizes, in the launch configuration bench.py times
 (acf_pair_count / acf_pair_count_weighted on whole catalogues):
 
-  * sampled outputs the oracle can compute one by one: the histogram of a few row blocks
-    (acf_pair_count_rows vs oracle rows), u64-equal;
+  * the WHOLE DD / DR / RR histograms of the full calls against tests/golden/fullsize_<config>.txt, written by the
+    CPU oracle alone (tests/golden/make_fullsize_histograms.py, the paper's own bin-by-bin CPU/GPU
+    comparison, with exact parity as the bar), through every fast kernel;
+  * sampled outputs the oracle can compute one by one: the histogram of row blocks
+    (acf_pair_count_rows vs oracle rows), u64-equal -- narrow blocks (ragged tiles: the masked paths) and
+    blocks of more than two whole tiles plus a ragged rest (full tiles and full groups: the unmasked loops
+    that classify nearly all pairs of a full call);
   * properties that hold at any size, on the full calls: the single-edge window path and the
     table path (two different kernels paths) give identical u64 counts; DR(a, b) == DR(b, a);
     row-block additivity; totals; the closed-form expectation on the uniform sphere.
 
 Run on the B200 box:  python -m pytest tests/test_gpu_fullsize.py -m gpu -x -q
 """
+import hashlib
+import os
+
 import numpy as np
 import pytest
 
+from conftest import GOLDEN, read_golden
 from workloads import make_config
 
 pytestmark = pytest.mark.gpu
@@ -70,16 +79,58 @@ def count(acf, ctx, d, which, rows=None, windows=1, kernel=None, bulk=0):
     return acf.counts_to_numpy(out[0]), out[1].cpu().numpy(), st
 
 
+# configurations whose theta_max is a few degrees: the oracle's Dec + RA window loop (pinned to the plain
+# loop in tests/test_oracle_pins.py) makes wide row blocks of 2M and 8M-point catalogues affordable
+CELLWINDOW = {"survey_scale", "pruning_stress"}
+
+
 def oracle_rows(oracle, d, which, rows):
-    a, wa, b, wb, auto = {"dd": (d.h_xd, d.w.w_d, None, None, True), "dr": (d.h_xd, d.w.w_d, d.h_xr, d.w.w_r, False),
-                          "rr": (d.h_xr, d.w.w_r, None, None, True)}[which]
-    return oracle.pair_count(a, b, d.w.cos_edges, auto, w_a=wa, w_b=wb, rows=rows)
+    w = d.w
+    a, ra, da, wa, b, rb, db, wb, auto = {
+        "dd": (d.h_xd, w.ra_d, w.dec_d, w.w_d, None, None, None, None, True),
+        "dr": (d.h_xd, w.ra_d, w.dec_d, w.w_d, d.h_xr, w.ra_r, w.dec_r, w.w_r, False),
+        "rr": (d.h_xr, w.ra_r, w.dec_r, w.w_r, None, None, None, None, True)}[which]
+    if w.name in CELLWINDOW and wa is None:
+        return oracle.pair_count_cellwindow(a, ra, da, b, rb, db, w.cos_edges, auto, rows=rows)
+    return oracle.pair_count(a, b, w.cos_edges, auto, w_a=wa, w_b=wb, rows=rows)
 
 
 def sample_blocks(n, width):
     """Row blocks at the start, around the middle (straddling a tile boundary) and at the ragged end."""
     mid = (n // 2 // 1024) * 1024
     return [(0, width), (max(0, mid - width // 2), min(n, mid + width // 2)), (n - width, n)]
+
+
+def wide_blocks(n, seed):
+    """Row blocks of more than two whole tiles of 1024 plus a ragged rest: as catalogues of their own they are
+    full i-tiles of full groups, which the kernels run through their unmasked loops (the single-edge window
+    loop in registers, the multi-edge chunks, the unmasked table path) at the full density of the j side."""
+    rng = np.random.default_rng(seed)
+    width = 2048 + 529
+    mid = (n // 2 // 1024) * 1024 - 1300
+    off = int(rng.integers(0, n - width))
+    return [(0, width), (mid, mid + width + 5), (off, off + width)]
+
+
+def read_fullsize_golden(name):
+    """tests/golden/fullsize_<name>.txt -> dict, or None if the file is not there."""
+    if not os.path.exists(os.path.join(GOLDEN, "fullsize_%s.txt" % name)):
+        return None
+    g = {}
+    for r in read_golden("fullsize_%s.txt" % name):
+        if r[0] in ("dd", "dr", "rr"):
+            g[r[0]] = np.array([int(v) for v in r[1:]], dtype=np.uint64)
+        elif r[0] in ("wdd", "wdr", "wrr"):
+            g[r[0]] = np.array([float.fromhex(v) for v in r[1:]], dtype=np.float64)
+        elif r[0].startswith("sha256_"):
+            g[r[0]] = r[1]
+        else:
+            g[r[0]] = int(r[1])
+    return g
+
+
+def sha(a):
+    return hashlib.sha256(np.ascontiguousarray(a).tobytes()).hexdigest()
 
 
 @pytest.mark.parametrize("name,width", [("tiny", 256), ("clustered_patch", 192), ("survey_scale", 96),
@@ -100,9 +151,35 @@ def test_fullsize_sampled_rows_and_properties(acf, ctx, oracle, name, width):
                 np.testing.assert_allclose(got_w, want[1], rtol=WSUM_RTOL, atol=0, err_msg="%s %s" % (which, rows))
             else:
                 assert got_c.tolist() == want.tolist(), (which, rows)
+    # ---- wide blocks (full tiles, full groups: the unmasked loops), through both fast kernels
+    for which, n in (("dd", w.n_d), ("dr", w.n_d), ("rr", w.n_r)):
+        for rows in wide_blocks(n, 7 + len(name)):
+            want = oracle_rows(oracle, d, which, rows)
+            for kern in (acf.ACF_KERNEL_WINDOW, acf.ACF_KERNEL_TABLE):
+                got_c, got_w, st = count(acf, ctx, d, which, rows=rows, kernel=kern)
+                if weighted:
+                    assert got_c.tolist() == want[0].tolist(), (which, rows, kern)
+                    np.testing.assert_allclose(got_w, want[1], rtol=WSUM_RTOL, atol=0, err_msg="%s %s" % (which, rows))
+                else:
+                    assert got_c.tolist() == want.tolist(), (which, rows, kern)
+                if name == "full_sky" and kern == acf.ACF_KERNEL_WINDOW:
+                    # the unmasked single-edge loop did classify most of the block's pairs
+                    assert st["pairs_window"] > 0.5 * st["pairs_evaluated"], st
 
     # ---- the full calls, as bench.py makes them
     full = {k: count(acf, ctx, d, k) for k in ("dd", "dr", "rr")}
+    # the whole histograms against the CPU oracle's (tests/golden/fullsize_<name>.txt)
+    g = read_fullsize_golden(name)
+    assert g is not None or name not in ("tiny", "clustered_patch"), "tests/golden/fullsize_%s.txt is missing" % name
+    if g is not None:
+        assert (g["n_d"], g["n_r"], g["nbins"]) == (w.n_d, w.n_r, w.nbins)
+        assert g["sha256_xyz_d"] == sha(d.h_xd) and g["sha256_xyz_r"] == sha(d.h_xr) and g["sha256_cos_edges"] == sha(w.cos_edges)
+        if weighted:
+            assert g["sha256_w_d"] == sha(w.w_d) and g["sha256_w_r"] == sha(w.w_r)
+        for k in ("dd", "dr", "rr"):
+            assert full[k][0].tolist() == g[k].tolist(), k
+            if weighted:
+                np.testing.assert_allclose(full[k][1], g["w" + k], rtol=WSUM_RTOL, atol=0, err_msg=k)
     for k, (c, s, st) in full.items():
         n_a = w.n_d if k != "rr" else w.n_r
         nominal = n_a * (n_a - 1) // 2 if k != "dr" else w.n_d * w.n_r
@@ -110,11 +187,13 @@ def test_fullsize_sampled_rows_and_properties(acf, ctx, oracle, name, width):
         assert int(c.sum()) <= nominal
     # three independent classification codes, bit for bit: the window kernel (edges of a window against
     # register tallies), the table kernel with its single-edge windows, and the table kernel's cell table alone
-    for k in ("dd", "dr"):
+    for k in ("dd", "dr", "rr"):
         for kern, windows in ((acf.ACF_KERNEL_WINDOW, 1), (acf.ACF_KERNEL_TABLE, 1), (acf.ACF_KERNEL_TABLE, 0)):
+            if k == "rr" and windows == 0:
+                continue
             c2, s2, st2 = count(acf, ctx, d, k, windows=windows, kernel=kern)
             assert windows == 1 or st2["pairs_window"] == 0
-            nominal = w.n_d * (w.n_d - 1) // 2 if k == "dd" else w.n_d * w.n_r
+            nominal = {"dd": w.n_d * (w.n_d - 1) // 2, "dr": w.n_d * w.n_r, "rr": w.n_r * (w.n_r - 1) // 2}[k]
             assert 0 < st2["pairs_evaluated"] <= nominal    # (the kernels prune groups of points to different depths)
             assert c2.tolist() == full[k][0].tolist(), (k, kern, windows)
             if weighted:

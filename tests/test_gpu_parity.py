@@ -171,6 +171,62 @@ def test_edge_inclusivity_adversarial(acf, ctx, oracle, kernel):
         assert gpu_counts(acf, ctx, xa, one, edges, False, kernel=kern).tolist() == oracle.pair_count(xa, one, edges, False).tolist(), c
 
 
+def great_circle_grid(n, first, step_rad, jitter=None):
+    """n points on the great circle z = 0 at longitudes (first + k) * step_rad (+ jitter[k]): pairs of such points
+    have separations that are whole multiples of the step (plus the jitter), whatever their position."""
+    phi = (first + np.arange(n)) * step_rad
+    if jitter is not None:
+        phi = phi + jitter
+    return soa(np.stack([np.cos(phi), np.sin(phi), np.zeros(n)], axis=1))
+
+
+@pytest.mark.parametrize("nb_arcsec,what", [(600, "single-edge windows"), (47, "windows of several edges")])
+@pytest.mark.parametrize("kernel", ["auto", "table", "window"])
+def test_near_edge_pairs_on_the_unmasked_paths(acf, ctx, oracle, kernel, nb_arcsec, what):
+    """Adversarial pairs at full tiles and full groups, i.e. through the unmasked loops that classify nearly
+    every pair of a full-size call (the one-point catalogues of test_edge_inclusivity_adversarial reach the
+    masked variants only).  3 tiles of i-points and 2 tiles + a ragged rest of j-points sit on a 1-arcsec grid
+    along a great circle; the bin edges are whole multiples of the grid step, so every j-point makes a pair
+    with several i-points whose separation is an edge up to a chosen offset: 0, a few ulps, and offsets of the
+    cosine around the guard bands of the kernels (3.0e-7 / 7.0e-7 window kernel, 4.5e-7 / 6.7e-7 table kernel).
+    Counts must equal the oracle's, cross and auto."""
+    kern = {"auto": acf.ACF_KERNEL_AUTO, "table": acf.ACF_KERNEL_TABLE, "window": acf.ACF_KERNEL_WINDOW}[kernel]
+    h = math.radians(1.0 / 3600.0)
+    n_i, n_j = 3 * 1024, 2 * 1024 + 300
+    sep0 = 2 * 3600                                  # the j arc starts 2 degrees after the i arc
+    m_edges = np.arange(sep0 - n_i - nb_arcsec, sep0 + n_j + 2 * nb_arcsec, nb_arcsec)   # edges, in grid steps
+    m_edges = m_edges[m_edges > 0]
+    edges = np.cos(m_edges * h)
+    assert np.all(np.diff(edges) < 0)
+    # offsets of the pair cosine from the edge; d(cos) = -sin(theta) d(theta), theta ~ 2 degrees
+    offs = np.array([0.0, 1e-16, -1e-16, 1e-13, -1e-13, 1e-8, -1e-8, 1e-7, -1e-7, 2.5e-7, -2.5e-7, 2.7e-7, -2.7e-7,
+                     2.9e-7, -2.9e-7, 3.0e-7, -3.0e-7, 3.1e-7, -3.1e-7, 4.4e-7, -4.6e-7, 6.6e-7, -6.8e-7, 7.1e-7, -6.9e-7])
+    jit = -offs[np.arange(n_j) % offs.size] / math.sin(sep0 * h)
+    xa = great_circle_grid(n_i, 0, h)
+    xb = great_circle_grid(n_j, sep0, h, jit)
+    want = oracle.pair_count(xa, xb, edges, False)
+    got = gpu_counts(acf, ctx, xa, xb, edges, False, kernel=kern)
+    st = acf.acf_get_stats(ctx)
+    assert got.tolist() == want.tolist(), what
+    assert st["pairs_fp64"] + st["pairs_chord"] > n_j, st        # the near-edge pairs were seen as such
+    if kernel == "window" and nb_arcsec == 600:
+        assert st["pairs_window"] > 0.4 * n_i * n_j, st          # the unmasked single-edge loop ran
+    got = gpu_counts(acf, ctx, xb, xa, edges, False, kernel=kern)
+    assert got.tolist() == want.tolist(), what
+    # weighted, through the packed accumulators of the window kernel (and pair by pair in the table kernel)
+    rng = np.random.default_rng(5)
+    wa, wb = rng.uniform(0.5, 2.0, n_i).astype(np.float32), rng.uniform(0.5, 2.0, n_j).astype(np.float32)
+    got = gpu_counts(acf, ctx, xa, xb, edges, False, wa=wa, wb=wb, kernel=kern)
+    want_w = oracle.pair_count(xa, xb, edges, False, w_a=wa, w_b=wb)
+    assert got[0].tolist() == want_w[0].tolist() == want.tolist()
+    np.testing.assert_allclose(got[1], want_w[1], rtol=WSUM_RTOL, atol=0)
+    # auto-count of both arcs together: diagonal tiles (i < j mask) beside unmasked off-diagonal ones
+    xab = np.concatenate([xa.reshape(3, -1), xb.reshape(3, -1)], axis=1).reshape(-1)
+    near = np.cos(np.arange(1, 40) * 97 * h)                      # edges inside the arcs as well
+    e2 = np.sort(np.concatenate([edges, near]))[::-1].copy()
+    assert gpu_counts(acf, ctx, xab, None, e2, True, kernel=kern).tolist() == oracle.pair_count(xab, None, e2, True).tolist()
+
+
 def test_duplicates_and_clamp(acf, ctx, oracle):
     # coincident points: c may round above 1 and is clamped; counted iff e_0 = 1
     ra, dec = full_sky(500, 7)

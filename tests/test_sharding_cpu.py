@@ -52,6 +52,10 @@ def _worker(rank, world, port, q):
             st = torch.from_numpy(np.asarray(s, dtype=np.float64).copy())
             all_reduce_counts(ct, st)
             res[key] = (ct.numpy().astype(np.uint64), st.numpy())
+            # the slice holds the pairs pairs_before_row says it does: bins over [0, 180] deg catch them all
+            from paper_1208_3658_b200.sharding import pairs_before_row
+            c_all = O.pair_count(a, b, np.array([1.0, 0.0, -1.0]), auto, rows=(lo, hi))
+            assert int(c_all.sum()) == pairs_before_row(hi, n_a, n_b, auto) - pairs_before_row(lo, n_a, n_b, auto)
         if rank == 0:
             q.put(res)
     finally:
