@@ -100,7 +100,8 @@ typedef struct acf_stats {
     uint64_t kernel_launches;    /* CUDA kernels launched by the call */
     double device_ms;            /* device time of the call, CUDA events on the ctx stream */
     double pair_kernel_ms;       /* of which: first to last pair-kernel launch (the dominant kernel) */
-    uint64_t pairs_chord;        /* pairs the fp32 cosine left open and the fp32 chord length decided (not in pairs_fp64) */
+    uint64_t pairs_chord;        /* pairs whose row the fp32 chord length decided: those of windows at small separations,
+                                    which are classified on it, and those the fp32 cosine had left open (not in pairs_fp64) */
     uint64_t pairs_bulk;         /* pairs counted group by group without being evaluated (ACF_OPT_BULK) */
 } acf_stats;
 

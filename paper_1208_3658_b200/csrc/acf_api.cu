@@ -85,6 +85,7 @@ extern "C" void acf_destroy(acf_ctx *ctx)
         ctx->s_keys[i].release();
         ctx->s_caps[i].release();
         ctx->s_gcaps[i].release();
+        ctx->s_scaps[i].release();
         ctx->s_pts2[i].release();
         ctx->s_vj[i].release();
         ctx->s_pack[i].release();

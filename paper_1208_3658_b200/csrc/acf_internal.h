@@ -61,9 +61,12 @@ constexpr int kTile = 1024;      // points per tile (both the register-resident 
 constexpr int kItemTiles = 8;    // at most this many consecutive j-tiles per work item
 constexpr int kGroup = 128;      // points per group: a warp's i-points, and the j-points of one window
 constexpr int kGroupsPerTile = kTile / kGroup;
+constexpr int kSub = 32;         // points per sub-group: the finer caps a window of several edges is split by
+constexpr int kSubsPerGroup = kGroup / kSub;
 
-// Bounding cap of one group of kGroup consecutive sorted points, in double: every point p of the
-// group has centre . p >= cos_r.  sin_r = sqrt(1 - cos_r^2); wsum = sum of the group's weights.
+// Bounding cap of one group of kGroup (or sub-group of kSub) consecutive sorted points, in double: every
+// point p of the group has centre . p / |p| >= cos_r (a bound on the directions; the points' norms may be
+// off 1 by the 1e-6 the validation accepts).  sin_r = sqrt(1 - cos_r^2); wsum = sum of the group's weights.
 // A group without points has cos_r = 2.
 struct GroupCap {
     double cx, cy, cz, cos_r, sin_r, wsum;
@@ -94,6 +97,7 @@ struct Prepared {
     uint32_t *perm = nullptr;     // sorted position -> original index
     double4 *caps = nullptr;      // per tile: unit centre (x, y, z) and cos of the bounding radius
     GroupCap *gcaps = nullptr;    // per group of kGroup points (kGroupsPerTile per tile)
+    GroupCap *scaps = nullptr;    // per sub-group of kSub points (kSubsPerGroup per group)
     int n_tiles = 0;
 };
 
@@ -128,6 +132,7 @@ struct acf_ctx {
     acf::Scratch s_keys[2];          // sort keys (double-buffered inside)
     acf::Scratch s_caps[2];          // tile caps
     acf::Scratch s_gcaps[2];         // group caps
+    acf::Scratch s_scaps[2];         // sub-group caps
     acf::Scratch s_pts2[2];          // paired layout of the sorted points
     acf::Scratch s_vj[2];            // fp64 window-path weights
     acf::Scratch s_pack[2];          // PackInfo + weight-range words

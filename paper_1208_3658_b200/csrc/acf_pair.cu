@@ -193,14 +193,14 @@ struct Window {
 // when rows(c_lo) - rows(c_hi) <= 1.  theta = angle between the centres, rho = sum of the radii:
 // cos(theta -+ rho) = cos(theta) cos(rho) +- sin(theta) sin(rho), clamped at the poles.
 __device__ __forceinline__ Window make_window(const GroupCap &a, const GroupCap &b, const double *__restrict__ edges, int nbins,
-                                              bool prune)
+                                              bool prune, double slack)
 {
     Window w;
     w.edge = -1;
     w.e32 = 0.f;
     w.wsum = b.wsum;
     double c_lo, c_hi;
-    if (!cap_window(a, b, c_lo, c_hi)) return w;
+    if (!cap_window(a, b, slack, c_lo, c_hi)) return w;
     const int r_lo = row_of_cos(c_hi, edges, nbins), r_hi = row_of_cos(c_lo, edges, nbins);
     if (r_hi - r_lo > 1) return w;
     if (prune && r_hi == r_lo && (r_lo == 0 || r_lo == nbins + 1)) {  // all closer than theta_min or all beyond theta_max
@@ -208,7 +208,7 @@ __device__ __forceinline__ Window make_window(const GroupCap &a, const GroupCap 
         return w;
     }
     w.edge = r_lo <= nbins ? r_lo : nbins;  // rows edge (c > e[edge]) and edge + 1
-    w.e32 = (float)edges[w.edge];
+    w.e32 = edge32(edges[w.edge]);
     return w;
 }
 
@@ -536,7 +536,7 @@ __global__ void __launch_bounds__(kThreads + 32, kWeighted ? 1 : 2) pair_kernel(
             mine.wsum = 0.0;
             if (lane < n_groups && (lane + 1) * kGroup <= jn)
                 mine = make_window(p.gcaps_a[(size_t)m.ti * kGroupsPerTile + warp], p.gcaps_b[(size_t)tj * kGroupsPerTile + lane],
-                                   p.edges, p.nbins, p.prune != 0);
+                                   p.edges, p.nbins, p.prune != 0, cap_slack(norm_eps(p.counters)));
             for (int g = 0; g < n_groups; ++g) {
                 Window win;
                 win.edge = __shfl_sync(0xffffffffu, mine.edge, g);

@@ -155,10 +155,27 @@ __device__ __forceinline__ float chord_margin(const unsigned long long *counters
     return (float)(2.02 * eps + 3.0e-15) * 1.0001f;
 }
 
-// All pairs between points of caps a and b have c_lo <= cos(theta) <= c_hi (theta = angle between the
-// centres, rho = sum of the radii: cos(theta -+ rho) = cos(theta) cos(rho) +- sin(theta) sin(rho), clamped
-// at the poles, widened by 1e-9).  Returns false when the caps give no bound.
-__device__ __forceinline__ bool cap_window(const GroupCap &a, const GroupCap &b, double &c_lo, double &c_hi)
+// Largest | |u|^2 - 1 | over the validated points of the call (validate_kernel), as a double.
+__device__ __forceinline__ double norm_eps(const unsigned long long *counters)
+{
+    return __longlong_as_double((long long)counters[kCtrNormDev]);
+}
+// What the cap bounds are widened by.  The caps bound the DIRECTIONS of the points (gather_caps_kernel divides
+// by the norms); the pair cosine of include/acf.h is the dot product of the vectors as given, i.e. the cosine of
+// the angle times |u_i| |u_j|, and | |u_i| |u_j| - 1 | <= eps (1 + eps) for | |u|^2 - 1 | <= eps.  1e-9 covers the
+// rounding of the few fp64 operations of the bound itself (~1e-15).
+__device__ __forceinline__ double cap_slack(double eps) { return 1.001 * eps + 1e-9; }
+
+// fp32 stand-in of an edge in the cosine tests d = e - c.  The pair cosine is clamped to [-1, 1], so nothing lies
+// beyond a pole edge: it is never tested in fp32 (an unclamped c32 marginally outside, or vectors a little longer
+// than 1, would be misfiled); +-4 decides every pair the clamped way and keeps |d| far above any guard band.
+__device__ __forceinline__ float edge32(double e) { return e >= 1.0 ? 4.0f : (e <= -1.0 ? -4.0f : (float)e); }
+
+// All pairs between points of caps a and b have c_lo <= c <= c_hi for the pair cosine c of include/acf.h
+// (theta = angle between the centres, rho = sum of the radii: cos(theta -+ rho) = cos(theta) cos(rho) +-
+// sin(theta) sin(rho), clamped at the poles, widened by `slack` = cap_slack(eps)).  Returns false when the caps
+// give no bound.
+__device__ __forceinline__ bool cap_window(const GroupCap &a, const GroupCap &b, double slack, double &c_lo, double &c_hi)
 {
     c_lo = -1.0;
     c_hi = 1.0;
@@ -170,8 +187,8 @@ __device__ __forceinline__ bool cap_window(const GroupCap &a, const GroupCap &b,
     const double sd = sqrt(fmax(0.0, 1.0 - d * d));
     c_hi = d >= C ? 1.0 : d * C + sd * S;
     c_lo = d <= -C ? -1.0 : d * C - sd * S;
-    c_hi = fmin(1.0, c_hi + 1e-9);  // rounding of the few operations above is ~1e-15
-    c_lo = fmax(-1.0, c_lo - 1e-9);
+    c_hi = fmin(1.0, c_hi + slack);
+    c_lo = fmax(-1.0, c_lo - slack);
     return true;
 }
 

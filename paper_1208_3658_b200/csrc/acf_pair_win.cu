@@ -1,14 +1,20 @@
 // acf_pair_win.cu -- the window kernel: every pair classified against the bin edges that can matter
 // for its window, tallies in registers, no per-pair shared-memory traffic.
 //
-// Points are sorted along a space-filling curve, so the kGroup i-points of a warp and a group of kGroup
-// staged j-points each sit in a small cap; the two caps bound the cosines of all their pairs to a window
-// [c_lo, c_hi] (fp64, rigorous), i.e. to the histogram rows r_lo .. r_hi and the k = r_hi - r_lo edges
-// e[r_lo] .. e[r_hi - 1] between them.  The edges are taken kChunk at a time.  Per pair and chunk:
+// Points are sorted along a space-filling curve, so the kGroup i-points a warp holds and a group of kGroup
+// (or a sub-group of kSub) j-points each sit in a small cap; the two caps bound the cosines of all their
+// pairs to a window [c_lo, c_hi] (fp64, rigorous), i.e. to the histogram rows r_lo .. r_hi and the
+// k = r_hi - r_lo edges e[r_lo] .. e[r_hi - 1] between them.  The edges are taken kChunk at a time.  Per
+// pair and chunk, on the cosine:
 //   d_0 = e_m - (x_i x_j + y_i y_j + z_i z_j)      three fp32 FMAs seeded with fp32(e_m)  (two j-points per FFMA2)
 //   d_q = d_0 + fp32(e_{m+q} - e_m)                 one add per further edge of the chunk
 //   above_q = d_q > 0                               the pair lies in a row beyond edge m + q
 //   certified iff |d_q| > G for every q             else the exact fp64 row of include/acf.h decides
+// or, for windows at small separations (1 - c_lo <= 2^-12, where the fp32 cosine cannot tell the edges
+// apart: SURVEY.md section 7, hard part 2), on the squared chord length s = |u_i - u_j|^2 = 2 (1 - c) up to
+// the norms, which does not cancel:
+//   d_0 = (x_j - x_i)^2 + (y_j - y_i)^2 + (z_j - z_i)^2 - s_m      s_m = fp32(2 (1 - e_m)); three adds, three FMAs
+//   d_q = d_0 + fp32(s_m - s_{m+q}),  above_q and the guard band as before, G = G(s_m) relative (chord_guard)
 // Per i-point and edge one fp64 accumulator takes t += [above_q] v_j (v_j = C + w_j packs the count and
 // the weight sum, see PackInfo: exact sums; weights of too wide a range for that are not tallied here
 // but pair by pair in acf_pair.cu; unweighted counts shift the sign bits of d_q into a word instead).
@@ -17,7 +23,13 @@
 // After a chunk the warp reduces its row tallies with shuffles and lane 0 adds them to the warp's rows in
 // shared memory; those go to global memory with u64 / f64 atomics (block histograms summed
 // into global memory -- here without a per-pair atomic, the 5-50 % serialisation the paper measures).
-// Ragged groups and the diagonal group of an auto-count (i < j) run the same loop with a per-pair mask.
+//
+// Every warp works on its own: it takes jobs {i-group, run of work items} from a global counter, bounds the
+// windows of its i-group against 16 j-groups at a time (one lane per j-group, fp64), drops the groups whose
+// window lies out of range without loading them, splits a window of several edges by the
+// j-side sub-group caps, and streams the surviving j-groups through its own ring of shared-memory stages with
+// TMA bulk copies (one mbarrier per stage).  No barrier is shared between warps: a warp whose groups are all
+// pruned runs ahead, one with many near-field groups takes its time, and neither waits for the other.
 #include <cmath>
 #include <cstring>
 
@@ -29,27 +41,50 @@ namespace acf {
 
 namespace {
 
-constexpr int kTeams = 2;              // teams of consumer warps: same i-points, alternate j-groups
-constexpr int kTeamWarps = kTile / kGroup;  // a team's warps hold the i-tile, kGroup points each
-constexpr int kWarps = kTeams * kTeamWarps;  // consumer warps
-constexpr int kThreads = 32 * kWarps;  // consumer threads
+constexpr int kWarps = 16;             // warps per CTA, each on its own stream of j-groups
+constexpr int kThreads = 32 * kWarps;
 constexpr int kR = kGroup / 32;        // i-points per thread
-#ifndef ACF_WIN_CHUNK
-#define ACF_WIN_CHUNK 3
-#endif
-constexpr int kChunk = ACF_WIN_CHUNK;  // edges per pass over a group
+constexpr int kChunk = 3;              // edges per pass over a group
 constexpr int kStep = 4;               // j-points per guard-band vote
-// Guard bands (u = 2^-24).  A wrong fp32 sign needs |d_0 - (e_m - c64)| >= |d_0|,
-// so only pairs with a small |d_0| matter; for those the partial sums of the chain are below 1 + 2e-6 in
-// magnitude (they differ from d_0 by products of coordinates whose absolute sum is at most 1 + 2e-6):
+constexpr int kWStages = 2;            // staged j-groups per warp
+constexpr int kQueue = 32;             // surviving j-groups a warp has bounded and not yet evaluated
+constexpr int kScan = 16;              // j-groups bounded at a time (two tiles, one lane each)
+constexpr int kMaxPassEdges = 6;       // windows of more edges than this go pair by pair (general_span)
+// The cell table of the pair-by-pair path: the values of the fp32 squared chord length s that share their sign,
+// exponent and top kCellBits mantissa bits form a cell; 2^kCellBits cells per octave from 2^kCellExpLo to 4.
+constexpr int kCellBits = 4;
+constexpr int kCellExpLo = -40;        // s below 2^-40 (0.2 arc seconds): no cell, the edges are searched
+constexpr int kCells = (2 - kCellExpLo) << kCellBits;
+struct Cell {
+    float thr;    // the one edge s_k (as stored, fp32) that can separate two rows inside the cell; +big if none
+    float guard;  // a pair is certified iff |s - thr| > guard (the bound of chord_row); thr = NaN: never (crowded cell)
+    int row;      // number of edges at or below the cell: the row of s < thr; s >= thr is one row on
+    int pad;
+};
+// Guard bands on the cosine (u = 2^-24).  A wrong fp32 sign needs
+// |d_0 - (e_m - c64)| >= |d_0|, so only pairs with a small |d_0| matter; for those the partial sums of the
+// chain are below 1 + 2e-6 in magnitude (they differ from d_0 by products of coordinates whose absolute sum is
+// at most 1 + 2e-6):
 //   2^-25 [fp32(e_m)] + 2u (1 + 1e-6) [the six rounded coordinates] + 2 * 2^-24 [the two inner FMAs]
 //   + 2^-24 |d_0| [the last FMA] + 4e-16 [c64 itself]  <=  2.69e-7.
 // d_q, q >= 1, is the sum of a d_0 that is not small and a rounded offset: partial sums below 4 (three
 // roundings of 2^-23), the offset (2^-24) and the six coordinates give 5.7e-7.
 constexpr float kGuard1 = 3.0e-7f;
 constexpr float kGuardK = 7.0e-7f;
-static_assert(kGroup == kR * 32 && (kTeamWarps & (kTeamWarps - 1)) == 0, "a warp's i-points are one group");
-static_assert(kGroup % 32 == 0 && 32 % kStep == 0 && kStep % 2 == 0, "");
+// A window with an edge inside it is classified on the chord length when it is narrower than this in the cosine
+// (and closer than 45 degrees).  A pair comes within the guard band of the edge with probability about 2 G / width --
+// 6e-7 / width on the cosine, (2.5e-7 sqrt(s) + 6e-7 s) / width on the chord, s = 2 (1 - c) -- and costs some
+// 1e4 thread-instructions of exact re-evaluation when it does, against 1.5 per pair for the chord's three extra adds:
+// below a width of 4e-3 the chord is the cheaper test.  Windows that hold no edge are tested on the cosine: their
+// pairs are near the edge that bounds their row only if the window itself is.
+constexpr double kChordWidth = 4.0e-3;
+constexpr double kChordCosMin = 0.7071;
+static_assert(kGroup == kR * 32 && kSub == 32 && kR == kSubsPerGroup, "register slot r of a warp is sub-group r of its i-group");
+static_assert(kGroup % 32 == 0 && 32 % kStep == 0 && kStep % 2 == 0 && kScan == 2 * kGroupsPerTile, "");
+
+constexpr size_t kGroupBytes = (size_t)kGroup * sizeof(float4);   // a staged j-group: the paired fp32 records
+constexpr size_t kGroupVjBytes = (size_t)kGroup * sizeof(double);  // and (weighted) its fp64 window weights
+__host__ __device__ constexpr size_t wstage_bytes(bool weighted) { return kGroupBytes + (weighted ? kGroupVjBytes : 0); }
 
 struct WinParams {
     const float4 *pts_a;
@@ -57,7 +92,7 @@ struct WinParams {
     const double *vj_b;
     const PackInfo *pack_b;
     const uint32_t *perm_a, *perm_b;
-    const GroupCap *gcaps_a, *gcaps_b;
+    const GroupCap *gcaps_a, *gcaps_b, *scaps_b;
     uint32_t n_a, n_b;
     const double *xyz_a, *xyz_b;
     size_t stride_a, stride_b;
@@ -70,10 +105,71 @@ struct WinParams {
     double *wsums;
     unsigned long long *counters;
     int is_auto;
-    int n_stages;
     int shared_rows;  // 1: one set of histogram rows per CTA instead of one per warp
     int prune;        // 1: groups whose window lies wholly out of range are not evaluated
     int bulk;         // 1: groups whose window lies wholly inside one bin are counted as a whole (ACF_OPT_BULK)
+    int refine;       // 1: windows of two or more edges are split by the j side's sub-group caps
+};
+
+// Shared-memory loads by 32-bit shared address: the loads of the pair loops are LDS whatever the compiler can
+// prove about a pointer, and an address costs one register.
+__device__ __forceinline__ ulonglong2 lds_u64x2(uint32_t a)
+{
+    ulonglong2 v;
+    asm volatile("ld.shared.v2.u64 {%0, %1}, [%2];" : "=l"(v.x), "=l"(v.y) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ unsigned long long lds_u64(uint32_t a)
+{
+    unsigned long long v;
+    asm volatile("ld.shared.u64 %0, [%1];" : "=l"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ double2 lds_f64x2(uint32_t a)
+{
+    double2 v;
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ double lds_f64(uint32_t a)
+{
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ int lds_f32_as_int(uint32_t a)
+{
+    int v;
+    asm volatile("ld.shared.s32 %0, [%1];" : "=r"(v) : "r"(a));
+    return v;
+}
+__device__ __forceinline__ float lds_f32(uint32_t a)
+{
+    float v;
+    asm volatile("ld.shared.f32 %0, [%1];" : "=f"(v) : "r"(a));
+    return v;
+}
+
+// Tables of a launch in shared memory (per CTA): nbins + 1 cosine edges (fp64), then four fp32 arrays of the same
+// length: the edges as squared chord lengths s_m (-1 / +inf at the poles), -s_m (the seed of the chord test), the
+// guard band of the chord test against edge m alone, and against edge m inside a chunk of several.
+struct Tables {
+    uint32_t base;  // shared address of the edges
+    int nbins;
+    const unsigned long long *counters;  // for chord_margin, on the rare paths that need it
+    __device__ __forceinline__ float margin() const { return chord_margin(counters); }
+    __device__ __forceinline__ const double *edges_ptr() const
+    {
+        return reinterpret_cast<const double *>(__cvta_shared_to_generic(base));
+    }
+    __device__ __forceinline__ const float *sed_ptr() const { return reinterpret_cast<const float *>(edges_ptr() + (nbins + 1)); }
+    __device__ __forceinline__ double edge(int m) const { return lds_f64(base + 8u * (uint32_t)m); }
+    __device__ __forceinline__ uint32_t f32_base(int k) const { return base + 8u * (uint32_t)(nbins + 1) + 4u * (uint32_t)(k * (nbins + 1)); }
+    __device__ __forceinline__ float sneg(int m) const { return lds_f32(f32_base(1) + 4u * (uint32_t)m); }
+    __device__ __forceinline__ float gs1(int m) const { return lds_f32(f32_base(2) + 4u * (uint32_t)m); }
+    __device__ __forceinline__ float gsk(int m) const { return lds_f32(f32_base(3) + 4u * (uint32_t)m); }
+    // the cell table of general_span, after the four fp32 arrays (16-byte aligned)
+    __device__ __forceinline__ uint32_t cells() const { return (f32_base(4) + 15u) & ~15u; }
 };
 
 __device__ __forceinline__ unsigned long long fadd2(unsigned long long a, unsigned long long b)
@@ -84,16 +180,10 @@ __device__ __forceinline__ unsigned long long fadd2(unsigned long long a, unsign
 }
 __device__ __forceinline__ float lo32(unsigned long long v) { return __uint_as_float((uint32_t)v); }
 __device__ __forceinline__ float hi32(unsigned long long v) { return __uint_as_float((uint32_t)(v >> 32)); }
-// 1.0f if v > 0 else 0.0f (SASS FSET.BF); read as the high word of a double it is 2^-7 or 0
-__device__ __forceinline__ float ind_gt0(float v)
-{
-    float r;
-    asm("set.gt.f32.f32 %0, %1, 0f00000000;" : "=f"(r) : "f"(v));
-    return r;
-}
 
-// The same comparison written into the high word of a 64-bit register whose low word is and stays zero:
-// the register then reads as the double 2^-7 [v > 0] with no instruction spent on the low word.
+// The comparison v > 0 written as 1.0f / 0.0f (SASS FSET.BF) into the high word of a 64-bit register whose low
+// word is and stays zero: the register then reads as the double 2^-7 [v > 0] with no instruction spent on
+// the low word.
 __device__ __forceinline__ double ind_gt0_f64(unsigned long long &reg, float v)
 {
     asm("{\n\t.reg .b32 lo, hi;\n\tmov.b64 {lo, hi}, %0;\n\tset.gt.f32.f32 hi, %1, 0f00000000;\n\tmov.b64 %0, {lo, hi};\n\t}"
@@ -102,8 +192,20 @@ __device__ __forceinline__ double ind_gt0_f64(unsigned long long &reg, float v)
     return __longlong_as_double((long long)reg);
 }
 
-// This warp's histogram rows in shared memory.  Lane 0 adds the reduced tallies; the rare exact
-// corrections come from any lane and are atomic.
+// Guard band of the chord test against the stored s_m (acf_pair_common.cuh "chord tier"): |s32 - s| <=
+// 2.4e-7 sqrt(s) + 3.1e-7 s + 6e-14 for the chain of chord_row; the chains here are seeded with -s_m (three
+// roundings of partial sums no larger than max(s, s_m)) and, inside a chunk, add a rounded offset to a d_0 that
+// is not small (2^-24 s_m each for the offset and the sum): 6e-7 s and 9e-7 s take that and the rounding of the
+// stored s_m; the edge's own uncertainty (norms, fp64 chain) is `margin` on both sides, as in chord_row.
+__device__ __forceinline__ float chord_guard(float se, float margin, bool in_chunk)
+{
+    if (!(se >= 0.f) || se > 3.0e38f) return 0.f;  // a pole: never within reach
+    const float sm = se + margin;
+    return 1.02f * (2.5e-7f * sqrtf(sm) + (in_chunk ? 9.0e-7f : 6.0e-7f) * sm + 1.0e-13f) + margin;
+}
+
+// This warp's histogram rows in shared memory.  Lane 0 adds the reduced tallies; the exact corrections, the
+// bulk counts and the pair-by-pair path come from any lane and are atomic.
 struct Rows {
     uint32_t *cnt;
     double *ws;
@@ -130,13 +232,21 @@ struct Rows {
 };
 // per-CTA statistics kept in shared memory until the kernel ends
 enum { kStatFp64 = 0, kStatWindow = 1, kStatEvaluated = 2, kStatChord = 3, kStatBulk = 4, kNumStats = 5 };
-// rows and weight of one window, parked in shared memory between its computation and its use
-struct WinRows {
-    int lo, hi;
-    double wsum;
-    float e32;  // fp32 of the edge a window with at most one edge is tested against
-    int pad;
+
+// One surviving j-group in a warp's queue: where it is, and the rows of its window (or of the windows of its
+// kSubsPerGroup sub-groups).
+struct Unit {
+    uint32_t i_first;      // index in catalogue a of the first point of the i-group the window was bounded for
+    uint32_t j_first;      // index in catalogue b of the group's first point
+    int16_t lo[kSubsPerGroup], hi[kSubsPerGroup];  // rows; nsub == 1: of the whole group, in [0]; lo < 0: nothing to evaluate
+    uint8_t nsub;          // 1 or kSubsPerGroup
+    uint8_t masked;        // ragged group on either side, or the diagonal group of an auto-count
+    uint8_t diag;          // count only pairs with (index of j) > (index of i)
+    uint8_t chord;         // bit s: (sub-)window s is classified on the chord length
+    int32_t jn;            // points of the j-group that exist
+    double wsum[kSubsPerGroup];  // weight sums of the (sub-)groups
 };
+static_assert(sizeof(Unit) == 64, "");
 
 __device__ __forceinline__ double warp_sum_f64(double v)
 {
@@ -145,26 +255,36 @@ __device__ __forceinline__ double warp_sum_f64(double v)
     return v;
 }
 
-// Thread (warp, lane) holds the i-points (warp % kTeamWarps) * kGroup + r * 32 + lane of the i-tile, r < kR.
-__device__ __forceinline__ uint32_t local_i(int r)
-{
-    return ((threadIdx.x >> 5) & (kTeamWarps - 1)) * kGroup + r * 32 + (threadIdx.x & 31);
-}
-
-
-// Which pairs of a group count: ragged ends of the catalogues and the diagonal group of an auto-count.
-struct Mask {
-    uint32_t valid;  // bit r: i-point r of this thread exists
-    int jn;          // j-points of the group that exist
-    int j0;          // index in the tile of the group's first j-point
-    bool diag;       // count only pairs with (index in tile of j) > (index in tile of i)
-    __device__ __forceinline__ bool on(int r, int jj) const
+// The j-points [jj0, jj1) of a staged group against this warp's i-group: what one pass works on.
+// Thread `lane` holds the i-points i_first + r * 32 + lane, r < kR.
+struct Span {
+    uint32_t grp2;       // shared address of the staged group, paired layout
+    uint32_t vgrp;       // shared address of its window weights
+    int jj0, jj1;        // multiples of kSub
+    double wsum;         // sum of the weights of the span's j-points
+    uint32_t i_first;    // index in catalogue a of the i-group's first point
+    uint32_t j_first;    // index in catalogue b of the staged group's first point
+    // point jj of the staged group
+    __device__ __forceinline__ float4 point(int jj) const
     {
-        return ((valid >> r) & 1u) && jj < jn && (!diag || (uint32_t)(j0 + jj) > local_i(r));
+        const uint32_t a = grp2 + 32u * (uint32_t)(jj >> 1) + 4u * (uint32_t)(jj & 1);
+        return make_float4(lds_f32(a), lds_f32(a + 8u), lds_f32(a + 16u), lds_f32(a + 24u));
     }
 };
 
-// The exact corrections of one chunk of a group, after its loop and before its tallies are read:
+// Which pairs of a span count: ragged ends of the catalogues and the diagonal group of an auto-count.
+struct Mask {
+    uint32_t gi;  // i-points of the group that exist
+    int jn;       // j-points of the group that exist
+    bool diag;    // count only pairs with (index of j) > (index of i); both catalogues are the same then
+    __device__ __forceinline__ bool on(const Span &sp, int r, int jj) const
+    {
+        const uint32_t il = (uint32_t)r * 32u + (threadIdx.x & 31u);
+        return il < gi && jj < jn && (!diag || sp.j_first + (uint32_t)jj > sp.i_first + il);
+    }
+};
+
+// The exact corrections of one chunk of a span, after its loop and before its tallies are read:
 // amb_steps has a bit per step of kStep j-points in which some pair came within the guard band of an
 // edge.  Every pair of those steps is re-derived bit for bit as the loop computed it; a pair within a
 // guard band gets its row from the chord tier or the fp64 definition of include/acf.h, and where that
@@ -174,41 +294,50 @@ struct Mask {
 //                   tally of the exact classification: no row ever sees a wrong pair added and taken back);
 //   dn[q]           to add to nb[q] (unweighted: pairs not above edge q).
 // One copy for all chunk shapes; it reloads the i-points rather than taking them in registers.
-template <bool kWeighted>
-__device__ __noinline__ void fixup_chunk(const WinParams &p, const float *__restrict__ grp2, const double *__restrict__ vgrp,
-                                         uint32_t amb_steps, int K, int m_a, bool masked, const Mask mk, uint32_t i_base,
-                                         uint32_t j_first, unsigned long long *stat, double *__restrict__ dt, int *__restrict__ dn)
+template <bool kWeighted, bool kChord>
+__device__ __noinline__ void fixup_chunk(const WinParams &p, const Tables tb, const Span sp, uint32_t amb_steps, int K, int m_a,
+                                         float G, unsigned long long *stat, double *__restrict__ dt, int *__restrict__ dn)
 {
+    const int lane = threadIdx.x & 31;
     float4 pi[kR];
 #pragma unroll
-    for (int r = 0; r < kR; ++r) pi[r] = p.pts_a[i_base + local_i(r)];  // the array is padded to a whole tile
+    for (int r = 0; r < kR; ++r) pi[r] = p.pts_a[sp.i_first + r * 32 + lane];  // the array is padded to a whole tile
     for (int i = 0; i < kChunk * kR; ++i) dt[i] = 0.0;
     for (int i = 0; i < kChunk; ++i) dn[i] = 0;
-    const double e0 = p.edges[m_a];
-    const float e32 = (float)e0;
-    const float G = K == 1 ? kGuard1 : kGuardK;
-    const float margin = chord_margin(p.counters);
-    float dl[kChunk];
+    float e32, dl[kChunk];
+    if constexpr (kChord) {
+        e32 = tb.sneg(m_a);
 #pragma unroll
-    for (int q = 0; q < kChunk; ++q) dl[q] = q > 0 && q < K ? (float)(p.edges[m_a + q] - e0) : 0.f;
+        for (int q = 0; q < kChunk; ++q) dl[q] = q > 0 && q < K ? __fsub_rn(tb.sneg(m_a + q), e32) : 0.f;
+    } else {
+        const double e0 = tb.edge(m_a);
+        e32 = edge32(e0);
+#pragma unroll
+        for (int q = 0; q < kChunk; ++q) dl[q] = q > 0 && q < K ? (tb.edge(m_a + q) <= -1.0 ? -8.0f : (float)(tb.edge(m_a + q) - e0)) : 0.f;
+    }
     while (amb_steps) {
-        const int jj0 = (__ffs(amb_steps) - 1) * kStep;
+        const int jj0 = sp.jj0 + (__ffs(amb_steps) - 1) * kStep;
         amb_steps &= amb_steps - 1;
         for (int u = 0; u < kStep; ++u) {
-            const float4 pj = tile_point(grp2, jj0 + u);
+            const float4 pj = sp.point(jj0 + u);
 #pragma unroll
             for (int r = 0; r < kR; ++r) {
-                if (masked && !mk.on(r, jj0 + u)) continue;
-                const float d0 = fmaf(-pi[r].x, pj.x, fmaf(-pi[r].y, pj.y, fmaf(-pi[r].z, pj.z, e32)));
+                float d0;
+                if constexpr (kChord) {
+                    const float dx = __fadd_rn(pj.x, -pi[r].x), dy = __fadd_rn(pj.y, -pi[r].y), dz = __fadd_rn(pj.z, -pi[r].z);
+                    d0 = fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, e32)));
+                } else {
+                    d0 = fmaf(-pi[r].x, pj.x, fmaf(-pi[r].y, pj.y, fmaf(-pi[r].z, pj.z, e32)));
+                }
                 bool amb = false;
 #pragma unroll
                 for (int q = 0; q < kChunk; ++q) amb |= q < K && !(fabsf(q == 0 ? d0 : __fadd_rn(d0, dl[q])) > G);
                 if (!amb) continue;
-                // the chord length decides where the cosine could not; what it leaves open, the definition
-                int exact = chord_row(pi[r].x, pi[r].y, pi[r].z, pj.x, pj.y, pj.z, p.sedges, p.nbins, margin);
+                // on the cosine, the chord length decides where it can; what is left open, the definition does
+                int exact = kChord ? -1 : chord_row(pi[r].x, pi[r].y, pi[r].z, pj.x, pj.y, pj.z, tb.sed_ptr(), tb.nbins, tb.margin());
                 if (exact < 0) {
-                    exact = exact_row(p.xyz_a, p.stride_a, p.perm_a[i_base + local_i(r)], p.xyz_b, p.stride_b,
-                                      p.perm_b[j_first + jj0 + u], p.edges, p.nbins);
+                    exact = exact_row(p.xyz_a, p.stride_a, p.perm_a[sp.i_first + r * 32 + lane], p.xyz_b, p.stride_b,
+                                      p.perm_b[sp.j_first + jj0 + u], p.edges, p.nbins);
                     atomicAdd(&stat[kStatFp64], 1ull);
                 } else {
                     atomicAdd(&stat[kStatChord], 1ull);
@@ -221,7 +350,7 @@ __device__ __noinline__ void fixup_chunk(const WinParams &p, const float *__rest
                     const bool fast_above = kWeighted ? dq > 0.f : (__float_as_uint(dq) >> 31) == 0u;
                     const bool exact_above = exact > m_a + q;
                     if (fast_above != exact_above) {
-                        if constexpr (kWeighted) dt[q * kR + r] += (exact_above ? 0.0078125 : -0.0078125) * vgrp[jj0 + u];
+                        if constexpr (kWeighted) dt[q * kR + r] += (exact_above ? 0.0078125 : -0.0078125) * lds_f64(sp.vgrp + 8u * (uint32_t)(jj0 + u));
                         else dn[q] += exact_above ? -1 : 1;
                     }
                 }
@@ -230,51 +359,35 @@ __device__ __noinline__ void fixup_chunk(const WinParams &p, const float *__rest
     }
 }
 
-// What a thread carries from one chunk of a group's edges to the next (registers of window_group): its
+// What a thread carries from one chunk of a window's edges to the next (registers of window_multi): its
 // pairs above the last edge done and, per i-point, the sum of their w_j.
 struct Carry {
     uint32_t c;
-    double s[kGroup / 32];
+    double s[kR];
 };
 
-// One thread's tallies of the two rows around an edge, kept in registers over consecutive groups that
-// are tested against the same edge (the common single-edge groups of the kernel's own loop).
+// One thread's tallies of the two rows around an edge, kept in registers over consecutive spans that
+// are tested against the same edge (the common single-edge windows of the kernel's own loop).
 struct LaneTally {
     uint32_t c_lo, c_hi;  // pairs in row m / row m + 1
     double w_lo, w_hi;    // and their weight
 };
 
-// Edges m_a .. m_a + K - 1 against one group of kGroup staged j-points and this thread's kR i-points.
-// A chunk fills rows m_a .. m_a + K - 1 (and m_a + K if it is the last of its group); the tallies above
-// its last edge go to the next chunk through `carry`.
-template <int K, bool kWeighted, bool kMasked, bool kDeferFix = false>
-__device__ __forceinline__ uint32_t window_chunk(const WinParams &p, const Rows rows, const float *__restrict__ grp2,
-                                             const double *__restrict__ vgrp, const float (&nx)[kR],
-                                             const float (&ny)[kR], const float (&nz)[kR],
-                                             const float (&wi)[kR], const int m_a, const bool first, const bool last, const double wsum_j,
-                                             const Mask &mk, uint32_t i_base, uint32_t j_first, unsigned long long *stat,
-                                             LaneTally *tally = nullptr, Carry *carry = nullptr, float e32_known = 0.f)
+// The pair loop: n_j staged j-points (a multiple of 32, paired layout at shared address grp2, window weights at
+// vgrp) against this thread's kR i-points and the K edges seeded by e32 and the offsets dl.  Returns the steps of
+// kStep j-points in which some pair came within the guard band G of an edge, one bit each (warp-uniform).
+//   t[q][r]  weighted: 2^-7 * sum of v_j over the pairs above edge q, per i-point
+//   nb[q]    unweighted: pairs not above edge q
+template <int K, bool kWeighted, bool kChord>
+__device__ __forceinline__ uint32_t pair_loop(const uint32_t grp2, const uint32_t vgrp, const int n_j, const float (&nx)[kR],
+                                              const float (&ny)[kR], const float (&nz)[kR], const float e32, const float (&dl)[K],
+                                              const float G, double (&t)[K][kR], uint32_t (&nb)[K])
 {
-    const int lane = threadIdx.x & 31;
-    const double e0 = kDeferFix ? 0.0 : p.edges[m_a];               // (the kernel's own loop has the edge at hand)
-    const float e32 = kDeferFix ? e32_known : (float)e0;
     const unsigned long long e2 = pack2(e32, e32);
-    float dl[K];
     unsigned long long dl2[K];
-    dl[0] = 0.f;
-    dl2[0] = 0ull;
 #pragma unroll
-    for (int q = 1; q < K; ++q) {
-        dl[q] = (float)(p.edges[m_a + q] - e0);
-        dl2[q] = pack2(dl[q], dl[q]);
-    }
-    const float G = K == 1 ? kGuard1 : kGuardK;
-
-    double t[K][kR];     // weighted: 2^-7 * sum of v_j over the pairs above edge q, per i-point
+    for (int q = 0; q < K; ++q) dl2[q] = pack2(dl[q], dl[q]);
     uint32_t sg[K][kR];  // unweighted: sign bits of d_q (1 = not above) of the last 32 j-points
-    uint32_t nb[K];      // unweighted: pairs not above edge q
-    double tall[kR];     // masked: 2^-7 * sum of v_j over the enabled pairs
-    uint32_t call = 0;   // masked: enabled pairs
 #pragma unroll
     for (int q = 0; q < K; ++q) {
         nb[q] = 0u;
@@ -284,8 +397,6 @@ __device__ __forceinline__ uint32_t window_chunk(const WinParams &p, const Rows 
             sg[q][r] = 0u;
         }
     }
-#pragma unroll
-    for (int r = 0; r < kR; ++r) tall[r] = 0.0;
     constexpr int kInd = (K == 1 ? kStep : 2) * kR;  // indicator registers: low words zero for the whole loop
     unsigned long long ind[kInd];
 #pragma unroll
@@ -294,62 +405,42 @@ __device__ __forceinline__ uint32_t window_chunk(const WinParams &p, const Rows 
     uint32_t amb_steps = 0;  // warp-uniform
     static_assert(kGroup / kStep <= 32, "one bit per step");
 #pragma unroll 1
-    for (int jj = 0; jj < kGroup; jj += kStep) {
-        float mn = 1.0f;  // min |d_q| over the enabled pairs of the step
+    for (int jj = 0; jj < n_j; jj += kStep) {
+        float mn = 1.0f;  // min |d_q| over the pairs of the step
 #pragma unroll
         for (int u = 0; u < kStep; u += 2) {
-            const ulonglong2 xy = *reinterpret_cast<const ulonglong2 *>(grp2 + (size_t)(jj + u) * 4);
-            const unsigned long long zz = *reinterpret_cast<const unsigned long long *>(grp2 + (size_t)(jj + u) * 4 + 4);
+            const ulonglong2 xy = lds_u64x2(grp2 + 16u * (uint32_t)(jj + u));
+            const unsigned long long zz = lds_u64(grp2 + 16u * (uint32_t)(jj + u) + 16u);
             double v0 = 0.0, v1 = 0.0;
             if constexpr (kWeighted) {
-                const double2 vv = *reinterpret_cast<const double2 *>(vgrp + jj + u);
+                const double2 vv = lds_f64x2(vgrp + 8u * (uint32_t)(jj + u));
                 v0 = vv.x;
                 v1 = vv.y;
             }
 #pragma unroll
             for (int r = 0; r < kR; ++r) {
-                // {n, n} packed at the use: the FFMA2 takes the one register for both halves
-                const unsigned long long d2 = ffma2(pack2(nx[r], nx[r]), xy.x,
-                                                    ffma2(pack2(ny[r], ny[r]), xy.y, ffma2(pack2(nz[r], nz[r]), zz, e2)));
-                bool on0 = true, on1 = true;
-                if constexpr (kMasked) {
-                    on0 = mk.on(r, jj + u);
-                    on1 = mk.on(r, jj + u + 1);
-                    call += (on0 ? 1u : 0u) + (on1 ? 1u : 0u);
-                    if constexpr (kWeighted) {
-                        tall[r] = fma(v0, __hiloint2double(on0 ? 0x3f800000 : 0, 0), tall[r]);
-                        tall[r] = fma(v1, __hiloint2double(on1 ? 0x3f800000 : 0, 0), tall[r]);
-                    }
+                unsigned long long d2;
+                if constexpr (kChord) {
+                    const unsigned long long dx = fadd2(xy.x, pack2(nx[r], nx[r])), dy = fadd2(xy.y, pack2(ny[r], ny[r])),
+                                             dz = fadd2(zz, pack2(nz[r], nz[r]));
+                    d2 = ffma2(dx, dx, ffma2(dy, dy, ffma2(dz, dz, e2)));
+                } else {
+                    // {n, n} packed at the use: the FFMA2 takes the one register for both halves
+                    d2 = ffma2(pack2(nx[r], nx[r]), xy.x, ffma2(pack2(ny[r], ny[r]), xy.y, ffma2(pack2(nz[r], nz[r]), zz, e2)));
                 }
 #pragma unroll
                 for (int q = 0; q < K; ++q) {
                     const unsigned long long dq2 = q == 0 ? d2 : fadd2(d2, dl2[q]);
                     const float a = lo32(dq2), b = hi32(dq2);
-                    if constexpr (kWeighted && !kMasked) {
+                    if constexpr (kWeighted) {
                         unsigned long long &g0 = ind[(u * kR + 2 * r) % kInd], &g1 = ind[(u * kR + 2 * r + 1) % kInd];
                         t[q][r] = fma(v0, ind_gt0_f64(g0, a), t[q][r]);
                         t[q][r] = fma(v1, ind_gt0_f64(g1, b), t[q][r]);
-                    } else if constexpr (kWeighted) {
-                        float i0 = ind_gt0(a), i1 = ind_gt0(b);
-                        i0 = on0 ? i0 : 0.f;
-                        i1 = on1 ? i1 : 0.f;
-                        t[q][r] = fma(v0, __hiloint2double(__float_as_int(i0), 0), t[q][r]);
-                        t[q][r] = fma(v1, __hiloint2double(__float_as_int(i1), 0), t[q][r]);
                     } else {
-                        uint32_t ba = __float_as_uint(a), bb = __float_as_uint(b);
-                        if constexpr (kMasked) {
-                            ba = on0 ? ba : 0x80000000u;
-                            bb = on1 ? bb : 0x80000000u;
-                        }
-                        asm("shf.l.wrap.b32 %0, %1, %0, 1;" : "+r"(sg[q][r]) : "r"(ba));
-                        asm("shf.l.wrap.b32 %0, %1, %0, 1;" : "+r"(sg[q][r]) : "r"(bb));
+                        asm("shf.l.wrap.b32 %0, %1, %0, 1;" : "+r"(sg[q][r]) : "r"(__float_as_uint(a)));
+                        asm("shf.l.wrap.b32 %0, %1, %0, 1;" : "+r"(sg[q][r]) : "r"(__float_as_uint(b)));
                     }
-                    float aa = fabsf(a), ab = fabsf(b);
-                    if constexpr (kMasked) {
-                        aa = on0 ? aa : 1.0f;
-                        ab = on1 ? ab : 1.0f;
-                    }
-                    asm("min.f32 %0, %0, %1, %2;" : "+f"(mn) : "f"(aa), "f"(ab));
+                    asm("min.f32 %0, %0, %1, %2;" : "+f"(mn) : "f"(fabsf(a)), "f"(fabsf(b)));
                 }
             }
         }
@@ -364,12 +455,48 @@ __device__ __forceinline__ uint32_t window_chunk(const WinParams &p, const Rows 
             }
         }
     }
+    return amb_steps;
+}
+
+// Edges m_a .. m_a + K - 1 against one span of staged j-points and this thread's kR i-points.
+// A chunk fills rows m_a .. m_a + K - 1 (and m_a + K if it is the last of its window); the tallies above
+// its last edge go to the next chunk through `carry`.
+template <int K, bool kWeighted, bool kChord>
+__device__ __forceinline__ void window_chunk(const WinParams &p, const Tables tb, const Rows rows, const Span sp,
+                                             const float (&nx)[kR], const float (&ny)[kR], const float (&nz)[kR],
+                                             const float *wi_of, const int wi_stride, const int m_a, const bool first, const bool last,
+                                             unsigned long long *stat, Carry *carry)
+{
+    // wi_of: the weights of this thread's i-points, wi_of[r * wi_stride]
+    const int lane = threadIdx.x & 31;
+    float e32, G;
+    float dl[K];
+    dl[0] = 0.f;
+    if constexpr (kChord) {
+        e32 = tb.sneg(m_a);
+        G = K == 1 ? tb.gs1(m_a) : tb.gsk(m_a);
+#pragma unroll
+        for (int q = 1; q < K; ++q) {
+            dl[q] = __fsub_rn(tb.sneg(m_a + q), e32);
+            G = fmaxf(G, tb.gsk(m_a + q));
+        }
+    } else {
+        const double e0 = tb.edge(m_a);
+        e32 = edge32(e0);
+        G = K == 1 ? kGuard1 : kGuardK;
+#pragma unroll
+        for (int q = 1; q < K; ++q) dl[q] = tb.edge(m_a + q) <= -1.0 ? -8.0f : (float)(tb.edge(m_a + q) - e0);
+    }
+    double t[K][kR];     // weighted: 2^-7 * sum of v_j over the pairs above edge q, per i-point
+    uint32_t nb[K];      // unweighted: pairs not above edge q
+    const uint32_t amb_steps = pair_loop<K, kWeighted, kChord>(sp.grp2 + 16u * (uint32_t)sp.jj0, sp.vgrp + 8u * (uint32_t)sp.jj0,
+                                                               sp.jj1 - sp.jj0, nx, ny, nz, e32, dl, G, t, nb);
 
     if (amb_steps) {
         // exact corrections, applied to the (exact) accumulators before anything is read from them
         double dt[kChunk * kR];
         int dn[kChunk];
-        fixup_chunk<kWeighted>(p, grp2, vgrp, amb_steps, K, m_a, kMasked, mk, i_base, j_first, stat, dt, dn);
+        fixup_chunk<kWeighted, kChord>(p, tb, sp, amb_steps, K, m_a, G, stat, dt, dn);
 #pragma unroll
         for (int q = 0; q < K; ++q) {
             if constexpr (kWeighted) {
@@ -381,6 +508,7 @@ __device__ __forceinline__ uint32_t window_chunk(const WinParams &p, const Rows 
         }
     }
     // ---- this thread's tallies -> row contributions -> the warp's rows
+    const uint32_t n_all = (uint32_t)(sp.jj1 - sp.jj0) * kR;  // this thread's pairs
     auto unpack = [&](double tt, uint32_t &n) -> double {  // 2^-7 (n C + sum of w) -> sum of w, n += count
         double sw = tt * 128.0;
         if constexpr (kWeighted) {
@@ -390,39 +518,12 @@ __device__ __forceinline__ uint32_t window_chunk(const WinParams &p, const Rows 
         }
         return sw;
     };
-    if constexpr (kDeferFix) {
-        // the kernel's own loop: one edge, nothing masked; the two rows' tallies stay with the thread
-        static_assert(K == 1 && !kMasked, "");
-        uint32_t c_hi = kWeighted ? 0u : (uint32_t)(kGroup * kR) - nb[0];
-        double w_lo = 0.0, w_hi = 0.0;
-        if constexpr (kWeighted) {
-#pragma unroll
-            for (int r = 0; r < kR; ++r) {
-                const double sw = unpack(t[0][r], c_hi);
-                w_lo = fma((double)wi[r], wsum_j - sw, w_lo);
-                w_hi = fma((double)wi[r], sw, w_hi);
-            }
-        }
-        const uint32_t c_lo = (uint32_t)(kGroup * kR) - c_hi;
-        tally->c_lo += c_lo;
-        tally->c_hi += c_hi;
-        if (c_lo != 0u) tally->w_lo += w_lo;  // no pair of this thread in the row: not even a rounding residue
-        if (c_hi != 0u) tally->w_hi += w_hi;
-        return 0u;
-    }
     uint32_t c_prev = 0;  // this thread's pairs above the previous edge (all its pairs before the first)
     double s_prev[kR];    // and, per i-point, the sum of their w_j
     if (first) {
-        if constexpr (kMasked) {
-            uint32_t n_unused = 0;
-            c_prev = call;
+        c_prev = n_all;
 #pragma unroll
-            for (int r = 0; r < kR; ++r) s_prev[r] = kWeighted ? unpack(tall[r], n_unused) : 0.0;
-        } else {
-            c_prev = (uint32_t)(kGroup * kR);
-#pragma unroll
-            for (int r = 0; r < kR; ++r) s_prev[r] = wsum_j;
-        }
+        for (int r = 0; r < kR; ++r) s_prev[r] = sp.wsum;
     } else {
         c_prev = carry->c;
 #pragma unroll
@@ -439,25 +540,23 @@ __device__ __forceinline__ uint32_t window_chunk(const WinParams &p, const Rows 
                 c_q = 0u;
 #pragma unroll
                 for (int r = 0; r < kR; ++r) {
-                    const double sw = unpack(t[q][r], c_q);
-                    rw = fma((double)wi[r], s_prev[r] - sw, rw);
+                    const double sw = unpack(t[q < K ? q : 0][r], c_q);
+                    rw = fma((double)wi_of[r * wi_stride], s_prev[r] - sw, rw);
                     s_prev[r] = sw;
                 }
             } else {
-                c_q = (uint32_t)(kGroup * kR) - nb[q];
+                c_q = n_all - nb[q < K ? q : 0];
             }
         } else if constexpr (kWeighted) {
 #pragma unroll
-            for (int r = 0; r < kR; ++r) rw = fma((double)wi[r], s_prev[r], rw);
+            for (int r = 0; r < kR; ++r) rw = fma((double)wi_of[r * wi_stride], s_prev[r], rw);
         }
         const uint32_t rc = c_prev - c_q;
         c_prev = c_q;
         if (rc == 0u) rw = 0.0;  // no pair of this thread in the row: not even a rounding residue
         const uint32_t rc_warp = __reduce_add_sync(0xffffffffu, rc);
         if constexpr (kWeighted) rw = warp_sum_f64(rw);
-        if (lane == 0) {
-            rows.template add<kWeighted>(m_a + q, rc_warp, rw);
-        }
+        if (lane == 0) rows.template add<kWeighted>(m_a + q, rc_warp, rw);
     }
     if (!last) {
         carry->c = c_prev;
@@ -465,202 +564,602 @@ __device__ __forceinline__ uint32_t window_chunk(const WinParams &p, const Rows 
         for (int r = 0; r < kR; ++r) carry->s[r] = s_prev[r];
     }
     __syncwarp();
-    return 0u;
 }
 
-// One group: all edges r_lo .. r_hi - 1 of its window, kChunk at a time.
-#define ACF_WIN_CHUNK_CALL(K, MASKED) \
-    window_chunk<K, kWeighted, MASKED>(p, rows, grp2, vgrp, nx, ny, nz, wi, m, m == r_lo, left <= K, wsum_j, mk, i_base, j_first, stat, \
-                                                nullptr, &carry)
-// Not inlined: only the common case (one edge, nothing masked) lives in the kernel's own loop, so that
-// the register allocation of that loop is not set by the rare variants.  It reloads the i-points.
-template <bool kWeighted>
-__device__ __noinline__ void window_group(const WinParams &p, const Rows rows, const float *__restrict__ grp2,
-                                          const double *__restrict__ vgrp, int r_lo, int r_hi,
-                                          double wsum_j, bool masked, const Mask mk, uint32_t i_base, uint32_t j_first,
+// A window of two or more edges (rows r_lo .. r_hi): its edges kChunk at a time, every pass over the whole span.
+// Not inlined: only the common case (one edge) lives in the kernel's own loop, so that the register
+// allocation of that loop is not set by the rare variants.  It reloads the i-points.
+template <bool kWeighted, bool kChord>
+__device__ __noinline__ void window_multi(const WinParams &p, const Tables tb, const Rows rows, const Span sp, int r_lo, int r_hi,
                                           unsigned long long *stat)
 {
-    float nx[kR], ny[kR], nz[kR], wi[kR];
+    const int lane = threadIdx.x & 31;
+    float nx[kR], ny[kR], nz[kR];
 #pragma unroll
     for (int r = 0; r < kR; ++r) {
-        const float4 v = p.pts_a[i_base + local_i(r)];  // the array is padded to a whole tile
+        const float4 v = p.pts_a[sp.i_first + r * 32 + lane];  // the array is padded to a whole tile
         nx[r] = -v.x;
         ny[r] = -v.y;
         nz[r] = -v.z;
-        wi[r] = v.w;
     }
+    const float *wi = &p.pts_a[sp.i_first + lane].w;  // the weight of i-point r: wi[r * 128] (float4 records, 32 apart)
     static_assert(kChunk == 3, "the dispatch below spells the chunk sizes out");
-    if (r_hi == r_lo) {  // one row: still every pair is evaluated, against the edge that bounds the row
-        if (r_lo > p.nbins) r_lo = p.nbins;
-        r_hi = r_lo + 1;
-    }
     Carry carry;
     carry.c = 0u;
 #pragma unroll
     for (int r = 0; r < kR; ++r) carry.s[r] = 0.0;
     int m = r_lo;  // edges below m are done
     while (m < r_hi) {
+        // passes of three edges, the last one or two passes of two (4 = 2 + 2, 5 = 3 + 2, 7 = 3 + 2 + 2): no pass of one
         const int left = r_hi - m;
-        if (masked) {
-            if (left == 1) ACF_WIN_CHUNK_CALL(1, true);
-            else if (left == 2) ACF_WIN_CHUNK_CALL(2, true);
-            else ACF_WIN_CHUNK_CALL(3, true);
-        } else {
-            if (left == 1) ACF_WIN_CHUNK_CALL(1, false);
-            else if (left == 2) ACF_WIN_CHUNK_CALL(2, false);
-            else ACF_WIN_CHUNK_CALL(3, false);
-        }
-        m += left < kChunk ? left : kChunk;
+        const int take = (left == 2 || left == 4) ? 2 : 3;
+        if (take == 2) window_chunk<2, kWeighted, kChord>(p, tb, rows, sp, nx, ny, nz, wi, 128, m, m == r_lo, left == 2, stat, &carry);
+        else window_chunk<3, kWeighted, kChord>(p, tb, rows, sp, nx, ny, nz, wi, 128, m, m == r_lo, left == 3, stat, &carry);
+        m += take;
     }
 }
-#undef ACF_WIN_CHUNK_CALL
+
+// Pair by pair: ragged groups, the diagonal group of an auto-count and windows of many edges.  The fp32 squared
+// chord length s of a pair picks a cell of the table (its float bits, shifted); the cell names the one edge that
+// can matter inside it and the guard band around that edge (the error bound of chord_row).  A certified pair goes
+// to its row at once; one within the guard band, or in a cell that holds several edges, gets its row from the
+// search of chord_row and, where that leaves it open, from the fp64 definition.
+template <bool kWeighted>
+__device__ __noinline__ void general_span(const WinParams &p, const Tables tb, const Rows rows, const Span sp, const Mask mk,
+                                          unsigned long long *stat)
+{
+    const int lane = threadIdx.x & 31;
+    float4 pi[kR];
+#pragma unroll
+    for (int r = 0; r < kR; ++r) pi[r] = p.pts_a[sp.i_first + r * 32 + lane];
+    const uint32_t cells = tb.cells();
+    constexpr int kShift = 23 - kCellBits;
+    constexpr int kKey0 = (127 + kCellExpLo) << kCellBits;
+    uint32_t n_exact = 0;
+    const int jj_end = sp.jj1 < mk.jn ? sp.jj1 : mk.jn;
+    for (int jj = sp.jj0; jj < jj_end; ++jj) {
+        const float4 pj = sp.point(jj);
+#pragma unroll
+        for (int r = 0; r < kR; ++r) {
+            if (!mk.on(sp, r, jj)) continue;
+            const float dx = __fsub_rn(pi[r].x, pj.x), dy = __fsub_rn(pi[r].y, pj.y), dz = __fsub_rn(pi[r].z, pj.z);
+            const float s32 = fmaf(dx, dx, fmaf(dy, dy, __fmul_rn(dz, dz)));  // as chord_row computes it
+            const int key = (int)(__float_as_uint(s32) >> kShift) - kKey0;
+            int row = -1;
+            if (key >= 0 && key < kCells) {
+                const uint32_t a = cells + 16u * (uint32_t)key;
+                const float thr = lds_f32(a), guard = lds_f32(a + 4u);
+                if (fabsf(s32 - thr) > guard) row = (int)lds_f32_as_int(a + 8u) + (s32 >= thr ? 1 : 0);
+            }
+            if (row < 0) {
+                row = chord_row(pi[r].x, pi[r].y, pi[r].z, pj.x, pj.y, pj.z, tb.sed_ptr(), tb.nbins, tb.margin());
+                if (row < 0) {
+                    row = exact_row(p.xyz_a, p.stride_a, p.perm_a[sp.i_first + r * 32 + lane], p.xyz_b, p.stride_b,
+                                    p.perm_b[sp.j_first + jj], p.edges, p.nbins);
+                    ++n_exact;
+                }
+            }
+            rows.template add_atomic<kWeighted>(row, 1u, (double)pi[r].w * (double)pj.w);
+        }
+    }
+    n_exact = __reduce_add_sync(0xffffffffu, n_exact);
+    if (lane == 0 && n_exact) atomicAdd(&stat[kStatFp64], (unsigned long long)n_exact);
+}
+
+// Fills the cell table of general_span from the edges as squared chord lengths (sed, ascending; -1 / +inf at the
+// poles).  A cell [lo, hi) is taken with the guard bands at its two ends: every edge a value of the cell could fail to
+// clear counts as inside it.  No edge inside: all of the cell is one row.  One: the edge and its guard band.  More:
+// the cell is marked crowded (NaN threshold) and its pairs are searched.
+__device__ __forceinline__ void fill_cells(uint32_t cells, const float *sed, int nbins, float margin, int tid, int n_threads)
+{
+    constexpr int kShift = 23 - kCellBits;
+    constexpr int kKey0 = (127 + kCellExpLo) << kCellBits;
+    auto guard_at = [&](float se) {  // chord_row's `cleared`, for an edge stored as se
+        const float sm = se + margin;
+        return 1.02f * (2.5e-7f * sqrtf(sm) + 4.0e-7f * sm + 1.0e-13f) + margin;
+    };
+    for (int key = tid; key < kCells; key += n_threads) {
+        const float lo = __uint_as_float((uint32_t)(key + kKey0) << kShift), hi = __uint_as_float((uint32_t)(key + kKey0 + 1) << kShift);
+        // a value s of the cell fails to clear edge k only if |s - se_k| <= guard_at(se_k)
+        int below = 0, inside = 0, first = -1;
+        for (int k = 0; k <= nbins; ++k) {
+            const float se = sed[k];
+            if (se < 0.f) {  // the pole edge e_0 = 1: every pair is at or beyond it
+                ++below;
+                continue;
+            }
+            if (se > 3.0e38f) continue;  // the pole edge e_n = -1: no pair is beyond it
+            const float g = 1.05f * guard_at(se);
+            if (se + g < lo) ++below;
+            else if (se - g <= hi) {
+                if (!inside) first = k;
+                ++inside;
+            }
+        }
+        Cell c;
+        c.row = below;
+        c.pad = 0;
+        if (inside == 0) {
+            c.thr = 3.0e38f;  // |s - thr| > guard always, s >= thr never
+            c.guard = 0.f;
+        } else if (inside == 1) {
+            c.thr = sed[first];
+            c.guard = guard_at(sed[first]);
+        } else {
+            c.thr = __uint_as_float(0x7fc00000u);  // NaN: no pair of the cell is certified, the edges are searched
+            c.guard = 0.f;
+        }
+        *reinterpret_cast<Cell *>(__cvta_shared_to_generic(cells + 16u * (uint32_t)key)) = c;
+    }
+}
 
 // ---- the kernel ---------------------------------------------------------------------------------
-// kWarps consumer warps and no producer warp (16 warps leave each thread 128 registers; a 17th would cost
-// 32 of them).  The j-tiles of the work items {i-tile, first j-tile, number of j-tiles} stream through a
-// ring of shared-memory stages filled by TMA bulk copies (full / empty mbarriers per stage).  Whichever
-// warp finds the ring's lock free refills the drained stages -- after it hands a stage back, and while it
-// waits for one -- pulling work items from a global counter.  Every warp walks the stream at its own
-// pace, holding its kGroup i-points of the current i-tile in registers.
-struct ProdState {
-    uint32_t lock;      // 0 free, 1 held
-    uint32_t produced;  // stages filled so far: slot = produced % n_stages, round = produced / n_stages
-    int ti, tj, left;   // the work item being streamed: its i-tile, next j-tile, j-tiles left
-    int done;           // the end-of-stream stage has been posted
-    unsigned long long n_items;
+// The warp-uniform state of a warp's stream.  It lives in shared memory (read a few times per j-group) so
+// that it does not occupy registers of the pair loops.
+struct WarpCtl {
+    uint32_t q_tail, n_issued, n_done;  // units [n_done, q_tail) are queued, [n_done, n_issued) have their loads in flight;
+                                        // unit number s lives in queue slot s % kQueue and stage s % kWStages
+    uint32_t it, it_end;                // work items of the job still to be scanned
+    int t, cx, cy, cz;                  // j-tiles of item `it` already scanned; that item {i-tile, first j-tile, j-tiles}
+    int ig;                             // the job's i-group within its i-tiles
+    int no_more;                        // the global job counter has run out
+    int sub;                            // the sub-group of the unit at the head of the queue that is being evaluated
+    uint32_t since_flush;               // j-groups tallied in the warp's unflushed rows
+    int tally_m;                        // the edge the threads' LaneTally belongs to, or -1
+    uint32_t loaded_first;              // i_first of the i-points in WarpSm::ipts
+    unsigned long long n_eval, n_win;   // pairs evaluated / of them by the single-edge loop
+    unsigned long long n_chord;         // pairs classified on the fp32 chord length (chord-domain windows, pair-by-pair path)
+};
+static_assert(sizeof(WarpCtl) <= 96 && sizeof(WarpCtl) % 8 == 0, "per-warp header: 32 bytes of mbarriers, then WarpCtl");
+constexpr int kWarpHeader = 128;
+
+// Per-CTA header of the shared memory.
+struct CtaHeader {
+    unsigned long long stat[8];
+    PackInfo pack;
+    uint32_t n_items, chunk, n_jobs, pad[3];
+};
+static_assert(kNumStats <= 8 && sizeof(CtaHeader) % 16 == 0, "");
+
+// A warp's shared memory, addressed from one 32-bit shared address:
+// [mbarriers, WarpCtl | queue | lane tallies | the i-points {-x, -y, -z, w} | stages | rows].
+template <bool kWeighted>
+struct WarpSm {
+    uint32_t base;
+    int rows_n;
+    static constexpr size_t kStage = wstage_bytes(kWeighted);
+    __device__ __forceinline__ unsigned char *ptr(uint32_t off) const
+    {
+        return reinterpret_cast<unsigned char *>(__cvta_shared_to_generic(base + off));
+    }
+    __device__ __forceinline__ uint32_t full(int st) const { return base + 8u * (uint32_t)st; }
+    __device__ __forceinline__ volatile WarpCtl *ctl() const { return reinterpret_cast<volatile WarpCtl *>(ptr(32)); }
+    __device__ __forceinline__ Unit *queue() const { return reinterpret_cast<Unit *>(ptr(kWarpHeader)); }
+    static constexpr uint32_t kFixed = kWarpHeader + (uint32_t)(sizeof(Unit) * kQueue) + 32u * (uint32_t)sizeof(LaneTally) + (uint32_t)(kGroup * sizeof(float4));
+    __device__ __forceinline__ LaneTally *tally() const { return reinterpret_cast<LaneTally *>(ptr(kWarpHeader + (uint32_t)(sizeof(Unit) * kQueue))); }
+    __device__ __forceinline__ float4 *ipts() const
+    {
+        return reinterpret_cast<float4 *>(ptr(kWarpHeader + (uint32_t)(sizeof(Unit) * kQueue) + 32u * (uint32_t)sizeof(LaneTally)));
+    }
+    __device__ __forceinline__ uint32_t stage(int st) const { return base + kFixed + (uint32_t)kStage * (uint32_t)st; }
+    __device__ __forceinline__ uint32_t *cnt_own() const { return reinterpret_cast<uint32_t *>(ptr(kFixed + (uint32_t)(kStage * kWStages))); }
+    __device__ __forceinline__ double *ws_own() const
+    {
+        return reinterpret_cast<double *>(reinterpret_cast<unsigned char *>(cnt_own()) + (((size_t)rows_n * sizeof(uint32_t) + 15) & ~size_t(15)));
+    }
 };
 
-template <bool kWeighted>
-__device__ __forceinline__ void try_produce(const WinParams &p, volatile ProdState *ps, uint64_t *full, uint64_t *empty,
-                                            StageMeta *meta, unsigned char *stages, int n_stages)
+__device__ __forceinline__ void mbar_wait_s(uint32_t bar, uint32_t parity)
 {
-    constexpr size_t kStage = stage_bytes(kWeighted);
-    if (ps->done || atomicCAS(const_cast<uint32_t *>(&ps->lock), 0u, 1u) != 0u) return;
-    while (!ps->done) {
-        const uint32_t produced = ps->produced;
-        const int slot = (int)(produced % (uint32_t)n_stages);
-        const uint32_t round = produced / (uint32_t)n_stages;
-        if (!mbar_test(&empty[slot], (round & 1u) ^ 1u)) break;  // not drained yet (round 0 passes at once)
-        if (ps->left == 0) {
-            const unsigned long long item = atomicAdd(&p.counters[kCtrWorkHead], 1ull);
-            if (item >= ps->n_items) {  // end of stream
-                StageMeta m;
-                m.ti = -1;
-                m.tj = m.jn = m.pad = 0;
-                meta[slot] = m;
-                ps->done = 1;
-                ps->produced = produced + 1;
-                mbar_arrive(&full[slot]);
-                break;
-            }
-            const int3 it = p.items[item];
-            ps->ti = it.x;
-            ps->tj = it.y;
-            ps->left = it.z;
-        }
-        const int tj = ps->tj;
-        const uint32_t j0 = (uint32_t)tj * kTile;
-        const uint32_t jn = p.n_b - j0 < (uint32_t)kTile ? p.n_b - j0 : (uint32_t)kTile;
-        StageMeta m;
-        m.ti = ps->ti;
-        m.tj = tj;
-        m.jn = (int)jn;
-        m.pad = 0;
-        meta[slot] = m;
-        ps->tj = tj + 1;
-        ps->left = ps->left - 1;
-        ps->produced = produced + 1;
-        // the arrays are padded to whole tiles: always a full tile
-        mbar_expect_tx(&full[slot], (uint32_t)kStage);
-        bulk_load(stages + (size_t)slot * kStage, p.pts2_b + (size_t)j0 * 4, (uint32_t)kTileBytes, &full[slot]);
-        if constexpr (kWeighted)
-            bulk_load(stages + (size_t)slot * kStage + kTileBytes, p.vj_b + (size_t)j0, (uint32_t)kVjBytes, &full[slot]);
+    asm volatile(
+        "{\n"
+        ".reg .pred p;\n"
+        "WAIT_LOOP_S:\n"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+        "@p bra WAIT_DONE_S;\n"
+        "bra WAIT_LOOP_S;\n"
+        "WAIT_DONE_S:\n"
+        "}\n" ::"r"(bar), "r"(parity) : "memory");
+}
+
+extern __shared__ __align__(128) unsigned char smem[];
+
+// The tables of the launch: right after the CtaHeader (pair_win_kernel); nothing of this needs a register.
+__device__ __forceinline__ Tables tables_of(const WinParams &p)
+{
+    Tables tb;
+    tb.base = smem_u32(smem) + (uint32_t)sizeof(CtaHeader);
+    tb.nbins = p.nbins;
+    tb.counters = p.counters;
+    return tb;
+}
+
+// The rows a warp tallies into: its own, or the CTA's (many bins).
+template <bool kWeighted>
+__device__ __forceinline__ Rows rows_of(const WinParams &p, const WarpSm<kWeighted> w)
+{
+    CtaHeader *h = reinterpret_cast<CtaHeader *>(smem);
+    Rows rows;
+    rows.shared = p.shared_rows != 0;
+    rows.pack = &h->pack;
+    if (rows.shared) {
+        // after the header, the edges and the chord tables (pair_win_kernel)
+        size_t off = sizeof(CtaHeader) + sizeof(double) * (size_t)(p.nbins + 1) + sizeof(float) * 4 * (size_t)(p.nbins + 1);
+        off = (off + 15) & ~size_t(15);
+        off += sizeof(Cell) * kCells;
+        rows.cnt = reinterpret_cast<uint32_t *>(smem + off);
+        off += sizeof(uint32_t) * (size_t)w.rows_n;
+        off = (off + 15) & ~size_t(15);
+        rows.ws = reinterpret_cast<double *>(smem + off);
+    } else {
+        rows.cnt = w.cnt_own();
+        rows.ws = w.ws_own();
     }
-    __threadfence_block();
-    atomicExch(const_cast<uint32_t *>(&ps->lock), 0u);
+    return rows;
+}
+
+// The kernel's own loop: the (sub-)window at the head of the warp's queue has at most one edge, WarpCtl::tally_m.
+// Everything but the i-points is read from the warp's shared memory -- before the pair loop what the loop needs,
+// after it what the tallies need (weight sum of the span, weights of the i-points, the lane's tallies of the two
+// rows around the edge) -- so that the loop has the registers to itself and the i-points are live across no call.
+template <bool kWeighted, bool kChord>
+__device__ __forceinline__ void single_edge_span(const WinParams &p, const WarpSm<kWeighted> w)
+{
+    const int lane = threadIdx.x & 31;
+    const Tables tb = tables_of(p);
+    uint32_t grp2, vgrp;
+    int n_j;
+    float e32, G;
+    float nx[kR], ny[kR], nz[kR];  // the i-points, negated: loaded here so that they are live across no call
+    {
+        volatile WarpCtl *c = w.ctl();
+        const uint32_t n_done = c->n_done;
+        const Unit *u = &w.queue()[n_done % kQueue];
+        const uint32_t i_first = u->i_first;
+        float4 *ip = w.ipts();
+        if (c->loaded_first != i_first) {
+            // another i-group: its points, negated, into the warp's shared memory (the array is padded to a whole tile)
+            __syncwarp();
+#pragma unroll
+            for (int r = 0; r < kR; ++r) {
+                const float4 v = p.pts_a[i_first + r * 32 + lane];
+                ip[r * 32 + lane] = make_float4(-v.x, -v.y, -v.z, v.w);
+            }
+            if (lane == 0) c->loaded_first = i_first;
+            __syncwarp();
+        }
+#pragma unroll
+        for (int r = 0; r < kR; ++r) {
+            const float4 v = ip[r * 32 + lane];
+            nx[r] = v.x;
+            ny[r] = v.y;
+            nz[r] = v.z;
+        }
+        const int jj0 = u->nsub == 1 ? 0 : c->sub * kSub;
+        n_j = u->nsub == 1 ? kGroup : kSub;
+        grp2 = w.stage((int)(n_done % kWStages)) + 16u * (uint32_t)jj0;
+        vgrp = w.stage((int)(n_done % kWStages)) + (uint32_t)kGroupBytes + 8u * (uint32_t)jj0;
+        const int m_edge = c->tally_m;
+        if constexpr (kChord) {
+            e32 = tb.sneg(m_edge);
+            G = tb.gs1(m_edge);
+        } else {
+            e32 = edge32(tb.edge(m_edge));
+            G = kGuard1;
+        }
+    }
+    const float dl[1] = {0.f};
+    double t[1][kR];
+    uint32_t nb[1];
+    const uint32_t amb_steps = pair_loop<1, kWeighted, kChord>(grp2, vgrp, n_j, nx, ny, nz, e32, dl, G, t, nb);
+
+    volatile WarpCtl *c = w.ctl();
+    const uint32_t n_done = c->n_done;
+    const Unit *u = &w.queue()[n_done % kQueue];
+    const int sub = u->nsub == 1 ? 0 : c->sub;
+    CtaHeader *h = reinterpret_cast<CtaHeader *>(smem);
+    if (amb_steps) {
+        // exact corrections, applied to the (exact) accumulators before anything is read from them
+        Span sp;
+        sp.grp2 = w.stage((int)(n_done % kWStages));
+        sp.vgrp = sp.grp2 + (uint32_t)kGroupBytes;
+        sp.jj0 = u->nsub == 1 ? 0 : sub * kSub;
+        sp.jj1 = sp.jj0 + n_j;
+        sp.wsum = 0.0;
+        sp.i_first = u->i_first;
+        sp.j_first = u->j_first;
+        double dt[kChunk * kR];
+        int dn[kChunk];
+        fixup_chunk<kWeighted, kChord>(p, tb, sp, amb_steps, 1, c->tally_m, G, h->stat, dt, dn);
+        if constexpr (kWeighted) {
+#pragma unroll
+            for (int r = 0; r < kR; ++r) t[0][r] += dt[r];
+        } else {
+            nb[0] += (uint32_t)dn[0];
+        }
+    }
+    // ---- this thread's tallies of the two rows around the edge
+    const uint32_t n_all = (uint32_t)n_j * kR;  // this thread's pairs
+    uint32_t c_hi = kWeighted ? 0u : n_all - nb[0];
+    double w_lo = 0.0, w_hi = 0.0;
+    if constexpr (kWeighted) {
+        const double wsum = u->wsum[sub], C = h->pack.C, inv_C = h->pack.inv_C;
+        const float *wi = &w.ipts()[lane].w;
+#pragma unroll
+        for (int r = 0; r < kR; ++r) {
+            // 2^-7 (n C + sum of w) -> n and the sum of w: C is a power of two and the sum of w is below C, so both are exact
+            double sw = t[0][r] * 128.0;
+            const double nn = floor(sw * inv_C);
+            sw -= nn * C;
+            c_hi += (uint32_t)nn;
+            w_lo = fma((double)wi[r * 128], wsum - sw, w_lo);
+            w_hi = fma((double)wi[r * 128], sw, w_hi);
+        }
+    }
+    const uint32_t c_lo = n_all - c_hi;
+    LaneTally *tally = w.tally() + lane;
+    tally->c_lo += c_lo;
+    tally->c_hi += c_hi;
+    if constexpr (kWeighted) {
+        if (c_lo != 0u) tally->w_lo += w_lo;  // no pair of this thread in the row: not even a rounding residue
+        if (c_hi != 0u) tally->w_hi += w_hi;
+    }
+}
+
+// Keeps the warp's queue filled: takes the next job from the global counter when the current one has been scanned,
+// and bounds the windows of the warp's i-group against the next (up to) kScan j-groups of its job -- two j-tiles,
+// one lane per j-group, fp64 -- queueing the survivors: groups whose window lies wholly out of range are dropped
+// (PAPER.md:126), a window of several edges is split by the sub-group caps of the j side.  Returns when kScan
+// units are queued or no job is left.  Not inlined: its registers are its own.
+template <bool kWeighted>
+__device__ __noinline__ void refill(const WinParams &p, const WarpSm<kWeighted> w, const Tables tb)
+{
+    const int lane = threadIdx.x & 31;
+    volatile WarpCtl *c = w.ctl();
+    Unit *queue = w.queue();
+    CtaHeader *h = reinterpret_cast<CtaHeader *>(smem);
+    const Rows rows = rows_of<kWeighted>(p, w);
+    const double slack = cap_slack(norm_eps(p.counters));
+    const double *edges_sm = tb.edges_ptr();
+    while (c->q_tail - c->n_done < (uint32_t)kScan) {
+        if (c->it >= c->it_end) {
+            // ---- the next job: {i-group of the tile, run of `chunk` work items}; 8 consecutive jobs share their items
+            uint32_t job = 0;
+            if (lane == 0) job = atomicAdd(reinterpret_cast<unsigned int *>(&p.counters[kCtrWorkHead]), 1u);  // (the low word: far fewer than 2^32 jobs)
+            job = __shfl_sync(0xffffffffu, job, 0);
+            if (job >= h->n_jobs) {
+                if (lane == 0) c->no_more = 1;
+                __syncwarp();
+                return;
+            }
+            if (lane == 0) {
+                const uint32_t it = job / kGroupsPerTile * h->chunk;
+                const int3 cur = p.items[it];
+                c->ig = (int)(job % kGroupsPerTile);
+                c->it = it;
+                c->it_end = it + h->chunk < h->n_items ? it + h->chunk : h->n_items;
+                c->t = 0;
+                c->cx = cur.x;
+                c->cy = cur.y;
+                c->cz = cur.z;
+            }
+            __syncwarp();
+        }
+        const int ig = c->ig;
+        uint32_t it = c->it;
+        const uint32_t it_end = c->it_end;
+        int t = c->t, cx = c->cx, cy = c->cy, cz = c->cz;
+        int ti0 = -1, tj0 = 0, ti1 = -1, tj1 = 0;
+        if (it < it_end) {
+            ti0 = cx;
+            tj0 = cy + t;
+            if (++t == cz) {
+                t = 0;
+                if (++it < it_end) {
+                    const int3 nxt = p.items[it];
+                    cx = nxt.x, cy = nxt.y, cz = nxt.z;
+                }
+            }
+        }
+        if (it < it_end) {
+            ti1 = cx;
+            tj1 = cy + t;
+            if (++t == cz) {
+                t = 0;
+                if (++it < it_end) {
+                    const int3 nxt = p.items[it];
+                    cx = nxt.x, cy = nxt.y, cz = nxt.z;
+                }
+            }
+        }
+        const int ti = lane < kGroupsPerTile ? ti0 : ti1, tj = lane < kGroupsPerTile ? tj0 : tj1;
+        const int g = lane & (kGroupsPerTile - 1);
+        bool live = lane < kScan && ti >= 0;
+        Unit u;
+        u.i_first = 0;
+        u.j_first = 0;
+        u.nsub = 1;
+        u.masked = u.diag = u.chord = 0;
+        u.jn = 0;
+#pragma unroll
+        for (int s = 0; s < kSubsPerGroup; ++s) {
+            u.lo[s] = u.hi[s] = -1;
+            u.wsum[s] = 0.0;
+        }
+        if (live) {
+            const uint32_t igx = (uint32_t)ti * kGroupsPerTile + ig, jgx = (uint32_t)tj * kGroupsPerTile + g;
+            const uint32_t i0 = igx * kGroup, j0 = jgx * kGroup;
+            const uint32_t gi = i0 < p.n_a ? (p.n_a - i0 < (uint32_t)kGroup ? p.n_a - i0 : (uint32_t)kGroup) : 0u;
+            const uint32_t gj = j0 < p.n_b ? (p.n_b - j0 < (uint32_t)kGroup ? p.n_b - j0 : (uint32_t)kGroup) : 0u;
+            const bool diag_tile = p.is_auto && tj == ti;
+            live = gi > 0 && gj > 0 && !(diag_tile && g < ig);
+            if (live) {
+                u.i_first = i0;
+                u.j_first = j0;
+                u.jn = (int32_t)gj;
+                u.diag = diag_tile && g == ig;
+                u.masked = gi < (uint32_t)kGroup || gj < (uint32_t)kGroup || u.diag;
+                const GroupCap ca = p.gcaps_a[igx], cb = p.gcaps_b[jgx];
+                auto bound = [&](const GroupCap &cj, int &lo, int &hi, bool &chord) {
+                    lo = 0;
+                    hi = p.nbins + 1;
+                    chord = false;
+                    double c_lo, c_hi;
+                    if (cap_window(ca, cj, slack, c_lo, c_hi)) {
+                        // rows of the two ends; the far end is a few rows on at most: walk there
+                        hi = lo = row_of_cos(c_hi, edges_sm, p.nbins);
+                        while (hi < p.nbins && c_lo <= edges_sm[hi]) ++hi;
+                        if (hi == p.nbins && c_lo < edges_sm[p.nbins]) ++hi;
+                        chord = hi > lo && c_hi - c_lo < kChordWidth && c_lo > kChordCosMin;
+                    }
+                };
+                int lo, hi;
+                bool chord;
+                bound(cb, lo, hi, chord);
+                const bool out = hi == lo && (lo == 0 || lo > p.nbins);  // all closer than theta_min or all beyond theta_max
+                if (p.prune && out) {
+                    live = false;  // pruned at the level of groups, like whole tiles in the work list
+                } else if (p.bulk && hi == lo && !out && !u.masked) {
+                    // all pairs of two full groups in one bin: the bin gets the groups' pair count and the product of
+                    // their weight sums, and nothing is evaluated (ACF_OPT_BULK)
+                    const unsigned long long all = (unsigned long long)kGroup * kGroup;
+                    rows.template add_atomic<kWeighted>(lo, (uint32_t)all, ca.wsum * cb.wsum);
+                    atomicAdd(&h->stat[kStatBulk], all);
+                    live = false;
+                } else {
+                    u.lo[0] = (int16_t)lo;
+                    u.hi[0] = (int16_t)hi;
+                    u.chord = chord ? 1 : 0;
+                    u.wsum[0] = cb.wsum;
+                    if (p.refine && !u.masked && hi - lo >= 2) {
+                        // several edges: the window of each sub-group of the j side is narrower
+                        u.nsub = kSubsPerGroup;
+                        u.chord = 0;
+#pragma unroll
+                        for (int s = 0; s < kSubsPerGroup; ++s) {
+                            const GroupCap cs = p.scaps_b[(size_t)jgx * kSubsPerGroup + s];
+                            int slo, shi;
+                            bool sch;
+                            bound(cs, slo, shi, sch);
+                            if (p.prune && shi == slo && (slo == 0 || slo > p.nbins)) slo = shi = -1;
+                            u.lo[s] = (int16_t)slo;
+                            u.hi[s] = (int16_t)shi;
+                            u.chord |= (sch ? 1 : 0) << s;
+                            u.wsum[s] = cs.wsum;
+                        }
+                    }
+                }
+            }
+        }
+        const uint32_t alive = __ballot_sync(0xffffffffu, live);
+        const uint32_t q_tail = c->q_tail;
+        if (live) queue[(q_tail + __popc(alive & ((1u << lane) - 1u))) % kQueue] = u;
+        __syncwarp();
+        if (lane == 0) {
+            c->q_tail = q_tail + __popc(alive);
+            c->it = it;
+            c->t = t;
+            c->cx = cx;
+            c->cy = cy;
+            c->cz = cz;
+        }
+        __syncwarp();
+    }
 }
 
 template <bool kWeighted>
-__global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p)
+__global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const __grid_constant__ WinParams p)
 {
     if (p.counters[kCtrBadInput] != 0) return;  // inputs failed validation
     if (kWeighted && p.pack_b->packed == 0) return;  // weights that do not pack: the table kernel does the call
-    extern __shared__ __align__(128) unsigned char smem[];
     const int rows_n = p.nbins + 2;
-    const int n_stages = p.n_stages;
-    constexpr size_t kStage = stage_bytes(kWeighted);
-    // layout: [full bars | empty bars | stage meta | producer state] (512 B) [stages][count rows per warp][weight rows per warp]
-    uint64_t *full = reinterpret_cast<uint64_t *>(smem);
-    uint64_t *empty = full + kMaxStages;
-    StageMeta *meta = reinterpret_cast<StageMeta *>(smem + 128);
-    volatile ProdState *ps = reinterpret_cast<volatile ProdState *>(smem + 128 + kMaxStages * sizeof(StageMeta));
-    unsigned long long *stat = reinterpret_cast<unsigned long long *>(smem + 128 + kMaxStages * sizeof(StageMeta) + sizeof(ProdState));
-    PackInfo *pack_sm = reinterpret_cast<PackInfo *>(stat + kNumStats);
-    static_assert(sizeof(ProdState) % 8 == 0 &&
-                      128 + kMaxStages * sizeof(StageMeta) + sizeof(ProdState) + kNumStats * 8 + sizeof(PackInfo) <= kSmemHeader,
-                  "header");
-    unsigned char *stages = smem + kSmemHeader;
-    size_t off = kSmemHeader + (size_t)n_stages * kStage;
-    uint32_t *cnt_all = reinterpret_cast<uint32_t *>(smem + off);
-    const int row_sets = p.shared_rows ? 1 : kWarps;
-    off += (size_t)row_sets * rows_n * sizeof(uint32_t);
-    off = (off + 15) & ~size_t(15);
-    double *ws_all = reinterpret_cast<double *>(smem + off);
-    if constexpr (kWeighted) off += (size_t)row_sets * rows_n * sizeof(double);
-    WinRows *win_all = reinterpret_cast<WinRows *>(smem + off);
-    off += (size_t)kWarps * kGroupsPerTile * sizeof(WinRows);
-    double *edges_sm = reinterpret_cast<double *>(smem + off);  // the edges, for the windows' row searches
-
+    const int n_edges = p.nbins + 1;
+    constexpr size_t kStage = wstage_bytes(kWeighted);
     const int tid = threadIdx.x, warp = tid >> 5, lane = tid & 31;
-    const int igrp = warp & (kTeamWarps - 1), team = warp / kTeamWarps;
-    for (int i = tid; i < row_sets * rows_n; i += blockDim.x) {
-        cnt_all[i] = 0;
-        if constexpr (kWeighted) ws_all[i] = 0.0;
-    }
-    for (int i = tid; i <= p.nbins; i += blockDim.x) edges_sm[i] = p.edges[i];
-    if (tid == 0) {
-        for (int s = 0; s < n_stages; ++s) {
-            mbar_init(&full[s], 1);
-            mbar_init(&empty[s], kWarps);
+
+    // ---- shared memory: per CTA [CtaHeader | edges | chord tables | shared rows], then per warp (WarpSm)
+    CtaHeader *h = reinterpret_cast<CtaHeader *>(smem);
+    size_t off = sizeof(CtaHeader);
+    double *edges_sm = reinterpret_cast<double *>(smem + off);
+    off += sizeof(double) * (size_t)n_edges;
+    float *sed_sm = reinterpret_cast<float *>(smem + off);
+    float *sneg_sm = sed_sm + n_edges, *gs1_sm = sneg_sm + n_edges, *gsk_sm = gs1_sm + n_edges;
+    off += sizeof(float) * 4 * (size_t)n_edges;
+    off = (off + 15) & ~size_t(15);
+    off += sizeof(Cell) * kCells;  // the cell table (Tables::cells)
+    if (p.shared_rows) {
+        uint32_t *cnt_shared = reinterpret_cast<uint32_t *>(smem + off);
+        off += sizeof(uint32_t) * (size_t)rows_n;
+        off = (off + 15) & ~size_t(15);
+        double *ws_shared = reinterpret_cast<double *>(smem + off);
+        if constexpr (kWeighted) off += sizeof(double) * (size_t)rows_n;
+        for (int i = tid; i < rows_n; i += blockDim.x) {
+            cnt_shared[i] = 0;
+            if constexpr (kWeighted) ws_shared[i] = 0.0;
         }
-        ps->lock = 0;
-        ps->produced = 0;
-        ps->ti = ps->tj = ps->left = 0;
-        ps->done = 0;
-        unsigned long long n_items = p.counters[kCtrWorkCount];
-        ps->n_items = n_items > p.capacity ? p.capacity : n_items;
-        for (int i = 0; i < kNumStats; ++i) stat[i] = 0ull;
-        *pack_sm = *p.pack_b;
-        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    off = (off + 127) & ~size_t(127);
+    size_t per_warp = WarpSm<kWeighted>::kFixed + kStage * kWStages;
+    if (!p.shared_rows) per_warp += (((size_t)rows_n * sizeof(uint32_t) + 15) & ~size_t(15)) + (kWeighted ? (size_t)rows_n * sizeof(double) : 0);
+    per_warp = (per_warp + 127) & ~size_t(127);
+    WarpSm<kWeighted> w;
+    w.base = smem_u32(smem + off + per_warp * (size_t)warp);
+    w.rows_n = rows_n;
+
+    const Tables tb = tables_of(p);
+    {
+        const float margin = tb.margin();
+        for (int i = tid; i < n_edges; i += blockDim.x) {
+            edges_sm[i] = p.edges[i];
+            const float se = p.sedges[i];
+            sed_sm[i] = se;
+            sneg_sm[i] = -se;
+            gs1_sm[i] = chord_guard(se, margin, false);
+            gsk_sm[i] = chord_guard(se, margin, true);
+        }
+        fill_cells(tb.cells(), p.sedges, p.nbins, margin, tid, blockDim.x);
+    }
+    if (!p.shared_rows)
+        for (int i = lane; i < rows_n; i += 32) {
+            w.cnt_own()[i] = 0;
+            if constexpr (kWeighted) w.ws_own()[i] = 0.0;
+        }
+    if (lane == 0) {
+        volatile WarpCtl *c = w.ctl();
+        for (int s = 0; s < kWStages; ++s) mbar_init(reinterpret_cast<uint64_t *>(w.ptr(8u * (uint32_t)s)), 1);
+        c->q_tail = c->n_issued = c->n_done = 0u;
+        c->it = c->it_end = 0u;
+        c->t = c->cx = c->cy = c->cz = c->ig = 0;
+        c->no_more = 0;
+        c->since_flush = 0u;
+        c->tally_m = -1;
+        c->loaded_first = 0xffffffffu;
+        c->n_eval = c->n_win = c->n_chord = 0ull;
+    }
+    if (tid == 0) {
+        for (int i = 0; i < 8; ++i) h->stat[i] = 0ull;
+        h->pack = *p.pack_b;
+        const uint32_t n_items = (uint32_t)(p.counters[kCtrWorkCount] > p.capacity ? p.capacity : p.counters[kCtrWorkCount]);
+        uint32_t chunk = (uint32_t)((unsigned long long)n_items * kGroupsPerTile / (64ull * gridDim.x * kWarps));
+        chunk = chunk < 1u ? 1u : (chunk > 4u ? 4u : chunk);
+        h->n_items = n_items;
+        h->chunk = chunk;
+        h->n_jobs = (n_items + chunk - 1u) / chunk * kGroupsPerTile;
+    }
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     __syncthreads();
 
-    if (tid == 0) try_produce<kWeighted>(p, ps, full, empty, meta, stages, n_stages);
+    w.tally()[lane] = LaneTally{0u, 0u, 0.0, 0.0};  // this thread's tallies of the rows around the edge WarpCtl::tally_m
 
-    // ---------------- consumers
-    Rows rows;
-    rows.shared = p.shared_rows != 0;
-    rows.pack = pack_sm;
-    rows.cnt = cnt_all + (rows.shared ? 0 : (size_t)warp * rows_n);
-    rows.ws = ws_all + (rows.shared ? 0 : (size_t)warp * rows_n);
-    WinRows *win = win_all + (size_t)warp * kGroupsPerTile;
-    uint32_t since_flush = 0;  // j-tiles this warp has tallied in its unflushed rows
-    // u32 rows: flush before the tallies could wrap (shared rows take the pairs of all the CTA's warps)
-    // (the rows are read as signed 32-bit numbers when flushed: half the range)
-    const uint32_t flush_every = (1u << 30) / (uint32_t)(kGroup * kTile) / (rows.shared ? (uint32_t)kWarps : 1u);
-    float wi[kR];
-    float nx[kR], ny[kR], nz[kR];  // the i-points, negated
-#pragma unroll
-    for (int r = 0; r < kR; ++r) wi[r] = nx[r] = ny[r] = nz[r] = 0.f;
-    uint32_t valid_mask = 0, i_base = 0, n_i = 0;
-    bool warp_full = false, warp_any = false;
-    int cur_ti = -1;
-
-    LaneTally tally{0u, 0u, 0.0, 0.0};
-    int tally_m = -1;  // the edge the tally belongs to (warp-uniform)
     auto flush_tally = [&]() {
         // the threads' tallies of rows tally_m and tally_m + 1 -> the warp's rows
+        volatile WarpCtl *c = w.ctl();
+        const int tally_m = c->tally_m;
         if (tally_m >= 0) {
+            const Rows rows = rows_of<kWeighted>(p, w);
+            LaneTally *tl = w.tally() + lane;
+            const LaneTally tally = *tl;
+            *tl = LaneTally{0u, 0u, 0.0, 0.0};
             const uint32_t c_lo = __reduce_add_sync(0xffffffffu, tally.c_lo), c_hi = __reduce_add_sync(0xffffffffu, tally.c_hi);
             double w_lo = 0.0, w_hi = 0.0;
             if constexpr (kWeighted) {
@@ -670,181 +1169,142 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const WinParams p
             if (lane == 0) {
                 rows.template add<kWeighted>(tally_m, c_lo, w_lo);
                 rows.template add<kWeighted>(tally_m + 1, c_hi, w_hi);
+                c->tally_m = -1;
             }
-            tally = LaneTally{0u, 0u, 0.0, 0.0};
-            tally_m = -1;
+            __syncwarp();
         }
     };
     auto flush_rows = [&]() {
         // this warp's rows -> global (u64 / f64 atomics); the rows restart from zero
         flush_tally();
         __syncwarp();
+        const Rows rows = rows_of<kWeighted>(p, w);
         for (int row = lane; row < rows_n; row += 32) {
             // (shared rows: other warps add while this one takes the value and leaves zero)
-            const uint32_t v = rows.shared ? atomicExch(&rows.cnt[row], 0u) : rows.cnt[row];
-            if (!rows.shared) rows.cnt[row] = 0;
-            // read as signed: with shared rows another warp's exact correction (-1 now, its tally later) may be
-            // caught in between; the two's-complement sum in global memory comes out the same
+            const uint32_t v = atomicExch(&rows.cnt[row], 0u);
+            // read as signed: a correction (-1 now, its tally later) may be caught in between; the two's-complement
+            // sum in global memory comes out the same
             if (row >= 1 && row <= p.nbins && v) atomicAdd(&p.counts[row - 1], (unsigned long long)(long long)(int32_t)v);
             if constexpr (kWeighted) {
-                const double w = rows.shared ? __longlong_as_double((long long)atomicExch(reinterpret_cast<unsigned long long *>(&rows.ws[row]), 0ull))
-                                             : rows.ws[row];
-                if (!rows.shared) rows.ws[row] = 0.0;
-                if (row >= 1 && row <= p.nbins && w != 0.0) atomicAdd(&p.wsums[row - 1], w);
+                const double ws = __longlong_as_double((long long)atomicExch(reinterpret_cast<unsigned long long *>(&rows.ws[row]), 0ull));
+                if (row >= 1 && row <= p.nbins && ws != 0.0) atomicAdd(&p.wsums[row - 1], ws);
             }
         }
+        if (lane == 0) w.ctl()->since_flush = 0u;
         __syncwarp();
-        since_flush = 0;
     };
 
-    for (uint32_t consumed = 0;; ++consumed) {
-        const int slot = (int)(consumed % (uint32_t)n_stages);
-        const uint32_t parity = (consumed / (uint32_t)n_stages) & 1u;
-        if (lane == 0)
-            while (!mbar_test(&full[slot], parity)) {
-                try_produce<kWeighted>(p, ps, full, empty, meta, stages, n_stages);
-                if (!mbar_test(&full[slot], parity)) __nanosleep(100);  // leave the issue slots to the warps that have work
+    while (true) {
+        volatile WarpCtl *c = w.ctl();
+        if (!c->no_more && c->q_tail - c->n_done < (uint32_t)kScan) refill<kWeighted>(p, w, tables_of(p));
+        // ---- issue: TMA loads of queued units into free stages
+        const uint32_t n_done = c->n_done;
+        {
+            const uint32_t q_tail = c->q_tail;
+            if (lane == 0) {
+                uint32_t n_issued = c->n_issued;
+                while (n_issued < q_tail && n_issued - n_done < (uint32_t)kWStages) {
+                    const uint32_t j0 = w.queue()[n_issued % kQueue].j_first;
+                    const int st = (int)(n_issued % kWStages);
+                    const uint32_t dst = w.stage(st), bar = w.full(st);
+                    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"((uint32_t)kStage) : "memory");
+                    // the arrays are padded to whole tiles: always a full group
+                    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                                 "l"(p.pts2_b + (size_t)j0 * 4), "r"((uint32_t)kGroupBytes), "r"(bar)
+                                 : "memory");
+                    if constexpr (kWeighted)
+                        asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                                         dst + (uint32_t)kGroupBytes),
+                                     "l"(p.vj_b + (size_t)j0), "r"((uint32_t)kGroupVjBytes), "r"(bar)
+                                     : "memory");
+                    ++n_issued;
+                }
+                c->n_issued = n_issued;
             }
-        __syncwarp();
-        mbar_wait(&full[slot], parity);  // every lane observes the completed phase
-        const StageMeta m = meta[slot];
-        if (m.ti < 0) break;
-        if (m.ti != cur_ti) {
-            cur_ti = m.ti;
-            i_base = (uint32_t)m.ti * kTile;
-            valid_mask = 0;
-#pragma unroll
-            for (int r = 0; r < kR; ++r) {
-                const uint32_t s = i_base + local_i(r);
-                const float4 v = p.pts_a[s];  // the array is padded to a whole tile
-                nx[r] = -v.x;
-                ny[r] = -v.y;
-                nz[r] = -v.z;
-                wi[r] = v.w;
-                valid_mask |= (s < p.n_a ? 1u : 0u) << r;
+            __syncwarp();
+            if (n_done == q_tail) {
+                if (c->no_more) break;
+                continue;
             }
-            n_i = i_base + kTile <= p.n_a ? kTile : p.n_a - i_base;
-            warp_full = (uint32_t)(igrp + 1) * kGroup <= n_i;
-            warp_any = (uint32_t)igrp * kGroup < n_i;
         }
-        const float *tile = reinterpret_cast<const float *>(stages + (size_t)slot * kStage);
-        const double *vtile = reinterpret_cast<const double *>(stages + (size_t)slot * kStage + kTileBytes);
-        const int tj = m.tj, jn = m.jn;
-        const bool diag = p.is_auto && tj == m.ti;
-        const uint32_t j_base = (uint32_t)tj * kTile;
-        // u32 rows: flush before this warp's tallies could wrap
-        if (since_flush >= flush_every) flush_rows();
-        ++since_flush;
-
-        if (warp_any) {
-            // lane l bounds the rows of this warp's i-group against the team's l-th j-group of the tile
-            const int n_groups = (jn + kGroup - 1) / kGroup;
-            __syncwarp();
-            const int my_g = lane * kTeams + team;
-            if (lane < kGroupsPerTile / kTeams && my_g < n_groups) {
-                WinRows wr;
-                wr.lo = 0;
-                wr.hi = p.nbins + 1;
-                const GroupCap gb = p.gcaps_b[(size_t)tj * kGroupsPerTile + my_g];
-                double c_lo, c_hi;
-                if (cap_window(p.gcaps_a[(size_t)m.ti * kGroupsPerTile + igrp], gb, c_lo, c_hi)) {
-                    // rows of the two ends; the far end is a few rows on at most: walk there
-                    int hi = wr.lo = row_of_cos(c_hi, edges_sm, p.nbins);
-                    while (hi < p.nbins && c_lo <= edges_sm[hi]) ++hi;
-                    if (hi == p.nbins && c_lo < edges_sm[p.nbins]) ++hi;
-                    wr.hi = hi;
-                }
-                if (p.prune && wr.hi == wr.lo && (wr.lo == 0 || wr.lo > p.nbins) && !(diag && my_g < igrp)) {
-                    // all closer than theta_min or all beyond theta_max: pruned at the level of groups, like whole
-                    // tiles in the work list; the tile's pair count in the statistics loses them
-                    const uint32_t gi = n_i - (uint32_t)igrp * kGroup < (uint32_t)kGroup ? n_i - (uint32_t)igrp * kGroup : (uint32_t)kGroup;
-                    const uint32_t gj = (uint32_t)(jn - my_g * kGroup < kGroup ? jn - my_g * kGroup : kGroup);
-                    const unsigned long long gone = diag && my_g == igrp ? (unsigned long long)gi * (gi - 1) / 2 : (unsigned long long)gi * gj;
-                    atomicAdd(&stat[kStatEvaluated], 0ull - gone);
-                    wr.lo = wr.hi = -1;
-                }
-                if (p.bulk && wr.lo >= 0 && wr.hi == wr.lo && warp_full && jn - my_g * kGroup >= kGroup && !(diag && my_g <= igrp)) {
-                    // all pairs of two full groups in one bin: the bin gets the groups' pair count and the product of
-                    // their weight sums, and nothing is evaluated (ACF_OPT_BULK)
-                    const unsigned long long all = (unsigned long long)kGroup * kGroup;
-                    rows.template add_atomic<kWeighted>(wr.lo, (uint32_t)all, p.gcaps_a[(size_t)m.ti * kGroupsPerTile + igrp].wsum * gb.wsum);
-                    atomicAdd(&stat[kStatEvaluated], 0ull - all);
-                    atomicAdd(&stat[kStatBulk], all);
-                    wr.lo = wr.hi = -1;
-                }
-                const int m_one = wr.hi > wr.lo ? wr.lo : (wr.lo > p.nbins ? p.nbins : (wr.lo < 0 ? 0 : wr.lo));
-                wr.e32 = (float)edges_sm[m_one];
-                wr.pad = 0;
-                wr.wsum = gb.wsum;
-                win[my_g] = wr;
-            }
-            __syncwarp();
-            // pass 1: the common groups (one edge, nothing masked), inline; the others are noted in slow_groups
-            uint32_t slow_groups = 0;
-            for (int g = diag ? igrp : 0; g < n_groups; ++g) {
-                if ((g & (kTeams - 1)) != team) continue;  // the other team's group
-                const int r_lo = win[g].lo, r_hi = win[g].hi;
-                if (r_lo < 0) continue;  // pruned (see where the windows are bounded)
-                const bool masked = !warp_full || jn - g * kGroup < kGroup || (diag && g == igrp);
-                if (masked || r_hi - r_lo > 1) {
-                    slow_groups |= 1u << g;
-                    continue;
-                }
+        // ---- evaluate the oldest unit
+        const Unit *u = &w.queue()[n_done % kQueue];
+        const int st = (int)(n_done % kWStages);
+        mbar_wait_s(w.full(st), (n_done / kWStages) & 1u);
+        Span sp;
+        sp.grp2 = w.stage(st);
+        sp.vgrp = sp.grp2 + (uint32_t)kGroupBytes;
+        sp.i_first = u->i_first;
+        sp.j_first = u->j_first;
+        // u32 rows, read as signed when flushed: flush before 2^30 pairs (shared rows take the pairs of all the CTA's warps)
+        if (c->since_flush >= (1u << 30) / (uint32_t)(kGroup * kGroup) / (p.shared_rows ? (uint32_t)kWarps : 1u)) flush_rows();
+        const int nsub = u->nsub;
+        const bool masked = u->masked != 0;
+        uint32_t pairs = 0, pairs_win = 0, pairs_chord = 0;
+        for (int s = 0; s < nsub; ++s) {
+            const int r_lo = u->lo[s], r_hi = u->hi[s];
+            if (r_lo < 0) continue;  // a sub-group whose window lies out of range
+            sp.jj0 = nsub == 1 ? 0 : s * kSub;
+            sp.jj1 = nsub == 1 ? kGroup : sp.jj0 + kSub;
+            sp.wsum = u->wsum[s];
+            const bool chord = (u->chord >> s) & 1;
+            const int K = r_hi - r_lo;
+            if (masked || K > kMaxPassEdges) {
+                Mask mk;
+                mk.gi = p.n_a - sp.i_first < (uint32_t)kGroup ? p.n_a - sp.i_first : (uint32_t)kGroup;
+                mk.jn = u->jn;
+                mk.diag = u->diag != 0;
+                general_span<kWeighted>(p, tables_of(p), rows_of<kWeighted>(p, w), sp, mk, h->stat);
+                const uint32_t n = !masked ? (uint32_t)(sp.jj1 - sp.jj0) * kGroup : (mk.diag ? mk.gi * (mk.gi - 1) / 2 : mk.gi * (uint32_t)mk.jn);
+                pairs += n;
+                pairs_chord += n;
+            } else if (K <= 1) {
                 // a window inside one row is tested against the edge that bounds the row
-                const int m_edge = r_hi > r_lo ? r_lo : (r_lo > p.nbins ? p.nbins : r_lo);
-                Mask mk{};
-                if (m_edge != tally_m) {
+                const int m_edge = K == 1 ? r_lo : (r_lo > p.nbins ? p.nbins : r_lo);
+                if (m_edge != c->tally_m) {
                     flush_tally();
-                    tally_m = m_edge;
+                    if (lane == 0) c->tally_m = m_edge;
                 }
-                window_chunk<1, kWeighted, false, true>(p, rows, tile + (size_t)g * kGroup * 4, vtile + g * kGroup,
-                                                                                      nx, ny, nz, wi, m_edge, true, true, win[g].wsum, mk,
-                                                                                      i_base, j_base + g * kGroup, stat, &tally, nullptr,
-                                                                                      win[g].e32);
-                if (lane == 0) atomicAdd(&stat[kStatWindow], (unsigned long long)(kGroup * kGroup));
+                if (lane == 0) c->sub = s;
+                __syncwarp();
+                if (chord) single_edge_span<kWeighted, true>(p, w);
+                else single_edge_span<kWeighted, false>(p, w);
+                pairs += (uint32_t)(sp.jj1 - sp.jj0) * kGroup;
+                pairs_win += (uint32_t)(sp.jj1 - sp.jj0) * kGroup;
+                if (chord) pairs_chord += (uint32_t)(sp.jj1 - sp.jj0) * kGroup;
+            } else {
+                if (chord) window_multi<kWeighted, true>(p, tables_of(p), rows_of<kWeighted>(p, w), sp, r_lo, r_hi, h->stat);
+                else window_multi<kWeighted, false>(p, tables_of(p), rows_of<kWeighted>(p, w), sp, r_lo, r_hi, h->stat);
+                pairs += (uint32_t)(sp.jj1 - sp.jj0) * kGroup;
+                if (chord) pairs_chord += (uint32_t)(sp.jj1 - sp.jj0) * kGroup;
             }
-            // pass 2: the rest through the function; it reloads the i-points, and so does this loop afterwards
-            // (they are not kept in registers across the calls)
-            if (slow_groups) {
-                for (int g = 0; g < n_groups; ++g) {
-                    if (!((slow_groups >> g) & 1u)) continue;
-                    const int r_lo = win[g].lo, r_hi = win[g].hi;
-                    Mask mk;
-                    mk.valid = valid_mask;
-                    mk.jn = jn - g * kGroup < kGroup ? jn - g * kGroup : kGroup;
-                    mk.j0 = g * kGroup;
-                    mk.diag = diag && g == igrp;
-                    const bool masked = !warp_full || mk.jn < kGroup || mk.diag;
-                    window_group<kWeighted>(p, rows, tile + (size_t)g * kGroup * 4, vtile + g * kGroup, r_lo, r_hi, win[g].wsum,
-                                                     masked, mk, i_base, j_base + g * kGroup, stat);
-                    if (lane == 0 && !masked && r_hi - r_lo <= 1) atomicAdd(&stat[kStatWindow], (unsigned long long)(kGroup * kGroup));
-                }
-#pragma unroll
-                for (int r = 0; r < kR; ++r) {
-                    const float4 v = p.pts_a[i_base + local_i(r)];
-                    nx[r] = -v.x;
-                    ny[r] = -v.y;
-                    nz[r] = -v.z;
-                    wi[r] = v.w;
-                }
-            }
+            __syncwarp();
         }
-        if (tid == 0) atomicAdd(&stat[kStatEvaluated], diag ? (unsigned long long)n_i * (n_i - 1) / 2 : (unsigned long long)n_i * (unsigned)jn);
-        __syncwarp();  // every lane has read the stage before it is handed back
+        __syncwarp();  // every lane has read the stage (and the queue slot) before either is reused
         if (lane == 0) {
-            mbar_arrive(&empty[slot]);
-            try_produce<kWeighted>(p, ps, full, empty, meta, stages, n_stages);
+            c->n_eval += pairs;
+            c->n_win += pairs_win;
+            c->n_chord += pairs_chord;
+            c->since_flush += 1u;
+            c->n_done = n_done + 1u;
         }
+        __syncwarp();
     }
 
     flush_rows();
+    if (lane == 0) {
+        volatile WarpCtl *c = w.ctl();
+        if (c->n_eval) atomicAdd(&h->stat[kStatEvaluated], c->n_eval);
+        if (c->n_win) atomicAdd(&h->stat[kStatWindow], c->n_win);
+        if (c->n_chord) atomicAdd(&h->stat[kStatChord], c->n_chord);
+    }
     __syncthreads();
     if (tid == 0) {
-        if (stat[kStatFp64]) atomicAdd(&p.counters[kCtrPairsFp64], stat[kStatFp64]);
-        if (stat[kStatWindow]) atomicAdd(&p.counters[kCtrPairsWindow], stat[kStatWindow]);
-        if (stat[kStatEvaluated]) atomicAdd(&p.counters[kCtrPairsEvaluated], stat[kStatEvaluated]);
-        if (stat[kStatChord]) atomicAdd(&p.counters[kCtrPairsChord], stat[kStatChord]);
-        if (stat[kStatBulk]) atomicAdd(&p.counters[kCtrPairsBulk], stat[kStatBulk]);
+        if (h->stat[kStatFp64]) atomicAdd(&p.counters[kCtrPairsFp64], h->stat[kStatFp64]);
+        if (h->stat[kStatWindow]) atomicAdd(&p.counters[kCtrPairsWindow], h->stat[kStatWindow]);
+        if (h->stat[kStatEvaluated]) atomicAdd(&p.counters[kCtrPairsEvaluated], h->stat[kStatEvaluated]);
+        if (h->stat[kStatChord]) atomicAdd(&p.counters[kCtrPairsChord], h->stat[kStatChord]);
+        if (h->stat[kStatBulk]) atomicAdd(&p.counters[kCtrPairsBulk], h->stat[kStatBulk]);
     }
 }
 
@@ -855,25 +1315,26 @@ int launch_pair_win(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_a
                     unsigned long long *d_counts, double *d_wsums)
 {
     const bool weighted = d_wsums != nullptr;
-    const int rows_n = nbins + 2;
-    int row_sets = kWarps;  // a set of rows per warp, or one per CTA when that leaves no room for the ring
-    auto smem_for = [&](int stages) {
-        size_t m = kSmemHeader + (size_t)stages * stage_bytes(weighted);
-        m += (size_t)row_sets * rows_n * sizeof(uint32_t);
+    const int rows_n = nbins + 2, n_edges = nbins + 1;
+    auto smem_for = [&](bool shared_rows) {
+        size_t m = sizeof(CtaHeader) + sizeof(double) * (size_t)n_edges + sizeof(float) * 4 * (size_t)n_edges;
         m = (m + 15) & ~size_t(15);
-        if (weighted) m += (size_t)row_sets * rows_n * sizeof(double);
-        m += (size_t)kWarps * kGroupsPerTile * sizeof(WinRows);
-        m += sizeof(double) * (size_t)(nbins + 1);
-        return m;
+        m += sizeof(Cell) * kCells;
+        if (shared_rows) {
+            m += sizeof(uint32_t) * (size_t)rows_n;
+            m = (m + 15) & ~size_t(15);
+            if (weighted) m += sizeof(double) * (size_t)rows_n;
+        }
+        m = (m + 127) & ~size_t(127);
+        size_t per_warp = kWarpHeader + sizeof(Unit) * kQueue + 32 * sizeof(LaneTally) + kGroup * sizeof(float4) + wstage_bytes(weighted) * kWStages;
+        if (!shared_rows) per_warp += (((size_t)rows_n * sizeof(uint32_t) + 15) & ~size_t(15)) + (weighted ? (size_t)rows_n * sizeof(double) : 0);
+        per_warp = (per_warp + 127) & ~size_t(127);
+        return m + per_warp * kWarps + 128;  // (+128: the dynamic segment need not start on a 128-byte boundary)
     };
-    // one CTA of 16 warps per SM: 128 registers a thread
-    const int ctas_per_sm = 1;
     const size_t budget = (size_t)ctx->max_smem_optin;
-    if (smem_for(4) > budget) row_sets = 1;
-    if (smem_for(2) > budget) return fail(ctx, ACF_EINVAL, "too many bins for the window kernel (%d)", nbins);
-    int n_stages = 2;
-    while (n_stages < kMaxStages && smem_for(n_stages + 1) <= budget) ++n_stages;
-    const size_t smem = smem_for(n_stages);
+    bool shared_rows = smem_for(false) > budget;  // a set of rows per warp, or one per CTA when that leaves no room
+    if (smem_for(shared_rows) > budget) return fail(ctx, ACF_EINVAL, "too many bins for the window kernel (%d)", nbins);
+    const size_t smem = smem_for(shared_rows);
 
     WinParams p{};
     p.pts_a = a.pts;
@@ -884,6 +1345,7 @@ int launch_pair_win(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_a
     p.perm_b = b.perm;
     p.gcaps_a = a.gcaps;
     p.gcaps_b = b.gcaps;
+    p.scaps_b = b.scaps;
     p.n_a = (uint32_t)a.n;
     p.n_b = (uint32_t)b.n;
     p.xyz_a = a.xyz;
@@ -899,12 +1361,12 @@ int launch_pair_win(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_a
     p.wsums = d_wsums;
     p.counters = ctx->d_counters;
     p.is_auto = is_auto;
-    p.n_stages = n_stages;
-    p.shared_rows = row_sets == 1 ? 1 : 0;
+    p.shared_rows = shared_rows ? 1 : 0;
     p.prune = ctx->opt_prune;
     p.bulk = ctx->opt_bulk;
+    p.refine = 1;
 
-    const int grid = ctx->num_sms * ctas_per_sm;
+    const int grid = ctx->num_sms;  // one CTA of 16 warps per SM: 128 registers a thread
     cudaError_t e = cudaSuccess;
     auto launch = [&](auto kern) {
         if (e != cudaSuccess) return;

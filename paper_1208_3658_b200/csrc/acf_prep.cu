@@ -185,7 +185,7 @@ __global__ void __launch_bounds__(256)
 gather_caps_kernel(const double *__restrict__ xyz, size_t stride, size_t off, const float *__restrict__ w,
                    const uint32_t *__restrict__ idx, uint32_t n, float4 *__restrict__ pts,
                    uint32_t *__restrict__ perm, double4 *__restrict__ caps, GroupCap *__restrict__ gcaps,
-                   float *__restrict__ pts2, double *__restrict__ vj, const uint32_t *__restrict__ range,
+                   GroupCap *__restrict__ scaps, float *__restrict__ pts2, double *__restrict__ vj, const uint32_t *__restrict__ range,
                    PackInfo *__restrict__ pack)
 {
     static_assert(kGroupsPerTile == 8 && kGroup == 128, "one warp of 256 threads per group");
@@ -194,8 +194,10 @@ gather_caps_kernel(const double *__restrict__ xyz, size_t stride, size_t off, co
     constexpr int kPer = kGroup / 32;
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t base = blockIdx.x * kTile + warp * kGroup;
-    double px[kPer], py[kPer], pz[kPer];
+    double px[kPer], py[kPer], pz[kPer];  // the points' directions (the vectors divided by their norms)
+    float wr[kPer];
     double sx = 0, sy = 0, sz = 0, sw = 0;
+    static_assert(kPer == kSubsPerGroup && kSub == 32, "register slot r of a warp is sub-group r of its group");
     // window-path weights (PackInfo): C = 2^(exponent(w_max) + 9) > 256 w_max, a power of two
     const uint32_t mx_bits = w ? range[0] : 0x3f800000u, mn_bits = w ? ~range[1] : 0x3f800000u;
     const int ex_max = (int)(mx_bits >> 23), ex_min = (int)(mn_bits >> 23);
@@ -220,6 +222,7 @@ gather_caps_kernel(const double *__restrict__ xyz, size_t stride, size_t off, co
             py[r] = xyz[stride + g];
             pz[r] = xyz[2 * stride + g];
             const float wi = w ? w[g] : 1.0f;
+            wr[r] = wi;
             pts[s] = make_float4((float)px[r], (float)py[r], (float)pz[r], wi);
             p2[0] = (float)px[r];
             p2[2] = (float)py[r];
@@ -227,15 +230,60 @@ gather_caps_kernel(const double *__restrict__ xyz, size_t stride, size_t off, co
             p2[6] = wi;
             vj[s] = packed ? packC + (double)wi : (double)wi;
             perm[s] = (uint32_t)g;  // index into the caller's catalogue
+            // the caps bound directions: norms may be off 1 by the 1e-6 the validation accepts (cap_slack)
+            const double inv = 1.0 / sqrt(fmax(1e-300, px[r] * px[r] + py[r] * py[r] + pz[r] * pz[r]));
+            px[r] *= inv;
+            py[r] *= inv;
+            pz[r] *= inv;
             sx += px[r];
             sy += py[r];
             sz += pz[r];
             sw += (double)wi;
         } else {
             px[r] = py[r] = pz[r] = 0.0;
+            wr[r] = 0.f;
             pts[s] = make_float4(0.f, 0.f, 0.f, 0.f);  // padding up to the tile boundary, never paired
             p2[0] = p2[2] = p2[4] = p2[6] = 0.f;
             vj[s] = 0.0;
+        }
+    }
+    // ---- sub-group caps: register slot r of the warp holds sub-group r (kSub consecutive sorted points)
+#pragma unroll
+    for (int r = 0; r < kPer; ++r) {
+        const bool have = base + r * 32 + lane < n;
+        double ux = have ? px[r] : 0.0, uy = have ? py[r] : 0.0, uz = have ? pz[r] : 0.0;
+        double uw = have ? (double)wr[r] : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) {
+            ux += __shfl_xor_sync(0xffffffffu, ux, o);
+            uy += __shfl_xor_sync(0xffffffffu, uy, o);
+            uz += __shfl_xor_sync(0xffffffffu, uz, o);
+            uw += __shfl_xor_sync(0xffffffffu, uw, o);
+        }
+        double cx = 0.0, cy = 0.0, cz = 1.0;
+        const double nrm = sqrt(ux * ux + uy * uy + uz * uz);
+        if (nrm > 1e-9) {
+            cx = ux / nrm;
+            cy = uy / nrm;
+            cz = uz / nrm;
+        }
+        double mind = have ? cx * px[r] + cy * py[r] + cz * pz[r] : 2.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) mind = fmin(mind, __shfl_xor_sync(0xffffffffu, mind, o));
+        if (lane == 0) {
+            GroupCap sc;
+            sc.cx = cx;
+            sc.cy = cy;
+            sc.cz = cz;
+            if (base + r * 32 < n) {
+                sc.cos_r = fmax(-1.0, fmin(1.0, mind) - 1e-9);
+                sc.sin_r = sqrt(fmax(0.0, 1.0 - sc.cos_r * sc.cos_r));
+            } else {
+                sc.cos_r = 2.0;  // no points
+                sc.sin_r = 0.0;
+            }
+            sc.wsum = uw;
+            scaps[((size_t)blockIdx.x * kGroupsPerTile + warp) * kSubsPerGroup + r] = sc;
         }
     }
 #pragma unroll
@@ -347,6 +395,7 @@ worklist_kernel(const double4 *__restrict__ caps_a, int ti_begin, int ti_end, co
     const int words = (n_tiles_b + 31) / 32;
     const int tj_first = is_auto ? ti : 0;
     const double4 ca = caps_a[ti];
+    const double slack = 1.001 * __longlong_as_double((long long)counters[kCtrNormDev]);
     uint32_t pruned = 0;
     for (int wbase = 0; wbase < words; wbase += blockDim.x / 32) {
         const int word = wbase + (threadIdx.x >> 5);
@@ -358,7 +407,8 @@ worklist_kernel(const double4 *__restrict__ caps_a, int ti_begin, int ti_end, co
                 double lo, hi;
                 cap_pair_bounds(ca, caps_b[tj], lo, hi);
                 // no pair can be in range: all beyond theta_max, or all closer than theta_min
-                if (hi < e_last - 1e-12 || lo > e_first + 1e-12) k = false;
+                // (the caps bound directions; the pair cosine carries the norms: cap_slack)
+                if (hi + slack < e_last - 1e-12 || lo - slack > e_first + 1e-12) k = false;
             }
             pruned += k ? 0u : 1u;
         }
@@ -413,6 +463,7 @@ int prepare_catalogue(acf_ctx *ctx, int slot, const double *xyz, size_t stride, 
     ACF_CUDA_TRY(ctx, ctx->s_perm[slot].reserve(sizeof(uint32_t) * padded));
     ACF_CUDA_TRY(ctx, ctx->s_caps[slot].reserve(sizeof(double4) * (size_t)n_tiles));
     ACF_CUDA_TRY(ctx, ctx->s_gcaps[slot].reserve(sizeof(GroupCap) * (size_t)n_tiles * kGroupsPerTile));
+    ACF_CUDA_TRY(ctx, ctx->s_scaps[slot].reserve(sizeof(GroupCap) * (size_t)n_tiles * kGroupsPerTile * kSubsPerGroup));
     ACF_CUDA_TRY(ctx, ctx->s_keys[slot].reserve(sizeof(uint32_t) * 4 * (size_t)n));  // keys x2, idx x2
     ACF_CUDA_TRY(ctx, ctx->s_pts2[slot].reserve(sizeof(float4) * padded));
     ACF_CUDA_TRY(ctx, ctx->s_vj[slot].reserve(sizeof(double) * padded));
@@ -423,6 +474,7 @@ int prepare_catalogue(acf_ctx *ctx, int slot, const double *xyz, size_t stride, 
     out->perm = ctx->s_perm[slot].as<uint32_t>();
     out->caps = ctx->s_caps[slot].as<double4>();
     out->gcaps = ctx->s_gcaps[slot].as<GroupCap>();
+    out->scaps = ctx->s_scaps[slot].as<GroupCap>();
     out->pts2 = ctx->s_pts2[slot].as<float>();
     out->vj = ctx->s_vj[slot].as<double>();
     out->pack = ctx->s_pack[slot].as<PackInfo>();
@@ -448,7 +500,7 @@ int prepare_catalogue(acf_ctx *ctx, int slot, const double *xyz, size_t stride, 
         wrange_kernel<<<blocks, 256, 0, st>>>(w, off, n, range);
         ctx->last.kernel_launches++;
     }
-    gather_caps_kernel<<<n_tiles, 256, 0, st>>>(xyz, stride, off, w, i0, n, out->pts, out->perm, out->caps, out->gcaps, out->pts2,
+    gather_caps_kernel<<<n_tiles, 256, 0, st>>>(xyz, stride, off, w, i0, n, out->pts, out->perm, out->caps, out->gcaps, out->scaps, out->pts2,
                                                out->vj, range, out->pack);
     ctx->last.kernel_launches++;
     ACF_CUDA_TRY(ctx, cudaGetLastError());
