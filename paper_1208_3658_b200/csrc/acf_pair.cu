@@ -683,9 +683,9 @@ int count_prepared(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_au
     int n_stages = 2;
     while (n_stages < 4 && smem_for(n_stages + 1) <= budget) ++n_stages;
     const size_t smem = smem_for(n_stages);
-    // which kernel: the window kernel for weighted counts, the table kernel for unweighted ones;
-    // with very many bins the table kernel's rows may not fit beside its table: the window kernel then takes over
-    bool use_win = ctx->opt_kernel == ACF_KERNEL_WINDOW || (ctx->opt_kernel == ACF_KERNEL_AUTO && weighted);
+    // which kernel: the window kernel; the table kernel on request, and behind the window kernel
+    // for weights that do not pack
+    bool use_win = ctx->opt_kernel == ACF_KERNEL_WINDOW || ctx->opt_kernel == ACF_KERNEL_AUTO;
     const bool table_fits = smem <= per_sm;
     if (!use_win && !table_fits) {
         if (ctx->opt_kernel != ACF_KERNEL_AUTO) return fail(ctx, ACF_EINVAL, "shared memory need %zu exceeds %d", smem, ctx->max_smem_optin);

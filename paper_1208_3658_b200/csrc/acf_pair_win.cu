@@ -49,7 +49,8 @@ constexpr int kStep = 4;               // j-points per guard-band vote
 constexpr int kWStages = 2;            // staged j-groups per warp
 constexpr int kQueue = 32;             // surviving j-groups a warp has bounded and not yet evaluated
 constexpr int kScan = 16;              // j-groups bounded at a time (two tiles, one lane each)
-constexpr int kMaxPassEdges = 6;       // windows of more edges than this go pair by pair (general_span)
+constexpr int kMaxPassEdges = 6;       // unweighted: windows of more edges than this go pair by pair (general_span); weighted ones
+                                       // take as many passes as it needs (their pair-by-pair tallies are fp64 atomics on shared memory)
 // The cell table of the pair-by-pair path: the values of the fp32 squared chord length s that share their sign,
 // exponent and top kCellBits mantissa bits form a cell; 2^kCellBits cells per octave from 2^kCellExpLo to 4.
 constexpr int kCellBits = 4;
@@ -702,6 +703,7 @@ struct WarpCtl {
     uint32_t it, it_end;                // work items of the job still to be scanned
     int t, cx, cy, cz;                  // j-tiles of item `it` already scanned; that item {i-tile, first j-tile, j-tiles}
     int ig;                             // the job's i-group within its i-tiles
+    int part;                           // the job takes the j-groups g of a tile with g % CtaHeader::split == part
     int no_more;                        // the global job counter has run out
     int sub;                            // the sub-group of the unit at the head of the queue that is being evaluated
     uint32_t since_flush;               // j-groups tallied in the warp's unflushed rows
@@ -717,7 +719,7 @@ constexpr int kWarpHeader = 128;
 struct CtaHeader {
     unsigned long long stat[8];
     PackInfo pack;
-    uint32_t n_items, chunk, n_jobs, pad[3];
+    uint32_t n_items, chunk, n_jobs, split, pad[2];
 };
 static_assert(kNumStats <= 8 && sizeof(CtaHeader) % 16 == 0, "");
 
@@ -906,6 +908,56 @@ __device__ __forceinline__ void single_edge_span(const WinParams &p, const WarpS
     }
 }
 
+// The threads' tallies of the rows around edge WarpCtl::tally_m -> the warp's rows.  (Not inlined, like
+// flush_rows: called when the edge changes, and the kernel's per-unit path should stay short.)
+template <bool kWeighted>
+__device__ __noinline__ void flush_tally(const WinParams &p, const WarpSm<kWeighted> w)
+{
+    const int lane = threadIdx.x & 31;
+    volatile WarpCtl *c = w.ctl();
+    const int tally_m = c->tally_m;
+    if (tally_m < 0) return;
+    const Rows rows = rows_of<kWeighted>(p, w);
+    LaneTally *tl = w.tally() + lane;
+    const LaneTally tally = *tl;
+    *tl = LaneTally{0u, 0u, 0.0, 0.0};
+    const uint32_t c_lo = __reduce_add_sync(0xffffffffu, tally.c_lo), c_hi = __reduce_add_sync(0xffffffffu, tally.c_hi);
+    double w_lo = 0.0, w_hi = 0.0;
+    if constexpr (kWeighted) {
+        w_lo = warp_sum_f64(tally.w_lo);
+        w_hi = warp_sum_f64(tally.w_hi);
+    }
+    if (lane == 0) {
+        rows.template add<kWeighted>(tally_m, c_lo, w_lo);
+        rows.template add<kWeighted>(tally_m + 1, c_hi, w_hi);
+        c->tally_m = -1;
+    }
+    __syncwarp();
+}
+
+// This warp's rows -> global memory (u64 / f64 atomics); the rows restart from zero.
+template <bool kWeighted>
+__device__ __noinline__ void flush_rows(const WinParams &p, const WarpSm<kWeighted> w)
+{
+    const int lane = threadIdx.x & 31;
+    flush_tally<kWeighted>(p, w);
+    __syncwarp();
+    const Rows rows = rows_of<kWeighted>(p, w);
+    for (int row = lane; row < w.rows_n; row += 32) {
+        // (shared rows: other warps add while this one takes the value and leaves zero)
+        const uint32_t v = atomicExch(&rows.cnt[row], 0u);
+        // read as signed: a correction (-1 now, its tally later) may be caught in between; the two's-complement
+        // sum in global memory comes out the same
+        if (row >= 1 && row <= p.nbins && v) atomicAdd(&p.counts[row - 1], (unsigned long long)(long long)(int32_t)v);
+        if constexpr (kWeighted) {
+            const double ws = __longlong_as_double((long long)atomicExch(reinterpret_cast<unsigned long long *>(&rows.ws[row]), 0ull));
+            if (row >= 1 && row <= p.nbins && ws != 0.0) atomicAdd(&p.wsums[row - 1], ws);
+        }
+    }
+    if (lane == 0) w.ctl()->since_flush = 0u;
+    __syncwarp();
+}
+
 // Keeps the warp's queue filled: takes the next job from the global counter when the current one has been scanned,
 // and bounds the windows of the warp's i-group against the next (up to) kScan j-groups of its job -- two j-tiles,
 // one lane per j-group, fp64 -- queueing the survivors: groups whose window lies wholly out of range are dropped
@@ -933,9 +985,10 @@ __device__ __noinline__ void refill(const WinParams &p, const WarpSm<kWeighted> 
                 return;
             }
             if (lane == 0) {
-                const uint32_t it = job / kGroupsPerTile * h->chunk;
+                const uint32_t it = job / (kGroupsPerTile * h->split) * h->chunk;
                 const int3 cur = p.items[it];
                 c->ig = (int)(job % kGroupsPerTile);
+                c->part = (int)(job / kGroupsPerTile % h->split);
                 c->it = it;
                 c->it_end = it + h->chunk < h->n_items ? it + h->chunk : h->n_items;
                 c->t = 0;
@@ -974,7 +1027,7 @@ __device__ __noinline__ void refill(const WinParams &p, const WarpSm<kWeighted> 
         }
         const int ti = lane < kGroupsPerTile ? ti0 : ti1, tj = lane < kGroupsPerTile ? tj0 : tj1;
         const int g = lane & (kGroupsPerTile - 1);
-        bool live = lane < kScan && ti >= 0;
+        bool live = lane < kScan && ti >= 0 && (g & (int)(h->split - 1u)) == c->part;
         Unit u;
         u.i_first = 0;
         u.j_first = 0;
@@ -1012,6 +1065,12 @@ __device__ __noinline__ void refill(const WinParams &p, const WarpSm<kWeighted> 
                         if (hi == p.nbins && c_lo < edges_sm[p.nbins]) ++hi;
                         chord = hi > lo && c_hi - c_lo < kChordWidth && c_lo > kChordCosMin;
                     }
+                    // The pair cosine is clamped to [-1, 1]: no pair lies before a pole edge e_0 = 1 or beyond e_n = -1, so
+                    // those two edges are in no window (and never tested in fp32: an unclamped c32 marginally outside, or
+                    // vectors a little longer than 1, would be misfiled).
+                    if (lo == 0 && edges_sm[0] >= 1.0) lo = 1;
+                    if (hi == p.nbins + 1 && edges_sm[p.nbins] <= -1.0) hi = p.nbins;
+                    if (hi < lo) hi = lo;
                 };
                 int lo, hi;
                 bool chord;
@@ -1129,7 +1188,7 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const __grid_cons
         for (int s = 0; s < kWStages; ++s) mbar_init(reinterpret_cast<uint64_t *>(w.ptr(8u * (uint32_t)s)), 1);
         c->q_tail = c->n_issued = c->n_done = 0u;
         c->it = c->it_end = 0u;
-        c->t = c->cx = c->cy = c->cz = c->ig = 0;
+        c->t = c->cx = c->cy = c->cz = c->ig = c->part = 0;
         c->no_more = 0;
         c->since_flush = 0u;
         c->tally_m = -1;
@@ -1142,57 +1201,18 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const __grid_cons
         const uint32_t n_items = (uint32_t)(p.counters[kCtrWorkCount] > p.capacity ? p.capacity : p.counters[kCtrWorkCount]);
         uint32_t chunk = (uint32_t)((unsigned long long)n_items * kGroupsPerTile / (64ull * gridDim.x * kWarps));
         chunk = chunk < 1u ? 1u : (chunk > 4u ? 4u : chunk);
+        // few items (small catalogues): a job takes only every split-th j-group of its items' tiles
+        uint32_t split = 1u;
+        while (split < (uint32_t)kGroupsPerTile && (unsigned long long)n_items * kGroupsPerTile * split < 2ull * gridDim.x * kWarps) split *= 2u;
         h->n_items = n_items;
         h->chunk = chunk;
-        h->n_jobs = (n_items + chunk - 1u) / chunk * kGroupsPerTile;
+        h->split = split;
+        h->n_jobs = (n_items + chunk - 1u) / chunk * kGroupsPerTile * split;
     }
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     __syncthreads();
 
     w.tally()[lane] = LaneTally{0u, 0u, 0.0, 0.0};  // this thread's tallies of the rows around the edge WarpCtl::tally_m
-
-    auto flush_tally = [&]() {
-        // the threads' tallies of rows tally_m and tally_m + 1 -> the warp's rows
-        volatile WarpCtl *c = w.ctl();
-        const int tally_m = c->tally_m;
-        if (tally_m >= 0) {
-            const Rows rows = rows_of<kWeighted>(p, w);
-            LaneTally *tl = w.tally() + lane;
-            const LaneTally tally = *tl;
-            *tl = LaneTally{0u, 0u, 0.0, 0.0};
-            const uint32_t c_lo = __reduce_add_sync(0xffffffffu, tally.c_lo), c_hi = __reduce_add_sync(0xffffffffu, tally.c_hi);
-            double w_lo = 0.0, w_hi = 0.0;
-            if constexpr (kWeighted) {
-                w_lo = warp_sum_f64(tally.w_lo);
-                w_hi = warp_sum_f64(tally.w_hi);
-            }
-            if (lane == 0) {
-                rows.template add<kWeighted>(tally_m, c_lo, w_lo);
-                rows.template add<kWeighted>(tally_m + 1, c_hi, w_hi);
-                c->tally_m = -1;
-            }
-            __syncwarp();
-        }
-    };
-    auto flush_rows = [&]() {
-        // this warp's rows -> global (u64 / f64 atomics); the rows restart from zero
-        flush_tally();
-        __syncwarp();
-        const Rows rows = rows_of<kWeighted>(p, w);
-        for (int row = lane; row < rows_n; row += 32) {
-            // (shared rows: other warps add while this one takes the value and leaves zero)
-            const uint32_t v = atomicExch(&rows.cnt[row], 0u);
-            // read as signed: a correction (-1 now, its tally later) may be caught in between; the two's-complement
-            // sum in global memory comes out the same
-            if (row >= 1 && row <= p.nbins && v) atomicAdd(&p.counts[row - 1], (unsigned long long)(long long)(int32_t)v);
-            if constexpr (kWeighted) {
-                const double ws = __longlong_as_double((long long)atomicExch(reinterpret_cast<unsigned long long *>(&rows.ws[row]), 0ull));
-                if (row >= 1 && row <= p.nbins && ws != 0.0) atomicAdd(&p.wsums[row - 1], ws);
-            }
-        }
-        if (lane == 0) w.ctl()->since_flush = 0u;
-        __syncwarp();
-    };
 
     while (true) {
         volatile WarpCtl *c = w.ctl();
@@ -1237,7 +1257,7 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const __grid_cons
         sp.i_first = u->i_first;
         sp.j_first = u->j_first;
         // u32 rows, read as signed when flushed: flush before 2^30 pairs (shared rows take the pairs of all the CTA's warps)
-        if (c->since_flush >= (1u << 30) / (uint32_t)(kGroup * kGroup) / (p.shared_rows ? (uint32_t)kWarps : 1u)) flush_rows();
+        if (c->since_flush >= (1u << 30) / (uint32_t)(kGroup * kGroup) / (p.shared_rows ? (uint32_t)kWarps : 1u)) flush_rows<kWeighted>(p, w);
         const int nsub = u->nsub;
         const bool masked = u->masked != 0;
         uint32_t pairs = 0, pairs_win = 0, pairs_chord = 0;
@@ -1249,7 +1269,7 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const __grid_cons
             sp.wsum = u->wsum[s];
             const bool chord = (u->chord >> s) & 1;
             const int K = r_hi - r_lo;
-            if (masked || K > kMaxPassEdges) {
+            if (masked || (!kWeighted && K > kMaxPassEdges)) {
                 Mask mk;
                 mk.gi = p.n_a - sp.i_first < (uint32_t)kGroup ? p.n_a - sp.i_first : (uint32_t)kGroup;
                 mk.jn = u->jn;
@@ -1262,7 +1282,7 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const __grid_cons
                 // a window inside one row is tested against the edge that bounds the row
                 const int m_edge = K == 1 ? r_lo : (r_lo > p.nbins ? p.nbins : r_lo);
                 if (m_edge != c->tally_m) {
-                    flush_tally();
+                    flush_tally<kWeighted>(p, w);
                     if (lane == 0) c->tally_m = m_edge;
                 }
                 if (lane == 0) c->sub = s;
@@ -1291,7 +1311,7 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const __grid_cons
         __syncwarp();
     }
 
-    flush_rows();
+    flush_rows<kWeighted>(p, w);
     if (lane == 0) {
         volatile WarpCtl *c = w.ctl();
         if (c->n_eval) atomicAdd(&h->stat[kStatEvaluated], c->n_eval);

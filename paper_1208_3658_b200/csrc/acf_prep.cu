@@ -386,7 +386,7 @@ __device__ __forceinline__ void cap_pair_bounds(const double4 a, const double4 b
 // and appends items {ti, first j-tile, number of j-tiles <= kItemTiles}.
 __global__ void __launch_bounds__(256)
 worklist_kernel(const double4 *__restrict__ caps_a, int ti_begin, int ti_end, const double4 *__restrict__ caps_b,
-                int n_tiles_b, int is_auto, int prune, double e_first, double e_last,
+                int n_tiles_b, int is_auto, int prune, int max_len, double e_first, double e_last,
                 int3 *__restrict__ items, uint32_t capacity, unsigned long long *__restrict__ counters)
 {
     extern __shared__ uint32_t keep[];  // bitmap over j tiles
@@ -435,7 +435,7 @@ worklist_kernel(const double4 *__restrict__ caps_a, int ti_begin, int ti_end, co
             int len = 1;
             // the diagonal tile of an auto count is always an item of its own (it runs the i<j variant)
             const bool diag = is_auto && tj == ti;
-            while (!diag && len < kItemTiles && tj + len < n_tiles_b && ((keep[(tj + len) >> 5] >> ((tj + len) & 31)) & 1u)) ++len;
+            while (!diag && len < max_len && tj + len < n_tiles_b && ((keep[(tj + len) >> 5] >> ((tj + len) & 31)) & 1u)) ++len;
             const unsigned long long slot = atomicAdd(&counters[kCtrWorkCount], 1ull);
             if (slot < capacity) items[slot] = make_int3(ti, tj, len);
             tj += len;
@@ -513,8 +513,11 @@ int build_worklist(acf_ctx *ctx, const Prepared &a, int ti_begin, int ti_end, co
     const int n_ti = ti_end - ti_begin;
     if (n_ti <= 0 || b.n_tiles == 0) return ACF_OK;
     const size_t smem = sizeof(uint32_t) * (size_t)((b.n_tiles + 31) / 32);
+    // items of up to kItemTiles j-tiles; shorter ones when the whole call is only a few tile pairs (small catalogues)
+    long long max_len = (long long)n_ti * b.n_tiles / ((long long)ctx->num_sms * 64);
+    max_len = max_len < 1 ? 1 : (max_len > kItemTiles ? kItemTiles : max_len);
     if (smem > 48 * 1024) return fail(ctx, ACF_EINVAL, "catalogue too large for the work-list kernel (%d tiles)", b.n_tiles);
-    worklist_kernel<<<n_ti, 256, smem, ctx->stream>>>(a.caps, ti_begin, ti_end, b.caps, b.n_tiles, is_auto, ctx->opt_prune,
+    worklist_kernel<<<n_ti, 256, smem, ctx->stream>>>(a.caps, ti_begin, ti_end, b.caps, b.n_tiles, is_auto, ctx->opt_prune, (int)max_len,
                                                      e_first, e_last, items, capacity, ctx->d_counters);
     ctx->last.kernel_launches++;
     ACF_CUDA_TRY(ctx, cudaGetLastError());
