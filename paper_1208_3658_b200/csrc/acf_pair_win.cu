@@ -265,6 +265,15 @@ struct Span {
     double wsum;         // sum of the weights of the span's j-points
     uint32_t i_first;    // index in catalogue a of the i-group's first point
     uint32_t j_first;    // index in catalogue b of the staged group's first point
+    uint32_t ipts;       // shared address of the warp's i-points {-x, -y, -z, w}, kGroup float4: thread `lane` reads r * 32 + lane
+    // i-point r of this thread, negated
+    __device__ __forceinline__ float4 ipoint(int r) const
+    {
+        const uint32_t a = ipts + 16u * (uint32_t)(r * 32 + (int)(threadIdx.x & 31u));
+        float4 v;
+        asm volatile("ld.shared.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "r"(a));
+        return v;
+    }
     // point jj of the staged group
     __device__ __forceinline__ float4 point(int jj) const
     {
@@ -302,7 +311,12 @@ __device__ __noinline__ void fixup_chunk(const WinParams &p, const Tables tb, co
     const int lane = threadIdx.x & 31;
     float4 pi[kR];
 #pragma unroll
-    for (int r = 0; r < kR; ++r) pi[r] = p.pts_a[sp.i_first + r * 32 + lane];  // the array is padded to a whole tile
+    for (int r = 0; r < kR; ++r) {
+        pi[r] = sp.ipoint(r);  // negated in the stash
+        pi[r].x = -pi[r].x;
+        pi[r].y = -pi[r].y;
+        pi[r].z = -pi[r].z;
+    }
     for (int i = 0; i < kChunk * kR; ++i) dt[i] = 0.0;
     for (int i = 0; i < kChunk; ++i) dn[i] = 0;
     float e32, dl[kChunk];
@@ -459,13 +473,15 @@ __device__ __forceinline__ uint32_t pair_loop(const uint32_t grp2, const uint32_
     return amb_steps;
 }
 
-// Edges m_a .. m_a + K - 1 against one span of staged j-points and this thread's kR i-points.
-// A chunk fills rows m_a .. m_a + K - 1 (and m_a + K if it is the last of its window); the tallies above
-// its last edge go to the next chunk through `carry`.
+// Edges m_a .. m_a + n_real - 1 (n_real <= K) against one span of staged j-points and this thread's kR i-points.
+// A chunk fills rows m_a .. m_a + n_real - 1 (and m_a + n_real if it is the last of its window); the tallies above
+// its last edge go to the next chunk through `carry`.  A chunk of fewer than K edges repeats its last edge: the
+// repeated tallies are equal, the rows between them get nothing, and one compiled loop serves every window
+// (the code of the rare shapes must not crowd the instruction cache of the common one).
 template <int K, bool kWeighted, bool kChord>
 __device__ __forceinline__ void window_chunk(const WinParams &p, const Tables tb, const Rows rows, const Span sp,
                                              const float (&nx)[kR], const float (&ny)[kR], const float (&nz)[kR],
-                                             const float *wi_of, const int wi_stride, const int m_a, const bool first, const bool last,
+                                             const float *wi_of, const int wi_stride, const int m_a, const int n_real, const bool first, const bool last,
                                              unsigned long long *stat, Carry *carry)
 {
     // wi_of: the weights of this thread's i-points, wi_of[r * wi_stride]
@@ -478,15 +494,19 @@ __device__ __forceinline__ void window_chunk(const WinParams &p, const Tables tb
         G = K == 1 ? tb.gs1(m_a) : tb.gsk(m_a);
 #pragma unroll
         for (int q = 1; q < K; ++q) {
-            dl[q] = __fsub_rn(tb.sneg(m_a + q), e32);
-            G = fmaxf(G, tb.gsk(m_a + q));
+            const int mq = m_a + (q < n_real ? q : n_real - 1);
+            dl[q] = __fsub_rn(tb.sneg(mq), e32);
+            G = fmaxf(G, tb.gsk(mq));
         }
     } else {
         const double e0 = tb.edge(m_a);
         e32 = edge32(e0);
         G = K == 1 ? kGuard1 : kGuardK;
 #pragma unroll
-        for (int q = 1; q < K; ++q) dl[q] = tb.edge(m_a + q) <= -1.0 ? -8.0f : (float)(tb.edge(m_a + q) - e0);
+        for (int q = 1; q < K; ++q) {
+            const double eq = tb.edge(m_a + (q < n_real ? q : n_real - 1));
+            dl[q] = eq <= -1.0 ? -8.0f : (float)(eq - e0);
+        }
     }
     double t[K][kR];     // weighted: 2^-7 * sum of v_j over the pairs above edge q, per i-point
     uint32_t nb[K];      // unweighted: pairs not above edge q
@@ -497,14 +517,15 @@ __device__ __forceinline__ void window_chunk(const WinParams &p, const Tables tb
         // exact corrections, applied to the (exact) accumulators before anything is read from them
         double dt[kChunk * kR];
         int dn[kChunk];
-        fixup_chunk<kWeighted, kChord>(p, tb, sp, amb_steps, K, m_a, G, stat, dt, dn);
+        fixup_chunk<kWeighted, kChord>(p, tb, sp, amb_steps, n_real, m_a, G, stat, dt, dn);
 #pragma unroll
         for (int q = 0; q < K; ++q) {
+            const int qq = q < n_real ? q : n_real - 1;  // a repeated edge gets the corrections of the edge it repeats
             if constexpr (kWeighted) {
 #pragma unroll
-                for (int r = 0; r < kR; ++r) t[q][r] += dt[q * kR + r];
+                for (int r = 0; r < kR; ++r) t[q][r] += dt[qq * kR + r];
             } else {
-                nb[q] += (uint32_t)dn[q];
+                nb[q] += (uint32_t)dn[qq];
             }
         }
     }
@@ -557,7 +578,7 @@ __device__ __forceinline__ void window_chunk(const WinParams &p, const Tables tb
         if (rc == 0u) rw = 0.0;  // no pair of this thread in the row: not even a rounding residue
         const uint32_t rc_warp = __reduce_add_sync(0xffffffffu, rc);
         if constexpr (kWeighted) rw = warp_sum_f64(rw);
-        if (lane == 0) rows.template add<kWeighted>(m_a + q, rc_warp, rw);
+        if (lane == 0) rows.template add<kWeighted>(m_a + (q < n_real ? q : n_real), rc_warp, rw);
     }
     if (!last) {
         carry->c = c_prev;
@@ -578,24 +599,22 @@ __device__ __noinline__ void window_multi(const WinParams &p, const Tables tb, c
     float nx[kR], ny[kR], nz[kR];
 #pragma unroll
     for (int r = 0; r < kR; ++r) {
-        const float4 v = p.pts_a[sp.i_first + r * 32 + lane];  // the array is padded to a whole tile
-        nx[r] = -v.x;
-        ny[r] = -v.y;
-        nz[r] = -v.z;
+        const float4 v = sp.ipoint(r);
+        nx[r] = v.x;
+        ny[r] = v.y;
+        nz[r] = v.z;
     }
-    const float *wi = &p.pts_a[sp.i_first + lane].w;  // the weight of i-point r: wi[r * 128] (float4 records, 32 apart)
-    static_assert(kChunk == 3, "the dispatch below spells the chunk sizes out");
+    // the weight of i-point r: wi[r * 128] (float4 records, 32 apart)
+    const float *wi = reinterpret_cast<const float *>(__cvta_shared_to_generic(sp.ipts)) + 4 * lane + 3;
     Carry carry;
     carry.c = 0u;
 #pragma unroll
     for (int r = 0; r < kR; ++r) carry.s[r] = 0.0;
     int m = r_lo;  // edges below m are done
     while (m < r_hi) {
-        // passes of three edges, the last one or two passes of two (4 = 2 + 2, 5 = 3 + 2, 7 = 3 + 2 + 2): no pass of one
         const int left = r_hi - m;
-        const int take = (left == 2 || left == 4) ? 2 : 3;
-        if (take == 2) window_chunk<2, kWeighted, kChord>(p, tb, rows, sp, nx, ny, nz, wi, 128, m, m == r_lo, left == 2, stat, &carry);
-        else window_chunk<3, kWeighted, kChord>(p, tb, rows, sp, nx, ny, nz, wi, 128, m, m == r_lo, left == 3, stat, &carry);
+        const int take = left < kChunk ? left : kChunk;
+        window_chunk<kChunk, kWeighted, kChord>(p, tb, rows, sp, nx, ny, nz, wi, 128, m, take, m == r_lo, left <= kChunk, stat, &carry);
         m += take;
     }
 }
@@ -612,7 +631,12 @@ __device__ __noinline__ void general_span(const WinParams &p, const Tables tb, c
     const int lane = threadIdx.x & 31;
     float4 pi[kR];
 #pragma unroll
-    for (int r = 0; r < kR; ++r) pi[r] = p.pts_a[sp.i_first + r * 32 + lane];
+    for (int r = 0; r < kR; ++r) {
+        pi[r] = sp.ipoint(r);  // negated in the stash
+        pi[r].x = -pi[r].x;
+        pi[r].y = -pi[r].y;
+        pi[r].z = -pi[r].z;
+    }
     const uint32_t cells = tb.cells();
     constexpr int kShift = 23 - kCellBits;
     constexpr int kKey0 = (127 + kCellExpLo) << kCellBits;
@@ -817,19 +841,7 @@ __device__ __forceinline__ void single_edge_span(const WinParams &p, const WarpS
         volatile WarpCtl *c = w.ctl();
         const uint32_t n_done = c->n_done;
         const Unit *u = &w.queue()[n_done % kQueue];
-        const uint32_t i_first = u->i_first;
-        float4 *ip = w.ipts();
-        if (c->loaded_first != i_first) {
-            // another i-group: its points, negated, into the warp's shared memory (the array is padded to a whole tile)
-            __syncwarp();
-#pragma unroll
-            for (int r = 0; r < kR; ++r) {
-                const float4 v = p.pts_a[i_first + r * 32 + lane];
-                ip[r * 32 + lane] = make_float4(-v.x, -v.y, -v.z, v.w);
-            }
-            if (lane == 0) c->loaded_first = i_first;
-            __syncwarp();
-        }
+        const float4 *ip = w.ipts();  // (the kernel has seen to it that they are the unit's)
 #pragma unroll
         for (int r = 0; r < kR; ++r) {
             const float4 v = ip[r * 32 + lane];
@@ -870,6 +882,7 @@ __device__ __forceinline__ void single_edge_span(const WinParams &p, const WarpS
         sp.wsum = 0.0;
         sp.i_first = u->i_first;
         sp.j_first = u->j_first;
+        sp.ipts = smem_u32(w.ipts());
         double dt[kChunk * kR];
         int dn[kChunk];
         fixup_chunk<kWeighted, kChord>(p, tb, sp, amb_steps, 1, c->tally_m, G, h->stat, dt, dn);
@@ -906,6 +919,15 @@ __device__ __forceinline__ void single_edge_span(const WinParams &p, const WarpS
         if (c_lo != 0u) tally->w_lo += w_lo;  // no pair of this thread in the row: not even a rounding residue
         if (c_hi != 0u) tally->w_hi += w_hi;
     }
+}
+
+// The chord-domain form of the kernel's own loop, out of line: a call is either in the regime of one form or of the
+// other (wide windows on the cosine, arc-minute windows on the chord), and the form it does not use should not
+// sit in the instruction cache between the pieces of the one it does.
+template <bool kWeighted>
+__device__ __noinline__ void single_edge_span_chord(const WinParams &p, const WarpSm<kWeighted> w)
+{
+    single_edge_span<kWeighted, true>(p, w);
 }
 
 // The threads' tallies of the rows around edge WarpCtl::tally_m -> the warp's rows.  (Not inlined, like
@@ -1106,6 +1128,13 @@ __device__ __noinline__ void refill(const WinParams &p, const WarpSm<kWeighted> 
                             u.chord |= (sch ? 1 : 0) << s;
                             u.wsum[s] = cs.wsum;
                         }
+                        // the same window four times over: one span after all (one prologue, one epilogue)
+                        if (u.lo[0] >= 0 && u.lo[1] == u.lo[0] && u.lo[2] == u.lo[0] && u.lo[3] == u.lo[0] && u.hi[1] == u.hi[0] &&
+                            u.hi[2] == u.hi[0] && u.hi[3] == u.hi[0] && (u.chord == 0 || u.chord == 15)) {
+                            u.nsub = 1;
+                            u.chord &= 1;
+                            u.wsum[0] = cb.wsum;
+                        }
                     }
                 }
             }
@@ -1256,6 +1285,18 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const __grid_cons
         sp.vgrp = sp.grp2 + (uint32_t)kGroupBytes;
         sp.i_first = u->i_first;
         sp.j_first = u->j_first;
+        sp.ipts = smem_u32(w.ipts());
+        if (c->loaded_first != sp.i_first) {
+            // another i-group: its points, negated, into the warp's shared memory (the array is padded to a whole tile)
+            float4 *ip = w.ipts();
+#pragma unroll
+            for (int r = 0; r < kR; ++r) {
+                const float4 v = p.pts_a[sp.i_first + r * 32 + lane];
+                ip[r * 32 + lane] = make_float4(-v.x, -v.y, -v.z, v.w);
+            }
+            if (lane == 0) c->loaded_first = sp.i_first;
+            __syncwarp();
+        }
         // u32 rows, read as signed when flushed: flush before 2^30 pairs (shared rows take the pairs of all the CTA's warps)
         if (c->since_flush >= (1u << 30) / (uint32_t)(kGroup * kGroup) / (p.shared_rows ? (uint32_t)kWarps : 1u)) flush_rows<kWeighted>(p, w);
         const int nsub = u->nsub;
@@ -1287,7 +1328,7 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const __grid_cons
                 }
                 if (lane == 0) c->sub = s;
                 __syncwarp();
-                if (chord) single_edge_span<kWeighted, true>(p, w);
+                if (chord) single_edge_span_chord<kWeighted>(p, w);
                 else single_edge_span<kWeighted, false>(p, w);
                 pairs += (uint32_t)(sp.jj1 - sp.jj0) * kGroup;
                 pairs_win += (uint32_t)(sp.jj1 - sp.jj0) * kGroup;
