@@ -705,7 +705,7 @@ int count_prepared(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_au
     // i-tiles are handed out in batches so that the item buffer stays bounded
     // (worst case one item per surviving j-tile: survivors may alternate with pruned tiles)
     const uint64_t items_per_ti = (uint64_t)b.n_tiles;
-    const uint64_t max_items = 8u << 20;
+    const uint64_t max_items = 64u << 20;  // 768 MB of items at most (8 M x 8 M points: 61 M tile pairs, one launch)
     int ti_per_batch = (int)(max_items / items_per_ti);
     if (ti_per_batch < 1) ti_per_batch = 1;
     if (ti_per_batch > a.n_tiles) ti_per_batch = a.n_tiles;
