@@ -53,7 +53,8 @@ extern "C" {
 
 #define ACF_MAX_BINS 1024
 
-typedef struct acf_ctx acf_ctx; /* opaque; library-owned */
+typedef struct acf_ctx acf_ctx;         /* opaque; library-owned */
+typedef struct acf_catalog acf_catalog; /* opaque; a catalogue prepared on the device (acf_prepare) */
 
 /* Options for acf_set_option. */
 enum {
@@ -140,6 +141,8 @@ int acf_radec_to_xyz(const double *ra_deg, const double *dec_deg, size_t n, doub
  *              0 counts all n_a*n_b pairs.
  *   d_counts : DEVICE, nbins uint64, overwritten.
  * n = 0 (or n = 1 in auto mode) gives all-zero counts and ACF_OK.
+ * The call prepares both catalogues (sort, caps) every time and waits on the host for the validation verdict while the
+ * pair kernel is already running; counts that share catalogues are better made on handles (acf_prepare).
  */
 int acf_pair_count(acf_ctx *ctx, const double *d_a, size_t n_a, const double *d_b, size_t n_b,
                    const double *cos_edges, int nbins, int is_auto, uint64_t *d_counts);
@@ -165,6 +168,38 @@ int acf_pair_count_rows(acf_ctx *ctx, const double *d_a, const float *d_wa, size
                         size_t i_end, const double *d_b, const float *d_wb, size_t n_b,
                         const double *cos_edges, int nbins, int is_auto, uint64_t *d_counts,
                         double *d_wsums);
+
+/*
+ * Prepared catalogues (sect. 2.1: the coordinates are copied to the device once and many
+ * sub-matrix kernels are launched on them).  acf_prepare validates a catalogue (as acf_pair_count does), sorts it
+ * along a space-filling curve and builds its fp32 copies and bounding caps ONCE; any number of counts can then be
+ * made on the handle -- DD, DR and RR of an estimate prepare each catalogue once instead of twice, a jackknife
+ * prepares every region once -- and those counts are truly asynchronous: the validation verdict was fetched by
+ * acf_prepare, so acf_pair_count_prepared never waits on the host.
+ *   d_xyz, d_w : DEVICE, as for acf_pair_count_weighted (d_w NULL: unit weights).  The handle REFERS to these
+ *                buffers (the exact re-evaluation of near-edge pairs reads the caller's doubles): they must stay
+ *                allocated and unchanged until acf_release.
+ *   [i_begin, i_end) : the rows that make up the catalogue (acf_prepare: all n of them)
+ * acf_prepare* synchronise the stream once (the verdict); ACF_EINVAL for non-unit / non-finite points or bad weights.
+ * acf_release frees the handle's device memory after the stream has drained; NULL is a no-op.  acf_destroy frees
+ * the handles that are still alive.
+ */
+int acf_prepare(acf_ctx *ctx, const double *d_xyz, const float *d_w, size_t n, acf_catalog **out);
+int acf_prepare_rows(acf_ctx *ctx, const double *d_xyz, const float *d_w, size_t n, size_t i_begin, size_t i_end,
+                     acf_catalog **out);
+void acf_release(acf_ctx *ctx, acf_catalog *cat);
+
+/*
+ * Pair-count histogram of prepared catalogues: b == NULL (or b == a) counts the unordered pairs of a (DD, RR),
+ * otherwise all pairs of a x b (DR).  Weighted sums are produced iff d_wsums != NULL (both catalogues must then
+ * have been prepared with weights).  Asynchronous on the context's stream; d_counts / d_wsums are overwritten.
+ *   part, n_parts : the call counts slice `part` of `n_parts` disjoint slices of the pair matrix (rows of a in the
+ *                   order of the prepared catalogue, dealt out tile by tile: balanced whatever is pruned).  The
+ *                   histograms of the n_parts slices add up to the whole count: this is the unit of work of a job
+ *                   sharded over GPUs, every rank holding both catalogues.  0, 1: the whole count.
+ */
+int acf_pair_count_prepared(acf_ctx *ctx, const acf_catalog *a, const acf_catalog *b, const double *cos_edges, int nbins,
+                            int part, int n_parts, uint64_t *d_counts, double *d_wsums);
 
 /*
  * Landy-Szalay estimator, Eq. 2, pure host, O(nbins):

@@ -26,6 +26,7 @@ EXPORTS = [
     "acf_create", "acf_destroy", "acf_last_error", "acf_set_option", "acf_set_stream", "acf_radec_to_xyz",
     "acf_pair_count", "acf_pair_count_weighted", "acf_pair_count_rows", "acf_wtheta", "acf_wtheta_weighted",
     "acf_estimator", "acf_theta_edges", "acf_cos_edges", "acf_jackknife", "acf_correlate_host", "acf_get_stats", "acf_version",
+    "acf_prepare", "acf_prepare_rows", "acf_release", "acf_pair_count_prepared",
 ]
 
 
@@ -81,6 +82,11 @@ def load_library(build_if_missing: bool = True):
     lib.acf_cos_edges.argtypes = [vp, i32, vp]
     lib.acf_jackknife.argtypes = [vp, vp, sz, vp, vp, sz, vp, i32, vp, i32, i32, vp, vp, vp]
     lib.acf_correlate_host.argtypes = [vp, vp, vp, vp, sz, vp, vp, vp, sz, vp, i32, vp, vp, vp, vp, vp, vp, vp]
+    lib.acf_prepare.argtypes = [vp, vp, vp, sz, ctypes.POINTER(vp)]
+    lib.acf_prepare_rows.argtypes = [vp, vp, vp, sz, sz, sz, ctypes.POINTER(vp)]
+    lib.acf_release.argtypes = [vp, vp]
+    lib.acf_release.restype = None
+    lib.acf_pair_count_prepared.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp, vp]
     lib.acf_get_stats.argtypes = [vp, ctypes.POINTER(acf_stats)]
     lib.acf_version.restype = ctypes.c_char_p
     for name in EXPORTS:
@@ -123,7 +129,9 @@ def acf_version() -> str:
 
 
 def acf_create(device: int = 0, cuda_stream: int | None = None):
-    """-> opaque context handle.  cuda_stream: a raw cudaStream_t (int) or None for torch's current stream."""
+    """-> opaque context handle.  cuda_stream: a raw cudaStream_t (int) or None for torch's current stream AT THIS
+    MOMENT: the context stays bound to that stream (acf_set_stream changes it); tensors produced on another
+    stream must be synchronised with it by the caller."""
     import torch
     lib = load_library()
     if not torch.cuda.is_available():
@@ -202,6 +210,65 @@ def acf_pair_count_rows(ctx, d_a, d_wa, i_begin, i_end, d_b, d_wb, cos_edges, is
     return (d_counts, d_wsums) if weighted else d_counts
 
 
+class Catalog:
+    """A prepared catalogue (acf_prepare).  Keeps the tensors the handle refers to alive."""
+
+    def __init__(self, ctx, handle, d_xyz, d_w, n):
+        self.ctx, self.handle, self.d_xyz, self.d_w, self.n = ctx, handle, d_xyz, d_w, n
+
+
+def acf_prepare(ctx, d_xyz, d_w=None, rows=None) -> Catalog:
+    """DEVICE tensors in; validates, sorts and builds the caps once.  rows=(i_begin, i_end): acf_prepare_rows."""
+    import torch
+    a, pa = _dev(d_xyz, torch.float64, "d_xyz")
+    n = _n_points(a)
+    w, pw = _dev(d_w, torch.float32, "d_w")
+    if w is not None and w.numel() != n:
+        raise ValueError("weight length mismatch")
+    h = ctypes.c_void_p()
+    if rows is None:
+        rc = load_library().acf_prepare(ctx, pa, pw, n, ctypes.byref(h))
+        cnt = n
+    else:
+        rc = load_library().acf_prepare_rows(ctx, pa, pw, n, int(rows[0]), int(rows[1]), ctypes.byref(h))
+        cnt = int(rows[1]) - int(rows[0])
+    if rc != ACF_OK:
+        _raise(ctx, rc)
+    return Catalog(ctx, h, a, w, cnt)
+
+
+def acf_prepare_rows(ctx, d_xyz, d_w, i_begin, i_end) -> Catalog:
+    return acf_prepare(ctx, d_xyz, d_w, rows=(i_begin, i_end))
+
+
+def acf_release(ctx, cat: Catalog) -> None:
+    if cat is not None and cat.handle is not None:
+        load_library().acf_release(ctx, cat.handle)
+        cat.handle = None
+
+
+def acf_pair_count_prepared(ctx, a: Catalog, b: Catalog | None, cos_edges, part: int = 0, n_parts: int = 1, weighted=None,
+                            d_counts=None, d_wsums=None):
+    """Counts on prepared catalogues; b None: auto-count of a.  Asynchronous.  weighted defaults to "a has weights".
+    -> d_counts, or (d_counts, d_wsums)."""
+    import torch
+    e, pe = _host(cos_edges, np.float64)
+    nbins = e.size - 1
+    if weighted is None:
+        weighted = a.d_w is not None and (b is None or b.d_w is not None)
+    dev = a.d_xyz.device
+    if d_counts is None:
+        d_counts = torch.empty(max(nbins, 1), dtype=torch.int64, device=dev)
+    if weighted and d_wsums is None:
+        d_wsums = torch.empty(max(nbins, 1), dtype=torch.float64, device=dev)
+    _, pc = _dev(d_counts, torch.int64, "d_counts")
+    _, pw = _dev(d_wsums, torch.float64, "d_wsums") if weighted else (None, 0)
+    rc = load_library().acf_pair_count_prepared(ctx, a.handle, None if b is None else b.handle, pe, nbins, int(part), int(n_parts), pc, pw)
+    if rc != ACF_OK:
+        _raise(ctx, rc)
+    return (d_counts, d_wsums) if weighted else d_counts
+
+
 def acf_pair_count(ctx, d_a, d_b, cos_edges, is_auto, d_counts=None):
     import torch
     a, pa = _dev(d_a, torch.float64, "d_a")
@@ -272,6 +339,9 @@ def acf_cos_edges(theta_deg) -> np.ndarray:
 def acf_jackknife(ctx, d_xyz_d, off_d, d_xyz_r, off_r, cos_edges, estimator: int = ACF_EST_LANDY_SZALAY) -> dict:
     """Delete-one jackknife over regions; the catalogues (device tensors) are ordered by region and
     off_d / off_r give each region's row range.  -> {"w": ..., "w_jk": (regions, nbins), "cov": (nbins, nbins)}."""
+    import torch
+    d_xyz_d, _ = _dev(d_xyz_d, torch.float64, "d_xyz_d")
+    d_xyz_r, _ = _dev(d_xyz_r, torch.float64, "d_xyz_r")
     off_d = np.ascontiguousarray(off_d, dtype=np.uint64)
     off_r = np.ascontiguousarray(off_r, dtype=np.uint64)
     edges, pe = _host(cos_edges, np.float64)

@@ -60,14 +60,18 @@ extern "C" int acf_create(acf_ctx **out, int device, void *cuda_stream)
     bool ok = cudaEventCreate(&ctx->ev_start) == cudaSuccess && cudaEventCreate(&ctx->ev_stop) == cudaSuccess &&
               cudaEventCreateWithFlags(&ctx->ev_flag, cudaEventDisableTiming) == cudaSuccess &&
               cudaEventCreate(&ctx->ev_k0) == cudaSuccess && cudaEventCreate(&ctx->ev_k1) == cudaSuccess &&
+              cudaEventCreateWithFlags(&ctx->ev_tables, cudaEventDisableTiming) == cudaSuccess &&
+              cudaEventCreateWithFlags(&ctx->ev_copy, cudaEventDisableTiming) == cudaSuccess &&
+              cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking) == cudaSuccess &&
               cudaMalloc(&ctx->d_counters, sizeof(unsigned long long) * acf::kNumCounters) == cudaSuccess &&
-              cudaHostAlloc(&ctx->h_counters, sizeof(unsigned long long) * acf::kNumCounters, cudaHostAllocDefault) == cudaSuccess;
+              cudaHostAlloc(&ctx->h_counters, sizeof(unsigned long long) * (acf::kNumCounters + 2), cudaHostAllocDefault) == cudaSuccess;
     if (!ok) {
         e = cudaGetLastError();
         acf_destroy(ctx);
         return create_fail(ACF_ECUDA, "context allocation failed", e);
     }
-    memset(ctx->h_counters, 0, sizeof(unsigned long long) * acf::kNumCounters);
+    memset(ctx->h_counters, 0, sizeof(unsigned long long) * (acf::kNumCounters + 2));
+    ctx->h_verdict = reinterpret_cast<int *>(ctx->h_counters + acf::kNumCounters);
     g_create_error[0] = 0;
     *out = ctx;
     return ACF_OK;
@@ -78,22 +82,19 @@ extern "C" void acf_destroy(acf_ctx *ctx)
     if (!ctx) return;
     cudaSetDevice(ctx->device);
     cudaStreamSynchronize(ctx->stream);
+    if (ctx->copy_stream) cudaStreamSynchronize(ctx->copy_stream);
+    while (ctx->catalogs) acf_release(ctx, ctx->catalogs);
     ctx->s_edges.release();
-    for (int i = 0; i < 2; ++i) {
-        ctx->s_pts[i].release();
-        ctx->s_perm[i].release();
-        ctx->s_keys[i].release();
-        ctx->s_caps[i].release();
-        ctx->s_gcaps[i].release();
-        ctx->s_scaps[i].release();
-        ctx->s_pts2[i].release();
-        ctx->s_vj[i].release();
-        ctx->s_pack[i].release();
-    }
+    for (int i = 0; i < 2; ++i) ctx->cat[i].release();
+    ctx->s_keys.release();
     ctx->s_work.release();
     ctx->s_misc.release();
     for (auto &s : ctx->s_host_stage) s.release();
     if (ctx->h_stage) cudaFreeHost(ctx->h_stage);
+    if (ctx->h_tables) cudaFreeHost(ctx->h_tables);
+    if (ctx->ev_tables) cudaEventDestroy(ctx->ev_tables);
+    if (ctx->ev_copy) cudaEventDestroy(ctx->ev_copy);
+    if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
     if (ctx->d_counters) cudaFree(ctx->d_counters);
     if (ctx->h_counters) cudaFreeHost(ctx->h_counters);
     if (ctx->ev_start) cudaEventDestroy(ctx->ev_start);
@@ -178,37 +179,69 @@ extern "C" int acf_pair_count_rows(acf_ctx *ctx, const double *d_a, const float 
     ctx->stats_pending = true;
 
     const bool empty = i_begin == i_end || n_b == 0 || (is_auto && n_a < 2);
-    if (!empty) {
-        ACF_CUDA_TRY(ctx, acf::launch_validate(ctx, d_a, d_wa, n_a));
-        if (!is_auto) ACF_CUDA_TRY(ctx, acf::launch_validate(ctx, d_b, d_wb, n_b));
-        ACF_CUDA_TRY(ctx, cudaMemcpyAsync(&ctx->h_counters[acf::kCtrBadInput], &ctx->d_counters[acf::kCtrBadInput],
-                                          sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+    if (!empty && ctx->opt_kernel == ACF_KERNEL_FP64) {
+        // the reference kernel: validation into the slot's PackInfo, then the definition for every pair
+        acf::Prepared a, b;
+        for (int k = 0; k < 2; ++k) {
+            ACF_CUDA_TRY(ctx, ctx->cat[k].pack.reserve(64));
+            ACF_CUDA_TRY(ctx, cudaMemsetAsync(ctx->cat[k].pack.ptr, 0, 64, st));
+        }
+        a.pack = ctx->cat[0].pack.as<acf::PackInfo>();
+        b.pack = ctx->cat[1].pack.as<acf::PackInfo>();
+        ACF_CUDA_TRY(ctx, acf::launch_validate(ctx, d_a, n_a, 0, n_a, d_wa, a.pack));
+        if (!is_auto) ACF_CUDA_TRY(ctx, acf::launch_validate(ctx, d_b, n_b, 0, n_b, d_wb, b.pack));
+        ACF_CUDA_TRY(ctx, cudaMemcpyAsync(&ctx->h_verdict[0], &a.pack->bad, sizeof(int), cudaMemcpyDeviceToHost, st));
+        ACF_CUDA_TRY(ctx, cudaMemcpyAsync(&ctx->h_verdict[1], &b.pack->bad, sizeof(int), cudaMemcpyDeviceToHost, st));
         ACF_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_flag, st));
-
-        if (ctx->opt_kernel != ACF_KERNEL_FP64) {
-            int rc = acf::run_pair_count_fast(ctx, d_a, d_wa, n_a, i_begin, i_end, d_b, d_wb, n_b, cos_edges, nbins,
-                                              is_auto, reinterpret_cast<unsigned long long *>(d_counts), d_wsums);
-            if (rc != ACF_OK) return rc;
-        } else {
+        ACF_CUDA_TRY(ctx, cudaEventSynchronize(ctx->ev_flag));  // (this kernel indexes nothing by the data, but a refused call must count nothing)
+        if (ctx->h_verdict[0] == 0 && ctx->h_verdict[1] == 0) {
             ACF_CUDA_TRY(ctx, ctx->s_edges.reserve(sizeof(double) * (size_t)(nbins + 1)));
             ACF_CUDA_TRY(ctx, cudaMemcpyAsync(ctx->s_edges.ptr, cos_edges, sizeof(double) * (size_t)(nbins + 1), cudaMemcpyHostToDevice, st));
             ACF_CUDA_TRY(ctx, acf::launch_pair_count_fp64(ctx, d_a, d_wa, n_a, i_begin, i_end, d_b, d_wb, n_b,
                                                           ctx->s_edges.as<double>(), nbins, is_auto,
                                                           reinterpret_cast<unsigned long long *>(d_counts), d_wsums));
+            ACF_CUDA_TRY(ctx, cudaStreamSynchronize(st));  // (cos_edges was copied from the caller's pageable array)
         }
+    } else if (!empty) {
+        // prepare what the call pairs -- rows [i_begin, i_end) of a as a catalogue of their own; for an auto-count
+        // the rows after them as the second one -- and count; the verdicts of the validations travel behind
+        acf::Prepared a, b;
+        unsigned long long *cnt = reinterpret_cast<unsigned long long *>(d_counts);
+        int rc = acf::prepare_catalogue(ctx, ctx->cat[0], d_a, n_a, i_begin, i_end - i_begin, d_wa, &a);
+        if (rc != ACF_OK) return rc;
+        ACF_CUDA_TRY(ctx, cudaMemcpyAsync(&ctx->h_verdict[0], &a.pack->bad, sizeof(int), cudaMemcpyDeviceToHost, st));
+        ctx->h_verdict[1] = 0;
+        if (is_auto) {
+            if (i_end < n_a) {
+                rc = acf::prepare_catalogue(ctx, ctx->cat[1], d_a, n_a, i_end, n_a - i_end, d_wa, &b);
+                if (rc != ACF_OK) return rc;
+                ACF_CUDA_TRY(ctx, cudaMemcpyAsync(&ctx->h_verdict[1], &b.pack->bad, sizeof(int), cudaMemcpyDeviceToHost, st));
+            }
+            ACF_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_flag, st));
+            rc = acf::count_prepared_part(ctx, a, a, 1, cos_edges, nbins, 0, 1, cnt, d_wsums);
+            if (rc == ACF_OK && i_end < n_a) rc = acf::count_prepared_part(ctx, a, b, 0, cos_edges, nbins, 0, 1, cnt, d_wsums);
+        } else {
+            rc = acf::prepare_catalogue(ctx, ctx->cat[1], d_b, n_b, 0, n_b, d_wb, &b);
+            if (rc != ACF_OK) return rc;
+            ACF_CUDA_TRY(ctx, cudaMemcpyAsync(&ctx->h_verdict[1], &b.pack->bad, sizeof(int), cudaMemcpyDeviceToHost, st));
+            ACF_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_flag, st));
+            rc = acf::count_prepared_part(ctx, a, b, 0, cos_edges, nbins, 0, 1, cnt, d_wsums);
+        }
+        if (rc != ACF_OK) return rc;
     }
     ACF_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_stop, st));
 
     if (!empty) {
-        // wait for the validation verdict only (the pair kernel keeps running asynchronously)
+        // wait for the validation verdict only (the pair kernel keeps running asynchronously; it has seen the same
+        // verdict on the device and counts nothing if it is bad)
         ACF_CUDA_TRY(ctx, cudaEventSynchronize(ctx->ev_flag));
-        if (ctx->h_counters[acf::kCtrBadInput] != 0) {
+        const long long bad = (long long)ctx->h_verdict[0] + ctx->h_verdict[1];
+        if (bad != 0) {
             cudaStreamSynchronize(st);
             cudaMemsetAsync(d_counts, 0, sizeof(uint64_t) * (size_t)nbins, st);
             if (weighted) cudaMemsetAsync(d_wsums, 0, sizeof(double) * (size_t)nbins, st);
             cudaStreamSynchronize(st);
-            return acf::fail(ctx, ACF_EINVAL, "%llu input points are not finite unit vectors (|r^2 - 1| <= 1e-6) or carry a negative / non-finite weight",
-                             ctx->h_counters[acf::kCtrBadInput]);
+            return acf::fail(ctx, ACF_EINVAL, "%lld input points are not finite unit vectors (|r^2 - 1| <= 1e-6) or carry a negative / non-finite weight", bad);
         }
     }
     return ACF_OK;
@@ -253,9 +286,100 @@ extern "C" int acf_get_stats(acf_ctx *ctx, acf_stats *out)
     return ACF_OK;
 }
 
-// Delete-one jackknife (include/acf.h).  Pairs with a point in region k, for a catalogue ordered by region:
-// rows k of the auto-count (pairs inside k and from k to the regions after it) plus the rows before k
-// against region k.  The cross-count loses D_k x R, D x R_k and gets D_k x R_k back.
+// ---- prepared catalogues -------------------------------------------------------------------------------------------
+extern "C" int acf_prepare_rows(acf_ctx *ctx, const double *d_xyz, const float *d_w, size_t n, size_t i_begin, size_t i_end,
+                                acf_catalog **out)
+{
+    if (!ctx) return ACF_EINVAL;
+    ctx->err[0] = 0;
+    if (!out) return acf::fail(ctx, ACF_EINVAL, "out is NULL");
+    *out = nullptr;
+    if (n && !d_xyz) return acf::fail(ctx, ACF_EINVAL, "catalogue pointer is NULL");
+    if (i_begin > i_end || i_end > n) return acf::fail(ctx, ACF_EINVAL, "row range [%zu, %zu) outside [0, %zu]", i_begin, i_end, n);
+    if (n >= (size_t(1) << 31)) return acf::fail(ctx, ACF_EINVAL, "catalogues are limited to 2^31-1 points");
+    ACF_CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    acf_catalog *cat = new (std::nothrow) acf_catalog();
+    if (!cat) return acf::fail(ctx, ACF_ENOMEM, "out of host memory");
+    cat->ctx = ctx;
+    cat->weighted = d_w != nullptr;
+    int rc = acf::prepare_catalogue(ctx, cat->buf, d_xyz, n, i_begin, i_end - i_begin, d_w, &cat->p);
+    if (rc == ACF_OK) {
+        cudaError_t e = cudaMemcpyAsync(&ctx->h_verdict[0], &cat->p.pack->bad, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+        if (e != cudaSuccess) rc = acf::fail(ctx, ACF_ECUDA, "acf_prepare: %s", cudaGetErrorString(e));
+        else if (ctx->h_verdict[0] != 0)
+            rc = acf::fail(ctx, ACF_EINVAL, "%d input points are not finite unit vectors (|r^2 - 1| <= 1e-6) or carry a negative / non-finite weight",
+                           ctx->h_verdict[0]);
+    }
+    if (rc != ACF_OK) {
+        cudaStreamSynchronize(ctx->stream);
+        cat->buf.release();
+        delete cat;
+        return rc;
+    }
+    cat->next = ctx->catalogs;
+    if (ctx->catalogs) ctx->catalogs->prev = cat;
+    ctx->catalogs = cat;
+    ctx->n_catalogs++;
+    *out = cat;
+    return ACF_OK;
+}
+
+extern "C" int acf_prepare(acf_ctx *ctx, const double *d_xyz, const float *d_w, size_t n, acf_catalog **out)
+{
+    return acf_prepare_rows(ctx, d_xyz, d_w, n, 0, n, out);
+}
+
+extern "C" void acf_release(acf_ctx *ctx, acf_catalog *cat)
+{
+    if (!ctx || !cat || cat->ctx != ctx) return;
+    cudaSetDevice(ctx->device);
+    cudaStreamSynchronize(ctx->stream);  // counts on the handle may still be running
+    if (cat->prev) cat->prev->next = cat->next;
+    else ctx->catalogs = cat->next;
+    if (cat->next) cat->next->prev = cat->prev;
+    ctx->n_catalogs--;
+    cat->buf.release();
+    delete cat;
+}
+
+extern "C" int acf_pair_count_prepared(acf_ctx *ctx, const acf_catalog *a, const acf_catalog *b, const double *cos_edges, int nbins,
+                                       int part, int n_parts, uint64_t *d_counts, double *d_wsums)
+{
+    if (!ctx) return ACF_EINVAL;
+    ctx->err[0] = 0;
+    if (const char *why = check_edges(cos_edges, nbins)) return acf::fail(ctx, ACF_EINVAL, "%s", why);
+    if (!a || a->ctx != ctx || (b && b->ctx != ctx)) return acf::fail(ctx, ACF_EINVAL, "catalogue handle is NULL or of another context");
+    if (!d_counts) return acf::fail(ctx, ACF_EINVAL, "d_counts is NULL");
+    if (n_parts < 1 || part < 0 || part >= n_parts) return acf::fail(ctx, ACF_EINVAL, "part %d of %d", part, n_parts);
+    const bool is_auto = b == nullptr || b == a;
+    if (is_auto) b = a;
+    const bool weighted = d_wsums != nullptr;
+    if (weighted && (!a->weighted || !b->weighted)) return acf::fail(ctx, ACF_EINVAL, "weighted count of a catalogue prepared without weights");
+    if (ctx->opt_kernel == ACF_KERNEL_FP64) return acf::fail(ctx, ACF_EINVAL, "the fp64 reference kernel counts unprepared catalogues only");
+    ACF_CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t st = ctx->stream;
+    ctx->last = acf_stats{};
+    ctx->pair_timed = false;
+    ctx->last.pairs_nominal = is_auto ? (uint64_t)a->p.n * (a->p.n ? a->p.n - 1 : 0) / 2 : (uint64_t)a->p.n * (uint64_t)b->p.n;  // (of all parts)
+    ACF_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_start, st));
+    ACF_CUDA_TRY(ctx, cudaMemsetAsync(ctx->d_counters, 0, sizeof(unsigned long long) * acf::kNumCounters, st));
+    ACF_CUDA_TRY(ctx, cudaMemsetAsync(d_counts, 0, sizeof(uint64_t) * (size_t)nbins, st));
+    if (weighted) ACF_CUDA_TRY(ctx, cudaMemsetAsync(d_wsums, 0, sizeof(double) * (size_t)nbins, st));
+    ctx->stats_pending = true;
+    // a catalogue prepared with weights counts unweighted as well: the kernels then read only its coordinates
+    acf::Prepared pa = a->p, pb = b->p;
+    int rc = acf::count_prepared_part(ctx, pa, pb, is_auto ? 1 : 0, cos_edges, nbins, part, n_parts,
+                                      reinterpret_cast<unsigned long long *>(d_counts), d_wsums);
+    if (rc != ACF_OK) return rc;
+    ACF_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_stop, st));
+    return ACF_OK;
+}
+
+// Delete-one jackknife (include/acf.h).  Every region of either catalogue is prepared once; the histograms of all pairs
+// of regions -- DD and RR: K (K + 1) / 2 counts each, DR: K^2 -- are counted on the handles into one device array and
+// fetched once.  Together they are exactly the pairs of one DD, one DR and one RR count; the full histograms are their
+// sums, and the histograms without region k are the full ones minus row and column k.
 extern "C" int acf_jackknife(acf_ctx *ctx, const double *d_xyz_d, size_t n_d, const size_t *off_d, const double *d_xyz_r,
                              size_t n_r, const size_t *off_r, int n_regions, const double *cos_edges, int nbins,
                              int estimator, double *w_full, double *w_jk, double *cov)
@@ -266,79 +390,91 @@ extern "C" int acf_jackknife(acf_ctx *ctx, const double *d_xyz_d, size_t n_d, co
     if (!d_xyz_d || !d_xyz_r || !off_d || !off_r || !w_full || !w_jk) return acf::fail(ctx, ACF_EINVAL, "NULL argument");
     if (n_regions < 2) return acf::fail(ctx, ACF_EINVAL, "n_regions must be at least 2");
     if (estimator < ACF_EST_LANDY_SZALAY || estimator > ACF_EST_HAMILTON) return acf::fail(ctx, ACF_EINVAL, "unknown estimator");
-    size_t max_d = 0, max_r = 0;
-    for (int k = 0; k < n_regions; ++k) {
+    for (int k = 0; k < n_regions; ++k)
         if (off_d[k + 1] < off_d[k] || off_r[k + 1] < off_r[k]) return acf::fail(ctx, ACF_EINVAL, "region offsets must not decrease");
-        if (off_d[k + 1] - off_d[k] > max_d) max_d = off_d[k + 1] - off_d[k];
-        if (off_r[k + 1] - off_r[k] > max_r) max_r = off_r[k + 1] - off_r[k];
-    }
     if (off_d[0] != 0 || off_r[0] != 0 || off_d[n_regions] != n_d || off_r[n_regions] != n_r)
         return acf::fail(ctx, ACF_EINVAL, "region offsets must run from 0 to n");
+    if (ctx->opt_kernel == ACF_KERNEL_FP64) return acf::fail(ctx, ACF_EINVAL, "the jackknife runs on prepared catalogues: not with the fp64 reference kernel");
     ACF_CUDA_TRY(ctx, cudaSetDevice(ctx->device));
     cudaStream_t st = ctx->stream;
-    const size_t nb = (size_t)nbins;
-    // scratch: the points of region k of either catalogue as catalogues of their own, and 8 histograms
-    ACF_CUDA_TRY(ctx, ctx->s_host_stage[0].reserve(sizeof(double) * 3 * (max_d ? max_d : 1)));
-    ACF_CUDA_TRY(ctx, ctx->s_host_stage[1].reserve(sizeof(double) * 3 * (max_r ? max_r : 1)));
-    ACF_CUDA_TRY(ctx, ctx->s_host_stage[4].reserve(sizeof(uint64_t) * 8 * nb));
-    double *d_dk = ctx->s_host_stage[0].as<double>(), *d_rk = ctx->s_host_stage[1].as<double>();
-    uint64_t *d_cnt = ctx->s_host_stage[4].as<uint64_t>();
-    std::vector<uint64_t> h((size_t)8 * nb), tot((size_t)3 * nb), dd(nb), dr(nb), rr(nb);
-
-    int rc;
-    auto count = [&](const double *a, size_t na, size_t i0, size_t i1, const double *b, size_t nbp, int is_auto, int slot) -> int {
-        return acf_pair_count_rows(ctx, a, nullptr, na, i0, i1, b, nullptr, nbp, cos_edges, nbins, is_auto, d_cnt + (size_t)slot * nb, nullptr);
-    };
-    auto fetch = [&](int slots) -> int {
-        ACF_CUDA_TRY(ctx, cudaMemcpyAsync(h.data(), d_cnt, sizeof(uint64_t) * (size_t)slots * nb, cudaMemcpyDeviceToHost, st));
-        ACF_CUDA_TRY(ctx, cudaStreamSynchronize(st));
-        return ACF_OK;
-    };
-    auto subset = [&](const double *src, size_t n, size_t lo, size_t cnt, double *dst) -> int {
-        for (int c = 0; c < 3 && cnt; ++c)
-            ACF_CUDA_TRY(ctx, cudaMemcpyAsync(dst + (size_t)c * cnt, src + (size_t)c * n + lo, sizeof(double) * cnt, cudaMemcpyDeviceToDevice, st));
-        return ACF_OK;
-    };
-    if ((rc = count(d_xyz_d, n_d, 0, n_d, d_xyz_d, n_d, 1, 0)) != ACF_OK) return rc;
-    if ((rc = count(d_xyz_d, n_d, 0, n_d, d_xyz_r, n_r, 0, 1)) != ACF_OK) return rc;
-    if ((rc = count(d_xyz_r, n_r, 0, n_r, d_xyz_r, n_r, 1, 2)) != ACF_OK) return rc;
-    if ((rc = fetch(3)) != ACF_OK) return rc;
-    tot.assign(h.begin(), h.begin() + 3 * (long)nb);
-    if ((rc = acf_estimator(estimator, tot.data(), tot.data() + nb, tot.data() + 2 * nb, n_d, n_r, nbins, w_full)) != ACF_OK) return rc;
-
-    for (int k = 0; k < n_regions; ++k) {
-        const size_t d0 = off_d[k], d1 = off_d[k + 1], r0 = off_r[k], r1 = off_r[k + 1];
-        const size_t ndk = d1 - d0, nrk = r1 - r0;
-        if ((rc = subset(d_xyz_d, n_d, d0, ndk, d_dk)) != ACF_OK) return rc;
-        if ((rc = subset(d_xyz_r, n_r, r0, nrk, d_rk)) != ACF_OK) return rc;
-        // slots: 0 DD rows k, 1 DD rows before k x D_k, 2 RR rows k, 3 RR rows before k x R_k,
-        //        4 D_k x R, 5 D x R_k, 6 D_k x R_k
-        if ((rc = count(d_xyz_d, n_d, d0, d1, d_xyz_d, n_d, 1, 0)) != ACF_OK) return rc;
-        if ((rc = count(d_xyz_d, n_d, 0, d0, d_dk, ndk, 0, 1)) != ACF_OK) return rc;
-        if ((rc = count(d_xyz_r, n_r, r0, r1, d_xyz_r, n_r, 1, 2)) != ACF_OK) return rc;
-        if ((rc = count(d_xyz_r, n_r, 0, r0, d_rk, nrk, 0, 3)) != ACF_OK) return rc;
-        if ((rc = count(d_xyz_d, n_d, d0, d1, d_xyz_r, n_r, 0, 4)) != ACF_OK) return rc;
-        if ((rc = count(d_xyz_d, n_d, 0, n_d, d_rk, nrk, 0, 5)) != ACF_OK) return rc;
-        if ((rc = count(d_dk, ndk, 0, ndk, d_rk, nrk, 0, 6)) != ACF_OK) return rc;
-        if ((rc = fetch(7)) != ACF_OK) return rc;
-        for (size_t b = 0; b < nb; ++b) {
-            dd[b] = tot[b] - h[b] - h[nb + b];
-            rr[b] = tot[2 * nb + b] - h[2 * nb + b] - h[3 * nb + b];
-            dr[b] = tot[nb + b] - h[4 * nb + b] - h[5 * nb + b] + h[6 * nb + b];
+    const size_t nb = (size_t)nbins, K = (size_t)n_regions;
+    std::vector<acf_catalog *> cd(K, nullptr), cr(K, nullptr);
+    auto cleanup = [&]() {
+        for (size_t k = 0; k < K; ++k) {
+            acf_release(ctx, cd[k]);
+            acf_release(ctx, cr[k]);
         }
-        if ((rc = acf_estimator(estimator, dd.data(), dr.data(), rr.data(), n_d - ndk, n_r - nrk, nbins, w_jk + (size_t)k * nb)) != ACF_OK)
-            return rc;
+    };
+    int rc = ACF_OK;
+    for (size_t k = 0; k < K && rc == ACF_OK; ++k) {
+        rc = acf_prepare_rows(ctx, d_xyz_d, nullptr, n_d, off_d[k], off_d[k + 1], &cd[k]);
+        if (rc == ACF_OK) rc = acf_prepare_rows(ctx, d_xyz_r, nullptr, n_r, off_r[k], off_r[k + 1], &cr[k]);
+    }
+    // histograms: DD[k][l] (k <= l), DR[k][l], RR[k][l] (k <= l): 3 K^2 slots of nbins
+    const size_t slots = 3 * K * K;
+    if (rc == ACF_OK && ctx->s_host_stage[4].reserve(sizeof(uint64_t) * slots * nb) != cudaSuccess) rc = acf::fail(ctx, ACF_ENOMEM, "out of device memory");
+    uint64_t *d_cnt = ctx->s_host_stage[4].as<uint64_t>();
+    if (rc == ACF_OK && cudaMemsetAsync(d_cnt, 0, sizeof(uint64_t) * slots * nb, st) != cudaSuccess) rc = acf::fail(ctx, ACF_ECUDA, "memset failed");
+    unsigned long long launches = 0;
+    for (size_t k = 0; k < K && rc == ACF_OK; ++k)
+        for (size_t l = 0; l < K && rc == ACF_OK; ++l) {
+            if (l >= k) {
+                rc = acf_pair_count_prepared(ctx, cd[k], l == k ? nullptr : cd[l], cos_edges, nbins, 0, 1, d_cnt + (k * K + l) * nb, nullptr);
+                launches += ctx->last.kernel_launches;
+                if (rc == ACF_OK) rc = acf_pair_count_prepared(ctx, cr[k], l == k ? nullptr : cr[l], cos_edges, nbins, 0, 1, d_cnt + ((2 * K + k) * K + l) * nb, nullptr);
+                launches += ctx->last.kernel_launches;
+            }
+            if (rc == ACF_OK) rc = acf_pair_count_prepared(ctx, cd[k], cr[l], cos_edges, nbins, 0, 1, d_cnt + ((K + k) * K + l) * nb, nullptr);
+            launches += ctx->last.kernel_launches;
+        }
+    std::vector<uint64_t> h(slots * nb);
+    if (rc == ACF_OK) {
+        cudaError_t e = cudaMemcpyAsync(h.data(), d_cnt, sizeof(uint64_t) * slots * nb, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) rc = acf::fail(ctx, ACF_ECUDA, "acf_jackknife: %s", cudaGetErrorString(e));
+    }
+    cleanup();
+    if (rc != ACF_OK) return rc;
+    ctx->last.kernel_launches = launches;
+
+    // totals, and per region the pairs that touch it
+    std::vector<uint64_t> tot(3 * nb, 0), touch(3 * K * nb, 0), dd(nb), dr(nb), rr(nb);
+    for (size_t k = 0; k < K; ++k)
+        for (size_t l = 0; l < K; ++l)
+            for (size_t b = 0; b < nb; ++b) {
+                const uint64_t vdd = l >= k ? h[(k * K + l) * nb + b] : 0, vrr = l >= k ? h[((2 * K + k) * K + l) * nb + b] : 0;
+                const uint64_t vdr = h[((K + k) * K + l) * nb + b];
+                tot[b] += vdd;
+                tot[nb + b] += vdr;
+                tot[2 * nb + b] += vrr;
+                // a pair of regions (k, l) touches k and l; DR[k][l] touches data region k and random region l
+                touch[k * nb + b] += vdd;
+                if (l != k) touch[l * nb + b] += vdd;
+                touch[(2 * K + k) * nb + b] += vrr;
+                if (l != k) touch[(2 * K + l) * nb + b] += vrr;
+                touch[(K + k) * nb + b] += vdr;
+                if (l != k) touch[(K + l) * nb + b] += vdr;
+            }
+    if ((rc = acf_estimator(estimator, tot.data(), tot.data() + nb, tot.data() + 2 * nb, n_d, n_r, nbins, w_full)) != ACF_OK) return rc;
+    for (size_t k = 0; k < K; ++k) {
+        const size_t ndk = off_d[k + 1] - off_d[k], nrk = off_r[k + 1] - off_r[k];
+        for (size_t b = 0; b < nb; ++b) {
+            dd[b] = tot[b] - touch[k * nb + b];
+            dr[b] = tot[nb + b] - touch[(K + k) * nb + b];
+            rr[b] = tot[2 * nb + b] - touch[(2 * K + k) * nb + b];
+        }
+        if ((rc = acf_estimator(estimator, dd.data(), dr.data(), rr.data(), n_d - ndk, n_r - nrk, nbins, w_jk + k * nb)) != ACF_OK) return rc;
     }
     if (cov) {
         std::vector<double> mean(nb, 0.0);
-        for (int k = 0; k < n_regions; ++k)
-            for (size_t b = 0; b < nb; ++b) mean[b] += w_jk[(size_t)k * nb + b];
+        for (size_t k = 0; k < K; ++k)
+            for (size_t b = 0; b < nb; ++b) mean[b] += w_jk[k * nb + b];
         for (size_t b = 0; b < nb; ++b) mean[b] /= (double)n_regions;
         const double f = (double)(n_regions - 1) / (double)n_regions;
         for (size_t a = 0; a < nb; ++a)
             for (size_t b = 0; b < nb; ++b) {
                 double sum = 0.0;
-                for (int k = 0; k < n_regions; ++k) sum += (w_jk[(size_t)k * nb + a] - mean[a]) * (w_jk[(size_t)k * nb + b] - mean[b]);
+                for (size_t k = 0; k < K; ++k) sum += (w_jk[k * nb + a] - mean[a]) * (w_jk[k * nb + b] - mean[b]);
                 cov[a * nb + b] = f * sum;
             }
     }
@@ -361,22 +497,21 @@ extern "C" int acf_correlate_host(acf_ctx *ctx, const double *ra_d, const double
     ACF_CUDA_TRY(ctx, cudaSetDevice(ctx->device));
     cudaStream_t st = ctx->stream;
 
-    // pinned staging: xyz of both catalogues, then the outputs
+    // pinned staging: xyz of both catalogues, their weights, then the outputs
     const size_t xyz_bytes = sizeof(double) * 3 * (n_d + n_r);
+    const size_t w_bytes = weighted ? ((sizeof(float) * (n_d + n_r) + 15) & ~size_t(15)) : 0;
     const size_t out_bytes = (sizeof(uint64_t) + sizeof(double)) * 3 * (size_t)nbins;
-    if (ctx->h_stage_bytes < xyz_bytes + out_bytes) {
+    if (ctx->h_stage_bytes < xyz_bytes + w_bytes + out_bytes) {
         if (ctx->h_stage) cudaFreeHost(ctx->h_stage);
         ctx->h_stage = nullptr;
         ctx->h_stage_bytes = 0;
-        ACF_CUDA_TRY(ctx, cudaHostAlloc(&ctx->h_stage, xyz_bytes + out_bytes, cudaHostAllocDefault));
-        ctx->h_stage_bytes = xyz_bytes + out_bytes;
+        ACF_CUDA_TRY(ctx, cudaHostAlloc(&ctx->h_stage, xyz_bytes + w_bytes + out_bytes, cudaHostAllocDefault));
+        ctx->h_stage_bytes = xyz_bytes + w_bytes + out_bytes;
     }
     double *h_xyz_d = static_cast<double *>(ctx->h_stage), *h_xyz_r = h_xyz_d + 3 * n_d;
-    uint64_t *h_cnt = reinterpret_cast<uint64_t *>(h_xyz_r + 3 * n_r);
+    float *h_wd = reinterpret_cast<float *>(h_xyz_r + 3 * n_r), *h_wr = h_wd + n_d;
+    uint64_t *h_cnt = reinterpret_cast<uint64_t *>(reinterpret_cast<char *>(h_wd) + w_bytes);
     double *h_ws = reinterpret_cast<double *>(h_cnt + 3 * (size_t)nbins);
-    // the randoms are canonicalised on the host while the device counts DD (PAPER.md:128 names the
-    // overlap of transfers and kernels as the step its own code did not take)
-    acf_radec_to_xyz(ra_d, dec_d, n_d, h_xyz_d);
 
     ACF_CUDA_TRY(ctx, ctx->s_host_stage[0].reserve(sizeof(double) * 3 * (n_d ? n_d : 1)));
     ACF_CUDA_TRY(ctx, ctx->s_host_stage[1].reserve(sizeof(double) * 3 * (n_r ? n_r : 1)));
@@ -388,23 +523,56 @@ extern "C" int acf_correlate_host(acf_ctx *ctx, const double *ra_d, const double
     float *d_wd = weighted ? ctx->s_host_stage[2].as<float>() : nullptr, *d_wr = weighted ? ctx->s_host_stage[3].as<float>() : nullptr;
     uint64_t *d_cnt = ctx->s_host_stage[4].as<uint64_t>();
     double *d_ws = weighted ? ctx->s_host_stage[5].as<double>() : nullptr;
-    if (n_d) ACF_CUDA_TRY(ctx, cudaMemcpyAsync(d_xd, h_xyz_d, sizeof(double) * 3 * n_d, cudaMemcpyHostToDevice, st));
-    if (weighted && n_d) ACF_CUDA_TRY(ctx, cudaMemcpyAsync(d_wd, w_d, sizeof(float) * n_d, cudaMemcpyHostToDevice, st));
 
-    int rc;
-    rc = acf_pair_count_rows(ctx, d_xd, d_wd, n_d, 0, n_d, d_xd, d_wd, n_d, cos_edges, nbins, 1, d_cnt, d_ws);
+    // The data: canonicalise, copy, prepare, and start DD.  The randoms are canonicalised on the host and copied on a
+    // second stream while the device counts DD (PAPER.md:128 names the overlap of transfers and kernels as the step the
+    // paper's own code did not take); the main stream waits for that copy before it touches them.
+    acf_radec_to_xyz(ra_d, dec_d, n_d, h_xyz_d);
+    if (weighted && n_d) memcpy(h_wd, w_d, sizeof(float) * n_d);
+    if (n_d) ACF_CUDA_TRY(ctx, cudaMemcpyAsync(d_xd, h_xyz_d, sizeof(double) * 3 * n_d, cudaMemcpyHostToDevice, st));
+    if (weighted && n_d) ACF_CUDA_TRY(ctx, cudaMemcpyAsync(d_wd, h_wd, sizeof(float) * n_d, cudaMemcpyHostToDevice, st));
+    acf_catalog *cd = nullptr, *cr = nullptr;
+    int rc = acf_prepare(ctx, d_xd, d_wd, n_d, &cd);
     if (rc != ACF_OK) return rc;
+    auto bail = [&](int code) {
+        cudaStreamSynchronize(ctx->copy_stream);
+        acf_release(ctx, cd);
+        acf_release(ctx, cr);
+        return code;
+    };
+    acf_stats st_sum{};
+    auto add_stats = [&]() {
+        st_sum.pairs_nominal += ctx->last.pairs_nominal;
+        st_sum.kernel_launches += ctx->last.kernel_launches;
+    };
+    rc = acf_pair_count_prepared(ctx, cd, nullptr, cos_edges, nbins, 0, 1, d_cnt, d_ws);
+    if (rc != ACF_OK) return bail(rc);
+    add_stats();
     acf_radec_to_xyz(ra_r, dec_r, n_r, h_xyz_r);
-    if (n_r) ACF_CUDA_TRY(ctx, cudaMemcpyAsync(d_xr, h_xyz_r, sizeof(double) * 3 * n_r, cudaMemcpyHostToDevice, st));
-    if (weighted && n_r) ACF_CUDA_TRY(ctx, cudaMemcpyAsync(d_wr, w_r, sizeof(float) * n_r, cudaMemcpyHostToDevice, st));
-    rc = acf_pair_count_rows(ctx, d_xd, d_wd, n_d, 0, n_d, d_xr, d_wr, n_r, cos_edges, nbins, 0, d_cnt + nbins, d_ws ? d_ws + nbins : nullptr);
-    if (rc != ACF_OK) return rc;
-    rc = acf_pair_count_rows(ctx, d_xr, d_wr, n_r, 0, n_r, d_xr, d_wr, n_r, cos_edges, nbins, 1, d_cnt + 2 * nbins, d_ws ? d_ws + 2 * nbins : nullptr);
-    if (rc != ACF_OK) return rc;
+    if (weighted && n_r) memcpy(h_wr, w_r, sizeof(float) * n_r);
+    if (n_r) ACF_CUDA_TRY(ctx, cudaMemcpyAsync(d_xr, h_xyz_r, sizeof(double) * 3 * n_r, cudaMemcpyHostToDevice, ctx->copy_stream));
+    if (weighted && n_r) ACF_CUDA_TRY(ctx, cudaMemcpyAsync(d_wr, h_wr, sizeof(float) * n_r, cudaMemcpyHostToDevice, ctx->copy_stream));
+    ACF_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_copy, ctx->copy_stream));
+    ACF_CUDA_TRY(ctx, cudaStreamWaitEvent(st, ctx->ev_copy, 0));
+    rc = acf_prepare(ctx, d_xr, d_wr, n_r, &cr);
+    if (rc != ACF_OK) return bail(rc);
+    rc = acf_pair_count_prepared(ctx, cd, cr, cos_edges, nbins, 0, 1, d_cnt + nbins, d_ws ? d_ws + nbins : nullptr);
+    if (rc != ACF_OK) return bail(rc);
+    add_stats();
+    rc = acf_pair_count_prepared(ctx, cr, nullptr, cos_edges, nbins, 0, 1, d_cnt + 2 * nbins, d_ws ? d_ws + 2 * nbins : nullptr);
+    if (rc != ACF_OK) return bail(rc);
+    add_stats();
 
     ACF_CUDA_TRY(ctx, cudaMemcpyAsync(h_cnt, d_cnt, sizeof(uint64_t) * 3 * (size_t)nbins, cudaMemcpyDeviceToHost, st));
     if (weighted) ACF_CUDA_TRY(ctx, cudaMemcpyAsync(h_ws, d_ws, sizeof(double) * 3 * (size_t)nbins, cudaMemcpyDeviceToHost, st));
-    ACF_CUDA_TRY(ctx, cudaStreamSynchronize(st));
+    {
+        const cudaError_t e = cudaStreamSynchronize(st);
+        acf_release(ctx, cd);
+        acf_release(ctx, cr);
+        if (e != cudaSuccess) return acf::fail(ctx, ACF_ECUDA, "acf_correlate_host: %s", cudaGetErrorString(e));
+        ctx->last.pairs_nominal = st_sum.pairs_nominal;
+        ctx->last.kernel_launches = st_sum.kernel_launches;
+    }
     memcpy(dd, h_cnt, sizeof(uint64_t) * (size_t)nbins);
     memcpy(dr, h_cnt + nbins, sizeof(uint64_t) * (size_t)nbins);
     memcpy(rr, h_cnt + 2 * nbins, sizeof(uint64_t) * (size_t)nbins);

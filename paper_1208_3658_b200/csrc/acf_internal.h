@@ -81,7 +81,9 @@ struct GroupCap {
 // path for every pair, which adds each w_i w_j to its row directly (acf_pair.cu).
 struct PackInfo {
     double C, inv_C;
-    int packed, pad;
+    int packed;
+    int bad;     // points of the catalogue that failed validation (validate_kernel): its counts are refused
+    double eps;  // max over the catalogue's points of | |u|^2 - 1 | (what the chord margins and the cap slack are made of)
 };
 
 // One catalogue prepared for the fast path (all device pointers live in ctx scratch).
@@ -99,6 +101,23 @@ struct Prepared {
     GroupCap *gcaps = nullptr;    // per group of kGroup points (kGroupsPerTile per tile)
     GroupCap *scaps = nullptr;    // per sub-group of kSub points (kSubsPerGroup per group)
     int n_tiles = 0;
+};
+
+// The device buffers of one prepared catalogue (grown lazily, freed with their owner: the context's two slots of
+// the calls that prepare on the fly, or an acf_catalog handle).
+struct CatBuffers {
+    Scratch pts, perm, caps, gcaps, scaps, pts2, vj, pack;
+    void release()
+    {
+        pts.release();
+        perm.release();
+        caps.release();
+        gcaps.release();
+        scaps.release();
+        pts2.release();
+        vj.release();
+        pack.release();
+    }
 };
 
 }  // namespace acf
@@ -121,26 +140,36 @@ struct acf_ctx {
     bool pair_timed = false;
     unsigned long long *d_counters = nullptr;  // acf::kNumCounters
     unsigned long long *h_counters = nullptr;  // pinned mirror
+    int *h_verdict = nullptr;                  // pinned (behind h_counters): bad-point counts of the catalogues of a call
     acf_stats last{};
     bool stats_pending = false;
 
     // scratch, grown lazily
     acf::Scratch s_edges;            // device copy of cos_edges (+ fp32 tables of the fast path)
     const float *d_sedges = nullptr; // inside s_edges: the edges as squared chord lengths (chord tier)
-    acf::Scratch s_pts[2];           // sorted float4 points of catalogue a / b
-    acf::Scratch s_perm[2];          // permutations
-    acf::Scratch s_keys[2];          // sort keys (double-buffered inside)
-    acf::Scratch s_caps[2];          // tile caps
-    acf::Scratch s_gcaps[2];         // group caps
-    acf::Scratch s_scaps[2];         // sub-group caps
-    acf::Scratch s_pts2[2];          // paired layout of the sorted points
-    acf::Scratch s_vj[2];            // fp64 window-path weights
-    acf::Scratch s_pack[2];          // PackInfo + weight-range words
+    acf::CatBuffers cat[2];          // catalogues a / b of the calls that prepare on the fly
+    acf::Scratch s_keys;             // sort keys and indices (double-buffered inside): scratch of a preparation
     acf::Scratch s_work;             // work list
     acf::Scratch s_misc;             // radix-sort histograms etc.
     acf::Scratch s_host_stage[6];    // acf_correlate_host: device copies of xyz / weights / outputs
     void *h_stage = nullptr;         // acf_correlate_host: pinned host staging
     size_t h_stage_bytes = 0;
+    void *h_tables = nullptr;        // pinned staging of the per-call tables (edges, chord edges, cell table)
+    size_t h_tables_bytes = 0;
+    cudaEvent_t ev_tables = nullptr; // the last copy out of h_tables
+    cudaStream_t copy_stream = nullptr;  // acf_correlate_host: host-to-device copies that overlap the counts
+    cudaEvent_t ev_copy = nullptr;
+    int n_catalogs = 0;              // acf_catalog handles alive (acf_destroy refuses to leave them dangling: it frees them)
+    struct acf_catalog *catalogs = nullptr;  // intrusive list of the handles
+};
+
+// A catalogue prepared once for any number of counts (include/acf.h: acf_prepare).
+struct acf_catalog {
+    acf_ctx *ctx = nullptr;
+    acf::Prepared p;
+    acf::CatBuffers buf;
+    bool weighted = false;
+    acf_catalog *next = nullptr, *prev = nullptr;
 };
 
 namespace acf {
@@ -184,12 +213,21 @@ int launch_pair_win(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_a
 
 // ---- acf_prep.cu: sort + gather + caps of points [off, off+cnt) of a catalogue with `stride` points;
 // and the work list of (i-tile, j-tile run) items for i-tiles [ti_begin, ti_end).
-int prepare_catalogue(acf_ctx *ctx, int slot, const double *xyz, size_t stride, size_t off, size_t cnt,
+// Validation (finite unit vectors, finite non-negative weights) is part of it: the verdict and the largest norm
+// deviation land in the catalogue's PackInfo.
+int prepare_catalogue(acf_ctx *ctx, CatBuffers &buf, const double *xyz, size_t stride, size_t off, size_t cnt,
                       const float *w, Prepared *out);
-int build_worklist(acf_ctx *ctx, const Prepared &a, int ti_begin, int ti_end, const Prepared &b, int is_auto,
+// i-tiles ti_begin + k * ti_stride < ti_end.
+int build_worklist(acf_ctx *ctx, const Prepared &a, int ti_begin, int ti_end, int ti_stride, const Prepared &b, int is_auto,
                    double e_first, double e_last, int3 *items, uint32_t capacity);
 
-// Validates unit vectors (and weights): bumps counters[kCtrBadInput] per bad point.
-cudaError_t launch_validate(acf_ctx *ctx, const double *d_xyz, const float *d_w, size_t n);
+// Validates points [off, off + cnt) of a catalogue with `stride` points (unit vectors, weights): pack->bad = number of
+// bad points, pack->eps = max | |u|^2 - 1 |.
+cudaError_t launch_validate(acf_ctx *ctx, const double *d_xyz, size_t stride, size_t off, size_t cnt, const float *d_w, PackInfo *pack);
+
+// ---- acf_pair.cu: the counts of part `part` of `n_parts` (i-tiles t = part mod n_parts) of prepared a against prepared b,
+// added into d_counts / d_wsums.  Enqueues only.
+int count_prepared_part(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_auto, const double *h_edges, int nbins,
+                        int part, int n_parts, unsigned long long *d_counts, double *d_wsums);
 
 }  // namespace acf

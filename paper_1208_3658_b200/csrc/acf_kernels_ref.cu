@@ -94,13 +94,14 @@ pair_count_fp64_kernel(const double *__restrict__ a, const float *__restrict__ w
     }
 }
 
-__global__ void validate_kernel(const double *__restrict__ xyz, const float *__restrict__ w, size_t n,
-                                unsigned long long *__restrict__ counters)
+__global__ void validate_kernel(const double *__restrict__ xyz, size_t stride, size_t off, size_t cnt, const float *__restrict__ w,
+                                PackInfo *__restrict__ pack)
 {
     unsigned int bad = 0;
-    double dev = 0.0;  // largest |r^2 - 1| seen: the chord tier of the pair kernels needs it (acf_pair_common.cuh)
-    for (size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x) {
-        const double x = xyz[i], y = xyz[n + i], z = xyz[2 * n + i];
+    double dev = 0.0;  // largest |r^2 - 1| seen: the chord tier and the cap bounds of the pair kernels need it (acf_pair_common.cuh)
+    for (size_t k = (size_t)blockIdx.x * blockDim.x + threadIdx.x; k < cnt; k += (size_t)gridDim.x * blockDim.x) {
+        const size_t i = off + k;
+        const double x = xyz[i], y = xyz[stride + i], z = xyz[2 * stride + i];
         const double r2 = x * x + y * y + z * z;
         bool ok = isfinite(x) && isfinite(y) && isfinite(z) && fabs(r2 - 1.0) <= 1e-6;
         if (ok) dev = fmax(dev, fabs(r2 - 1.0));
@@ -111,21 +112,22 @@ __global__ void validate_kernel(const double *__restrict__ xyz, const float *__r
         bad += ok ? 0u : 1u;
     }
     bad = __reduce_add_sync(0xffffffffu, bad);
-    if ((threadIdx.x & 31) == 0 && bad) atomicAdd(&counters[kCtrBadInput], (unsigned long long)bad);
+    if ((threadIdx.x & 31) == 0 && bad) atomicAdd(&pack->bad, (int)(bad > 0x3fffffffu ? 0x3fffffffu : bad));
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) dev = fmax(dev, __shfl_xor_sync(0xffffffffu, dev, o));
     // non-negative doubles order like their bit patterns
-    if ((threadIdx.x & 31) == 0 && dev > 0.0) atomicMax(&counters[kCtrNormDev], (unsigned long long)__double_as_longlong(dev));
+    if ((threadIdx.x & 31) == 0 && dev > 0.0)
+        atomicMax(reinterpret_cast<unsigned long long *>(&pack->eps), (unsigned long long)__double_as_longlong(dev));
 }
 
 }  // namespace
 
-cudaError_t launch_validate(acf_ctx *ctx, const double *d_xyz, const float *d_w, size_t n)
+cudaError_t launch_validate(acf_ctx *ctx, const double *d_xyz, size_t stride, size_t off, size_t cnt, const float *d_w, PackInfo *pack)
 {
-    if (n == 0) return cudaSuccess;
-    int blocks = (int)((n + 255) / 256);
+    if (cnt == 0) return cudaSuccess;
+    int blocks = (int)((cnt + 255) / 256);
     if (blocks > ctx->num_sms * 8) blocks = ctx->num_sms * 8;
-    validate_kernel<<<blocks, 256, 0, ctx->stream>>>(d_xyz, d_w, n, ctx->d_counters);
+    validate_kernel<<<blocks, 256, 0, ctx->stream>>>(d_xyz, stride, off, cnt, d_w, pack);
     ctx->last.kernel_launches++;
     return cudaGetLastError();
 }

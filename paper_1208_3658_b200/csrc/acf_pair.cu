@@ -659,10 +659,21 @@ cudaError_t launch(acf_ctx *ctx, const PairParams &p, size_t smem, int grid)
     return cudaGetLastError();
 }
 
-int count_prepared(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_auto, const double *h_edges, int nbins,
-                   const Lut &L, const uint2 *d_lut, unsigned long long *d_counts, double *d_wsums)
+// The verdicts of the two catalogues' validations -> the call's counters, where the kernels look for them.
+__global__ void seed_counters_kernel(unsigned long long *__restrict__ counters, const PackInfo *__restrict__ pa, const PackInfo *__restrict__ pb)
 {
-    if (a.n == 0 || b.n == 0) return ACF_OK;
+    const int bad = pa->bad + (pb != pa ? pb->bad : 0);
+    if (bad) atomicAdd(&counters[kCtrBadInput], (unsigned long long)bad);
+    const double eps = fmax(pa->eps, pb->eps);
+    atomicMax(&counters[kCtrNormDev], (unsigned long long)__double_as_longlong(eps));
+}
+
+int count_prepared(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_auto, const double *h_edges, int nbins,
+                   const Lut &L, const uint2 *d_lut, int part, int n_parts, unsigned long long *d_counts, double *d_wsums)
+{
+    if (a.n == 0 || b.n == 0 || part >= a.n_tiles) return ACF_OK;
+    seed_counters_kernel<<<1, 1, 0, ctx->stream>>>(ctx->d_counters, a.pack, b.pack);
+    ctx->last.kernel_launches++;
     const bool weighted = d_wsums != nullptr;
     const int rows = nbins + 2;
     const bool priv = rows <= kMaxPrivateRows;
@@ -695,10 +706,10 @@ int count_prepared(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_au
     // weight range); otherwise it returns at once and the table kernel, launched behind it, does the call.  Where the
     // table kernel's histograms do not fit either, the verdict is fetched and the call refused.
     if (use_win && weighted && !table_fits) {
-        int packed = 0;
-        ACF_CUDA_TRY(ctx, cudaMemcpyAsync(&packed, &b.pack->packed, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream));
+        PackInfo pk{};
+        ACF_CUDA_TRY(ctx, cudaMemcpyAsync(&pk, b.pack, sizeof(PackInfo), cudaMemcpyDeviceToHost, ctx->stream));
         ACF_CUDA_TRY(ctx, cudaStreamSynchronize(ctx->stream));
-        if (!packed && ctx->h_counters[kCtrBadInput] == 0)
+        if (!pk.packed && pk.bad == 0)
             return fail(ctx, ACF_EINVAL, "weights ranging over more than 2^13 cannot be tallied with %d bins (at most about 600)", nbins);
     }
 
@@ -706,9 +717,10 @@ int count_prepared(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_au
     // (worst case one item per surviving j-tile: survivors may alternate with pruned tiles)
     const uint64_t items_per_ti = (uint64_t)b.n_tiles;
     const uint64_t max_items = 64u << 20;  // 768 MB of items at most (8 M x 8 M points: 61 M tile pairs, one launch)
+    const int n_mine = (a.n_tiles - part + n_parts - 1) / n_parts;  // i-tiles part, part + n_parts, ...
     int ti_per_batch = (int)(max_items / items_per_ti);
     if (ti_per_batch < 1) ti_per_batch = 1;
-    if (ti_per_batch > a.n_tiles) ti_per_batch = a.n_tiles;
+    if (ti_per_batch > n_mine) ti_per_batch = n_mine;
     const uint32_t capacity = (uint32_t)(items_per_ti * (uint64_t)ti_per_batch);
     ACF_CUDA_TRY(ctx, ctx->s_work.reserve(sizeof(int3) * (size_t)capacity));
 
@@ -745,10 +757,12 @@ int count_prepared(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_au
     p.n_stages = n_stages;
 
     const int grid = ctx->num_sms * ctas_per_sm;
-    for (int ti0 = 0; ti0 < a.n_tiles; ti0 += ti_per_batch) {
-        const int ti1 = ti0 + ti_per_batch < a.n_tiles ? ti0 + ti_per_batch : a.n_tiles;
+    for (int k0 = 0; k0 < n_mine; k0 += ti_per_batch) {
+        const int k1 = k0 + ti_per_batch < n_mine ? k0 + ti_per_batch : n_mine;
+        const int ti0 = part + k0 * n_parts;
+        const int ti1 = part + (k1 - 1) * n_parts + 1;
         ACF_CUDA_TRY(ctx, cudaMemsetAsync(&ctx->d_counters[kCtrWorkHead], 0, 2 * sizeof(unsigned long long), ctx->stream));
-        int rc = build_worklist(ctx, a, ti0, ti1, b, is_auto, h_edges[0], h_edges[nbins], ctx->s_work.as<int3>(), capacity);
+        int rc = build_worklist(ctx, a, ti0, ti1, n_parts, b, is_auto, h_edges[0], h_edges[nbins], ctx->s_work.as<int3>(), capacity);
         if (rc != ACF_OK) return rc;
         cudaError_t e;
         if (!ctx->pair_timed) {
@@ -777,57 +791,69 @@ int count_prepared(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_au
 
 }  // namespace
 
-int run_pair_count_fast(acf_ctx *ctx, const double *d_a, const float *d_wa, size_t n_a, size_t i_begin,
-                        size_t i_end, const double *d_b, const float *d_wb, size_t n_b, const double *h_edges,
-                        int nbins, int is_auto, unsigned long long *d_counts, double *d_wsums)
+namespace {
+
+// The device tables of a call: the edges (fp64), the edges as squared chord lengths (fp32, chord tier) and, when the
+// table kernel may run (on request, or behind the window kernel for weights that do not pack), its cell table.
+int upload_tables(acf_ctx *ctx, const double *h_edges, int nbins, bool weighted, Lut &L, const uint2 *&d_lut)
 {
-    // cell table: the coarsest resolution that leaves no resolvable cell crowded
-    Lut L = build_lut(h_edges, nbins, 6);
-    for (int m = 7; m <= 9 && crowded_resolvable(L) > 0; ++m) L = build_lut(h_edges, nbins, m);
-    {   // with very many bins a coarser table (more cells left to the re-checks) may be what lets the kernel fit
-        const bool weighted = d_wsums != nullptr;
+    const bool want_lut = ctx->opt_kernel == ACF_KERNEL_TABLE || weighted;
+    if (want_lut) {
+        // cell table: the coarsest resolution that leaves no resolvable cell crowded
+        L = build_lut(h_edges, nbins, 6);
+        for (int m = 7; m <= 9 && crowded_resolvable(L) > 0; ++m) L = build_lut(h_edges, nbins, m);
+        // with very many bins a coarser table (more cells left to the re-checks) may be what lets the kernel fit
         const int rows = nbins + 2;
         const size_t words = rows <= kMaxPrivateRows ? (size_t)kWarps * rows * 32 : (size_t)kWarps * rows;
         auto need = [&](const Lut &t) {
             return kSmemHeader + 2 * stage_bytes(weighted) + t.cells.size() * sizeof(uint2) + words * (weighted ? 12 : 4) + 32;
         };
         while (L.m > 6 && need(L) > (size_t)ctx->max_smem_optin) L = build_lut(h_edges, nbins, L.m - 1);
+    } else {
+        L = Lut{};
+        L.m = 6;
+        L.shift = 23 - 6;
+        L.key0 = 0;
     }
-    // device tables: the edges (fp64), the edges as squared chord lengths (fp32, chord tier), the cell table
     const size_t edge_bytes = (sizeof(double) * (size_t)(nbins + 1) + 15) & ~size_t(15);
     const size_t sed_bytes = (sizeof(float) * (size_t)(nbins + 1) + 15) & ~size_t(15);
-    std::vector<float> sed((size_t)nbins + 1);
-    for (int k = 0; k <= nbins; ++k) sed[(size_t)k] = (float)(2.0 * (1.0 - h_edges[k]));
-    if (h_edges[0] >= 1.0) sed[0] = -1.0f;                                 // c is clamped: nothing lies beyond a pole
-    if (h_edges[nbins] <= -1.0) sed[(size_t)nbins] = std::numeric_limits<float>::infinity();
-    ACF_CUDA_TRY(ctx, ctx->s_edges.reserve(edge_bytes + sed_bytes + L.cells.size() * sizeof(uint2)));
-    ACF_CUDA_TRY(ctx, cudaMemcpyAsync(ctx->s_edges.ptr, h_edges, sizeof(double) * (size_t)(nbins + 1), cudaMemcpyHostToDevice, ctx->stream));
-    float *d_sed = reinterpret_cast<float *>(static_cast<char *>(ctx->s_edges.ptr) + edge_bytes);
-    ACF_CUDA_TRY(ctx, cudaMemcpyAsync(d_sed, sed.data(), sizeof(float) * sed.size(), cudaMemcpyHostToDevice, ctx->stream));
-    ctx->d_sedges = d_sed;
-    uint2 *d_lut = reinterpret_cast<uint2 *>(static_cast<char *>(ctx->s_edges.ptr) + edge_bytes + sed_bytes);
-    ACF_CUDA_TRY(ctx, cudaMemcpyAsync(d_lut, L.cells.data(), L.cells.size() * sizeof(uint2), cudaMemcpyHostToDevice, ctx->stream));
-
-    Prepared a, b;
-    int rc;
-    if (is_auto) {
-        // rows [i_begin, i_end): pairs inside the row block, plus the block against everything after it
-        rc = prepare_catalogue(ctx, 0, d_a, n_a, i_begin, i_end - i_begin, d_wa, &a);
-        if (rc != ACF_OK) return rc;
-        rc = count_prepared(ctx, a, a, 1, h_edges, nbins, L, d_lut, d_counts, d_wsums);
-        if (rc != ACF_OK) return rc;
-        if (i_end < n_a) {
-            rc = prepare_catalogue(ctx, 1, d_a, n_a, i_end, n_a - i_end, d_wa, &b);
-            if (rc != ACF_OK) return rc;
-            rc = count_prepared(ctx, a, b, 0, h_edges, nbins, L, d_lut, d_counts, d_wsums);
-        }
-        return rc;
+    // staged through pinned memory: the copies are asynchronous and the caller's array may go away at once
+    const size_t total = edge_bytes + sed_bytes + L.cells.size() * sizeof(uint2);
+    if (ctx->h_tables_bytes < total) {
+        if (ctx->h_tables) cudaFreeHost(ctx->h_tables);
+        ctx->h_tables = nullptr;
+        ctx->h_tables_bytes = 0;
+        ACF_CUDA_TRY(ctx, cudaHostAlloc(&ctx->h_tables, total + 4096, cudaHostAllocDefault));
+        ctx->h_tables_bytes = total + 4096;
+    } else {
+        // the previous call's copy out of this buffer must have been made
+        ACF_CUDA_TRY(ctx, cudaEventSynchronize(ctx->ev_tables));
     }
-    rc = prepare_catalogue(ctx, 0, d_a, n_a, i_begin, i_end - i_begin, d_wa, &a);
+    char *h = static_cast<char *>(ctx->h_tables);
+    memcpy(h, h_edges, sizeof(double) * (size_t)(nbins + 1));
+    float *sed = reinterpret_cast<float *>(h + edge_bytes);
+    for (int k = 0; k <= nbins; ++k) sed[k] = (float)(2.0 * (1.0 - h_edges[k]));
+    if (h_edges[0] >= 1.0) sed[0] = -1.0f;  // c is clamped: nothing lies beyond a pole
+    if (h_edges[nbins] <= -1.0) sed[nbins] = std::numeric_limits<float>::infinity();
+    if (!L.cells.empty()) memcpy(h + edge_bytes + sed_bytes, L.cells.data(), L.cells.size() * sizeof(uint2));
+    ACF_CUDA_TRY(ctx, ctx->s_edges.reserve(total));
+    ACF_CUDA_TRY(ctx, cudaMemcpyAsync(ctx->s_edges.ptr, h, total, cudaMemcpyHostToDevice, ctx->stream));
+    ACF_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_tables, ctx->stream));
+    ctx->d_sedges = reinterpret_cast<float *>(static_cast<char *>(ctx->s_edges.ptr) + edge_bytes);
+    d_lut = reinterpret_cast<const uint2 *>(static_cast<char *>(ctx->s_edges.ptr) + edge_bytes + sed_bytes);
+    return ACF_OK;
+}
+
+}  // namespace
+
+int count_prepared_part(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_auto, const double *h_edges, int nbins,
+                        int part, int n_parts, unsigned long long *d_counts, double *d_wsums)
+{
+    Lut L;
+    const uint2 *d_lut = nullptr;
+    int rc = upload_tables(ctx, h_edges, nbins, d_wsums != nullptr, L, d_lut);
     if (rc != ACF_OK) return rc;
-    rc = prepare_catalogue(ctx, 1, d_b, n_b, 0, n_b, d_wb, &b);
-    if (rc != ACF_OK) return rc;
-    return count_prepared(ctx, a, b, 0, h_edges, nbins, L, d_lut, d_counts, d_wsums);
+    return count_prepared(ctx, a, b, is_auto, h_edges, nbins, L, d_lut, part, n_parts, d_counts, d_wsums);
 }
 
 }  // namespace acf

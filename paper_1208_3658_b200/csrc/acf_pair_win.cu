@@ -823,7 +823,7 @@ constexpr int kWarpHeader = 128;
 struct CtaHeader {
     unsigned long long stat[8];
     PackInfo pack;
-    uint32_t n_items, chunk, n_jobs, split, pad[2];
+    uint32_t n_items, chunk, n_jobs, split, pad[4];
 };
 static_assert(kNumStats <= 8 && sizeof(CtaHeader) % 16 == 0, "");
 

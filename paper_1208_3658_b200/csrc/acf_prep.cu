@@ -204,12 +204,9 @@ gather_caps_kernel(const double *__restrict__ xyz, size_t stride, size_t off, co
     const bool packed = mx_bits != 0u && ex_min >= 1 && ex_max - ex_min <= 13;
     const double packC = __hiloint2double((ex_max - 127 + 9 + 1023) << 20, 0);
     if (blockIdx.x == 0 && threadIdx.x == 0) {
-        PackInfo pi;
-        pi.C = packC;
-        pi.inv_C = __hiloint2double((127 - 9 - ex_max + 1023) << 20, 0);
-        pi.packed = packed ? 1 : 0;
-        pi.pad = 0;
-        *pack = pi;
+        pack->C = packC;  // (bad and eps are the validation's)
+        pack->inv_C = __hiloint2double((127 - 9 - ex_max + 1023) << 20, 0);
+        pack->packed = packed ? 1 : 0;
     }
 #pragma unroll
     for (int r = 0; r < kPer; ++r) {
@@ -386,11 +383,11 @@ __device__ __forceinline__ void cap_pair_bounds(const double4 a, const double4 b
 // and appends items {ti, first j-tile, number of j-tiles <= kItemTiles}.
 __global__ void __launch_bounds__(256)
 worklist_kernel(const double4 *__restrict__ caps_a, int ti_begin, int ti_end, const double4 *__restrict__ caps_b,
-                int n_tiles_b, int is_auto, int prune, int max_len, double e_first, double e_last,
+                int n_tiles_b, int is_auto, int prune, int max_len, int ti_stride, double e_first, double e_last,
                 int3 *__restrict__ items, uint32_t capacity, unsigned long long *__restrict__ counters)
 {
     extern __shared__ uint32_t keep[];  // bitmap over j tiles
-    const int ti = ti_begin + blockIdx.x;
+    const int ti = ti_begin + blockIdx.x * ti_stride;
     if (ti >= ti_end) return;
     const int words = (n_tiles_b + 31) / 32;
     const int tj_first = is_auto ? ti : 0;
@@ -446,7 +443,7 @@ worklist_kernel(const double4 *__restrict__ caps_a, int ti_begin, int ti_end, co
 }  // namespace
 
 // ------------------------------------------------------------------ host side
-int prepare_catalogue(acf_ctx *ctx, int slot, const double *xyz, size_t stride, size_t off, size_t cnt,
+int prepare_catalogue(acf_ctx *ctx, CatBuffers &buf, const double *xyz, size_t stride, size_t off, size_t cnt,
                       const float *w, Prepared *out)
 {
     cudaStream_t st = ctx->stream;
@@ -457,29 +454,31 @@ int prepare_catalogue(acf_ctx *ctx, int slot, const double *xyz, size_t stride, 
     out->stride = stride;
     out->n = cnt;
     out->n_tiles = n_tiles;
+    ACF_CUDA_TRY(ctx, buf.pack.reserve(64));
+    out->pack = buf.pack.as<PackInfo>();
+    ACF_CUDA_TRY(ctx, cudaMemsetAsync(out->pack, 0, 64, st));
     if (cnt == 0) return ACF_OK;
+    ACF_CUDA_TRY(ctx, launch_validate(ctx, xyz, stride, off, cnt, w, out->pack));
     const size_t padded = (size_t)n_tiles * kTile;
-    ACF_CUDA_TRY(ctx, ctx->s_pts[slot].reserve(sizeof(float4) * padded));
-    ACF_CUDA_TRY(ctx, ctx->s_perm[slot].reserve(sizeof(uint32_t) * padded));
-    ACF_CUDA_TRY(ctx, ctx->s_caps[slot].reserve(sizeof(double4) * (size_t)n_tiles));
-    ACF_CUDA_TRY(ctx, ctx->s_gcaps[slot].reserve(sizeof(GroupCap) * (size_t)n_tiles * kGroupsPerTile));
-    ACF_CUDA_TRY(ctx, ctx->s_scaps[slot].reserve(sizeof(GroupCap) * (size_t)n_tiles * kGroupsPerTile * kSubsPerGroup));
-    ACF_CUDA_TRY(ctx, ctx->s_keys[slot].reserve(sizeof(uint32_t) * 4 * (size_t)n));  // keys x2, idx x2
-    ACF_CUDA_TRY(ctx, ctx->s_pts2[slot].reserve(sizeof(float4) * padded));
-    ACF_CUDA_TRY(ctx, ctx->s_vj[slot].reserve(sizeof(double) * padded));
-    ACF_CUDA_TRY(ctx, ctx->s_pack[slot].reserve(64));
+    ACF_CUDA_TRY(ctx, buf.pts.reserve(sizeof(float4) * padded));
+    ACF_CUDA_TRY(ctx, buf.perm.reserve(sizeof(uint32_t) * padded));
+    ACF_CUDA_TRY(ctx, buf.caps.reserve(sizeof(double4) * (size_t)n_tiles));
+    ACF_CUDA_TRY(ctx, buf.gcaps.reserve(sizeof(GroupCap) * (size_t)n_tiles * kGroupsPerTile));
+    ACF_CUDA_TRY(ctx, buf.scaps.reserve(sizeof(GroupCap) * (size_t)n_tiles * kGroupsPerTile * kSubsPerGroup));
+    ACF_CUDA_TRY(ctx, ctx->s_keys.reserve(sizeof(uint32_t) * 4 * (size_t)n));  // keys x2, idx x2
+    ACF_CUDA_TRY(ctx, buf.pts2.reserve(sizeof(float4) * padded));
+    ACF_CUDA_TRY(ctx, buf.vj.reserve(sizeof(double) * padded));
     const uint32_t nblocks = (n + kSortBlockChunk - 1) / kSortBlockChunk;
     ACF_CUDA_TRY(ctx, ctx->s_misc.reserve(sizeof(uint32_t) * 256 * (size_t)nblocks));
-    out->pts = ctx->s_pts[slot].as<float4>();
-    out->perm = ctx->s_perm[slot].as<uint32_t>();
-    out->caps = ctx->s_caps[slot].as<double4>();
-    out->gcaps = ctx->s_gcaps[slot].as<GroupCap>();
-    out->scaps = ctx->s_scaps[slot].as<GroupCap>();
-    out->pts2 = ctx->s_pts2[slot].as<float>();
-    out->vj = ctx->s_vj[slot].as<double>();
-    out->pack = ctx->s_pack[slot].as<PackInfo>();
-    uint32_t *range = reinterpret_cast<uint32_t *>(ctx->s_pack[slot].as<char>() + 32);
-    uint32_t *k0 = ctx->s_keys[slot].as<uint32_t>(), *k1 = k0 + n, *i0 = k1 + n, *i1 = i0 + n;
+    out->pts = buf.pts.as<float4>();
+    out->perm = buf.perm.as<uint32_t>();
+    out->caps = buf.caps.as<double4>();
+    out->gcaps = buf.gcaps.as<GroupCap>();
+    out->scaps = buf.scaps.as<GroupCap>();
+    out->pts2 = buf.pts2.as<float>();
+    out->vj = buf.vj.as<double>();
+    uint32_t *range = reinterpret_cast<uint32_t *>(buf.pack.as<char>() + 48);
+    uint32_t *k0 = ctx->s_keys.as<uint32_t>(), *k1 = k0 + n, *i0 = k1 + n, *i1 = i0 + n;
     uint32_t *counts = ctx->s_misc.as<uint32_t>();
 
     int blocks = (int)((n + 255) / 256);
@@ -496,7 +495,6 @@ int prepare_catalogue(acf_ctx *ctx, int slot, const double *xyz, size_t stride, 
         t = i0; i0 = i1; i1 = t;
     }
     if (w) {
-        ACF_CUDA_TRY(ctx, cudaMemsetAsync(range, 0, 2 * sizeof(uint32_t), st));
         wrange_kernel<<<blocks, 256, 0, st>>>(w, off, n, range);
         ctx->last.kernel_launches++;
     }
@@ -507,17 +505,17 @@ int prepare_catalogue(acf_ctx *ctx, int slot, const double *xyz, size_t stride, 
     return ACF_OK;
 }
 
-int build_worklist(acf_ctx *ctx, const Prepared &a, int ti_begin, int ti_end, const Prepared &b, int is_auto,
+int build_worklist(acf_ctx *ctx, const Prepared &a, int ti_begin, int ti_end, int ti_stride, const Prepared &b, int is_auto,
                    double e_first, double e_last, int3 *items, uint32_t capacity)
 {
-    const int n_ti = ti_end - ti_begin;
+    const int n_ti = (ti_end - ti_begin + ti_stride - 1) / ti_stride;
     if (n_ti <= 0 || b.n_tiles == 0) return ACF_OK;
     const size_t smem = sizeof(uint32_t) * (size_t)((b.n_tiles + 31) / 32);
     // items of up to kItemTiles j-tiles; shorter ones when the whole call is only a few tile pairs (small catalogues)
     long long max_len = (long long)n_ti * b.n_tiles / ((long long)ctx->num_sms * 64);
     max_len = max_len < 1 ? 1 : (max_len > kItemTiles ? kItemTiles : max_len);
     if (smem > 48 * 1024) return fail(ctx, ACF_EINVAL, "catalogue too large for the work-list kernel (%d tiles)", b.n_tiles);
-    worklist_kernel<<<n_ti, 256, smem, ctx->stream>>>(a.caps, ti_begin, ti_end, b.caps, b.n_tiles, is_auto, ctx->opt_prune, (int)max_len,
+    worklist_kernel<<<n_ti, 256, smem, ctx->stream>>>(a.caps, ti_begin, ti_end, b.caps, b.n_tiles, is_auto, ctx->opt_prune, (int)max_len, ti_stride,
                                                      e_first, e_last, items, capacity, ctx->d_counters);
     ctx->last.kernel_launches++;
     ACF_CUDA_TRY(ctx, cudaGetLastError());

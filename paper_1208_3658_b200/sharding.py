@@ -64,3 +64,13 @@ def sharded_pair_count(ctx, d_a, d_wa, d_b, d_wb, cos_edges, is_auto, rank: int,
     out = B.acf_pair_count_rows(ctx, d_a, d_wa, lo, hi, d_b, d_wb, cos_edges, is_auto)
     counts, wsums = out if d_wa is not None else (out, None)
     return all_reduce_counts(counts, wsums, group)
+
+
+def sharded_pair_count_prepared(ctx, cat_a, cat_b, cos_edges, rank: int, world_size: int, weighted=None, group=None):
+    """The same on prepared catalogues (acf_prepare on every rank): rank r counts part r of world_size interleaved
+    slices of the pair matrix -- the i-tiles of the sorted catalogue dealt out in turn, so that the slices are
+    balanced whatever the pruning leaves of them -- and the histograms are summed.  Nothing is prepared again."""
+    from . import binding as B
+    out = B.acf_pair_count_prepared(ctx, cat_a, cat_b, cos_edges, part=rank, n_parts=world_size, weighted=weighted)
+    counts, wsums = out if isinstance(out, tuple) else (out, None)
+    return all_reduce_counts(counts, wsums, group)

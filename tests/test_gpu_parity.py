@@ -468,3 +468,57 @@ def test_correlate_host_end_to_end(acf, ctx, oracle):
                   oracle.pair_count(xr, None, t.cos_edges, True))
     assert res["dd"].tolist() == dd.tolist() and res["dr"].tolist() == dr.tolist() and res["rr"].tolist() == rr.tolist()
     np.testing.assert_allclose(res["w"], oracle.wtheta(dd, dr, rr, t.n_d, t.n_r), rtol=0, atol=WTHETA_ATOL, equal_nan=True)
+
+
+def test_prepared_catalogues(acf, ctx, oracle):
+    """acf_prepare / acf_pair_count_prepared: the catalogues of an estimate prepared once, DD, DR, RR counted on
+    the handles (weighted and not), the interleaved parts of a count adding up to the whole, a row range prepared
+    as a catalogue of its own, bad input refused when it is prepared."""
+    import torch
+    w = make_config("full_sky", 0.006)
+    xd, xr = acf.acf_radec_to_xyz(w.ra_d, w.dec_d), acf.acf_radec_to_xyz(w.ra_r, w.dec_r)
+    dxd, dxr, dwd, dwr = dev(xd), dev(xr), dev(w.w_d), dev(w.w_r)
+    cd, cr = acf.acf_prepare(ctx, dxd, dwd), acf.acf_prepare(ctx, dxr, dwr)
+    try:
+        for a, b, xa, xb, wa, wb, auto in ((cd, None, xd, None, w.w_d, None, True), (cd, cr, xd, xr, w.w_d, w.w_r, False),
+                                           (cr, None, xr, None, w.w_r, None, True)):
+            want = oracle.pair_count(xa, xb, w.cos_edges, auto, w_a=wa, w_b=wb)
+            c, s = acf.acf_pair_count_prepared(ctx, a, b, w.cos_edges)
+            torch.cuda.synchronize()
+            assert acf.counts_to_numpy(c).tolist() == want[0].tolist()
+            np.testing.assert_allclose(s.cpu().numpy(), want[1], rtol=WSUM_RTOL, atol=0)
+            st = acf.acf_get_stats(ctx)
+            assert st["pairs_evaluated"] == st["pairs_nominal"] == (a.n * (a.n - 1) // 2 if auto else a.n * b.n)
+            # the same handles, unweighted
+            cu = acf.acf_pair_count_prepared(ctx, a, b, w.cos_edges, weighted=False)
+            torch.cuda.synchronize()
+            assert acf.counts_to_numpy(cu).tolist() == want[0].tolist()
+            # parts: the slices of the pair matrix add up, more parts than tiles included
+            for n_parts in (3, 40):
+                tot_c, tot_s = np.zeros_like(want[0]), np.zeros_like(want[1])
+                for part in range(n_parts):
+                    c, s = acf.acf_pair_count_prepared(ctx, a, b, w.cos_edges, part=part, n_parts=n_parts)
+                    torch.cuda.synchronize()
+                    tot_c += acf.counts_to_numpy(c)
+                    tot_s += s.cpu().numpy()
+                assert tot_c.tolist() == want[0].tolist()
+                np.testing.assert_allclose(tot_s, want[1], rtol=WSUM_RTOL, atol=0)
+        # rows of the data as a catalogue of their own against the randoms
+        rows = (1000, 3500)
+        ck = acf.acf_prepare_rows(ctx, dxd, None, *rows)
+        c = acf.acf_pair_count_prepared(ctx, ck, cr, w.cos_edges, weighted=False)
+        torch.cuda.synchronize()
+        assert acf.counts_to_numpy(c).tolist() == oracle.pair_count(xd, xr, w.cos_edges, False, rows=rows).tolist()
+        acf.acf_release(ctx, ck)
+        with pytest.raises(acf.AcfError):
+            acf.acf_pair_count_prepared(ctx, cd, cr, w.cos_edges, part=3, n_parts=3)
+    finally:
+        acf.acf_release(ctx, cd)
+        acf.acf_release(ctx, cr)
+    bad = xd.copy()
+    bad[5] = 3.0
+    with pytest.raises(acf.AcfError) as ei:
+        acf.acf_prepare(ctx, dev(bad))
+    assert ei.value.code == -1 and "unit" in str(ei.value)
+    # the context still works afterwards
+    assert int(acf.counts_to_numpy(acf.acf_pair_count(ctx, dxd, None, np.array([1.0, -1.0]), True)).sum()) == w.n_d * (w.n_d - 1) // 2

@@ -9,7 +9,7 @@ one-call result bit for bit (weighted sums to 1e-12), at the full sizes of confi
 import numpy as np
 import pytest
 
-from paper_1208_3658_b200.sharding import pairs_before_row, row_ranges, sharded_pair_count
+from paper_1208_3658_b200.sharding import pairs_before_row, row_ranges, sharded_pair_count, sharded_pair_count_prepared
 from workloads import make_config
 
 pytestmark = pytest.mark.gpu
@@ -71,6 +71,27 @@ def test_rank_slices_add_up_to_the_unsharded_count(acf, ctx, name, scale, world)
         assert sum_c.tolist() == whole_c.tolist(), (name, auto)
         if weighted:
             np.testing.assert_allclose(sum_w, whole_w, rtol=1e-12, atol=0)
+        # the same job on prepared catalogues: interleaved tile slices, nothing prepared twice
+        ca = acf.acf_prepare(ctx, a, wa)
+        cb = None if auto else acf.acf_prepare(ctx, b, wb)
+        sum_c[:] = 0
+        sum_w[:] = 0
+        evaluated = []
+        for rank in range(world):
+            out = sharded_pair_count_prepared(ctx, ca, cb, w.cos_edges, rank, world)
+            torch.cuda.synchronize()
+            c, s = to_np(acf, out, weighted)
+            evaluated.append(acf.acf_get_stats(ctx)["pairs_evaluated"])
+            sum_c += c
+            if weighted:
+                sum_w += s
+        acf.acf_release(ctx, ca)
+        acf.acf_release(ctx, cb)
+        assert sum_c.tolist() == whole_c.tolist(), (name, auto, "prepared")
+        if weighted:
+            np.testing.assert_allclose(sum_w, whole_w, rtol=1e-12, atol=0)
+        if scale == 1.0:
+            assert max(evaluated) <= 1.15 * (sum(evaluated) / world), evaluated   # the slices are balanced
     if scale < 0.01:
         # more ranks than rows: empty slices are legal and count nothing
         assert any(lo == hi for lo, hi in row_ranges(w.n_d, w.n_d, True, 64))
