@@ -31,6 +31,10 @@
  *     (cosines of ascending angle edges).  1 <= nbins <= ACF_MAX_BINS.
  *   - Device work is enqueued on the context's stream and is asynchronous unless
  *     stated; results in device buffers are valid after that stream is synchronised.
+ *     (acf_pair_count* prepare their catalogues on the fly and wait on the host for the validation verdict; the
+ *     counts on prepared handles never wait.)
+ *   - A catalogue holds at most 2^31 - 1 points; the tile-level work list keeps one bit per tile of 1024 points
+ *     of the second catalogue in 48 KB of shared memory, i.e. up to 4.0e8 points there (ACF_EINVAL beyond).
  *   - Every function returns ACF_OK (0) or a negative ACF_E* code, never throws,
  *     aborts or prints; acf_last_error() gives the message of the last failure on
  *     that context.  A context is not thread-safe: one caller at a time.
@@ -187,6 +191,12 @@ int acf_pair_count_rows(acf_ctx *ctx, const double *d_a, const float *d_wa, size
 int acf_prepare(acf_ctx *ctx, const double *d_xyz, const float *d_w, size_t n, acf_catalog **out);
 int acf_prepare_rows(acf_ctx *ctx, const double *d_xyz, const float *d_w, size_t n, size_t i_begin, size_t i_end,
                      acf_catalog **out);
+/* Prepares `cat` again on new data (or the same buffers with new contents), reusing its device memory: a pipeline
+ * that counts one catalogue after another of about the same size (the many random catalogues of a Monte-Carlo error
+ * estimate) allocates once.  Same arguments, waits and errors as acf_prepare_rows; after an error the
+ * handle holds an empty catalogue. */
+int acf_prepare_again(acf_ctx *ctx, acf_catalog *cat, const double *d_xyz, const float *d_w, size_t n, size_t i_begin,
+                      size_t i_end);
 void acf_release(acf_ctx *ctx, acf_catalog *cat);
 
 /*

@@ -26,7 +26,7 @@ EXPORTS = [
     "acf_create", "acf_destroy", "acf_last_error", "acf_set_option", "acf_set_stream", "acf_radec_to_xyz",
     "acf_pair_count", "acf_pair_count_weighted", "acf_pair_count_rows", "acf_wtheta", "acf_wtheta_weighted",
     "acf_estimator", "acf_theta_edges", "acf_cos_edges", "acf_jackknife", "acf_correlate_host", "acf_get_stats", "acf_version",
-    "acf_prepare", "acf_prepare_rows", "acf_release", "acf_pair_count_prepared",
+    "acf_prepare", "acf_prepare_rows", "acf_prepare_again", "acf_release", "acf_pair_count_prepared",
 ]
 
 
@@ -84,6 +84,7 @@ def load_library(build_if_missing: bool = True):
     lib.acf_correlate_host.argtypes = [vp, vp, vp, vp, sz, vp, vp, vp, sz, vp, i32, vp, vp, vp, vp, vp, vp, vp]
     lib.acf_prepare.argtypes = [vp, vp, vp, sz, ctypes.POINTER(vp)]
     lib.acf_prepare_rows.argtypes = [vp, vp, vp, sz, sz, sz, ctypes.POINTER(vp)]
+    lib.acf_prepare_again.argtypes = [vp, vp, vp, vp, sz, sz, sz]
     lib.acf_release.argtypes = [vp, vp]
     lib.acf_release.restype = None
     lib.acf_pair_count_prepared.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp, vp]
@@ -239,6 +240,20 @@ def acf_prepare(ctx, d_xyz, d_w=None, rows=None) -> Catalog:
 
 def acf_prepare_rows(ctx, d_xyz, d_w, i_begin, i_end) -> Catalog:
     return acf_prepare(ctx, d_xyz, d_w, rows=(i_begin, i_end))
+
+
+def acf_prepare_again(ctx, cat: Catalog, d_xyz, d_w=None, rows=None) -> Catalog:
+    """Re-prepares the handle on new data, reusing its device memory."""
+    import torch
+    a, pa = _dev(d_xyz, torch.float64, "d_xyz")
+    n = _n_points(a)
+    w, pw = _dev(d_w, torch.float32, "d_w")
+    lo, hi = (0, n) if rows is None else (int(rows[0]), int(rows[1]))
+    rc = load_library().acf_prepare_again(ctx, cat.handle, pa, pw, n, lo, hi)
+    cat.d_xyz, cat.d_w, cat.n = a, w, hi - lo
+    if rc != ACF_OK:
+        _raise(ctx, rc)
+    return cat
 
 
 def acf_release(ctx, cat: Catalog) -> None:

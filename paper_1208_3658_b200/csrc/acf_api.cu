@@ -302,6 +302,8 @@ extern "C" int acf_prepare_rows(acf_ctx *ctx, const double *d_xyz, const float *
     if (!cat) return acf::fail(ctx, ACF_ENOMEM, "out of host memory");
     cat->ctx = ctx;
     cat->weighted = d_w != nullptr;
+    ctx->last = acf_stats{};  // (acf_get_stats after a preparation: its kernel launches)
+    ctx->stats_pending = false;
     int rc = acf::prepare_catalogue(ctx, cat->buf, d_xyz, n, i_begin, i_end - i_begin, d_w, &cat->p);
     if (rc == ACF_OK) {
         cudaError_t e = cudaMemcpyAsync(&ctx->h_verdict[0], &cat->p.pack->bad, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream);
@@ -323,6 +325,35 @@ extern "C" int acf_prepare_rows(acf_ctx *ctx, const double *d_xyz, const float *
     ctx->n_catalogs++;
     *out = cat;
     return ACF_OK;
+}
+
+extern "C" int acf_prepare_again(acf_ctx *ctx, acf_catalog *cat, const double *d_xyz, const float *d_w, size_t n, size_t i_begin,
+                                 size_t i_end)
+{
+    if (!ctx) return ACF_EINVAL;
+    ctx->err[0] = 0;
+    if (!cat || cat->ctx != ctx) return acf::fail(ctx, ACF_EINVAL, "catalogue handle is NULL or of another context");
+    if (n && !d_xyz) return acf::fail(ctx, ACF_EINVAL, "catalogue pointer is NULL");
+    if (i_begin > i_end || i_end > n) return acf::fail(ctx, ACF_EINVAL, "row range [%zu, %zu) outside [0, %zu]", i_begin, i_end, n);
+    if (n >= (size_t(1) << 31)) return acf::fail(ctx, ACF_EINVAL, "catalogues are limited to 2^31-1 points");
+    ACF_CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    cat->weighted = d_w != nullptr;
+    ctx->last = acf_stats{};  // (acf_get_stats after a preparation: its kernel launches)
+    ctx->stats_pending = false;
+    int rc = acf::prepare_catalogue(ctx, cat->buf, d_xyz, n, i_begin, i_end - i_begin, d_w, &cat->p);
+    if (rc == ACF_OK) {
+        cudaError_t e = cudaMemcpyAsync(&ctx->h_verdict[0], &cat->p.pack->bad, sizeof(int), cudaMemcpyDeviceToHost, ctx->stream);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(ctx->stream);
+        if (e != cudaSuccess) rc = acf::fail(ctx, ACF_ECUDA, "acf_prepare: %s", cudaGetErrorString(e));
+        else if (ctx->h_verdict[0] != 0)
+            rc = acf::fail(ctx, ACF_EINVAL, "%d input points are not finite unit vectors (|r^2 - 1| <= 1e-6) or carry a negative / non-finite weight",
+                           ctx->h_verdict[0]);
+    }
+    if (rc != ACF_OK) {
+        cat->p.n = 0;
+        cat->p.n_tiles = 0;
+    }
+    return rc;
 }
 
 extern "C" int acf_prepare(acf_ctx *ctx, const double *d_xyz, const float *d_w, size_t n, acf_catalog **out)
@@ -531,13 +562,17 @@ extern "C" int acf_correlate_host(acf_ctx *ctx, const double *ra_d, const double
     if (weighted && n_d) memcpy(h_wd, w_d, sizeof(float) * n_d);
     if (n_d) ACF_CUDA_TRY(ctx, cudaMemcpyAsync(d_xd, h_xyz_d, sizeof(double) * 3 * n_d, cudaMemcpyHostToDevice, st));
     if (weighted && n_d) ACF_CUDA_TRY(ctx, cudaMemcpyAsync(d_wd, h_wd, sizeof(float) * n_d, cudaMemcpyHostToDevice, st));
-    acf_catalog *cd = nullptr, *cr = nullptr;
-    int rc = acf_prepare(ctx, d_xd, d_wd, n_d, &cd);
+    // the two handles live with the context: prepared again on every call, their device memory reused
+    auto prepare = [&](int k, const double *x, const float *wt, size_t n) -> int {
+        if (!ctx->e2e_cat[k]) return acf_prepare(ctx, x, wt, n, &ctx->e2e_cat[k]);
+        return acf_prepare_again(ctx, ctx->e2e_cat[k], x, wt, n, 0, n);
+    };
+    int rc = prepare(0, d_xd, d_wd, n_d);
     if (rc != ACF_OK) return rc;
+    acf_catalog *&cd = ctx->e2e_cat[0], *&cr = ctx->e2e_cat[1];
     auto bail = [&](int code) {
         cudaStreamSynchronize(ctx->copy_stream);
-        acf_release(ctx, cd);
-        acf_release(ctx, cr);
+        cudaStreamSynchronize(st);
         return code;
     };
     acf_stats st_sum{};
@@ -554,7 +589,7 @@ extern "C" int acf_correlate_host(acf_ctx *ctx, const double *ra_d, const double
     if (weighted && n_r) ACF_CUDA_TRY(ctx, cudaMemcpyAsync(d_wr, h_wr, sizeof(float) * n_r, cudaMemcpyHostToDevice, ctx->copy_stream));
     ACF_CUDA_TRY(ctx, cudaEventRecord(ctx->ev_copy, ctx->copy_stream));
     ACF_CUDA_TRY(ctx, cudaStreamWaitEvent(st, ctx->ev_copy, 0));
-    rc = acf_prepare(ctx, d_xr, d_wr, n_r, &cr);
+    rc = prepare(1, d_xr, d_wr, n_r);
     if (rc != ACF_OK) return bail(rc);
     rc = acf_pair_count_prepared(ctx, cd, cr, cos_edges, nbins, 0, 1, d_cnt + nbins, d_ws ? d_ws + nbins : nullptr);
     if (rc != ACF_OK) return bail(rc);
@@ -567,8 +602,6 @@ extern "C" int acf_correlate_host(acf_ctx *ctx, const double *ra_d, const double
     if (weighted) ACF_CUDA_TRY(ctx, cudaMemcpyAsync(h_ws, d_ws, sizeof(double) * 3 * (size_t)nbins, cudaMemcpyDeviceToHost, st));
     {
         const cudaError_t e = cudaStreamSynchronize(st);
-        acf_release(ctx, cd);
-        acf_release(ctx, cr);
         if (e != cudaSuccess) return acf::fail(ctx, ACF_ECUDA, "acf_correlate_host: %s", cudaGetErrorString(e));
         ctx->last.pairs_nominal = st_sum.pairs_nominal;
         ctx->last.kernel_launches = st_sum.kernel_launches;

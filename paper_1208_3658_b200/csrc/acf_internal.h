@@ -159,6 +159,7 @@ struct acf_ctx {
     cudaEvent_t ev_tables = nullptr; // the last copy out of h_tables
     cudaStream_t copy_stream = nullptr;  // acf_correlate_host: host-to-device copies that overlap the counts
     cudaEvent_t ev_copy = nullptr;
+    struct acf_catalog *e2e_cat[2] = {nullptr, nullptr};  // acf_correlate_host: its two handles, kept between calls (no cudaMalloc / cudaFree per call)
     int n_catalogs = 0;              // acf_catalog handles alive (acf_destroy refuses to leave them dangling: it frees them)
     struct acf_catalog *catalogs = nullptr;  // intrusive list of the handles
 };

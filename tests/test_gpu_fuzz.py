@@ -114,3 +114,61 @@ def test_random_cases_all_kernels(acf, oracle, seed):
                     np.testing.assert_allclose(out[1].cpu().numpy(), want[1], rtol=WSUM_RTOL, atol=0, err_msg=str((seed, kern, bulk)))
     finally:
         acf.acf_destroy(ctx)
+
+
+@pytest.mark.parametrize("kernel", ["window", "table"])
+@pytest.mark.parametrize("bulk", [0, 1])
+def test_inexact_norms_and_tight_groups(acf, oracle, kernel, bulk):
+    """Vectors whose norms are off 1 by what the validation accepts (| |u|^2 - 1 | <= 1e-6), in tight groups: the
+    pair cosine of the definition carries the norms, so a bounding cap built from the directions alone would put a
+    whole window on the wrong side of an edge (round-1 advice).  First the constructed case -- 1024 copies of
+    a (1 + 4e-7) against 1024 copies of b (1 + 4e-7), 1e-3 rad apart, an edge at cos(theta) (1 + 4e-7): every pair has
+    c = (1 + 8e-7) cos(theta) > e_m and lies before the edge, although the directions alone say beyond it -- then
+    antipodal points with norms above 1 and e_n = -1, then seeded clumps with random norms and edges at the clumps'
+    separations.  Both fast kernels, with and without ACF_OPT_BULK."""
+    import torch
+    kern = {"window": acf.ACF_KERNEL_WINDOW, "table": acf.ACF_KERNEL_TABLE}[kernel]
+    ctx = acf.acf_create(0)
+    acf.acf_set_option(ctx, acf.ACF_OPT_KERNEL, kern)
+    acf.acf_set_option(ctx, acf.ACF_OPT_BULK, bulk)
+
+    def run(a, b, edges, auto=False):
+        da = torch.from_numpy(a).cuda()
+        db = None if auto else torch.from_numpy(b).cuda()
+        out = acf.acf_pair_count_rows(ctx, da, None, 0, a.size // 3, db, None, edges, auto)
+        torch.cuda.synchronize()
+        return acf.counts_to_numpy(out).tolist()
+
+    try:
+        theta = 1.0e-3
+        s = 1.0 + 4.0e-7
+        a = np.tile(np.array([[1.0], [0.0], [0.0]]) * s, (1, 1024)).reshape(-1)
+        b = np.tile(np.array([[np.cos(theta)], [np.sin(theta)], [0.0]]) * s, (1, 1024)).reshape(-1)
+        edges = np.array([1.0, np.cos(theta) * s, np.cos(2 * theta), 0.0, -1.0])
+        want = oracle.pair_count(a, b, edges, False).tolist()
+        assert want[0] == 1024 * 1024   # the definition puts every pair before the edge
+        assert run(a, b, edges) == want
+        # antipodal points a little longer than 1, last edge at the pole: c clamps to -1 and belongs to the last bin
+        a2 = np.concatenate([a.reshape(3, -1), -a.reshape(3, -1)], axis=1).reshape(-1)
+        assert run(a2, None, edges, auto=True) == oracle.pair_count(a2, None, edges, True).tolist()
+        rng = np.random.default_rng(99)
+        for trial in range(6):
+            n_cl = int(rng.integers(3, 40))
+            centres = rng.normal(size=(n_cl, 3))
+            centres /= np.linalg.norm(centres, axis=1, keepdims=True)
+            sig = float(rng.choice([1e-6, 1e-4, 1e-3]))
+            def clumps(n):
+                p = centres[rng.integers(0, n_cl, n)] + sig * rng.normal(size=(n, 3))
+                p /= np.linalg.norm(p, axis=1, keepdims=True)
+                p *= (1.0 + rng.uniform(-4.5e-7, 4.5e-7, n))[:, None]
+                return np.ascontiguousarray(p.T).reshape(-1)
+            a, b = clumps(int(rng.choice([1024, 1500, 2600]))), clumps(int(rng.choice([1024, 2048, 3000])))
+            # edges at the cosines of the separations of the clump centres, nudged by the size of the norm effect
+            c = np.unique(np.clip(centres @ centres.T, -1, 1).round(12))
+            c = c[(c > -0.999) & (c < 0.999999)]
+            pick = rng.choice(c, size=min(12, c.size), replace=False) * (1.0 + rng.uniform(-8e-7, 8e-7, min(12, c.size)))
+            edges = np.unique(np.concatenate([[1.0, -1.0], pick]))[::-1].copy()
+            assert run(a, b, edges) == oracle.pair_count(a, b, edges, False).tolist(), (trial, "cross")
+            assert run(a, None, edges, auto=True) == oracle.pair_count(a, None, edges, True).tolist(), (trial, "auto")
+    finally:
+        acf.acf_destroy(ctx)
