@@ -385,6 +385,30 @@ def jackknife_line(P, ctx, dev):
     return out
 
 
+def ensemble_line(P, ctx, dev):
+    """acf_random_ensemble: the clustered patch's data against 8 random catalogues (detail.mc_randoms)."""
+    import torch
+    w = make_config("clustered_patch", 1.0)
+    K = 8
+    xd = torch.from_numpy(P.acf_radec_to_xyz(w.ra_d, w.dec_d)).to(dev)
+    rands = []
+    for k in range(K):
+        r = make_config("clustered_patch", 1.0, seed_offset=100 + k)
+        rands.append(torch.from_numpy(P.acf_radec_to_xyz(r.ra_r, r.dec_r)).to(dev))
+    cat = P.acf_prepare(ctx, xd)
+    P.acf_random_ensemble(ctx, cat, rands[:2], w.cos_edges)
+    torch.cuda.synchronize(dev)
+    t0 = time.perf_counter()
+    res = P.acf_random_ensemble(ctx, cat, rands, w.cos_edges)
+    dt = time.perf_counter() - t0
+    launches = P.acf_get_stats(ctx)["kernel_launches"]
+    P.acf_release(ctx, cat)
+    pairs = w.n_d * (w.n_d - 1) // 2 + K * (w.n_d * w.n_r + w.n_r * (w.n_r - 1) // 2)
+    sd = np.sqrt(np.diag(res["cov"]))
+    return {"workload": "clustered_patch x1 data, %d random catalogues of %d points, Landy-Szalay" % (K, w.n_r), "seconds": dt,
+            "launches": launches, "gpairs_s_nominal": pairs / dt / 1e9, "median_sigma_w": float(np.nanmedian(sd))}
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
@@ -509,7 +533,7 @@ def main():
     }
 
     # ---- the five configurations and the jackknife, one short measurement each (one GPU, rank 0's box only)
-    configs = jk = None
+    configs = jk = mc = None
     if world == 1 and not args.no_configs:
         configs = {}
         for name in ALL_CONFIGS:
@@ -517,6 +541,7 @@ def main():
             configs[name] = config_line(P, ctx, dev, name, flush_buf, stream, peak_tinst, runner=runner if same else None,
                                         e2e=name in ("tiny", "clustered_patch"))
         jk = jackknife_line(P, ctx, dev)
+        mc = ensemble_line(P, ctx, dev)
 
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -537,7 +562,7 @@ def main():
             "detail": {"ms_steps": ms_steps, "wall_s_timed_region": t_wall, "pairs_fp64_per_step": acc["fp64"],
                        "pairs_evaluated_per_step": evaluated_per_step, "pairs_single_edge_window_per_step": acc["window"],
                        "pairs_on_chord_per_step": acc["chord"], "launches_per_step": launches_per_step,
-                       "source_sha16": source_hash(), "version": P.acf_version(), "configs": configs, "jackknife": jk},
+                       "source_sha16": source_hash(), "version": P.acf_version(), "configs": configs, "jackknife": jk, "mc_randoms": mc},
         }
         print(json.dumps(out), flush=True)
     runner.close()

@@ -273,6 +273,25 @@ int acf_jackknife(acf_ctx *ctx, const double *d_xyz_d, size_t n_d, const size_t 
                   int estimator, double *w_full, double *w_jk, double *cov);
 
 /*
+ * Monte-Carlo errors from an ensemble of random catalogues (the speed-up makes "a full MC-based
+ * calculation of the errors" affordable): the data are counted once (DD), every random catalogue k of the ensemble
+ * gives DR_k and RR_k, and the estimator is formed n_random times.  The catalogues stream through two internal
+ * handles (prepared on the device one after the other, nothing allocated per catalogue) and all 2 n_random + 1
+ * counts are enqueued without a host wait in between; the validation verdicts are collected at the end.
+ *   data       : the prepared data catalogue (acf_prepare)
+ *   d_xyz_r    : HOST array of n_random DEVICE pointers, catalogue k: canonical xyz SoA of n_r[k] points
+ *   n_r        : HOST, n_random sizes
+ *   dd         : HOST, nbins uint64;  dr, rr : HOST, n_random x nbins uint64 (row k = catalogue k)
+ *   w          : HOST, n_random x nbins doubles: the estimator with random catalogue k
+ *   mean, cov  : HOST, nbins / nbins x nbins doubles or NULL: mean over k and the sample covariance
+ *                cov[a][b] = 1/(K - 1) sum_k (w_k[a] - mean[a]) (w_k[b] - mean[b])  (K = n_random >= 2 for cov)
+ * Unweighted.  Synchronous.  ACF_EINVAL if any catalogue fails validation (nothing is returned then).
+ */
+int acf_random_ensemble(acf_ctx *ctx, const acf_catalog *data, const double *const *d_xyz_r, const size_t *n_r, int n_random,
+                        const double *cos_edges, int nbins, int estimator, uint64_t *dd, uint64_t *dr, uint64_t *rr,
+                        double *w, double *mean, double *cov);
+
+/*
  * The whole job from HOST buffers: canonicalise both catalogues (acf_radec_to_xyz), copy them
  * to the device, count DD, DR, RR, copy the histograms back and apply Eq. 2.  Synchronous.
  *   ra_*, dec_* : HOST doubles (degrees);  w_d, w_r : HOST floats or both NULL (unweighted)

@@ -4,9 +4,10 @@ Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl refere
 legs may import this module.  It builds the C oracle with gcc on first use (or when
 the source is newer than the shared object) and marshals numpy arrays.  The definition
 (O1-O8) lives in acf_oracle.c, with citations into PAPER.md (arXiv 1208.3658 sect. 2, Eq. 2,
-Appendix A); the only arithmetic written here is the delete-one jackknife at the end of
-the file (`jackknife`, `jackknife_cov`: remove a region, recount with the C functions,
-numpy mean and outer products), pinned on a hand example in tests/test_oracle_pins.py.
+Appendix A); the only arithmetic written here is the resampling at the end of the file: the delete-one
+jackknife (`jackknife`, `jackknife_cov`: remove a region, recount with the C functions, numpy mean
+and outer products) and the ensemble of random catalogues (`random_ensemble`: one count per
+catalogue, numpy mean and sample covariance), pinned on hand examples in tests/test_oracle_pins.py.
 """
 from __future__ import annotations
 
@@ -280,6 +281,28 @@ def jackknife(xyz_d, region_d, xyz_r, region_r, n_regions: int, cos_edges, kind:
     w_full = est(xd, xr)
     w_jk = np.stack([est(xd[:, region_d != k], xr[:, region_r != k]) for k in range(n_regions)])
     return w_full, w_jk, jackknife_cov(w_jk)
+
+
+def ensemble_cov(w_k) -> np.ndarray:
+    """Sample covariance of K estimates (rows of w_k): 1/(K - 1) sum_k (w_k - mean)(w_k - mean)^T."""
+    w_k = np.asarray(w_k, dtype=np.float64)
+    dev = w_k - w_k.mean(axis=0)
+    return dev.T @ dev / (w_k.shape[0] - 1)
+
+
+def random_ensemble(xyz_d, xyz_r_list, cos_edges, kind: int = 0):
+    """PAPER.md:201 (Monte-Carlo errors), by the definition: the data counted once, every random catalogue of the
+    ensemble counted on its own (DR_k, RR_k), the estimator formed with each.  -> (dd, dr[K], rr[K], w[K], mean, cov)."""
+    xd = np.ascontiguousarray(xyz_d, dtype=np.float64)
+    dd = pair_count(xd, None, cos_edges, True)
+    dr, rr, w = [], [], []
+    for xr in xyz_r_list:
+        xr = np.ascontiguousarray(xr, dtype=np.float64)
+        dr.append(pair_count(xd, xr, cos_edges, False))
+        rr.append(pair_count(xr, None, cos_edges, True))
+        w.append(estimator(kind, dd, dr[-1], rr[-1], xd.size // 3, xr.size // 3))
+    w = np.stack(w)
+    return dd, np.stack(dr), np.stack(rr), w, w.mean(axis=0), (ensemble_cov(w) if len(xyz_r_list) > 1 else None)
 
 
 def wtheta_weighted(dd, dr, rr, w_d, w_r) -> np.ndarray:

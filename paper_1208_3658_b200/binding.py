@@ -26,7 +26,7 @@ EXPORTS = [
     "acf_create", "acf_destroy", "acf_last_error", "acf_set_option", "acf_set_stream", "acf_radec_to_xyz",
     "acf_pair_count", "acf_pair_count_weighted", "acf_pair_count_rows", "acf_wtheta", "acf_wtheta_weighted",
     "acf_estimator", "acf_theta_edges", "acf_cos_edges", "acf_jackknife", "acf_correlate_host", "acf_get_stats", "acf_version",
-    "acf_prepare", "acf_prepare_rows", "acf_prepare_again", "acf_release", "acf_pair_count_prepared",
+    "acf_prepare", "acf_prepare_rows", "acf_prepare_again", "acf_release", "acf_pair_count_prepared", "acf_random_ensemble",
 ]
 
 
@@ -88,6 +88,7 @@ def load_library(build_if_missing: bool = True):
     lib.acf_release.argtypes = [vp, vp]
     lib.acf_release.restype = None
     lib.acf_pair_count_prepared.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp, vp]
+    lib.acf_random_ensemble.argtypes = [vp, vp, vp, vp, i32, vp, i32, i32, vp, vp, vp, vp, vp, vp]
     lib.acf_get_stats.argtypes = [vp, ctypes.POINTER(acf_stats)]
     lib.acf_version.restype = ctypes.c_char_p
     for name in EXPORTS:
@@ -372,6 +373,26 @@ def acf_jackknife(ctx, d_xyz_d, off_d, d_xyz_r, off_r, cos_edges, estimator: int
     if rc != ACF_OK:
         raise AcfError(rc, acf_last_error(ctx))
     return {"w": w, "w_jk": w_jk, "cov": cov}
+
+
+def acf_random_ensemble(ctx, data: Catalog, d_xyz_r_list, cos_edges, estimator: int = ACF_EST_LANDY_SZALAY) -> dict:
+    """Monte-Carlo errors from an ensemble of random catalogues (device tensors).
+    -> {"dd", "dr" (K, nbins), "rr" (K, nbins), "w" (K, nbins), "mean", "cov"}."""
+    import torch
+    K = len(d_xyz_r_list)
+    tensors = [_dev(t, torch.float64, "d_xyz_r[%d]" % k)[0] for k, t in enumerate(d_xyz_r_list)]
+    ptrs = (ctypes.c_void_p * K)(*[t.data_ptr() for t in tensors])
+    sizes = (ctypes.c_size_t * K)(*[_n_points(t) for t in tensors])
+    e, pe = _host(cos_edges, np.float64)
+    nbins = e.size - 1
+    out = {"dd": np.zeros(nbins, np.uint64), "dr": np.zeros((K, nbins), np.uint64), "rr": np.zeros((K, nbins), np.uint64),
+           "w": np.zeros((K, nbins)), "mean": np.zeros(nbins), "cov": np.zeros((nbins, nbins)) if K > 1 else None}
+    rc = load_library().acf_random_ensemble(ctx, data.handle, ctypes.cast(ptrs, ctypes.c_void_p), ctypes.cast(sizes, ctypes.c_void_p), K, pe, nbins,
+                                            int(estimator), out["dd"].ctypes.data, out["dr"].ctypes.data, out["rr"].ctypes.data,
+                                            out["w"].ctypes.data, out["mean"].ctypes.data, out["cov"].ctypes.data if K > 1 else None)
+    if rc != ACF_OK:
+        _raise(ctx, rc)
+    return out
 
 
 def acf_wtheta_weighted(wdd, wdr, wrr, w_d, w_r) -> np.ndarray:

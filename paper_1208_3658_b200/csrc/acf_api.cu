@@ -512,6 +512,97 @@ extern "C" int acf_jackknife(acf_ctx *ctx, const double *d_xyz_d, size_t n_d, co
     return ACF_OK;
 }
 
+// Monte-Carlo errors from an ensemble of random catalogues (include/acf.h).
+extern "C" int acf_random_ensemble(acf_ctx *ctx, const acf_catalog *data, const double *const *d_xyz_r, const size_t *n_r, int n_random,
+                                   const double *cos_edges, int nbins, int estimator, uint64_t *dd, uint64_t *dr, uint64_t *rr,
+                                   double *w, double *mean, double *cov)
+{
+    if (!ctx) return ACF_EINVAL;
+    ctx->err[0] = 0;
+    if (const char *why = check_edges(cos_edges, nbins)) return acf::fail(ctx, ACF_EINVAL, "%s", why);
+    if (!data || data->ctx != ctx) return acf::fail(ctx, ACF_EINVAL, "catalogue handle is NULL or of another context");
+    if (n_random < 1 || !d_xyz_r || !n_r || !dd || !dr || !rr || !w) return acf::fail(ctx, ACF_EINVAL, "NULL argument or no random catalogue");
+    if (cov && n_random < 2) return acf::fail(ctx, ACF_EINVAL, "a covariance needs at least two random catalogues");
+    if (estimator < ACF_EST_LANDY_SZALAY || estimator > ACF_EST_HAMILTON) return acf::fail(ctx, ACF_EINVAL, "unknown estimator");
+    if (ctx->opt_kernel == ACF_KERNEL_FP64) return acf::fail(ctx, ACF_EINVAL, "the ensemble runs on prepared catalogues: not with the fp64 reference kernel");
+    for (int k = 0; k < n_random; ++k) {
+        if (n_r[k] && !d_xyz_r[k]) return acf::fail(ctx, ACF_EINVAL, "random catalogue %d is NULL", k);
+        if (n_r[k] >= (size_t(1) << 31)) return acf::fail(ctx, ACF_EINVAL, "catalogues are limited to 2^31-1 points");
+    }
+    ACF_CUDA_TRY(ctx, cudaSetDevice(ctx->device));
+    cudaStream_t st = ctx->stream;
+    const size_t nb = (size_t)nbins, K = (size_t)n_random;
+    // device: DD, then DR_k and RR_k; pinned host: the same, then the verdicts
+    ACF_CUDA_TRY(ctx, ctx->s_host_stage[4].reserve(sizeof(uint64_t) * (2 * K + 1) * nb));
+    uint64_t *d_cnt = ctx->s_host_stage[4].as<uint64_t>();
+    const size_t host_bytes = sizeof(uint64_t) * (2 * K + 1) * nb + sizeof(int) * K;
+    if (ctx->h_stage_bytes < host_bytes) {
+        if (ctx->h_stage) cudaFreeHost(ctx->h_stage);
+        ctx->h_stage = nullptr;
+        ctx->h_stage_bytes = 0;
+        ACF_CUDA_TRY(ctx, cudaHostAlloc(&ctx->h_stage, host_bytes, cudaHostAllocDefault));
+        ctx->h_stage_bytes = host_bytes;
+    }
+    uint64_t *h_cnt = static_cast<uint64_t *>(ctx->h_stage);
+    int *h_bad = reinterpret_cast<int *>(h_cnt + (2 * K + 1) * nb);
+    // two internal handles, used in turn: the preparation of catalogue k + 1 is enqueued behind the counts of catalogue k
+    // (one stream: the buffers of a handle are free again when its counts have run)
+    acf_catalog ring[2];
+    ring[0].ctx = ring[1].ctx = ctx;
+    unsigned long long launches = 0;
+    int rc = acf_pair_count_prepared(ctx, data, nullptr, cos_edges, nbins, 0, 1, d_cnt, nullptr);
+    launches += ctx->last.kernel_launches;
+    for (size_t k = 0; k < K && rc == ACF_OK; ++k) {
+        acf_catalog &c = ring[k & 1];
+        ctx->last = acf_stats{};
+        rc = acf::prepare_catalogue(ctx, c.buf, d_xyz_r[k], n_r[k], 0, n_r[k], nullptr, &c.p);
+        launches += ctx->last.kernel_launches;
+        if (rc != ACF_OK) break;
+        if (cudaMemcpyAsync(&h_bad[k], &c.p.pack->bad, sizeof(int), cudaMemcpyDeviceToHost, st) != cudaSuccess) {
+            rc = acf::fail(ctx, ACF_ECUDA, "copy of the verdict failed");
+            break;
+        }
+        rc = acf_pair_count_prepared(ctx, data, &c, cos_edges, nbins, 0, 1, d_cnt + (1 + k) * nb, nullptr);
+        launches += ctx->last.kernel_launches;
+        if (rc == ACF_OK) rc = acf_pair_count_prepared(ctx, &c, nullptr, cos_edges, nbins, 0, 1, d_cnt + (1 + K + k) * nb, nullptr);
+        launches += ctx->last.kernel_launches;
+    }
+    if (rc == ACF_OK) {
+        cudaError_t e = cudaMemcpyAsync(h_cnt, d_cnt, sizeof(uint64_t) * (2 * K + 1) * nb, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+        if (e != cudaSuccess) rc = acf::fail(ctx, ACF_ECUDA, "acf_random_ensemble: %s", cudaGetErrorString(e));
+    } else {
+        cudaStreamSynchronize(st);
+    }
+    ring[0].buf.release();
+    ring[1].buf.release();
+    if (rc != ACF_OK) return rc;
+    ctx->last.kernel_launches = launches;
+    for (size_t k = 0; k < K; ++k)
+        if (h_bad[k] != 0)
+            return acf::fail(ctx, ACF_EINVAL, "random catalogue %zu: %d points are not finite unit vectors (|r^2 - 1| <= 1e-6)", k, h_bad[k]);
+    memcpy(dd, h_cnt, sizeof(uint64_t) * nb);
+    memcpy(dr, h_cnt + nb, sizeof(uint64_t) * K * nb);
+    memcpy(rr, h_cnt + (1 + K) * nb, sizeof(uint64_t) * K * nb);
+    for (size_t k = 0; k < K; ++k)
+        if ((rc = acf_estimator(estimator, dd, dr + k * nb, rr + k * nb, data->p.n, n_r[k], nbins, w + k * nb)) != ACF_OK) return rc;
+    if (mean || cov) {
+        std::vector<double> m(nb, 0.0);
+        for (size_t k = 0; k < K; ++k)
+            for (size_t b = 0; b < nb; ++b) m[b] += w[k * nb + b];
+        for (size_t b = 0; b < nb; ++b) m[b] /= (double)K;
+        if (mean) memcpy(mean, m.data(), sizeof(double) * nb);
+        if (cov)
+            for (size_t a = 0; a < nb; ++a)
+                for (size_t b = 0; b < nb; ++b) {
+                    double sum = 0.0;
+                    for (size_t k = 0; k < K; ++k) sum += (w[k * nb + a] - m[a]) * (w[k * nb + b] - m[b]);
+                    cov[a * nb + b] = sum / (double)(K - 1);
+                }
+    }
+    return ACF_OK;
+}
+
 extern "C" int acf_correlate_host(acf_ctx *ctx, const double *ra_d, const double *dec_d, const float *w_d, size_t n_d,
                                   const double *ra_r, const double *dec_r, const float *w_r, size_t n_r,
                                   const double *cos_edges, int nbins, uint64_t *dd, uint64_t *dr, uint64_t *rr,

@@ -522,3 +522,34 @@ def test_prepared_catalogues(acf, ctx, oracle):
     assert ei.value.code == -1 and "unit" in str(ei.value)
     # the context still works afterwards
     assert int(acf.counts_to_numpy(acf.acf_pair_count(ctx, dxd, None, np.array([1.0, -1.0]), True)).sum()) == w.n_d * (w.n_d - 1) // 2
+
+
+@pytest.mark.parametrize("est", [0, 1])
+def test_random_ensemble_against_separate_counts(acf, ctx, oracle, est):
+    """acf_random_ensemble (random catalogues of unequal sizes streamed through two handles, every count enqueued
+    without a host wait) against the oracle's one count per catalogue: the same integers, so the same estimates,
+    mean and covariance; a bad catalogue in the ensemble is refused."""
+    w = make_config("clustered_patch", 0.02)
+    xd = acf.acf_radec_to_xyz(w.ra_d, w.dec_d)
+    rands = []
+    for k in range(5):
+        r = make_config("clustered_patch", 0.02 + 0.003 * k, seed_offset=50 + k)
+        rands.append(acf.acf_radec_to_xyz(r.ra_r, r.dec_r))
+    dxd = dev(xd)
+    cat = acf.acf_prepare(ctx, dxd)
+    try:
+        got = acf.acf_random_ensemble(ctx, cat, [dev(x) for x in rands], w.cos_edges, est)
+        dd, dr, rr, wk, mean, cov = oracle.random_ensemble(xd, rands, w.cos_edges, est)
+        assert got["dd"].tolist() == dd.tolist() and got["dr"].tolist() == dr.tolist() and got["rr"].tolist() == rr.tolist()
+        np.testing.assert_allclose(got["w"], wk, rtol=0, atol=WTHETA_ATOL, equal_nan=True)
+        np.testing.assert_allclose(got["mean"], mean, rtol=0, atol=WTHETA_ATOL, equal_nan=True)
+        ok = np.isfinite(cov)
+        assert np.array_equal(np.isfinite(got["cov"]), ok)
+        np.testing.assert_allclose(got["cov"][ok], cov[ok], rtol=1e-9, atol=1e-12)
+        bad = rands[2].copy()
+        bad[7] = float("nan")
+        with pytest.raises(acf.AcfError) as ei:
+            acf.acf_random_ensemble(ctx, cat, [dev(rands[0]), dev(rands[1]), dev(bad)], w.cos_edges, est)
+        assert ei.value.code == -1 and "catalogue 2" in str(ei.value)
+    finally:
+        acf.acf_release(ctx, cat)

@@ -322,6 +322,35 @@ def test_jackknife_pins(oracle):
     assert np.all(np.diag(cov)[ok] >= 0)
 
 
+def test_random_ensemble_pins(oracle):
+    """Monte-Carlo errors from an ensemble of random catalogues.  The covariance formula on a hand
+    example; the ensemble is one count per catalogue (identical catalogues give identical estimates and a zero
+    covariance); on unclustered data the estimates scatter around zero by about their Poisson error."""
+    # rows (1,2),(3,4),(5,6): mean (3,4), deviations (-2,-2),(0,0),(2,2), sum of outer products 8, / (K - 1) = 4
+    np.testing.assert_allclose(oracle.ensemble_cov([[1, 2], [3, 4], [5, 6]]), np.full((2, 2), 4.0), rtol=1e-15)
+    c = oracle.ensemble_cov([[0, 1], [2, 1], [4, 1], [6, 1]])      # variance of 0, 2, 4, 6 is 20 / 3
+    assert c[0, 0] == pytest.approx(20.0 / 3.0) and c[1, 1] == 0 and c[0, 1] == 0
+    w = make_config("tiny", scale=0.08)
+    xd = oracle.radec_to_xyz(w.ra_d, w.dec_d)
+    rands = []
+    for k in range(5):
+        r = make_config("tiny", scale=0.08, seed_offset=100 + k)
+        rands.append(oracle.radec_to_xyz(r.ra_r, r.dec_r))
+    dd, dr, rr, wk, mean, cov = oracle.random_ensemble(xd, rands, w.cos_edges, 0)
+    assert dd.tolist() == oracle.pair_count(xd, None, w.cos_edges, True).tolist()
+    for k in range(5):
+        assert dr[k].tolist() == oracle.pair_count(xd, rands[k], w.cos_edges, False).tolist()
+        assert rr[k].tolist() == oracle.pair_count(rands[k], None, w.cos_edges, True).tolist()
+        np.testing.assert_array_equal(wk[k], oracle.wtheta(dd, dr[k], rr[k], xd.size // 3, rands[k].size // 3))
+    ok = np.isfinite(wk).all(axis=0) & (rr.min(axis=0) > 200)
+    assert ok.sum() >= 3
+    np.testing.assert_allclose(mean[ok], wk[:, ok].mean(axis=0), rtol=1e-15)
+    sd = np.sqrt(np.diag(cov)[ok])
+    assert np.all(sd < 5.0 * np.sqrt(2.0 / rr[:, ok].mean(axis=0)) + 0.02) and np.all(np.abs(mean[ok]) < 5 * sd + 0.05)
+    same = oracle.random_ensemble(xd, [rands[0], rands[0], rands[0]], w.cos_edges, 0)
+    assert np.all(np.abs(same[5][np.isfinite(same[5])]) < 1e-30) and same[3][0].tobytes() == same[3][2].tobytes()
+
+
 def test_O7_unclustered_is_zero_within_noise(oracle):
     # north_star: w(theta) ~ 0 within Poisson noise for an unclustered uniform catalogue
     w = make_config("tiny", scale=0.4)
