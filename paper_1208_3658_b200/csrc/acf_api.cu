@@ -183,11 +183,11 @@ extern "C" int acf_pair_count_rows(acf_ctx *ctx, const double *d_a, const float 
         // the reference kernel: validation into the slot's PackInfo, then the definition for every pair
         acf::Prepared a, b;
         for (int k = 0; k < 2; ++k) {
-            ACF_CUDA_TRY(ctx, ctx->cat[k].pack.reserve(64));
-            ACF_CUDA_TRY(ctx, cudaMemsetAsync(ctx->cat[k].pack.ptr, 0, 64, st));
+            ACF_CUDA_TRY(ctx, ctx->cat[k].slab.reserve(64));
+            ACF_CUDA_TRY(ctx, cudaMemsetAsync(ctx->cat[k].slab.ptr, 0, 64, st));
         }
-        a.pack = ctx->cat[0].pack.as<acf::PackInfo>();
-        b.pack = ctx->cat[1].pack.as<acf::PackInfo>();
+        a.pack = ctx->cat[0].slab.as<acf::PackInfo>();
+        b.pack = ctx->cat[1].slab.as<acf::PackInfo>();
         ACF_CUDA_TRY(ctx, acf::launch_validate(ctx, d_a, n_a, 0, n_a, d_wa, a.pack));
         if (!is_auto) ACF_CUDA_TRY(ctx, acf::launch_validate(ctx, d_b, n_b, 0, n_b, d_wb, b.pack));
         ACF_CUDA_TRY(ctx, cudaMemcpyAsync(&ctx->h_verdict[0], &a.pack->bad, sizeof(int), cudaMemcpyDeviceToHost, st));

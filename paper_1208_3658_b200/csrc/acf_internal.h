@@ -106,18 +106,8 @@ struct Prepared {
 // The device buffers of one prepared catalogue (grown lazily, freed with their owner: the context's two slots of
 // the calls that prepare on the fly, or an acf_catalog handle).
 struct CatBuffers {
-    Scratch pts, perm, caps, gcaps, scaps, pts2, vj, pack;
-    void release()
-    {
-        pts.release();
-        perm.release();
-        caps.release();
-        gcaps.release();
-        scaps.release();
-        pts2.release();
-        vj.release();
-        pack.release();
-    }
+    Scratch slab;  // one allocation, carved up by prepare_catalogue
+    void release() { slab.release(); }
 };
 
 }  // namespace acf

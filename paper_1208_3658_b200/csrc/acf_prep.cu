@@ -454,30 +454,31 @@ int prepare_catalogue(acf_ctx *ctx, CatBuffers &buf, const double *xyz, size_t s
     out->stride = stride;
     out->n = cnt;
     out->n_tiles = n_tiles;
-    ACF_CUDA_TRY(ctx, buf.pack.reserve(64));
-    out->pack = buf.pack.as<PackInfo>();
+    // one slab per catalogue: [PackInfo + weight range (64 B) | pts | pts2 | vj | perm | caps | gcaps | scaps]
+    const size_t padded = (size_t)n_tiles * kTile;
+    auto up = [](size_t v) { return (v + 255) & ~size_t(255); };
+    const size_t o_pts = 256, o_pts2 = o_pts + up(sizeof(float4) * padded), o_vj = o_pts2 + up(sizeof(float4) * padded),
+                 o_perm = o_vj + up(sizeof(double) * padded), o_caps = o_perm + up(sizeof(uint32_t) * padded),
+                 o_gcaps = o_caps + up(sizeof(double4) * (size_t)n_tiles),
+                 o_scaps = o_gcaps + up(sizeof(GroupCap) * (size_t)n_tiles * kGroupsPerTile),
+                 total = o_scaps + up(sizeof(GroupCap) * (size_t)n_tiles * kGroupsPerTile * kSubsPerGroup);
+    ACF_CUDA_TRY(ctx, buf.slab.reserve(total));
+    char *base = buf.slab.as<char>();
+    out->pack = reinterpret_cast<PackInfo *>(base);
     ACF_CUDA_TRY(ctx, cudaMemsetAsync(out->pack, 0, 64, st));
     if (cnt == 0) return ACF_OK;
     ACF_CUDA_TRY(ctx, launch_validate(ctx, xyz, stride, off, cnt, w, out->pack));
-    const size_t padded = (size_t)n_tiles * kTile;
-    ACF_CUDA_TRY(ctx, buf.pts.reserve(sizeof(float4) * padded));
-    ACF_CUDA_TRY(ctx, buf.perm.reserve(sizeof(uint32_t) * padded));
-    ACF_CUDA_TRY(ctx, buf.caps.reserve(sizeof(double4) * (size_t)n_tiles));
-    ACF_CUDA_TRY(ctx, buf.gcaps.reserve(sizeof(GroupCap) * (size_t)n_tiles * kGroupsPerTile));
-    ACF_CUDA_TRY(ctx, buf.scaps.reserve(sizeof(GroupCap) * (size_t)n_tiles * kGroupsPerTile * kSubsPerGroup));
     ACF_CUDA_TRY(ctx, ctx->s_keys.reserve(sizeof(uint32_t) * 4 * (size_t)n));  // keys x2, idx x2
-    ACF_CUDA_TRY(ctx, buf.pts2.reserve(sizeof(float4) * padded));
-    ACF_CUDA_TRY(ctx, buf.vj.reserve(sizeof(double) * padded));
     const uint32_t nblocks = (n + kSortBlockChunk - 1) / kSortBlockChunk;
     ACF_CUDA_TRY(ctx, ctx->s_misc.reserve(sizeof(uint32_t) * 256 * (size_t)nblocks));
-    out->pts = buf.pts.as<float4>();
-    out->perm = buf.perm.as<uint32_t>();
-    out->caps = buf.caps.as<double4>();
-    out->gcaps = buf.gcaps.as<GroupCap>();
-    out->scaps = buf.scaps.as<GroupCap>();
-    out->pts2 = buf.pts2.as<float>();
-    out->vj = buf.vj.as<double>();
-    uint32_t *range = reinterpret_cast<uint32_t *>(buf.pack.as<char>() + 48);
+    out->pts = reinterpret_cast<float4 *>(base + o_pts);
+    out->pts2 = reinterpret_cast<float *>(base + o_pts2);
+    out->vj = reinterpret_cast<double *>(base + o_vj);
+    out->perm = reinterpret_cast<uint32_t *>(base + o_perm);
+    out->caps = reinterpret_cast<double4 *>(base + o_caps);
+    out->gcaps = reinterpret_cast<GroupCap *>(base + o_gcaps);
+    out->scaps = reinterpret_cast<GroupCap *>(base + o_scaps);
+    uint32_t *range = reinterpret_cast<uint32_t *>(base + 48);
     uint32_t *k0 = ctx->s_keys.as<uint32_t>(), *k1 = k0 + n, *i0 = k1 + n, *i1 = i0 + n;
     uint32_t *counts = ctx->s_misc.as<uint32_t>();
 
