@@ -114,6 +114,13 @@ struct WinParams {
     int refine;       // 1: windows of two or more edges are split by the j side's sub-group caps
 };
 
+// chord_row out of line: the exact corrections and the pair-by-pair paths call it from unrolled loops, and one copy of
+// its search is what should be resident.
+__device__ __noinline__ int chord_row_ool(float xi, float yi, float zi, float xj, float yj, float zj, const float *sed, int nbins, float margin)
+{
+    return chord_row(xi, yi, zi, xj, yj, zj, sed, nbins, margin);
+}
+
 // Shared-memory loads by 32-bit shared address: the loads of the pair loops are LDS whatever the compiler can
 // prove about a pointer, and an address costs one register.
 __device__ __forceinline__ ulonglong2 lds_u64x2(uint32_t a)
@@ -352,7 +359,7 @@ __device__ __noinline__ void fixup_chunk(const WinParams &p, const Tables tb, co
                 for (int q = 0; q < kChunk; ++q) amb |= q < K && !(fabsf(q == 0 ? d0 : __fadd_rn(d0, dl[q])) > G);
                 if (!amb) continue;
                 // on the cosine, the chord length decides where it can; what is left open, the definition does
-                int exact = kChord ? -1 : chord_row(pi[r].x, pi[r].y, pi[r].z, pj.x, pj.y, pj.z, tb.sed_ptr(), tb.nbins, tb.margin());
+                int exact = kChord ? -1 : chord_row_ool(pi[r].x, pi[r].y, pi[r].z, pj.x, pj.y, pj.z, tb.sed_ptr(), tb.nbins, tb.margin());
                 if (exact < 0) {
                     exact = exact_row(p.xyz_a, p.stride_a, p.perm_a[sp.i_first + r * 32 + lane], p.xyz_b, p.stride_b,
                                       p.perm_b[sp.j_first + jj0 + u], p.edges, p.nbins);
@@ -661,7 +668,7 @@ __device__ __noinline__ void general_span(const WinParams &p, const Tables tb, c
                 if (fabsf(s32 - thr) > guard) row = (int)lds_f32_as_int(a + 8u) + (s32 >= thr ? 1 : 0);
             }
             if (row < 0) {
-                row = chord_row(pi[r].x, pi[r].y, pi[r].z, pj.x, pj.y, pj.z, tb.sed_ptr(), tb.nbins, tb.margin());
+                row = chord_row_ool(pi[r].x, pi[r].y, pi[r].z, pj.x, pj.y, pj.z, tb.sed_ptr(), tb.nbins, tb.margin());
                 if (row < 0) {
                     row = exact_row(p.xyz_a, p.stride_a, p.perm_a[sp.i_first + r * 32 + lane], p.xyz_b, p.stride_b,
                                     p.perm_b[sp.j_first + jj], p.edges, p.nbins);
@@ -732,7 +739,7 @@ __device__ __noinline__ void general_span_full(const WinParams &p, const Tables 
                 for (int h = 0; h < 2; ++h) {
                     if (row[r][h] >= 0) continue;
                     const float xj = h ? hi32(xy.x) : lo32(xy.x), yj = h ? hi32(xy.y) : lo32(xy.y), zj = h ? hi32(zw.x) : lo32(zw.x);
-                    int rw = chord_row(-nx[r], -ny[r], -nz[r], xj, yj, zj, tb.sed_ptr(), tb.nbins, tb.margin());
+                    int rw = chord_row_ool(-nx[r], -ny[r], -nz[r], xj, yj, zj, tb.sed_ptr(), tb.nbins, tb.margin());
                     if (rw < 0) {
                         rw = exact_row(p.xyz_a, p.stride_a, p.perm_a[sp.i_first + r * 32 + lane], p.xyz_b, p.stride_b,
                                        p.perm_b[sp.j_first + jj + h], p.edges, p.nbins);
@@ -1060,6 +1067,30 @@ __device__ __noinline__ void flush_rows(const WinParams &p, const WarpSm<kWeight
     __syncwarp();
 }
 
+// The rows r_lo .. r_hi of the window of two caps, and whether it is classified on the chord length: r_lo | r_hi << 12 |
+// chord << 24.  Out of line: refill calls it once per j-group and four times more per window of several edges, and its
+// fp64 code should be resident once.
+__device__ __noinline__ uint32_t bound_rows(const GroupCap ca, const GroupCap cj, const double slack, const double *edges_sm, const int nbins)
+{
+    int lo = 0, hi = nbins + 1;
+    bool chord = false;
+    double c_lo, c_hi;
+    if (cap_window(ca, cj, slack, c_lo, c_hi)) {
+        // rows of the two ends; the far end is a few rows on at most: walk there
+        hi = lo = row_of_cos(c_hi, edges_sm, nbins);
+        while (hi < nbins && c_lo <= edges_sm[hi]) ++hi;
+        if (hi == nbins && c_lo < edges_sm[nbins]) ++hi;
+        chord = hi > lo && c_hi - c_lo < kChordWidth && c_lo > kChordCosMin;
+    }
+    // The pair cosine is clamped to [-1, 1]: no pair lies before a pole edge e_0 = 1 or beyond e_n = -1, so
+    // those two edges are in no window (and never tested in fp32: an unclamped c32 marginally outside, or
+    // vectors a little longer than 1, would be misfiled).
+    if (lo == 0 && edges_sm[0] >= 1.0) lo = 1;
+    if (hi == nbins + 1 && edges_sm[nbins] <= -1.0) hi = nbins;
+    if (hi < lo) hi = lo;
+    return (uint32_t)lo | ((uint32_t)hi << 12) | (chord ? 1u << 24 : 0u);
+}
+
 // Keeps the warp's queue filled: takes the next job from the global counter when the current one has been scanned,
 // and bounds the windows of the warp's i-group against the next (up to) kScan j-groups of its job -- two j-tiles,
 // one lane per j-group, fp64 -- queueing the survivors: groups whose window lies wholly out of range are dropped
@@ -1156,23 +1187,10 @@ __device__ __noinline__ void refill(const WinParams &p, const WarpSm<kWeighted> 
                 u.masked = gi < (uint32_t)kGroup || gj < (uint32_t)kGroup || u.diag;
                 const GroupCap ca = p.gcaps_a[igx], cb = p.gcaps_b[jgx];
                 auto bound = [&](const GroupCap &cj, int &lo, int &hi, bool &chord) {
-                    lo = 0;
-                    hi = p.nbins + 1;
-                    chord = false;
-                    double c_lo, c_hi;
-                    if (cap_window(ca, cj, slack, c_lo, c_hi)) {
-                        // rows of the two ends; the far end is a few rows on at most: walk there
-                        hi = lo = row_of_cos(c_hi, edges_sm, p.nbins);
-                        while (hi < p.nbins && c_lo <= edges_sm[hi]) ++hi;
-                        if (hi == p.nbins && c_lo < edges_sm[p.nbins]) ++hi;
-                        chord = hi > lo && c_hi - c_lo < kChordWidth && c_lo > kChordCosMin;
-                    }
-                    // The pair cosine is clamped to [-1, 1]: no pair lies before a pole edge e_0 = 1 or beyond e_n = -1, so
-                    // those two edges are in no window (and never tested in fp32: an unclamped c32 marginally outside, or
-                    // vectors a little longer than 1, would be misfiled).
-                    if (lo == 0 && edges_sm[0] >= 1.0) lo = 1;
-                    if (hi == p.nbins + 1 && edges_sm[p.nbins] <= -1.0) hi = p.nbins;
-                    if (hi < lo) hi = lo;
+                    const uint32_t r = bound_rows(ca, cj, slack, edges_sm, p.nbins);
+                    lo = (int)(r & 0xfffu);
+                    hi = (int)((r >> 12) & 0xfffu);
+                    chord = (r >> 24) != 0u;
                 };
                 int lo, hi;
                 bool chord;
