@@ -71,7 +71,7 @@ def read_ncu_profile():
         for key in ("source_sha16", "launch", "dram_bytes", "sass_thread_inst_per_pair", "issue_active_pct", "kernel_ms"):
             if line.startswith(key + ":"):
                 v = line.split(":", 1)[1].strip().strip("`")
-                out[key] = v if key in ("source_sha16", "launch") else float(v)
+                out[key] = v if key in ("source_sha16", "launch") else (int(v) if key == "dram_bytes" else float(v))
     if "source_sha16" not in out or "sass_thread_inst_per_pair" not in out:
         return None
     out["stale"] = out["source_sha16"] != source_hash()

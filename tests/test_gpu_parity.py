@@ -509,6 +509,15 @@ def test_prepared_catalogues(acf, ctx, oracle):
         c = acf.acf_pair_count_prepared(ctx, ck, cr, w.cos_edges, weighted=False)
         torch.cuda.synchronize()
         assert acf.counts_to_numpy(c).tolist() == oracle.pair_count(xd, xr, w.cos_edges, False, rows=rows).tolist()
+        # the handle prepared again on other data (another, smaller catalogue): its memory reused, the counts the new data's
+        w2 = make_config("full_sky", 0.004, seed_offset=7)
+        x2 = acf.acf_radec_to_xyz(w2.ra_d, w2.dec_d)
+        acf.acf_prepare_again(ctx, ck, dev(x2), dev(w2.w_d))
+        c, s = acf.acf_pair_count_prepared(ctx, ck, None, w.cos_edges)
+        torch.cuda.synchronize()
+        want2 = oracle.pair_count(x2, None, w.cos_edges, True, w_a=w2.w_d)
+        assert acf.counts_to_numpy(c).tolist() == want2[0].tolist()
+        np.testing.assert_allclose(s.cpu().numpy(), want2[1], rtol=WSUM_RTOL, atol=0)
         acf.acf_release(ctx, ck)
         with pytest.raises(acf.AcfError):
             acf.acf_pair_count_prepared(ctx, cd, cr, w.cos_edges, part=3, n_parts=3)
