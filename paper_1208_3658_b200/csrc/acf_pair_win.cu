@@ -484,6 +484,40 @@ __device__ __forceinline__ uint32_t pair_loop(const uint32_t grp2, const uint32_
     return amb_steps;
 }
 
+// The pair loop of a window that holds no edge: its caps prove that every pair lies in one row, on the near side of the
+// edge e_m that bounds the row.  Every pair's d = e_m - c (or s - s_m) is still computed and must come out below -G --
+// certified on that side -- but nothing is tallied pair by pair: the row gets the span's pair count and weight at once.
+// Returns false if some pair is not certified (the span is then redone by pair_loop and its exact corrections).
+template <bool kChord>
+__device__ __forceinline__ bool verify_loop(const uint32_t grp2, const int n_j, const float (&nx)[kR], const float (&ny)[kR],
+                                            const float (&nz)[kR], const float e32, const float G)
+{
+    const unsigned long long e2 = pack2(e32, e32);
+    float mx0 = -3.0e38f, mx1 = -3.0e38f;  // max d over the pairs, two chains
+#pragma unroll 1
+    for (int jj = 0; jj < n_j; jj += 4) {
+#pragma unroll
+        for (int u = 0; u < 4; u += 2) {
+            const ulonglong2 xy = lds_u64x2(grp2 + 16u * (uint32_t)(jj + u));
+            const unsigned long long zz = lds_u64(grp2 + 16u * (uint32_t)(jj + u) + 16u);
+#pragma unroll
+            for (int r = 0; r < kR; ++r) {
+                unsigned long long d2;
+                if constexpr (kChord) {
+                    const unsigned long long dx = fadd2(xy.x, pack2(nx[r], nx[r])), dy = fadd2(xy.y, pack2(ny[r], ny[r])),
+                                             dz = fadd2(zz, pack2(nz[r], nz[r]));
+                    d2 = ffma2(dx, dx, ffma2(dy, dy, ffma2(dz, dz, e2)));
+                } else {
+                    d2 = ffma2(pack2(nx[r], nx[r]), xy.x, ffma2(pack2(ny[r], ny[r]), xy.y, ffma2(pack2(nz[r], nz[r]), zz, e2)));
+                }
+                if (r & 1) asm("max.f32 %0, %0, %1, %2;" : "+f"(mx1) : "f"(lo32(d2)), "f"(hi32(d2)));
+                else asm("max.f32 %0, %0, %1, %2;" : "+f"(mx0) : "f"(lo32(d2)), "f"(hi32(d2)));
+            }
+        }
+    }
+    return __all_sync(0xffffffffu, fmaxf(mx0, mx1) < -G);
+}
+
 // Edges m_a .. m_a + n_real - 1 (n_real <= K) against one span of staged j-points and this thread's kR i-points.
 // A chunk fills rows m_a .. m_a + n_real - 1 (and m_a + n_real if it is the last of its window); the tallies above
 // its last edge go to the next chunk through `carry`.  A chunk of fewer than K edges repeats its last edge: the
@@ -923,6 +957,7 @@ __device__ __forceinline__ void single_edge_span(const WinParams &p, const WarpS
     uint32_t grp2, vgrp;
     int n_j;
     float e32, G;
+    bool no_edge;
     float nx[kR], ny[kR], nz[kR];  // the i-points, negated: loaded here so that they are live across no call
     {
         volatile WarpCtl *c = w.ctl();
@@ -948,11 +983,24 @@ __device__ __forceinline__ void single_edge_span(const WinParams &p, const WarpS
             e32 = edge32(tb.edge(m_edge));
             G = kGuard1;
         }
+        // a window with no edge inside, all of it in a row of the histogram: every pair is expected before the row's far edge
+        const int s0 = u->nsub == 1 ? 0 : c->sub;
+        no_edge = u->hi[s0] == u->lo[s0] && u->lo[s0] <= tb.nbins;
     }
     const float dl[1] = {0.f};
     double t[1][kR];
     uint32_t nb[1];
-    const uint32_t amb_steps = pair_loop<1, kWeighted, kChord>(grp2, vgrp, n_j, nx, ny, nz, e32, dl, G, t, nb);
+    uint32_t amb_steps = 0;
+    bool verified = false;
+    if constexpr (!kChord) verified = no_edge && verify_loop<false>(grp2, n_j, nx, ny, nz, e32, G);
+    if (verified) {
+        // every pair certified in row m_edge: nothing above the edge
+        nb[0] = (uint32_t)n_j * kR;
+#pragma unroll
+        for (int r = 0; r < kR; ++r) t[0][r] = 0.0;
+    } else {
+        amb_steps = pair_loop<1, kWeighted, kChord>(grp2, vgrp, n_j, nx, ny, nz, e32, dl, G, t, nb);
+    }
 
     volatile WarpCtl *c = w.ctl();
     const uint32_t n_done = c->n_done;
@@ -1080,7 +1128,8 @@ __device__ __noinline__ uint32_t bound_rows(const GroupCap ca, const GroupCap cj
         hi = lo = row_of_cos(c_hi, edges_sm, nbins);
         while (hi < nbins && c_lo <= edges_sm[hi]) ++hi;
         if (hi == nbins && c_lo < edges_sm[nbins]) ++hi;
-        chord = hi > lo && c_hi - c_lo < kChordWidth && c_lo > kChordCosMin;
+        // (a window with no edge inside is tested against the far edge of its row: on the chord only if it comes close to it)
+        chord = c_hi - c_lo < kChordWidth && c_lo > kChordCosMin && (hi > lo || (lo <= nbins && c_lo - edges_sm[lo] < 3.0e-6));
     }
     // The pair cosine is clamped to [-1, 1]: no pair lies before a pole edge e_0 = 1 or beyond e_n = -1, so
     // those two edges are in no window (and never tested in fp32: an unclamped c32 marginally outside, or
