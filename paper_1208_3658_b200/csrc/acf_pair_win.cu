@@ -597,26 +597,33 @@ __device__ __forceinline__ void window_chunk(const WinParams &p, const Tables tb
         for (int r = 0; r < kR; ++r) s_prev[r] = carry->s[r];
     }
     __syncwarp();
+    // The rows, one after the other in a rolled loop (this epilogue runs once per span of a rare shape: its code is kept
+    // short for the instruction cache, its tallies go through a copy in local memory that the loop can index).
+    double tl[K + 1][kR];
+    uint32_t nbl[K + 1];
 #pragma unroll
-    for (int q = 0; q <= K; ++q) {
-        if (q == K && !last) break;
-        uint32_t c_q = 0;  // pairs above edge q (q == K: nothing lies above the row after the last edge)
+    for (int q = 0; q < K; ++q) {
+        nbl[q] = nb[q];
+#pragma unroll
+        for (int r = 0; r < kR; ++r) tl[q][r] = t[q][r];
+    }
+    nbl[K] = n_all;  // nothing lies above the row after the last edge
+#pragma unroll
+    for (int r = 0; r < kR; ++r) tl[K][r] = 0.0;
+    const int q_end = last ? K + 1 : K;
+#pragma unroll 1
+    for (int q = 0; q < q_end; ++q) {
+        uint32_t c_q = 0;  // pairs above edge q
         double rw = 0.0;   // weight of this thread's pairs in row m_a + q
-        if (q < K) {
-            if constexpr (kWeighted) {
-                c_q = 0u;
+        if constexpr (kWeighted) {
 #pragma unroll
-                for (int r = 0; r < kR; ++r) {
-                    const double sw = unpack(t[q < K ? q : 0][r], c_q);
-                    rw = fma((double)wi_of[r * wi_stride], s_prev[r] - sw, rw);
-                    s_prev[r] = sw;
-                }
-            } else {
-                c_q = n_all - nb[q < K ? q : 0];
+            for (int r = 0; r < kR; ++r) {
+                const double sw = unpack(tl[q][r], c_q);
+                rw = fma((double)wi_of[r * wi_stride], s_prev[r] - sw, rw);
+                s_prev[r] = sw;
             }
-        } else if constexpr (kWeighted) {
-#pragma unroll
-            for (int r = 0; r < kR; ++r) rw = fma((double)wi_of[r * wi_stride], s_prev[r], rw);
+        } else {
+            c_q = n_all - nbl[q];
         }
         const uint32_t rc = c_prev - c_q;
         c_prev = c_q;
