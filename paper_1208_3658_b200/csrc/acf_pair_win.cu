@@ -433,7 +433,9 @@ __device__ __forceinline__ uint32_t pair_loop(const uint32_t grp2, const uint32_
 #pragma unroll 1
     for (int jj = 0; jj < n_j; jj += kStep) {
         float mn = 1.0f;  // min |d_q| over the pairs of the step
-#pragma unroll
+        // (the loops of several edges are not unrolled over the step's two pairs of j-points: they are the rare shapes,
+        // and half their code is what the instruction cache has for the common one)
+#pragma unroll(K == 1 ? kStep / 2 : 1)
         for (int u = 0; u < kStep; u += 2) {
             const ulonglong2 xy = lds_u64x2(grp2 + 16u * (uint32_t)(jj + u));
             const unsigned long long zz = lds_u64(grp2 + 16u * (uint32_t)(jj + u) + 16u);
