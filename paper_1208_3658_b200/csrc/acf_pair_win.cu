@@ -318,14 +318,6 @@ __device__ __noinline__ void fixup_chunk(const WinParams &p, const Tables tb, co
                                          float G, unsigned long long *stat, double *__restrict__ dt, int *__restrict__ dn)
 {
     const int lane = threadIdx.x & 31;
-    float4 pi[kR];
-#pragma unroll
-    for (int r = 0; r < kR; ++r) {
-        pi[r] = sp.ipoint(r);  // negated in the stash
-        pi[r].x = -pi[r].x;
-        pi[r].y = -pi[r].y;
-        pi[r].z = -pi[r].z;
-    }
     for (int i = 0; i < kChunk * kR; ++i) dt[i] = 0.0;
     for (int i = 0; i < kChunk; ++i) dn[i] = 0;
     float e32, dl[kChunk];
@@ -343,23 +335,29 @@ __device__ __noinline__ void fixup_chunk(const WinParams &p, const Tables tb, co
         constexpr int kStep = step_of(kWeighted);
         const int jj0 = sp.jj0 + (__ffs(amb_steps) - 1) * kStep;
         amb_steps &= amb_steps - 1;
+        // (rolled loops: this code runs for one unit in three and should be short)
+#pragma unroll 1
         for (int u = 0; u < kStep; ++u) {
             const float4 pj = sp.point(jj0 + u);
-#pragma unroll
+#pragma unroll 1
             for (int r = 0; r < kR; ++r) {
+                float4 pir = sp.ipoint(r);  // negated in the stash
+                pir.x = -pir.x;
+                pir.y = -pir.y;
+                pir.z = -pir.z;
                 float d0;
                 if constexpr (kChord) {
-                    const float dx = __fadd_rn(pj.x, -pi[r].x), dy = __fadd_rn(pj.y, -pi[r].y), dz = __fadd_rn(pj.z, -pi[r].z);
+                    const float dx = __fadd_rn(pj.x, -pir.x), dy = __fadd_rn(pj.y, -pir.y), dz = __fadd_rn(pj.z, -pir.z);
                     d0 = fmaf(dx, dx, fmaf(dy, dy, fmaf(dz, dz, e32)));
                 } else {
-                    d0 = fmaf(-pi[r].x, pj.x, fmaf(-pi[r].y, pj.y, fmaf(-pi[r].z, pj.z, e32)));
+                    d0 = fmaf(-pir.x, pj.x, fmaf(-pir.y, pj.y, fmaf(-pir.z, pj.z, e32)));
                 }
                 bool amb = false;
 #pragma unroll
                 for (int q = 0; q < kChunk; ++q) amb |= q < K && !(fabsf(q == 0 ? d0 : __fadd_rn(d0, dl[q])) > G);
                 if (!amb) continue;
                 // on the cosine, the chord length decides where it can; what is left open, the definition does
-                int exact = kChord ? -1 : chord_row_ool(pi[r].x, pi[r].y, pi[r].z, pj.x, pj.y, pj.z, tb.sed_ptr(), tb.nbins, tb.margin());
+                int exact = kChord ? -1 : chord_row_ool(pir.x, pir.y, pir.z, pj.x, pj.y, pj.z, tb.sed_ptr(), tb.nbins, tb.margin());
                 if (exact < 0) {
                     exact = exact_row(p.xyz_a, p.stride_a, p.perm_a[sp.i_first + r * 32 + lane], p.xyz_b, p.stride_b,
                                       p.perm_b[sp.j_first + jj0 + u], p.edges, p.nbins);
