@@ -1217,85 +1217,83 @@ __device__ __noinline__ void refill(const WinParams &p, const WarpSm<kWeighted> 
         const int ti = lane < kGroupsPerTile ? ti0 : ti1, tj = lane < kGroupsPerTile ? tj0 : tj1;
         const int g = lane & (kGroupsPerTile - 1);
         bool live = lane < kScan && ti >= 0 && (g & (int)(h->split - 1u)) == c->part;
-        Unit u;
-        u.i_first = 0;
-        u.j_first = 0;
-        u.nsub = 1;
-        u.masked = u.diag = u.chord = 0;
-        u.jn = 0;
-#pragma unroll
-        for (int s = 0; s < kSubsPerGroup; ++s) {
-            u.lo[s] = u.hi[s] = -1;
-            u.wsum[s] = 0.0;
-        }
+        // first the window of the whole j-group (registers), then the queue slot, then -- straight into the slot -- the
+        // windows of the sub-groups where the group's holds several edges (a rolled loop: this code should be short)
+        uint32_t i0 = 0, j0 = 0, gj = 0, jgx = 0;
+        int lo = 0, hi = 0;
+        bool chord = false, masked = false, diag = false;
+        double wsum_i = 0.0, wsum_j = 0.0;
+        GroupCap ca;
         if (live) {
-            const uint32_t igx = (uint32_t)ti * kGroupsPerTile + ig, jgx = (uint32_t)tj * kGroupsPerTile + g;
-            const uint32_t i0 = igx * kGroup, j0 = jgx * kGroup;
+            const uint32_t igx = (uint32_t)ti * kGroupsPerTile + ig;
+            jgx = (uint32_t)tj * kGroupsPerTile + g;
+            i0 = igx * kGroup;
+            j0 = jgx * kGroup;
             const uint32_t gi = i0 < p.n_a ? (p.n_a - i0 < (uint32_t)kGroup ? p.n_a - i0 : (uint32_t)kGroup) : 0u;
-            const uint32_t gj = j0 < p.n_b ? (p.n_b - j0 < (uint32_t)kGroup ? p.n_b - j0 : (uint32_t)kGroup) : 0u;
+            gj = j0 < p.n_b ? (p.n_b - j0 < (uint32_t)kGroup ? p.n_b - j0 : (uint32_t)kGroup) : 0u;
             const bool diag_tile = p.is_auto && tj == ti;
             live = gi > 0 && gj > 0 && !(diag_tile && g < ig);
             if (live) {
-                u.i_first = i0;
-                u.j_first = j0;
-                u.jn = (int32_t)gj;
-                u.diag = diag_tile && g == ig;
-                u.masked = gi < (uint32_t)kGroup || gj < (uint32_t)kGroup || u.diag;
-                const GroupCap ca = p.gcaps_a[igx], cb = p.gcaps_b[jgx];
-                auto bound = [&](const GroupCap &cj, int &lo, int &hi, bool &chord) {
-                    const uint32_t r = bound_rows(ca, cj, slack, edges_sm, p.nbins);
-                    lo = (int)(r & 0xfffu);
-                    hi = (int)((r >> 12) & 0xfffu);
-                    chord = (r >> 24) != 0u;
-                };
-                int lo, hi;
-                bool chord;
-                bound(cb, lo, hi, chord);
+                diag = diag_tile && g == ig;
+                masked = gi < (uint32_t)kGroup || gj < (uint32_t)kGroup || diag;
+                ca = p.gcaps_a[igx];
+                const GroupCap cb = p.gcaps_b[jgx];
+                wsum_i = ca.wsum;
+                wsum_j = cb.wsum;
+                const uint32_t r = bound_rows(ca, cb, slack, edges_sm, p.nbins);
+                lo = (int)(r & 0xfffu);
+                hi = (int)((r >> 12) & 0xfffu);
+                chord = (r >> 24) != 0u;
                 const bool out = hi == lo && (lo == 0 || lo > p.nbins);  // all closer than theta_min or all beyond theta_max
                 if (p.prune && out) {
                     live = false;  // pruned at the level of groups, like whole tiles in the work list
-                } else if (p.bulk && hi == lo && !out && !u.masked) {
+                } else if (p.bulk && hi == lo && !out && !masked) {
                     // all pairs of two full groups in one bin: the bin gets the groups' pair count and the product of
                     // their weight sums, and nothing is evaluated (ACF_OPT_BULK)
                     const unsigned long long all = (unsigned long long)kGroup * kGroup;
-                    rows.template add_atomic<kWeighted>(lo, (uint32_t)all, ca.wsum * cb.wsum);
+                    rows.template add_atomic<kWeighted>(lo, (uint32_t)all, wsum_i * wsum_j);
                     atomicAdd(&h->stat[kStatBulk], all);
                     live = false;
-                } else {
-                    u.lo[0] = (int16_t)lo;
-                    u.hi[0] = (int16_t)hi;
-                    u.chord = chord ? 1 : 0;
-                    u.wsum[0] = cb.wsum;
-                    if (p.refine && !u.masked && hi - lo >= 2) {
-                        // several edges: the window of each sub-group of the j side is narrower
-                        u.nsub = kSubsPerGroup;
-                        u.chord = 0;
-#pragma unroll
-                        for (int s = 0; s < kSubsPerGroup; ++s) {
-                            const GroupCap cs = p.scaps_b[(size_t)jgx * kSubsPerGroup + s];
-                            int slo, shi;
-                            bool sch;
-                            bound(cs, slo, shi, sch);
-                            if (p.prune && shi == slo && (slo == 0 || slo > p.nbins)) slo = shi = -1;
-                            u.lo[s] = (int16_t)slo;
-                            u.hi[s] = (int16_t)shi;
-                            u.chord |= (sch ? 1 : 0) << s;
-                            u.wsum[s] = cs.wsum;
-                        }
-                        // the same window four times over: one span after all (one prologue, one epilogue)
-                        if (u.lo[0] >= 0 && u.lo[1] == u.lo[0] && u.lo[2] == u.lo[0] && u.lo[3] == u.lo[0] && u.hi[1] == u.hi[0] &&
-                            u.hi[2] == u.hi[0] && u.hi[3] == u.hi[0] && (u.chord == 0 || u.chord == 15)) {
-                            u.nsub = 1;
-                            u.chord &= 1;
-                            u.wsum[0] = cb.wsum;
-                        }
-                    }
                 }
             }
         }
         const uint32_t alive = __ballot_sync(0xffffffffu, live);
         const uint32_t q_tail = c->q_tail;
-        if (live) queue[(q_tail + __popc(alive & ((1u << lane) - 1u))) % kQueue] = u;
+        if (live) {
+            Unit *q = &queue[(q_tail + __popc(alive & ((1u << lane) - 1u))) % kQueue];
+            q->i_first = i0;
+            q->j_first = j0;
+            q->jn = (int32_t)gj;
+            q->nsub = 1;
+            q->masked = masked;
+            q->diag = diag;
+            q->chord = chord ? 1 : 0;
+            q->lo[0] = (int16_t)lo;
+            q->hi[0] = (int16_t)hi;
+            q->wsum[0] = wsum_j;
+            if (p.refine && !masked && hi - lo >= 2) {
+                // several edges: the window of each sub-group of the j side is narrower
+                uint32_t chords = 0;
+                bool same = true;
+#pragma unroll
+                for (int s = 0; s < kSubsPerGroup; ++s) {
+                    const GroupCap cs = p.scaps_b[(size_t)jgx * kSubsPerGroup + s];
+                    const uint32_t r = bound_rows(ca, cs, slack, edges_sm, p.nbins);
+                    int slo = (int)(r & 0xfffu), shi = (int)((r >> 12) & 0xfffu);
+                    if (p.prune && shi == slo && (slo == 0 || slo > p.nbins)) slo = shi = -1;
+                    q->lo[s] = (int16_t)slo;
+                    q->hi[s] = (int16_t)shi;
+                    q->wsum[s] = cs.wsum;
+                    chords |= (r >> 24) << s;
+                    same = same && slo >= 0 && slo == q->lo[0] && shi == q->hi[0];
+                }
+                same = same && (chords == 0u || chords == 15u);
+                // the same window four times over: one span after all (one prologue, one epilogue)
+                q->nsub = same ? 1 : kSubsPerGroup;
+                q->chord = (uint8_t)(same ? (chords & 1u) : chords);
+                if (same) q->wsum[0] = wsum_j;
+            }
+        }
         __syncwarp();
         if (lane == 0) {
             c->q_tail = q_tail + __popc(alive);
