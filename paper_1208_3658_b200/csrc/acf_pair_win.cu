@@ -51,19 +51,35 @@ __host__ __device__ constexpr int step_of(bool) { return 4; }
 constexpr int kWStages = 2;            // staged j-groups per warp
 constexpr int kQueue = 32;             // surviving j-groups a warp has bounded and not yet evaluated
 constexpr int kScan = 16;              // j-groups bounded at a time (two tiles, one lane each)
-constexpr int kMaxPassEdges = 9;       // unweighted: windows of more edges than this go pair by pair (general_span); weighted ones
+constexpr int kMaxPassEdges = 3;       // unweighted: windows of more edges than this go pair by pair (general_span); weighted ones
                                        // take as many passes as it needs (their pair-by-pair tallies are fp64 atomics on shared memory)
 // The cell table of the pair-by-pair path: the values of the fp32 squared chord length s that share their sign,
 // exponent and top kCellBits mantissa bits form a cell; 2^kCellBits cells per octave from 2^kCellExpLo to 4.
 constexpr int kCellBits = 4;
 constexpr int kCellExpLo = -40;        // s below 2^-40 (0.2 arc seconds): no cell, the edges are searched
 constexpr int kCells = (2 - kCellExpLo) << kCellBits;
+constexpr int kCellSlots = kCells + 2;  // slot kCells: the values outside the table (never certified); one more for 16-byte alignment
 struct Cell {
-    float thr;    // the one edge s_k (as stored, fp32) that can separate two rows inside the cell; +big if none
-    float guard;  // a pair is certified iff |s - thr| > guard (the bound of chord_row); thr = NaN: never (crowded cell)
-    int row;      // number of edges at or below the cell: the row of s < thr; s >= thr is one row on
-    int pad;
+    float thr;      // the one edge s_k (as stored, fp32) that can separate two rows inside the cell; +big if none; NaN: the cell
+                    // holds several edges (or is the slot of the values outside the table) and certifies nothing
+    uint32_t word;  // bits 16..31: the guard band of that edge (the bound of chord_row) as the upper half of a float, rounded up:
+                    // a pair is certified iff |s - thr| > guard;  bits 0..15: the row of s >= thr (s < thr is the row before)
 };
+static_assert(sizeof(Cell) == 8 && (sizeof(Cell) * kCellSlots) % 16 == 0, "one LDS.64 per pair");
+constexpr int kCellShift = 23 - kCellBits;
+constexpr uint32_t kCellKey0 = (uint32_t)(127 + kCellExpLo) << kCellBits;
+// The row of the squared chord length s32 by its cell; false if the cell does not certify it.
+__device__ __forceinline__ bool cell_row(uint32_t cells, float s32, int &row)
+{
+    // (zero, values below 2^kCellExpLo and NaN wrap or run past the table: all of them land in slot kCells)
+    const uint32_t key = min((__float_as_uint(s32) >> kCellShift) - kCellKey0, (uint32_t)kCells);
+    float thr;
+    uint32_t word;
+    asm volatile("ld.shared.v2.b32 {%0, %1}, [%2];" : "=f"(thr), "=r"(word) : "r"(cells + 8u * key));
+    const float d = s32 - thr;
+    row = (int)(word & 0xffffu) + (__float_as_int(d) >> 31);
+    return fabsf(d) > __uint_as_float(word & 0xffff0000u);
+}
 // Guard bands on the cosine (u = 2^-24).  A wrong fp32 sign needs
 // |d_0 - (e_m - c64)| >= |d_0|, so only pairs with a small |d_0| matter; for those the partial sums of the
 // chain are below 1 + 2e-6 in magnitude (they differ from d_0 by products of coordinates whose absolute sum is
@@ -147,12 +163,6 @@ __device__ __forceinline__ double lds_f64(uint32_t a)
     asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(a));
     return v;
 }
-__device__ __forceinline__ int lds_f32_as_int(uint32_t a)
-{
-    int v;
-    asm volatile("ld.shared.s32 %0, [%1];" : "=r"(v) : "r"(a));
-    return v;
-}
 __device__ __forceinline__ float lds_f32(uint32_t a)
 {
     float v;
@@ -224,8 +234,9 @@ struct Rows {
     template <bool kWeighted>
     __device__ __forceinline__ void add_atomic(int row, uint32_t c, double w) const  // from any lane
     {
-        atomicAdd(&cnt[row], c);
-        if constexpr (kWeighted) atomicAdd(&ws[row], w);
+        // (by shared address: through the generic pointer the compiler emits a generic ATOM, ten times slower)
+        asm volatile("red.shared.add.u32 [%0], %1;" ::"r"(smem_u32(cnt + row)), "r"(c) : "memory");
+        if constexpr (kWeighted) asm volatile("red.shared.add.f64 [%0], %1;" ::"r"(smem_u32(ws + row)), "d"(w) : "memory");
     }
     template <bool kWeighted>
     __device__ __forceinline__ void add(int row, uint32_t c, double w) const  // lane 0 of the rows' warp
@@ -690,8 +701,6 @@ __device__ __noinline__ void general_span(const WinParams &p, const Tables tb, c
         pi[r].z = -pi[r].z;
     }
     const uint32_t cells = tb.cells();
-    constexpr int kShift = 23 - kCellBits;
-    constexpr int kKey0 = (127 + kCellExpLo) << kCellBits;
     uint32_t n_exact = 0;
     const int jj_end = sp.jj1 < mk.jn ? sp.jj1 : mk.jn;
     for (int jj = sp.jj0; jj < jj_end; ++jj) {
@@ -701,14 +710,8 @@ __device__ __noinline__ void general_span(const WinParams &p, const Tables tb, c
             if (!mk.on(sp, r, jj)) continue;
             const float dx = __fsub_rn(pi[r].x, pj.x), dy = __fsub_rn(pi[r].y, pj.y), dz = __fsub_rn(pi[r].z, pj.z);
             const float s32 = fmaf(dx, dx, fmaf(dy, dy, __fmul_rn(dz, dz)));  // as chord_row computes it
-            const int key = (int)(__float_as_uint(s32) >> kShift) - kKey0;
-            int row = -1;
-            if (key >= 0 && key < kCells) {
-                const uint32_t a = cells + 16u * (uint32_t)key;
-                const float thr = lds_f32(a), guard = lds_f32(a + 4u);
-                if (fabsf(s32 - thr) > guard) row = (int)lds_f32_as_int(a + 8u) + (s32 >= thr ? 1 : 0);
-            }
-            if (row < 0) {
+            int row;
+            if (!cell_row(cells, s32, row)) {
                 row = chord_row_ool(pi[r].x, pi[r].y, pi[r].z, pj.x, pj.y, pj.z, tb.sed_ptr(), tb.nbins, tb.margin());
                 if (row < 0) {
                     row = exact_row(p.xyz_a, p.stride_a, p.perm_a[sp.i_first + r * 32 + lane], p.xyz_b, p.stride_b,
@@ -723,14 +726,41 @@ __device__ __noinline__ void general_span(const WinParams &p, const Tables tb, c
     if (lane == 0 && n_exact) atomicAdd(&stat[kStatFp64], (unsigned long long)n_exact);
 }
 
+// The pairs of the j-points jj, jj + 1 that their cell did not certify (bit 2 r + h of `open`: i-point r, j-point jj + h):
+// the search of chord_row, then the fp64 definition.  Called by the whole warp; rolled, out of line.
+template <bool kWeighted>
+__device__ __noinline__ void resolve_open(const WinParams &p, const Tables tb, const Rows rows, const Span sp, int jj, uint32_t open,
+                                          unsigned long long *stat)
+{
+    const int lane = threadIdx.x & 31;
+    uint32_t n_exact = 0;
+#pragma unroll 1
+    while (open) {
+        const int b = __ffs((int)open) - 1;
+        open &= open - 1u;
+        const int r = b >> 1, h = b & 1;
+        const float4 pi = sp.ipoint(r);  // negated in the stash
+        const float4 pj = sp.point(jj + h);
+        int rw = chord_row_ool(-pi.x, -pi.y, -pi.z, pj.x, pj.y, pj.z, tb.sed_ptr(), tb.nbins, tb.margin());
+        if (rw < 0) {
+            rw = exact_row(p.xyz_a, p.stride_a, p.perm_a[sp.i_first + r * 32 + lane], p.xyz_b, p.stride_b, p.perm_b[sp.j_first + jj + h],
+                           p.edges, p.nbins);
+            ++n_exact;
+        }
+        rows.template add_atomic<kWeighted>(rw, 1u, (double)pi.w * (double)pj.w);
+    }
+    n_exact = __reduce_add_sync(0xffffffffu, n_exact);
+    if (lane == 0 && n_exact) atomicAdd(&stat[kStatFp64], (unsigned long long)n_exact);
+}
+
 // The same for a full span (nothing masked): two j-points at a time, their squared chord lengths by packed adds and
-// FMAs (bit for bit the values chord_row computes), one 16-byte load per pair for its cell, and the search only for
-// the pairs the cell does not certify.  Windows of many edges (the near field of a small-angle count) come here.
+// FMAs (bit for bit the values chord_row computes), one 8-byte load per pair for its cell, one shared-memory
+// reduction per pair for its row, and the search only for the pairs the cell does not certify.  Unweighted windows
+// of more than kMaxPassEdges edges (the near field of a small-angle count) come here.
 template <bool kWeighted>
 __device__ __noinline__ void general_span_full(const WinParams &p, const Tables tb, const Rows rows, const Span sp,
                                                unsigned long long *stat)
 {
-    const int lane = threadIdx.x & 31;
     float nx[kR], ny[kR], nz[kR], wi[kR];
 #pragma unroll
     for (int r = 0; r < kR; ++r) {
@@ -741,15 +771,13 @@ __device__ __noinline__ void general_span_full(const WinParams &p, const Tables 
         wi[r] = v.w;
     }
     const uint32_t cells = tb.cells();
-    constexpr int kShift = 23 - kCellBits;
-    constexpr int kKey0 = (127 + kCellExpLo) << kCellBits;
-    uint32_t n_exact = 0;
+    // (no branch around a pair's reduction: an uncertified pair adds to CtaHeader::trash, the last 16 bytes before the tables)
+    const uint32_t cnt_a = smem_u32(rows.cnt), ws_a = kWeighted ? smem_u32(rows.ws) : 0u, trash = tb.base - 16u;
 #pragma unroll 1
     for (int jj = sp.jj0; jj < sp.jj1; jj += 2) {
         const ulonglong2 xy = lds_u64x2(sp.grp2 + 16u * (uint32_t)jj);
         const ulonglong2 zw = lds_u64x2(sp.grp2 + 16u * (uint32_t)jj + 16u);  // {z0, z1}, {w0, w1}
-        int row[kR][2];
-        bool open = false;
+        uint32_t open = 0u;
 #pragma unroll
         for (int r = 0; r < kR; ++r) {
             const unsigned long long dx = fadd2(xy.x, pack2(nx[r], nx[r])), dy = fadd2(xy.y, pack2(ny[r], ny[r])),
@@ -759,44 +787,18 @@ __device__ __noinline__ void general_span_full(const WinParams &p, const Tables 
             const unsigned long long s2 = ffma2(dx, dx, ffma2(dy, dy, zz2));
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
-                const float s32 = h ? hi32(s2) : lo32(s2);
-                const uint32_t key = (__float_as_uint(s32) >> kShift) - (uint32_t)kKey0;
-                row[r][h] = -1;
-                if (key < (uint32_t)kCells) {
-                    float thr, guard;
-                    int base;
-                    asm volatile("ld.shared.v2.f32 {%0, %1}, [%2];" : "=f"(thr), "=f"(guard) : "r"(cells + 16u * key));
-                    base = lds_f32_as_int(cells + 16u * key + 8u);
-                    if (fabsf(s32 - thr) > guard) row[r][h] = base + (s32 >= thr ? 1 : 0);
-                }
-                open |= row[r][h] < 0;
+                int row;
+                const bool cert = cell_row(cells, h ? hi32(s2) : lo32(s2), row);
+                asm volatile("red.shared.add.u32 [%0], 1;" ::"r"(cert ? cnt_a + 4u * (uint32_t)row : trash) : "memory");
+                if constexpr (kWeighted)
+                    asm volatile("red.shared.add.f64 [%0], %1;" ::"r"(cert ? ws_a + 8u * (uint32_t)row : trash + 8u),
+                                 "d"((double)wi[r] * (double)(h ? hi32(zw.y) : lo32(zw.y)))
+                                 : "memory");
+                open |= cert ? 0u : 1u << (2 * r + h);
             }
         }
-        if (open) {
-            // the pairs their cell did not certify: the search of chord_row, then the fp64 definition
-#pragma unroll
-            for (int r = 0; r < kR; ++r)
-#pragma unroll
-                for (int h = 0; h < 2; ++h) {
-                    if (row[r][h] >= 0) continue;
-                    const float xj = h ? hi32(xy.x) : lo32(xy.x), yj = h ? hi32(xy.y) : lo32(xy.y), zj = h ? hi32(zw.x) : lo32(zw.x);
-                    int rw = chord_row_ool(-nx[r], -ny[r], -nz[r], xj, yj, zj, tb.sed_ptr(), tb.nbins, tb.margin());
-                    if (rw < 0) {
-                        rw = exact_row(p.xyz_a, p.stride_a, p.perm_a[sp.i_first + r * 32 + lane], p.xyz_b, p.stride_b,
-                                       p.perm_b[sp.j_first + jj + h], p.edges, p.nbins);
-                        ++n_exact;
-                    }
-                    row[r][h] = rw;
-                }
-        }
-#pragma unroll
-        for (int r = 0; r < kR; ++r)
-#pragma unroll
-            for (int h = 0; h < 2; ++h)
-                rows.template add_atomic<kWeighted>(row[r][h], 1u, (double)wi[r] * (double)(h ? hi32(zw.y) : lo32(zw.y)));
+        if (__any_sync(0xffffffffu, open != 0u)) resolve_open<kWeighted>(p, tb, rows, sp, jj, open, stat);
     }
-    n_exact = __reduce_add_sync(0xffffffffu, n_exact);
-    if (lane == 0 && n_exact) atomicAdd(&stat[kStatFp64], (unsigned long long)n_exact);
 }
 
 // Fills the cell table of general_span from the edges as squared chord lengths (sed, ascending; -1 / +inf at the
@@ -805,14 +807,20 @@ __device__ __noinline__ void general_span_full(const WinParams &p, const Tables 
 // the cell is marked crowded (NaN threshold) and its pairs are searched.
 __device__ __forceinline__ void fill_cells(uint32_t cells, const float *sed, int nbins, float margin, int tid, int n_threads)
 {
-    constexpr int kShift = 23 - kCellBits;
-    constexpr int kKey0 = (127 + kCellExpLo) << kCellBits;
     auto guard_at = [&](float se) {  // chord_row's `cleared`, for an edge stored as se
         const float sm = se + margin;
         return 1.02f * (2.5e-7f * sqrtf(sm) + 4.0e-7f * sm + 1.0e-13f) + margin;
     };
-    for (int key = tid; key < kCells; key += n_threads) {
-        const float lo = __uint_as_float((uint32_t)(key + kKey0) << kShift), hi = __uint_as_float((uint32_t)(key + kKey0 + 1) << kShift);
+    for (int key = tid; key < kCellSlots; key += n_threads) {
+        Cell c;
+        if (key >= kCells) {  // the slot of the values outside the table (and the padding after it)
+            c.thr = __uint_as_float(0x7fc00000u);
+            c.word = 0u;
+            *reinterpret_cast<Cell *>(__cvta_shared_to_generic(cells + 8u * (uint32_t)key)) = c;
+            continue;
+        }
+        const float lo = __uint_as_float(((uint32_t)key + kCellKey0) << kCellShift),
+                    hi = __uint_as_float(((uint32_t)key + kCellKey0 + 1u) << kCellShift);
         // a value s of the cell fails to clear edge k only if |s - se_k| <= guard_at(se_k)
         int below = 0, inside = 0, first = -1;
         for (int k = 0; k <= nbins; ++k) {
@@ -829,20 +837,16 @@ __device__ __forceinline__ void fill_cells(uint32_t cells, const float *sed, int
                 ++inside;
             }
         }
-        Cell c;
-        c.row = below;
-        c.pad = 0;
+        c.word = (uint32_t)(below + 1);  // the row of s >= thr
         if (inside == 0) {
-            c.thr = 3.0e38f;  // |s - thr| > guard always, s >= thr never
-            c.guard = 0.f;
+            c.thr = 3.0e38f;  // |s - thr| > 0 always, s >= thr never: all of the cell is row `below`
         } else if (inside == 1) {
             c.thr = sed[first];
-            c.guard = guard_at(sed[first]);
+            c.word |= (__float_as_uint(guard_at(sed[first])) + 0xffffu) & 0xffff0000u;  // rounded up to 8 mantissa bits
         } else {
             c.thr = __uint_as_float(0x7fc00000u);  // NaN: no pair of the cell is certified, the edges are searched
-            c.guard = 0.f;
         }
-        *reinterpret_cast<Cell *>(__cvta_shared_to_generic(cells + 16u * (uint32_t)key)) = c;
+        *reinterpret_cast<Cell *>(__cvta_shared_to_generic(cells + 8u * (uint32_t)key)) = c;
     }
 }
 
@@ -871,7 +875,8 @@ constexpr int kWarpHeader = 128;
 struct CtaHeader {
     unsigned long long stat[8];
     PackInfo pack;
-    uint32_t n_items, chunk, n_jobs, split, pad[4];
+    uint32_t n_items, chunk, n_jobs, split;
+    uint32_t trash[4];  // where the pair-by-pair loop sends the reductions of the pairs it has not certified: a u32, then a double
 };
 static_assert(kNumStats <= 8 && sizeof(CtaHeader) % 16 == 0, "");
 
@@ -940,7 +945,7 @@ __device__ __forceinline__ Rows rows_of(const WinParams &p, const WarpSm<kWeight
         // after the header, the edges and the chord tables (pair_win_kernel)
         size_t off = sizeof(CtaHeader) + sizeof(double) * (size_t)(p.nbins + 1) + sizeof(float) * 4 * (size_t)(p.nbins + 1);
         off = (off + 15) & ~size_t(15);
-        off += sizeof(Cell) * kCells;
+        off += sizeof(Cell) * kCellSlots;
         rows.cnt = reinterpret_cast<uint32_t *>(smem + off);
         off += sizeof(uint32_t) * (size_t)w.rows_n;
         off = (off + 15) & ~size_t(15);
@@ -1326,7 +1331,7 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const __grid_cons
     float *sneg_sm = sed_sm + n_edges, *gs1_sm = sneg_sm + n_edges, *gsk_sm = gs1_sm + n_edges;
     off += sizeof(float) * 4 * (size_t)n_edges;
     off = (off + 15) & ~size_t(15);
-    off += sizeof(Cell) * kCells;  // the cell table (Tables::cells)
+    off += sizeof(Cell) * kCellSlots;  // the cell table (Tables::cells)
     if (p.shared_rows) {
         uint32_t *cnt_shared = reinterpret_cast<uint32_t *>(smem + off);
         off += sizeof(uint32_t) * (size_t)rows_n;
@@ -1533,7 +1538,7 @@ int launch_pair_win(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_a
     auto smem_for = [&](bool shared_rows) {
         size_t m = sizeof(CtaHeader) + sizeof(double) * (size_t)n_edges + sizeof(float) * 4 * (size_t)n_edges;
         m = (m + 15) & ~size_t(15);
-        m += sizeof(Cell) * kCells;
+        m += sizeof(Cell) * kCellSlots;
         if (shared_rows) {
             m += sizeof(uint32_t) * (size_t)rows_n;
             m = (m + 15) & ~size_t(15);
