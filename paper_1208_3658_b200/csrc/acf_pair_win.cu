@@ -54,25 +54,31 @@ constexpr int kScan = 16;              // j-groups bounded at a time (two tiles,
 constexpr int kMaxPassEdges = 3;       // unweighted: windows of more edges than this go pair by pair (general_span); weighted ones
                                        // take as many passes as it needs (their pair-by-pair tallies are fp64 atomics on shared memory)
 // The cell table of the pair-by-pair path: the values of the fp32 squared chord length s that share their sign,
-// exponent and top kCellBits mantissa bits form a cell; 2^kCellBits cells per octave from 2^kCellExpLo to 4.
-constexpr int kCellBits = 4;
+// exponent and top cell_bits mantissa bits form a cell; 2^cell_bits cells per octave from 2^kCellExpLo to 4.
+// Unweighted counts send the windows of more than kMaxPassEdges edges through it: 64 cells per octave, so that bins
+// down to a ratio of 1.011 in s (0.55 % in theta: 100 even bins, 1000 logarithmic ones over four decades) still have a
+// cell to themselves; weighted counts use it for ragged and diagonal groups only and keep the shared memory for their
+// wider stages.
 constexpr int kCellExpLo = -40;        // s below 2^-40 (0.2 arc seconds): no cell, the edges are searched
-constexpr int kCells = (2 - kCellExpLo) << kCellBits;
-constexpr int kCellSlots = kCells + 2;  // slot kCells: the values outside the table (never certified); one more for 16-byte alignment
+__host__ __device__ constexpr int cell_bits(bool weighted) { return weighted ? 4 : 6; }
+__host__ __device__ constexpr int cell_count(bool weighted) { return (2 - kCellExpLo) << cell_bits(weighted); }
+// slot cell_count: the values outside the table (never certified); one more for 16-byte alignment
+__host__ __device__ constexpr int cell_slots(bool weighted) { return cell_count(weighted) + 2; }
 struct Cell {
     float thr;      // the one edge s_k (as stored, fp32) that can separate two rows inside the cell; +big if none; NaN: the cell
                     // holds several edges (or is the slot of the values outside the table) and certifies nothing
     uint32_t word;  // bits 16..31: the guard band of that edge (the bound of chord_row) as the upper half of a float, rounded up:
                     // a pair is certified iff |s - thr| > guard;  bits 0..15: the row of s >= thr (s < thr is the row before)
 };
-static_assert(sizeof(Cell) == 8 && (sizeof(Cell) * kCellSlots) % 16 == 0, "one LDS.64 per pair");
-constexpr int kCellShift = 23 - kCellBits;
-constexpr uint32_t kCellKey0 = (uint32_t)(127 + kCellExpLo) << kCellBits;
+static_assert(sizeof(Cell) == 8 && (sizeof(Cell) * cell_slots(false)) % 16 == 0 && (sizeof(Cell) * cell_slots(true)) % 16 == 0, "one LDS.64 per pair");
 // The row of the squared chord length s32 by its cell; false if the cell does not certify it.
+template <bool kWeighted>
 __device__ __forceinline__ bool cell_row(uint32_t cells, float s32, int &row)
 {
-    // (zero, values below 2^kCellExpLo and NaN wrap or run past the table: all of them land in slot kCells)
-    const uint32_t key = min((__float_as_uint(s32) >> kCellShift) - kCellKey0, (uint32_t)kCells);
+    constexpr int kShift = 23 - cell_bits(kWeighted);
+    constexpr uint32_t kKey0 = (uint32_t)(127 + kCellExpLo) << cell_bits(kWeighted);
+    // (zero, values below 2^kCellExpLo and NaN wrap or run past the table: all of them land in the slot after it)
+    const uint32_t key = min((__float_as_uint(s32) >> kShift) - kKey0, (uint32_t)cell_count(kWeighted));
     float thr;
     uint32_t word;
     asm volatile("ld.shared.v2.b32 {%0, %1}, [%2];" : "=f"(thr), "=r"(word) : "r"(cells + 8u * key));
@@ -711,7 +717,7 @@ __device__ __noinline__ void general_span(const WinParams &p, const Tables tb, c
             const float dx = __fsub_rn(pi[r].x, pj.x), dy = __fsub_rn(pi[r].y, pj.y), dz = __fsub_rn(pi[r].z, pj.z);
             const float s32 = fmaf(dx, dx, fmaf(dy, dy, __fmul_rn(dz, dz)));  // as chord_row computes it
             int row;
-            if (!cell_row(cells, s32, row)) {
+            if (!cell_row<kWeighted>(cells, s32, row)) {
                 row = chord_row_ool(pi[r].x, pi[r].y, pi[r].z, pj.x, pj.y, pj.z, tb.sed_ptr(), tb.nbins, tb.margin());
                 if (row < 0) {
                     row = exact_row(p.xyz_a, p.stride_a, p.perm_a[sp.i_first + r * 32 + lane], p.xyz_b, p.stride_b,
@@ -788,7 +794,7 @@ __device__ __noinline__ void general_span_full(const WinParams &p, const Tables 
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
                 int row;
-                const bool cert = cell_row(cells, h ? hi32(s2) : lo32(s2), row);
+                const bool cert = cell_row<kWeighted>(cells, h ? hi32(s2) : lo32(s2), row);
                 asm volatile("red.shared.add.u32 [%0], 1;" ::"r"(cert ? cnt_a + 4u * (uint32_t)row : trash) : "memory");
                 if constexpr (kWeighted)
                     asm volatile("red.shared.add.f64 [%0], %1;" ::"r"(cert ? ws_a + 8u * (uint32_t)row : trash + 8u),
@@ -805,38 +811,44 @@ __device__ __noinline__ void general_span_full(const WinParams &p, const Tables 
 // poles).  A cell [lo, hi) is taken with the guard bands at its two ends: every edge a value of the cell could fail to
 // clear counts as inside it.  No edge inside: all of the cell is one row.  One: the edge and its guard band.  More:
 // the cell is marked crowded (NaN threshold) and its pairs are searched.
+template <bool kWeighted>
 __device__ __forceinline__ void fill_cells(uint32_t cells, const float *sed, int nbins, float margin, int tid, int n_threads)
 {
+    constexpr int kShift = 23 - cell_bits(kWeighted);
+    constexpr uint32_t kKey0 = (uint32_t)(127 + kCellExpLo) << cell_bits(kWeighted);
     auto guard_at = [&](float se) {  // chord_row's `cleared`, for an edge stored as se
         const float sm = se + margin;
         return 1.02f * (2.5e-7f * sqrtf(sm) + 4.0e-7f * sm + 1.0e-13f) + margin;
     };
-    for (int key = tid; key < kCellSlots; key += n_threads) {
+    // a value s fails to clear edge k only if |s - se_k| <= guard_at(se_k); both ends of that band ascend with k
+    auto band_hi = [&](int k) { return sed[k] < 0.f ? -1.0f : (sed[k] > 3.0e38f ? 3.4e38f : sed[k] + 1.05f * guard_at(sed[k])); };
+    auto band_lo = [&](int k) { return sed[k] < 0.f ? -1.0f : (sed[k] > 3.0e38f ? 3.4e38f : sed[k] - 1.05f * guard_at(sed[k])); };
+    for (int key = tid; key < cell_slots(kWeighted); key += n_threads) {
         Cell c;
-        if (key >= kCells) {  // the slot of the values outside the table (and the padding after it)
+        if (key >= cell_count(kWeighted)) {  // the slot of the values outside the table (and the padding after it)
             c.thr = __uint_as_float(0x7fc00000u);
             c.word = 0u;
             *reinterpret_cast<Cell *>(__cvta_shared_to_generic(cells + 8u * (uint32_t)key)) = c;
             continue;
         }
-        const float lo = __uint_as_float(((uint32_t)key + kCellKey0) << kCellShift),
-                    hi = __uint_as_float(((uint32_t)key + kCellKey0 + 1u) << kCellShift);
-        // a value s of the cell fails to clear edge k only if |s - se_k| <= guard_at(se_k)
-        int below = 0, inside = 0, first = -1;
-        for (int k = 0; k <= nbins; ++k) {
-            const float se = sed[k];
-            if (se < 0.f) {  // the pole edge e_0 = 1: every pair is at or beyond it
-                ++below;
-                continue;
-            }
-            if (se > 3.0e38f) continue;  // the pole edge e_n = -1: no pair is beyond it
-            const float g = 1.05f * guard_at(se);
-            if (se + g < lo) ++below;
-            else if (se - g <= hi) {
-                if (!inside) first = k;
-                ++inside;
-            }
+        const float lo = __uint_as_float(((uint32_t)key + kKey0) << kShift), hi = __uint_as_float(((uint32_t)key + kKey0 + 1u) << kShift);
+        // below: the edges whose band ends before the cell (the pole edge e_0 = 1, stored as -1, always does: every pair is
+        // at or beyond it); up: those whose band starts at or before its end (the pole edge e_n = -1, stored as +inf, never
+        // does: no pair is beyond it).  Two binary searches over the nbins + 1 edges.
+        int below = 0, up = 0;
+        for (int a = 0, b = nbins + 1; a < b;) {
+            const int m = (a + b) >> 1;
+            if (band_hi(m) < lo) below = a = m + 1;
+            else b = m;
         }
+        for (int a = below, b = nbins + 1; a < b;) {
+            const int m = (a + b) >> 1;
+            if (band_lo(m) <= hi) a = m + 1;
+            else b = m;
+            up = a;
+        }
+        if (up < below) up = below;
+        const int inside = up - below, first = below;
         c.word = (uint32_t)(below + 1);  // the row of s >= thr
         if (inside == 0) {
             c.thr = 3.0e38f;  // |s - thr| > 0 always, s >= thr never: all of the cell is row `below`
@@ -945,7 +957,7 @@ __device__ __forceinline__ Rows rows_of(const WinParams &p, const WarpSm<kWeight
         // after the header, the edges and the chord tables (pair_win_kernel)
         size_t off = sizeof(CtaHeader) + sizeof(double) * (size_t)(p.nbins + 1) + sizeof(float) * 4 * (size_t)(p.nbins + 1);
         off = (off + 15) & ~size_t(15);
-        off += sizeof(Cell) * kCellSlots;
+        off += sizeof(Cell) * cell_slots(kWeighted);
         rows.cnt = reinterpret_cast<uint32_t *>(smem + off);
         off += sizeof(uint32_t) * (size_t)w.rows_n;
         off = (off + 15) & ~size_t(15);
@@ -1331,7 +1343,7 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const __grid_cons
     float *sneg_sm = sed_sm + n_edges, *gs1_sm = sneg_sm + n_edges, *gsk_sm = gs1_sm + n_edges;
     off += sizeof(float) * 4 * (size_t)n_edges;
     off = (off + 15) & ~size_t(15);
-    off += sizeof(Cell) * kCellSlots;  // the cell table (Tables::cells)
+    off += sizeof(Cell) * cell_slots(kWeighted);  // the cell table (Tables::cells)
     if (p.shared_rows) {
         uint32_t *cnt_shared = reinterpret_cast<uint32_t *>(smem + off);
         off += sizeof(uint32_t) * (size_t)rows_n;
@@ -1362,7 +1374,7 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const __grid_cons
             gs1_sm[i] = chord_guard(se, margin, false);
             gsk_sm[i] = chord_guard(se, margin, true);
         }
-        fill_cells(tb.cells(), p.sedges, p.nbins, margin, tid, blockDim.x);
+        fill_cells<kWeighted>(tb.cells(), p.sedges, p.nbins, margin, tid, blockDim.x);
     }
     if (!p.shared_rows)
         for (int i = lane; i < rows_n; i += 32) {
@@ -1538,7 +1550,7 @@ int launch_pair_win(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_a
     auto smem_for = [&](bool shared_rows) {
         size_t m = sizeof(CtaHeader) + sizeof(double) * (size_t)n_edges + sizeof(float) * 4 * (size_t)n_edges;
         m = (m + 15) & ~size_t(15);
-        m += sizeof(Cell) * kCellSlots;
+        m += sizeof(Cell) * (size_t)cell_slots(weighted);
         if (shared_rows) {
             m += sizeof(uint32_t) * (size_t)rows_n;
             m = (m + 15) & ~size_t(15);
