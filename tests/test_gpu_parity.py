@@ -291,6 +291,29 @@ def test_linear_bins_many(acf, ctx, oracle):
     acf.acf_set_option(ctx, acf.ACF_OPT_KERNEL, acf.ACF_KERNEL_AUTO)
 
 
+def test_fine_bins_dense_patch(acf, ctx, oracle):
+    """Narrow bins on a dense patch: every window holds many edges, unweighted counts classify such windows pair by
+    pair through the cell table of the squared chord length (64 cells per octave), weighted ones in passes of three
+    edges.  Even bins put up to two edges into a cell at the far end, logarithmic ones do not."""
+    ra, dec = uniform_patch(12000, (10.0, 12.0), (-1.0, 1.0), 17)
+    rb, db = uniform_patch(9000, (10.0, 12.0), (-1.0, 1.0), 18)
+    a, b = acf.acf_radec_to_xyz(ra, dec), acf.acf_radec_to_xyz(rb, db)
+    wa = (1.0 + np.random.default_rng(19).integers(0, 16, 12000) / 16.0).astype(np.float32)
+    wb = (1.0 + np.random.default_rng(20).integers(0, 16, 9000) / 16.0).astype(np.float32)
+    acf.acf_set_option(ctx, acf.ACF_OPT_KERNEL, acf.ACF_KERNEL_WINDOW)
+    for theta in (linear_theta_edges_deg(0.0, 1.0, 100), linear_theta_edges_deg(0.0, 1.5, 400), log_theta_edges_deg(1.0 / 3600, 2.0, 300)):
+        edges = cos_edges_from_theta_deg(theta)
+        assert gpu_counts(acf, ctx, a, None, edges, True).tolist() == oracle.pair_count(a, None, edges, True).tolist()
+        assert gpu_counts(acf, ctx, a, b, edges, False).tolist() == oracle.pair_count(a, b, edges, False).tolist()
+        got = gpu_counts(acf, ctx, a, b, edges, False, wa=wa, wb=wb)
+        want = oracle.pair_count(a, b, edges, False, w_a=wa, w_b=wb)
+        assert got[0].tolist() == want[0].tolist()
+        np.testing.assert_allclose(got[1], want[1], rtol=WSUM_RTOL, atol=0)
+    st = acf.acf_get_stats(ctx)
+    assert st["pairs_window"] < 0.5 * st["pairs_evaluated"]  # mostly windows of several edges
+    acf.acf_set_option(ctx, acf.ACF_OPT_KERNEL, acf.ACF_KERNEL_AUTO)
+
+
 @pytest.mark.parametrize("kernel", ["table", "window"])
 def test_small_angles_chord_tier_and_inexact_norms(acf, ctx, oracle, kernel):
     """Bins far below the fp32 resolution of 1 - cos(theta) (0.02 arcsec to 2 arcmin): the fp32 chord
