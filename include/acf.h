@@ -62,14 +62,16 @@ typedef struct acf_catalog acf_catalog; /* opaque; a catalogue prepared on the d
 
 /* Options for acf_set_option. */
 enum {
-    /* Which pair kernel runs.  ACF_KERNEL_AUTO (default) = the fast fp32-certify path, choosing
-     * between its two kernels; ACF_KERNEL_FP64 = the reference kernel that evaluates the definition
+    /* Which pair kernel runs.  ACF_KERNEL_AUTO (default) = the fast fp32-certify path: the window
+     * kernel for every call (the table kernel only where the window kernel's shared memory does not
+     * fit or its weights do not pack, see below); ACF_KERNEL_FP64 = the reference kernel that evaluates the definition
      * in double for every pair (slow; the arbiter the fast path defers to, kept callable for
      * debugging); ACF_KERNEL_TABLE = fast path, cell-table kernel (single-edge windows in registers,
      * everything else through a bin table and per-lane shared-memory histograms);
      * ACF_KERNEL_WINDOW = fast path, window kernel (every group of pairs classified in registers
-     * against the few edges its bounding caps allow; weights whose range exceeds 2^13 are handed to the
-     * table kernel's per-pair path, whatever the choice).  All four give the same counts.  With very many
+     * against the few edges its bounding caps allow; unweighted groups that more than three edges can
+     * separate, pair by pair through a cell table of the squared chord length; weights whose range
+     * exceeds 2^13 are handed to the table kernel's per-pair path, whatever the choice).  All four give the same counts.  With very many
      * bins a kernel's shared-memory histograms may not fit: AUTO then takes the other fast kernel, an
      * explicit choice returns ACF_EINVAL. */
     ACF_OPT_KERNEL = 1,
