@@ -409,6 +409,42 @@ def ensemble_line(P, ctx, dev):
             "launches": launches, "gpairs_s_nominal": pairs / dt / 1e9, "median_sigma_w": float(np.nanmedian(sd))}
 
 
+# PAPER.md:117-124 (Table 1): the DR component, n^2 pairs, 254 logarithmic bins; whole-program wall time on a Tesla
+# M2070 and on one core of a Xeon E5540, its own catalogue.  Context for detail.paper_shaped, not a
+# target: another machine, another dataset, a timed region that there included reading a text file.
+PAPER_TABLE1 = {"n": [10 ** 4, 10 ** 5, 10 ** 6], "gpu_seconds": [0.2, 16.0, 1254.0], "cpu_seconds": [23.9, 2305.0, 231225.0]}
+
+
+def paper_shaped_line(P, ctx, dev):
+    """The shape of the paper's own timing test: the DR count of n clustered galaxies against n
+    "flat" randoms on the octant 0 < RA, Dec < 90 deg, 254 logarithmic bins over a wide range (1 arcmin - 90 deg), n =
+    1e4, 1e5, 1e6.  Timed from host coordinates to host histogram: canonicalisation, H2D, the count, D2H
+    (detail.paper_shaped)."""
+    import torch
+    from workloads import cos_edges_from_theta_deg, log_theta_edges_deg, neyman_scott, uniform_patch
+    edges = cos_edges_from_theta_deg(log_theta_edges_deg(1.0 / 60.0, 90.0, 254))
+    octant = ((0.0, 90.0), (0.0, 90.0))
+    seconds, in_range = [], []
+    for k, n in enumerate(PAPER_TABLE1["n"]):
+        ra_d, dec_d = neyman_scott(n, max(1, n // 20), 5.0, octant[0], octant[1], 51 + k, children="poisson")
+        ra_r, dec_r = uniform_patch(n, octant[0], octant[1], 61 + k)
+        for rep in range(2 if n < 10 ** 6 else 1):  # (the small ones once more, warm)
+            torch.cuda.synchronize(dev)
+            t0 = time.perf_counter()
+            xa = torch.from_numpy(P.acf_radec_to_xyz(ra_d, dec_d)).to(dev)
+            xb = torch.from_numpy(P.acf_radec_to_xyz(ra_r, dec_r)).to(dev)
+            counts = P.counts_to_numpy(P.acf_pair_count(ctx, xa, xb, edges, False))
+            dt = time.perf_counter() - t0
+        seconds.append(dt)
+        in_range.append(int(counts.sum()))
+    return {"workload": "DR of n clustered points x n flat randoms on the octant 0 < RA, Dec < 90 deg, 254 log bins 1 arcmin - 90 deg, unweighted; "
+                        "host coordinates -> host histogram (canonicalise, H2D, prepare, count, D2H)",
+            "n": PAPER_TABLE1["n"], "seconds": seconds, "pairs_in_range": in_range,
+            "gpairs_s": [n * n / t / 1e9 for n, t in zip(PAPER_TABLE1["n"], seconds)],
+            "paper_table1": dict(PAPER_TABLE1, cite="PAPER.md:117-124", note="context only: Tesla M2070 / one Xeon E5540 core, the paper's "
+                                 "catalogue, whole-program wall time including the text file")}
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
@@ -533,7 +569,7 @@ def main():
     }
 
     # ---- the five configurations and the jackknife, one short measurement each (one GPU, rank 0's box only)
-    configs = jk = mc = None
+    configs = jk = mc = paper = None
     if world == 1 and not args.no_configs:
         configs = {}
         for name in ALL_CONFIGS:
@@ -542,6 +578,7 @@ def main():
                                         e2e=name in ("tiny", "clustered_patch"))
         jk = jackknife_line(P, ctx, dev)
         mc = ensemble_line(P, ctx, dev)
+        paper = paper_shaped_line(P, ctx, dev)
 
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -562,7 +599,8 @@ def main():
             "detail": {"ms_steps": ms_steps, "wall_s_timed_region": t_wall, "pairs_fp64_per_step": acc["fp64"],
                        "pairs_evaluated_per_step": evaluated_per_step, "pairs_single_edge_window_per_step": acc["window"],
                        "pairs_on_chord_per_step": acc["chord"], "launches_per_step": launches_per_step,
-                       "source_sha16": source_hash(), "version": P.acf_version(), "configs": configs, "jackknife": jk, "mc_randoms": mc},
+                       "source_sha16": source_hash(), "version": P.acf_version(), "configs": configs, "jackknife": jk, "mc_randoms": mc,
+                       "paper_shaped": paper},
         }
         print(json.dumps(out), flush=True)
     runner.close()
