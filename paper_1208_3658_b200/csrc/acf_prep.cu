@@ -65,19 +65,20 @@ __global__ void key_kernel(const double *__restrict__ xyz, size_t stride, size_t
 // ------------------------------------------------------------------ radix sort (stable, LSD)
 constexpr int kSortThreads = 256;
 constexpr int kSortWarps = kSortThreads / 32;
-constexpr int kSortPerLane = 16;                                  // elements per lane
-constexpr int kSortWarpChunk = 32 * kSortPerLane;                 // contiguous elements per warp
-constexpr int kSortBlockChunk = kSortWarps * kSortWarpChunk;      // 4096 per CTA
+// Elements per lane: 16 (4096 per CTA), or 64 for catalogues of more than 2 M points, so that the one-CTA scan of the
+// 256 x nblocks digit counts stays short (8 M points: 125 k counters instead of 500 k, 0.46 ms per pass before).
+__host__ __device__ constexpr int sort_per_lane(uint32_t n) { return n > (2u << 20) ? 64 : 16; }
+__host__ __device__ constexpr uint32_t sort_block_chunk(int per_lane) { return (uint32_t)(kSortWarps * 32 * per_lane); }
 
 // counts[d * nblocks + b] = number of keys of CTA b whose digit is d
 __global__ void __launch_bounds__(kSortThreads)
-radix_count_kernel(const uint32_t *__restrict__ keys, uint32_t n, int shift, uint32_t *__restrict__ counts, uint32_t nblocks)
+radix_count_kernel(const uint32_t *__restrict__ keys, uint32_t n, int shift, uint32_t *__restrict__ counts, uint32_t nblocks, int per_lane)
 {
     __shared__ uint32_t hist[256];
     hist[threadIdx.x] = 0;
     __syncthreads();
-    const uint32_t base = blockIdx.x * kSortBlockChunk;
-    for (int t = threadIdx.x; t < kSortBlockChunk; t += kSortThreads) {
+    const uint32_t chunk = sort_block_chunk(per_lane), base = blockIdx.x * chunk;
+    for (uint32_t t = threadIdx.x; t < chunk; t += kSortThreads) {
         const uint32_t i = base + t;
         if (i < n) atomicAdd(&hist[(keys[i] >> shift) & 255u], 1u);
     }
@@ -115,14 +116,14 @@ __global__ void __launch_bounds__(1024) scan_kernel(uint32_t *__restrict__ data,
 __global__ void __launch_bounds__(kSortThreads)
 radix_scatter_kernel(const uint32_t *__restrict__ keys_in, const uint32_t *__restrict__ idx_in,
                      uint32_t *__restrict__ keys_out, uint32_t *__restrict__ idx_out, uint32_t n, int shift,
-                     const uint32_t *__restrict__ offsets, uint32_t nblocks)
+                     const uint32_t *__restrict__ offsets, uint32_t nblocks, int per_lane)
 {
     __shared__ uint32_t whist[kSortWarps][256];  // per-warp digit counts, then running output positions
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     for (int t = threadIdx.x; t < kSortWarps * 256; t += kSortThreads) (&whist[0][0])[t] = 0;
     __syncthreads();
-    const uint32_t wbase = blockIdx.x * kSortBlockChunk + warp * kSortWarpChunk;
-    for (int r = 0; r < kSortPerLane; ++r) {
+    const uint32_t wbase = blockIdx.x * sort_block_chunk(per_lane) + (uint32_t)(warp * 32 * per_lane);
+    for (int r = 0; r < per_lane; ++r) {
         const uint32_t i = wbase + r * 32 + lane;
         if (i < n) atomicAdd(&whist[warp][(keys_in[i] >> shift) & 255u], 1u);
     }
@@ -137,7 +138,7 @@ radix_scatter_kernel(const uint32_t *__restrict__ keys_in, const uint32_t *__res
     }
     __syncthreads();
     const uint32_t lt_mask = (1u << lane) - 1u;
-    for (int r = 0; r < kSortPerLane; ++r) {
+    for (int r = 0; r < per_lane; ++r) {
         const uint32_t i = wbase + r * 32 + lane;
         const bool ok = i < n;
         const uint32_t key = ok ? keys_in[i] : 0u;
@@ -367,17 +368,26 @@ gather_caps_kernel(const double *__restrict__ xyz, size_t stride, size_t off, co
 }
 
 // ------------------------------------------------------------------ work list
-// Angular bounds of all pairs between two caps, as cosines: every pair has
-// cos_lo <= c <= cos_hi.  Radii are padded by 1e-7 rad.
-__device__ __forceinline__ void cap_pair_bounds(const double4 a, const double4 b, double &cos_lo, double &cos_hi)
-{
-    const double d = fmin(1.0, fmax(-1.0, a.x * b.x + a.y * b.y + a.z * b.z));
-    const double th = acos(d), ra = acos(a.w), rb = acos(b.w);
-    const double pad = 1e-7;
-    const double tmin = th - ra - rb - pad, tmax = th + ra + rb + pad;
-    cos_hi = tmin <= 0.0 ? 1.0 : cos(tmin);
-    cos_lo = tmax >= 3.141592653589793 ? -1.0 : cos(tmax);
-}
+// Whether no pair between two caps can be in range, without trigonometry: with R = rho_a + rho_b (both radii at most
+// 90 degrees, else nothing is decided) and d the cosine between the centres,
+//   all pairs beyond theta_max  <=>  theta_ab - R > theta_max  <=>  d < cos(theta_max + R)   (theta_max + R < 180 deg)
+//   all pairs closer than theta_min  <=>  theta_ab + R < theta_min  <=>  d > cos(theta_min - R)   (R < theta_min)
+// taken with a margin on the cosine: 3e-7 for the padding of the radii (1e-7 rad) and the rounding of these few
+// operations, plus `slack` (the caps bound directions; the pair cosine carries the norms: cap_slack).  sa = sin rho_a.
+struct RangeTest {
+    double c_max, s_max, c_min, s_min;  // cos and sin of theta_max (the last edge) and of theta_min (the first)
+    double margin;
+    __device__ __forceinline__ bool out_of_range(const double4 a, double sa, const double4 b) const
+    {
+        if (a.w < 0.0 || b.w < 0.0) return false;
+        const double d = a.x * b.x + a.y * b.y + a.z * b.z;
+        const double sb = sqrt(fmax(0.0, 1.0 - b.w * b.w));
+        const double cR = a.w * b.w - sa * sb, sR = sa * b.w + a.w * sb;  // R in [0, 180 deg]
+        if (cR > -c_max && d < c_max * cR - s_max * sR - margin) return true;  // beyond theta_max
+        if (cR > c_min && d > c_min * cR + s_min * sR + margin) return true;   // closer than theta_min
+        return false;
+    }
+};
 
 // One CTA per i-tile.  Tests every candidate j-tile cap, then one thread walks the survivor bitmap
 // and appends items {ti, first j-tile, number of j-tiles <= kItemTiles}.
@@ -393,6 +403,13 @@ worklist_kernel(const double4 *__restrict__ caps_a, int ti_begin, int ti_end, co
     const int tj_first = is_auto ? ti : 0;
     const double4 ca = caps_a[ti];
     const double slack = 1.001 * __longlong_as_double((long long)counters[kCtrNormDev]);
+    RangeTest rt;
+    rt.c_max = e_last;
+    rt.s_max = sqrt(fmax(0.0, 1.0 - e_last * e_last));
+    rt.c_min = e_first;
+    rt.s_min = sqrt(fmax(0.0, 1.0 - e_first * e_first));
+    rt.margin = slack + 3e-7;
+    const double sa = sqrt(fmax(0.0, 1.0 - ca.w * ca.w));
     uint32_t pruned = 0;
     for (int wbase = 0; wbase < words; wbase += blockDim.x / 32) {
         const int word = wbase + (threadIdx.x >> 5);
@@ -400,24 +417,21 @@ worklist_kernel(const double4 *__restrict__ caps_a, int ti_begin, int ti_end, co
         bool k = false;
         if (word < words && tj < n_tiles_b && tj >= tj_first) {
             k = true;
-            if (prune) {
-                double lo, hi;
-                cap_pair_bounds(ca, caps_b[tj], lo, hi);
-                // no pair can be in range: all beyond theta_max, or all closer than theta_min
-                // (the caps bound directions; the pair cosine carries the norms: cap_slack)
-                if (hi + slack < e_last - 1e-12 || lo - slack > e_first + 1e-12) k = false;
-            }
+            if (prune && rt.out_of_range(ca, sa, caps_b[tj])) k = false;
             pruned += k ? 0u : 1u;
         }
         const uint32_t bits = __ballot_sync(0xffffffffu, k);
         if ((threadIdx.x & 31) == 0 && word < words) keep[word] = bits;
     }
+    // (one atomic per CTA and counter: thousands of CTAs add to the same two words)
+    __shared__ uint32_t pruned_cta;
+    if (threadIdx.x == 0) pruned_cta = 0u;
+    __syncthreads();
     pruned = __reduce_add_sync(0xffffffffu, pruned);
-    if ((threadIdx.x & 31) == 0) {
-        if (pruned) atomicAdd(&counters[kCtrTilePairsPruned], (unsigned long long)pruned);
-    }
+    if ((threadIdx.x & 31) == 0 && pruned) atomicAdd(&pruned_cta, pruned);
     __syncthreads();
     if (threadIdx.x == 0) {
+        if (pruned_cta) atomicAdd(&counters[kCtrTilePairsPruned], (unsigned long long)pruned_cta);
         atomicAdd(&counters[kCtrTilePairsTotal], (unsigned long long)(n_tiles_b - tj_first));
         int tj = tj_first;
         while (tj < n_tiles_b) {
@@ -469,7 +483,8 @@ int prepare_catalogue(acf_ctx *ctx, CatBuffers &buf, const double *xyz, size_t s
     if (cnt == 0) return ACF_OK;
     ACF_CUDA_TRY(ctx, launch_validate(ctx, xyz, stride, off, cnt, w, out->pack));
     ACF_CUDA_TRY(ctx, ctx->s_keys.reserve(sizeof(uint32_t) * 4 * (size_t)n));  // keys x2, idx x2
-    const uint32_t nblocks = (n + kSortBlockChunk - 1) / kSortBlockChunk;
+    const int per_lane = sort_per_lane(n);
+    const uint32_t nblocks = (n + sort_block_chunk(per_lane) - 1) / sort_block_chunk(per_lane);
     ACF_CUDA_TRY(ctx, ctx->s_misc.reserve(sizeof(uint32_t) * 256 * (size_t)nblocks));
     out->pts = reinterpret_cast<float4 *>(base + o_pts);
     out->pts2 = reinterpret_cast<float *>(base + o_pts2);
@@ -488,9 +503,9 @@ int prepare_catalogue(acf_ctx *ctx, CatBuffers &buf, const double *xyz, size_t s
     ctx->last.kernel_launches++;
     for (int pass = 0; pass < 4; ++pass) {
         const int shift = 8 * pass;
-        radix_count_kernel<<<nblocks, kSortThreads, 0, st>>>(k0, n, shift, counts, nblocks);
+        radix_count_kernel<<<nblocks, kSortThreads, 0, st>>>(k0, n, shift, counts, nblocks, per_lane);
         scan_kernel<<<1, 1024, 0, st>>>(counts, 256u * nblocks);
-        radix_scatter_kernel<<<nblocks, kSortThreads, 0, st>>>(k0, i0, k1, i1, n, shift, counts, nblocks);
+        radix_scatter_kernel<<<nblocks, kSortThreads, 0, st>>>(k0, i0, k1, i1, n, shift, counts, nblocks, per_lane);
         ctx->last.kernel_launches += 3;
         uint32_t *t = k0; k0 = k1; k1 = t;
         t = i0; i0 = i1; i1 = t;
