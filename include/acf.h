@@ -154,6 +154,34 @@ int acf_pair_count(acf_ctx *ctx, const double *d_a, size_t n_a, const double *d_
                    const double *cos_edges, int nbins, int is_auto, uint64_t *d_counts);
 
 /*
+ * The same count without any allocation, for callers that cannot call cudaMalloc (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid it).  Needs no context.  Its kernel is a variant of the fp64
+ * reference kernel (every pair evaluated in double as defined above: the counts are those of acf_pair_count, bit
+ * for bit) whose scratch memory -- the device copy of the edges, a status word, one partial histogram per CTA --
+ * is a fixed array in the library's device image: 4.2 MB that every GPU which loads the library holds until the
+ * process exits.  Hence the limit: at most ACF_STATIC_MAX_POINTS points per catalogue, ACF_EINVAL beyond
+ * (unweighted counts only).  The call enqueues a memset, a copy of the edges and two kernels on cuda_stream and
+ * returns; it calls no cudaMalloc, cudaFree or allocating library routine.  The first call on a device asks the
+ * runtime for the array's address (and thereby loads the device image there): make it outside a capture.
+ *   device      : the GPU that d_a, d_b, d_counts, d_bad and cuda_stream belong to (the caller's current
+ *                 device is restored on return).
+ *   d_a, d_b, n_a, n_b, cos_edges, nbins, is_auto : as for acf_pair_count.
+ *   d_counts    : DEVICE, nbins uint64, overwritten (it need not be zeroed).
+ *   d_bad       : DEVICE, one uint32, or NULL: overwritten with the number of invalid points found (non-finite,
+ *                 or |x^2+y^2+z^2 - 1| > 1e-6).  The call does not wait for this verdict: where it is not
+ *                 zero, d_counts is not to be used.
+ *   cuda_stream : the cudaStream_t to enqueue on (NULL: the default stream).
+ *   err, err_len: HOST buffer that receives the message of a failure ("" on success), or NULL.
+ * All calls share the one array, which keeps the last call's contents: what must start at zero is cleared by
+ * every call, but calls that OVERLAP on one GPU (two streams, two host threads) race and give wrong counts.
+ * Calls on one stream are ordered and safe.
+ */
+#define ACF_STATIC_MAX_POINTS 131072
+int acf_pair_count_static(int device, const double *d_a, size_t n_a, const double *d_b, size_t n_b,
+                          const double *cos_edges, int nbins, int is_auto, uint64_t *d_counts, uint32_t *d_bad,
+                          void *cuda_stream, char *err, size_t err_len);
+
+/*
  * Same, with pair weight w_i * w_j (not in the paper; BASELINE.json config 4).
  *   d_wa, d_wb : DEVICE, n_a / n_b floats, finite and >= 0.  In auto mode d_wb must equal d_wa.
  *   d_wsums    : DEVICE, nbins doubles, overwritten with sum over counted pairs of

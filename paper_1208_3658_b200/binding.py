@@ -27,6 +27,7 @@ EXPORTS = [
     "acf_pair_count", "acf_pair_count_weighted", "acf_pair_count_rows", "acf_wtheta", "acf_wtheta_weighted",
     "acf_estimator", "acf_theta_edges", "acf_cos_edges", "acf_jackknife", "acf_correlate_host", "acf_get_stats", "acf_version",
     "acf_prepare", "acf_prepare_rows", "acf_prepare_again", "acf_release", "acf_pair_count_prepared", "acf_random_ensemble",
+    "acf_pair_count_static",
 ]
 
 
@@ -89,6 +90,7 @@ def load_library(build_if_missing: bool = True):
     lib.acf_release.restype = None
     lib.acf_pair_count_prepared.argtypes = [vp, vp, vp, vp, i32, i32, i32, vp, vp]
     lib.acf_random_ensemble.argtypes = [vp, vp, vp, vp, i32, vp, i32, i32, vp, vp, vp, vp, vp, vp]
+    lib.acf_pair_count_static.argtypes = [i32, vp, sz, vp, sz, vp, i32, i32, vp, vp, vp, ctypes.c_char_p, sz]
     lib.acf_get_stats.argtypes = [vp, ctypes.POINTER(acf_stats)]
     lib.acf_version.restype = ctypes.c_char_p
     for name in EXPORTS:
@@ -303,6 +305,40 @@ def acf_pair_count(ctx, d_a, d_b, cos_edges, is_auto, d_counts=None):
     if rc != ACF_OK:
         _raise(ctx, rc)
     return d_counts
+
+
+ACF_STATIC_MAX_POINTS = 131072
+
+
+def acf_pair_count_static(d_a, d_b, cos_edges, is_auto, d_counts=None, d_bad=None, cuda_stream=None):
+    """The count of acf_pair_count by the entry point that allocates nothing (no context; at most
+    ACF_STATIC_MAX_POINTS points per catalogue).  Pass d_counts (int64[nbins]) and d_bad (int32[1]) to keep this
+    wrapper from allocating too.  cuda_stream: a raw cudaStream_t (int) or None for torch's current stream.
+    -> (d_counts, d_bad); asynchronous."""
+    import torch
+    a, pa = _dev(d_a, torch.float64, "d_a")
+    n_a = _n_points(a)
+    if is_auto:
+        pb, n_b = pa, n_a
+    else:
+        b, pb = _dev(d_b, torch.float64, "d_b")
+        n_b = _n_points(b)
+    e, pe = _host(cos_edges, np.float64)
+    nbins = e.size - 1
+    if d_counts is None:
+        d_counts = torch.empty(max(nbins, 1), dtype=torch.int64, device=a.device)
+    if d_bad is None:
+        d_bad = torch.empty(1, dtype=torch.int32, device=a.device)
+    _, pc = _dev(d_counts, torch.int64, "d_counts")
+    _, pbad = _dev(d_bad, torch.int32, "d_bad")
+    if cuda_stream is None:
+        cuda_stream = torch.cuda.current_stream(a.device).cuda_stream
+    err = ctypes.create_string_buffer(512)
+    rc = load_library().acf_pair_count_static(a.device.index, pa, n_a, pb, n_b, pe, nbins, int(bool(is_auto)), pc, pbad,
+                                              cuda_stream, err, len(err))
+    if rc != ACF_OK:
+        raise AcfError(rc, err.value.decode())
+    return d_counts, d_bad
 
 
 def acf_pair_count_weighted(ctx, d_a, d_wa, d_b, d_wb, cos_edges, is_auto, d_counts=None, d_wsums=None):

@@ -18,7 +18,7 @@ INCLUDE = os.path.join(ROOT, "include")
 LIB = os.path.join(PKG, "libacf.so")
 BUILD = os.path.join(PKG, "build")
 
-CUDA_SOURCES = ["acf_api.cu", "acf_kernels_ref.cu", "acf_prep.cu", "acf_pair.cu", "acf_pair_win.cu"]
+CUDA_SOURCES = ["acf_api.cu", "acf_kernels_ref.cu", "acf_prep.cu", "acf_pair.cu", "acf_pair_win.cu", "acf_static.cu"]
 HOST_SOURCES = ["acf_host.cpp"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo",
