@@ -445,6 +445,44 @@ def paper_shaped_line(P, ctx, dev):
                                  "catalogue, whole-program wall time including the text file")}
 
 
+def binning_sweep_line(P, ctx, dev):
+    """The paper's binning sweep (the DR count of the 1e5 sample over bin counts, ranges and even or
+    logarithmic spacing took between 11 and 57 s there, "users should be aware that depending on their choice of
+    binning, timing results may vary"): the same kind of sweep on the octant catalogue of paper_shaped_line, n = 1e5,
+    catalogues resident and prepared once, each count timed on its own after one warm call (detail.binning_sweep)."""
+    import torch
+    from workloads import neyman_scott, uniform_patch
+    n = 10 ** 5
+    octant = ((0.0, 90.0), (0.0, 90.0))
+    ra_d, dec_d = neyman_scott(n, n // 20, 5.0, octant[0], octant[1], 52, children="poisson")
+    ra_r, dec_r = uniform_patch(n, octant[0], octant[1], 62)
+    cd = P.acf_prepare(ctx, torch.from_numpy(P.acf_radec_to_xyz(ra_d, dec_d)).to(dev))
+    cr = P.acf_prepare(ctx, torch.from_numpy(P.acf_radec_to_xyz(ra_r, dec_r)).to(dev))
+    cases = [("log", 1.0 / 60.0, 90.0, 254), ("log", 1.0 / 60.0, 90.0, 20), ("log", 1.0 / 60.0, 90.0, 1024),
+             ("even", 0.0, 90.0, 254), ("even", 0.0, 90.0, 20), ("even", 0.0, 90.0, 1024),
+             ("log", 1.0 / 60.0, 1.0, 254), ("even", 0.0, 10.0, 100)]
+    rows = []
+    for kind, lo, hi, nb in cases:
+        edges = P.acf_cos_edges(P.acf_theta_edges(P.ACF_BINS_LOG if kind == "log" else P.ACF_BINS_EVEN, lo, hi, nb))
+        out = torch.empty(nb, dtype=torch.int64, device=dev)
+        P.acf_pair_count_prepared(ctx, cd, cr, edges, d_counts=out)
+        torch.cuda.synchronize(dev)
+        t0 = time.perf_counter()
+        P.acf_pair_count_prepared(ctx, cd, cr, edges, d_counts=out)
+        torch.cuda.synchronize(dev)
+        dt = time.perf_counter() - t0
+        st = P.acf_get_stats(ctx)
+        rows.append({"bins": "%s, %d bins, %.4g - %.4g deg" % (kind, nb, lo, hi), "ms": 1e3 * dt, "gpairs_s_nominal": n * n / dt / 1e9,
+                     "pairs_evaluated": st["pairs_evaluated"], "pairs_in_range": int(P.counts_to_numpy(out).sum())})
+    P.acf_release(ctx, cd)
+    P.acf_release(ctx, cr)
+    ms = [r["ms"] for r in rows]
+    return {"workload": "DR of 1e5 clustered points x 1e5 flat randoms on the octant, unweighted, prepared catalogues; one count per binning",
+            "cases": rows, "ms_min": min(ms), "ms_max": max(ms),
+            "paper": {"seconds_min": 11.0, "seconds_max": 57.0, "cite": "PAPER.md:126",
+                      "note": "context only: Tesla M2070, the paper's catalogue and its own choice of binnings"}}
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
@@ -569,7 +607,7 @@ def main():
     }
 
     # ---- the five configurations and the jackknife, one short measurement each (one GPU, rank 0's box only)
-    configs = jk = mc = paper = None
+    configs = jk = mc = paper = sweep = None
     if world == 1 and not args.no_configs:
         configs = {}
         for name in ALL_CONFIGS:
@@ -579,6 +617,7 @@ def main():
         jk = jackknife_line(P, ctx, dev)
         mc = ensemble_line(P, ctx, dev)
         paper = paper_shaped_line(P, ctx, dev)
+        sweep = binning_sweep_line(P, ctx, dev)
 
     cpu_baseline = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
@@ -600,7 +639,7 @@ def main():
                        "pairs_evaluated_per_step": evaluated_per_step, "pairs_single_edge_window_per_step": acc["window"],
                        "pairs_on_chord_per_step": acc["chord"], "launches_per_step": launches_per_step,
                        "source_sha16": source_hash(), "version": P.acf_version(), "configs": configs, "jackknife": jk, "mc_randoms": mc,
-                       "paper_shaped": paper},
+                       "paper_shaped": paper, "binning_sweep": sweep},
         }
         print(json.dumps(out), flush=True)
     runner.close()
