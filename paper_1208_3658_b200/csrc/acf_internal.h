@@ -199,7 +199,7 @@ int run_pair_count_fast(acf_ctx *ctx, const double *d_a, const float *d_wa, size
                         int nbins, int is_auto, unsigned long long *d_counts, double *d_wsums);
 
 // ---- acf_pair_win.cu: the window kernel on the work items already in ctx->s_work (edges in ctx->s_edges).
-int launch_pair_win(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_auto, int nbins, uint32_t capacity,
+int launch_pair_win(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_auto, const double *h_edges, int nbins, uint32_t capacity,
                     unsigned long long *d_counts, double *d_wsums);
 
 // ---- acf_prep.cu: sort + gather + caps of points [off, off+cnt) of a catalogue with `stride` points;

@@ -770,7 +770,7 @@ int count_prepared(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_au
             ctx->pair_timed = true;
         }
         if (use_win) {
-            rc = launch_pair_win(ctx, a, b, is_auto, nbins, capacity, d_counts, d_wsums);
+            rc = launch_pair_win(ctx, a, b, is_auto, h_edges, nbins, capacity, d_counts, d_wsums);
             if (rc != ACF_OK) return rc;
             if (weighted && table_fits) {  // the same work list again, for weights that do not pack
                 ACF_CUDA_TRY(ctx, cudaMemsetAsync(&ctx->d_counters[kCtrWorkHead], 0, sizeof(unsigned long long), ctx->stream));

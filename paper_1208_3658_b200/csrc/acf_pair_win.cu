@@ -54,31 +54,37 @@ constexpr int kScan = 16;              // j-groups bounded at a time (two tiles,
 constexpr int kMaxPassEdges = 3;       // unweighted: windows of more edges than this go pair by pair (general_span); weighted ones
                                        // take as many passes as it needs (their pair-by-pair tallies are fp64 atomics on shared memory)
 // The cell table of the pair-by-pair path: the values of the fp32 squared chord length s that share their sign,
-// exponent and top cell_bits mantissa bits form a cell; 2^cell_bits cells per octave from 2^kCellExpLo to 4.
-// Unweighted counts send the windows of more than kMaxPassEdges edges through it: 64 cells per octave, so that bins
-// down to a ratio of 1.011 in s (0.55 % in theta: 100 even bins, 1000 logarithmic ones over four decades) still have a
-// cell to themselves; weighted counts use it for ragged and diagonal groups only and keep the shared memory for their
-// wider stages.
-constexpr int kCellExpLo = -40;        // s below 2^-40 (0.2 arc seconds): no cell, the edges are searched
-__host__ __device__ constexpr int cell_bits(bool weighted) { return weighted ? 4 : 6; }
-__host__ __device__ constexpr int cell_count(bool weighted) { return (2 - kCellExpLo) << cell_bits(weighted); }
-// slot cell_count: the values outside the table (never certified); one more for 16-byte alignment
-__host__ __device__ constexpr int cell_slots(bool weighted) { return cell_count(weighted) + 2; }
+// exponent and top `bits` mantissa bits form a cell; 2^bits cells per octave from 2^exp_lo to 4.  The host picks both
+// per call (cell_shape): exp_lo just below the first edge, and as many cells per octave as the narrowest bin needs to
+// have a cell to itself, between 64 and 1024 for unweighted counts (which send the windows of more than kMaxPassEdges
+// edges through the table) as far as the table stays within kCellBudget; weighted counts use the table for ragged and
+// diagonal groups only and keep 16 cells per octave: their shared memory goes to their wider stages.
+constexpr int kCellExpMin = -40;       // s below 2^-40 (0.2 arc seconds): never a cell, the edges are searched
+constexpr size_t kCellBudget = 48 << 10;
+struct CellShape {
+    int bits, exp_lo, count;  // count = (2 - exp_lo) << bits cells; slot `count` stands for the values outside the table
+    __host__ __device__ int slots() const { return count + 2; }  // (one more for 16-byte alignment)
+};
 struct Cell {
     float thr;      // the one edge s_k (as stored, fp32) that can separate two rows inside the cell; +big if none; NaN: the cell
                     // holds several edges (or is the slot of the values outside the table) and certifies nothing
     uint32_t word;  // bits 16..31: the guard band of that edge (the bound of chord_row) as the upper half of a float, rounded up:
                     // a pair is certified iff |s - thr| > guard;  bits 0..15: the row of s >= thr (s < thr is the row before)
 };
-static_assert(sizeof(Cell) == 8 && (sizeof(Cell) * cell_slots(false)) % 16 == 0 && (sizeof(Cell) * cell_slots(true)) % 16 == 0, "one LDS.64 per pair");
+static_assert(sizeof(Cell) == 8, "one LDS.64 per pair");
+// What the pair loops keep of a CellShape: the shift of the float bits, the key of the first cell, the number of cells.
+struct CellKey {
+    uint32_t shift, key0, count;
+    __device__ __forceinline__ explicit CellKey(const CellShape c)
+        : shift((uint32_t)(23 - c.bits)), key0((uint32_t)(127 + c.exp_lo) << c.bits), count((uint32_t)c.count)
+    {
+    }
+};
 // The row of the squared chord length s32 by its cell; false if the cell does not certify it.
-template <bool kWeighted>
-__device__ __forceinline__ bool cell_row(uint32_t cells, float s32, int &row)
+__device__ __forceinline__ bool cell_row(uint32_t cells, const CellKey ck, float s32, int &row)
 {
-    constexpr int kShift = 23 - cell_bits(kWeighted);
-    constexpr uint32_t kKey0 = (uint32_t)(127 + kCellExpLo) << cell_bits(kWeighted);
-    // (zero, values below 2^kCellExpLo and NaN wrap or run past the table: all of them land in the slot after it)
-    const uint32_t key = min((__float_as_uint(s32) >> kShift) - kKey0, (uint32_t)cell_count(kWeighted));
+    // (zero, values below 2^exp_lo and NaN wrap or run past the table: all of them land in the slot after it)
+    const uint32_t key = min((__float_as_uint(s32) >> ck.shift) - ck.key0, ck.count);
     float thr;
     uint32_t word;
     asm volatile("ld.shared.v2.b32 {%0, %1}, [%2];" : "=f"(thr), "=r"(word) : "r"(cells + 8u * key));
@@ -134,6 +140,7 @@ struct WinParams {
     int prune;        // 1: groups whose window lies wholly out of range are not evaluated
     int bulk;         // 1: groups whose window lies wholly inside one bin are counted as a whole (ACF_OPT_BULK)
     int refine;       // 1: windows of two or more edges are split by the j side's sub-group caps
+    CellShape cell;   // the cell table of the pair-by-pair path
 };
 
 // chord_row out of line: the exact corrections and the pair-by-pair paths call it from unrolled loops, and one copy of
@@ -707,6 +714,7 @@ __device__ __noinline__ void general_span(const WinParams &p, const Tables tb, c
         pi[r].z = -pi[r].z;
     }
     const uint32_t cells = tb.cells();
+    const CellKey ck(p.cell);
     uint32_t n_exact = 0;
     const int jj_end = sp.jj1 < mk.jn ? sp.jj1 : mk.jn;
     for (int jj = sp.jj0; jj < jj_end; ++jj) {
@@ -717,7 +725,7 @@ __device__ __noinline__ void general_span(const WinParams &p, const Tables tb, c
             const float dx = __fsub_rn(pi[r].x, pj.x), dy = __fsub_rn(pi[r].y, pj.y), dz = __fsub_rn(pi[r].z, pj.z);
             const float s32 = fmaf(dx, dx, fmaf(dy, dy, __fmul_rn(dz, dz)));  // as chord_row computes it
             int row;
-            if (!cell_row<kWeighted>(cells, s32, row)) {
+            if (!cell_row(cells, ck, s32, row)) {
                 row = chord_row_ool(pi[r].x, pi[r].y, pi[r].z, pj.x, pj.y, pj.z, tb.sed_ptr(), tb.nbins, tb.margin());
                 if (row < 0) {
                     row = exact_row(p.xyz_a, p.stride_a, p.perm_a[sp.i_first + r * 32 + lane], p.xyz_b, p.stride_b,
@@ -777,6 +785,7 @@ __device__ __noinline__ void general_span_full(const WinParams &p, const Tables 
         wi[r] = v.w;
     }
     const uint32_t cells = tb.cells();
+    const CellKey ck(p.cell);
     // (no branch around a pair's reduction: an uncertified pair adds to CtaHeader::trash, the last 16 bytes before the tables)
     const uint32_t cnt_a = smem_u32(rows.cnt), ws_a = kWeighted ? smem_u32(rows.ws) : 0u, trash = tb.base - 16u;
 #pragma unroll 1
@@ -794,7 +803,7 @@ __device__ __noinline__ void general_span_full(const WinParams &p, const Tables 
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
                 int row;
-                const bool cert = cell_row<kWeighted>(cells, h ? hi32(s2) : lo32(s2), row);
+                const bool cert = cell_row(cells, ck, h ? hi32(s2) : lo32(s2), row);
                 asm volatile("red.shared.add.u32 [%0], 1;" ::"r"(cert ? cnt_a + 4u * (uint32_t)row : trash) : "memory");
                 if constexpr (kWeighted)
                     asm volatile("red.shared.add.f64 [%0], %1;" ::"r"(cert ? ws_a + 8u * (uint32_t)row : trash + 8u),
@@ -811,11 +820,11 @@ __device__ __noinline__ void general_span_full(const WinParams &p, const Tables 
 // poles).  A cell [lo, hi) is taken with the guard bands at its two ends: every edge a value of the cell could fail to
 // clear counts as inside it.  No edge inside: all of the cell is one row.  One: the edge and its guard band.  More:
 // the cell is marked crowded (NaN threshold) and its pairs are searched.
-template <bool kWeighted>
-__device__ __forceinline__ void fill_cells(uint32_t cells, const float *sed, int nbins, float margin, int tid, int n_threads)
+__device__ __forceinline__ void fill_cells(uint32_t cells, const CellShape shape, const float *sed, int nbins, float margin, int tid,
+                                           int n_threads)
 {
-    constexpr int kShift = 23 - cell_bits(kWeighted);
-    constexpr uint32_t kKey0 = (uint32_t)(127 + kCellExpLo) << cell_bits(kWeighted);
+    const int kShift = 23 - shape.bits;
+    const uint32_t kKey0 = (uint32_t)(127 + shape.exp_lo) << shape.bits;
     auto guard_at = [&](float se) {  // chord_row's `cleared`, for an edge stored as se
         const float sm = se + margin;
         return 1.02f * (2.5e-7f * sqrtf(sm) + 4.0e-7f * sm + 1.0e-13f) + margin;
@@ -823,9 +832,9 @@ __device__ __forceinline__ void fill_cells(uint32_t cells, const float *sed, int
     // a value s fails to clear edge k only if |s - se_k| <= guard_at(se_k); both ends of that band ascend with k
     auto band_hi = [&](int k) { return sed[k] < 0.f ? -1.0f : (sed[k] > 3.0e38f ? 3.4e38f : sed[k] + 1.05f * guard_at(sed[k])); };
     auto band_lo = [&](int k) { return sed[k] < 0.f ? -1.0f : (sed[k] > 3.0e38f ? 3.4e38f : sed[k] - 1.05f * guard_at(sed[k])); };
-    for (int key = tid; key < cell_slots(kWeighted); key += n_threads) {
+    for (int key = tid; key < shape.slots(); key += n_threads) {
         Cell c;
-        if (key >= cell_count(kWeighted)) {  // the slot of the values outside the table (and the padding after it)
+        if (key >= shape.count) {  // the slot of the values outside the table (and the padding after it)
             c.thr = __uint_as_float(0x7fc00000u);
             c.word = 0u;
             *reinterpret_cast<Cell *>(__cvta_shared_to_generic(cells + 8u * (uint32_t)key)) = c;
@@ -957,7 +966,7 @@ __device__ __forceinline__ Rows rows_of(const WinParams &p, const WarpSm<kWeight
         // after the header, the edges and the chord tables (pair_win_kernel)
         size_t off = sizeof(CtaHeader) + sizeof(double) * (size_t)(p.nbins + 1) + sizeof(float) * 4 * (size_t)(p.nbins + 1);
         off = (off + 15) & ~size_t(15);
-        off += sizeof(Cell) * cell_slots(kWeighted);
+        off += sizeof(Cell) * (size_t)p.cell.slots();
         rows.cnt = reinterpret_cast<uint32_t *>(smem + off);
         off += sizeof(uint32_t) * (size_t)w.rows_n;
         off = (off + 15) & ~size_t(15);
@@ -1343,7 +1352,7 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const __grid_cons
     float *sneg_sm = sed_sm + n_edges, *gs1_sm = sneg_sm + n_edges, *gsk_sm = gs1_sm + n_edges;
     off += sizeof(float) * 4 * (size_t)n_edges;
     off = (off + 15) & ~size_t(15);
-    off += sizeof(Cell) * cell_slots(kWeighted);  // the cell table (Tables::cells)
+    off += sizeof(Cell) * (size_t)p.cell.slots();  // the cell table (Tables::cells)
     if (p.shared_rows) {
         uint32_t *cnt_shared = reinterpret_cast<uint32_t *>(smem + off);
         off += sizeof(uint32_t) * (size_t)rows_n;
@@ -1374,7 +1383,7 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const __grid_cons
             gs1_sm[i] = chord_guard(se, margin, false);
             gsk_sm[i] = chord_guard(se, margin, true);
         }
-        fill_cells<kWeighted>(tb.cells(), p.sedges, p.nbins, margin, tid, blockDim.x);
+        fill_cells(tb.cells(), p.cell, p.sedges, p.nbins, margin, tid, blockDim.x);
     }
     if (!p.shared_rows)
         for (int i = lane; i < rows_n; i += 32) {
@@ -1542,15 +1551,40 @@ __global__ void __launch_bounds__(kThreads, 1) pair_win_kernel(const __grid_cons
 }  // namespace
 
 // Launches the window kernel on the work items of the context's work list.
-int launch_pair_win(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_auto, int nbins, uint32_t capacity,
+// The shape of the cell table for a call's edges (see CellShape): the table starts two octaves below the octave of the
+// first edge that is not a pole (closer pairs, a factor 2 to 2.8 below theta_min, are searched); a cell is 0.69 / 2^bits
+// of its s wide, and the narrowest bin should be at least two cells wide.
+static CellShape cell_shape(const double *h_edges, int nbins, bool weighted)
+{
+    double s_first = 4.0, rel_min = 1.0;
+    double prev = -1.0;
+    for (int k = 0; k <= nbins; ++k) {
+        const double sk = 2.0 * (1.0 - h_edges[k]);  // ascending
+        if (sk > 0.0 && sk < s_first) s_first = sk;
+        if (prev > 0.0 && sk > prev) rel_min = std::min(rel_min, (sk - prev) / sk);
+        prev = sk;
+    }
+    CellShape c;
+    int e = 0;
+    std::frexp(s_first, &e);  // s_first = f 2^e, f in [0.5, 1): the octave of s_first starts at 2^(e - 1)
+    c.exp_lo = std::max(kCellExpMin, std::min(1, e - 3));
+    c.bits = weighted ? 4 : 6;
+    if (!weighted)
+        while (c.bits < 10 && 0.69 / (double)(1 << c.bits) > 0.5 * rel_min && sizeof(Cell) * ((size_t)(2 - c.exp_lo) << (c.bits + 1)) <= kCellBudget) ++c.bits;
+    c.count = (2 - c.exp_lo) << c.bits;
+    return c;
+}
+
+int launch_pair_win(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_auto, const double *h_edges, int nbins, uint32_t capacity,
                     unsigned long long *d_counts, double *d_wsums)
 {
     const bool weighted = d_wsums != nullptr;
+    const CellShape cell = cell_shape(h_edges, nbins, weighted);
     const int rows_n = nbins + 2, n_edges = nbins + 1;
     auto smem_for = [&](bool shared_rows) {
         size_t m = sizeof(CtaHeader) + sizeof(double) * (size_t)n_edges + sizeof(float) * 4 * (size_t)n_edges;
         m = (m + 15) & ~size_t(15);
-        m += sizeof(Cell) * (size_t)cell_slots(weighted);
+        m += sizeof(Cell) * (size_t)cell.slots();
         if (shared_rows) {
             m += sizeof(uint32_t) * (size_t)rows_n;
             m = (m + 15) & ~size_t(15);
@@ -1596,6 +1630,7 @@ int launch_pair_win(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_a
     p.prune = ctx->opt_prune;
     p.bulk = ctx->opt_bulk;
     p.refine = 1;
+    p.cell = cell;
 
     const int grid = ctx->num_sms;  // one CTA of 16 warps per SM: 128 registers a thread
     cudaError_t e = cudaSuccess;
