@@ -1579,7 +1579,7 @@ int launch_pair_win(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_a
                     unsigned long long *d_counts, double *d_wsums)
 {
     const bool weighted = d_wsums != nullptr;
-    const CellShape cell = cell_shape(h_edges, nbins, weighted);
+    CellShape cell = cell_shape(h_edges, nbins, weighted);
     const int rows_n = nbins + 2, n_edges = nbins + 1;
     auto smem_for = [&](bool shared_rows) {
         size_t m = sizeof(CtaHeader) + sizeof(double) * (size_t)n_edges + sizeof(float) * 4 * (size_t)n_edges;
@@ -1597,7 +1597,20 @@ int launch_pair_win(acf_ctx *ctx, const Prepared &a, const Prepared &b, int is_a
         return m + per_warp * kWarps + 128;  // (+128: the dynamic segment need not start on a 128-byte boundary)
     };
     const size_t budget = (size_t)ctx->max_smem_optin;
-    bool shared_rows = smem_for(false) > budget;  // a set of rows per warp, or one per CTA when that leaves no room
+    // what gives way when the shared memory is short: first the cell table's resolution, then the rows per warp (one
+    // set per CTA instead, every update atomic), then the resolution again
+    auto shrink_cells = [&](bool shared_rows) {
+        while (smem_for(shared_rows) > budget && cell.bits > (weighted ? 4 : 6)) {
+            --cell.bits;
+            cell.count = (2 - cell.exp_lo) << cell.bits;
+        }
+    };
+    shrink_cells(false);
+    const bool shared_rows = smem_for(false) > budget;
+    if (shared_rows) {
+        cell = cell_shape(h_edges, nbins, weighted);
+        shrink_cells(true);
+    }
     if (smem_for(shared_rows) > budget) return fail(ctx, ACF_EINVAL, "too many bins for the window kernel (%d)", nbins);
     const size_t smem = smem_for(shared_rows);
 

@@ -301,7 +301,9 @@ def test_fine_bins_dense_patch(acf, ctx, oracle):
     wa = (1.0 + np.random.default_rng(19).integers(0, 16, 12000) / 16.0).astype(np.float32)
     wb = (1.0 + np.random.default_rng(20).integers(0, 16, 9000) / 16.0).astype(np.float32)
     acf.acf_set_option(ctx, acf.ACF_OPT_KERNEL, acf.ACF_KERNEL_WINDOW)
-    for theta in (linear_theta_edges_deg(0.0, 1.0, 100), linear_theta_edges_deg(0.0, 1.5, 400), log_theta_edges_deg(1.0 / 3600, 2.0, 300)):
+    # (the last: so many bins that the cell table gives up resolution for the rows' shared memory)
+    for theta in (linear_theta_edges_deg(0.0, 1.0, 100), linear_theta_edges_deg(0.0, 1.5, 400), log_theta_edges_deg(1.0 / 3600, 2.0, 300),
+                  linear_theta_edges_deg(0.0, 90.0, 640)):
         edges = cos_edges_from_theta_deg(theta)
         assert gpu_counts(acf, ctx, a, None, edges, True).tolist() == oracle.pair_count(a, None, edges, True).tolist()
         assert gpu_counts(acf, ctx, a, b, edges, False).tolist() == oracle.pair_count(a, b, edges, False).tolist()
