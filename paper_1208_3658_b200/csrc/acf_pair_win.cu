@@ -80,17 +80,26 @@ struct CellKey {
     {
     }
 };
-// The row of the squared chord length s32 by its cell; false if the cell does not certify it.
-__device__ __forceinline__ bool cell_row(uint32_t cells, const CellKey ck, float s32, int &row)
+// The cell of the squared chord length s32 ...
+__device__ __forceinline__ void cell_load(uint32_t cells, const CellKey ck, float s32, float &thr, uint32_t &word)
 {
     // (zero, values below 2^exp_lo and NaN wrap or run past the table: all of them land in the slot after it)
     const uint32_t key = min((__float_as_uint(s32) >> ck.shift) - ck.key0, ck.count);
-    float thr;
-    uint32_t word;
     asm volatile("ld.shared.v2.b32 {%0, %1}, [%2];" : "=f"(thr), "=r"(word) : "r"(cells + 8u * key));
+}
+// ... and its row by that cell; false if the cell does not certify it.
+__device__ __forceinline__ bool cell_decide(float s32, float thr, uint32_t word, int &row)
+{
     const float d = s32 - thr;
     row = (int)(word & 0xffffu) + (__float_as_int(d) >> 31);
     return fabsf(d) > __uint_as_float(word & 0xffff0000u);
+}
+__device__ __forceinline__ bool cell_row(uint32_t cells, const CellKey ck, float s32, int &row)
+{
+    float thr;
+    uint32_t word;
+    cell_load(cells, ck, s32, thr, word);
+    return cell_decide(s32, thr, word, row);
 }
 // Guard bands on the cosine (u = 2^-24).  A wrong fp32 sign needs
 // |d_0 - (e_m - c64)| >= |d_0|, so only pairs with a small |d_0| matter; for those the partial sums of the
@@ -793,17 +802,28 @@ __device__ __noinline__ void general_span_full(const WinParams &p, const Tables 
         const ulonglong2 xy = lds_u64x2(sp.grp2 + 16u * (uint32_t)jj);
         const ulonglong2 zw = lds_u64x2(sp.grp2 + 16u * (uint32_t)jj + 16u);  // {z0, z1}, {w0, w1}
         uint32_t open = 0u;
+        // first all eight table loads, then the eight decisions and reductions: the loads and the reductions are
+        // volatile and keep their order, and a load that waited behind the previous pair's reduction was what the loop
+        // spent its time on
+        unsigned long long s2[kR];
+        float thr[kR][2];
+        uint32_t word[kR][2];
 #pragma unroll
         for (int r = 0; r < kR; ++r) {
             const unsigned long long dx = fadd2(xy.x, pack2(nx[r], nx[r])), dy = fadd2(xy.y, pack2(ny[r], ny[r])),
                                      dz = fadd2(zw.x, pack2(nz[r], nz[r]));
             unsigned long long zz2;
             asm("mul.rn.f32x2 %0, %1, %1;" : "=l"(zz2) : "l"(dz));
-            const unsigned long long s2 = ffma2(dx, dx, ffma2(dy, dy, zz2));
+            s2[r] = ffma2(dx, dx, ffma2(dy, dy, zz2));
+#pragma unroll
+            for (int h = 0; h < 2; ++h) cell_load(cells, ck, h ? hi32(s2[r]) : lo32(s2[r]), thr[r][h], word[r][h]);
+        }
+#pragma unroll
+        for (int r = 0; r < kR; ++r) {
 #pragma unroll
             for (int h = 0; h < 2; ++h) {
                 int row;
-                const bool cert = cell_row(cells, ck, h ? hi32(s2) : lo32(s2), row);
+                const bool cert = cell_decide(h ? hi32(s2[r]) : lo32(s2[r]), thr[r][h], word[r][h], row);
                 asm volatile("red.shared.add.u32 [%0], 1;" ::"r"(cert ? cnt_a + 4u * (uint32_t)row : trash) : "memory");
                 if constexpr (kWeighted)
                     asm volatile("red.shared.add.f64 [%0], %1;" ::"r"(cert ? ws_a + 8u * (uint32_t)row : trash + 8u),
