@@ -92,7 +92,8 @@ __device__ __forceinline__ bool cell_decide(float s32, float thr, uint32_t word,
 {
     const float d = s32 - thr;
     row = (int)(word & 0xffffu) + (__float_as_int(d) >> 31);
-    return fabsf(d) > __uint_as_float(word & 0xffff0000u);
+    // (the whole word as the float: the row in its low half adds less than 2^-7 of the guard band to it, on the safe side)
+    return fabsf(d) > __uint_as_float(word);
 }
 __device__ __forceinline__ bool cell_row(uint32_t cells, const CellKey ck, float s32, int &row)
 {
